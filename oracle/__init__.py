@@ -1,0 +1,37 @@
+"""CPU oracle for the Llumnix KV-cache live-migration hot path.  TEST INFRASTRUCTURE ONLY.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` /
+`--impl reference` legs may import this package.  It shares no code with the
+CUDA path (`paper_2406_03243_b200/`): no common kernels, headers, helpers,
+tables or constants; neither imports the other.  Inputs come from `synth/`,
+passed in as arrays by the caller.
+
+What it computes, and the passage each part follows (all `PAPER.md:<line>`):
+
+* `kv_migration.migrate_stage`   — one migration stage: the blocks of the request
+  named by (src_block_ids, dst_block_ids) are copied whole, every layer, K and V
+  (§4.2 live migration; block = K or V of `block_size` tokens of
+  one layer, §5 "Block fusion"; destination blocks are reserved
+  before the stage, §4.2 handshake).
+* `kv_migration.migrate_batch`   — the same for many requests (the source llumlet
+  migrates requests one after another, §4.4.3).
+* `kv_migration.pack` / `unpack` — block fusion: gather into / scatter from ONE
+  contiguous buffer (§5 "Block fusion"; buffer is what the
+  transport sends, §5 "KV cache transfer").
+* `kv_migration.append_tokens`   — the append-only growth of the cache while
+  decoding continues (§4.2).
+* `kv_migration.staged_migration`— stage 0..N with decoding in between (Fig. 6,
+  PAPER.md:134).
+* `kv_migration.plan_stage`, `stage_sizes` — which logical blocks a stage takes
+   and the shrinking-stage recurrence behind "only takes two
+  stages" (§6.2).
+* `decode_attention.decode_attention_fp64` — standard KV-cache attention for one
+  decode token per sequence, read through the block table (§2).
+
+Parity pins (tests/test_oracle_*.py, `-m "not gpu"`): every function above is
+pinned to something other than itself — pure-Python element-loop brute force on
+micro pools (P1–P8), the paper's printed block arithmetic (P12,
+tests/golden/paper_block_arithmetic.txt), closed-form special cases and
+`torch.nn.functional.scaled_dot_product_attention` in float64 (P11), and the
+closed form of the stage recurrence (P9).  Nothing here is "parity unpinned".
+"""
