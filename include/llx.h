@@ -1,0 +1,198 @@
+/* llx.h — C ABI of the B200-native live-migration path for a paged KV cache.
+ *
+ * What this library computes is fixed by Llumnix (arxiv 2406.03243); citations are
+ * "PAPER.md:<line>" of the paper text plus the section the line falls in.
+ *
+ *   - §4.2 "Live Migration of LLM Requests" (Fig. 6): the KV cache is
+ *     append-only, so the blocks of completed iterations are copied to the destination
+ *     instance in STAGES while decoding continues; a short final stage copies the last
+ *     blocks once the source has stopped the request.
+ *   - §4.2 handshake (Fig. 7): the destination RESERVES the blocks of a stage
+ *     before the stage runs; the caller therefore passes the destination block ids in.
+ *   - §5 "Block fusion": the copy unit is the block = K *or* V of block_size
+ *     tokens of ONE layer (128 KB for 16-bit LLaMA-7B); the many small blocks of a request
+ *     are fused into ONE contiguous buffer for the transport.
+ *   - §5 "KV cache transfer": copies run on their own CUDA stream so that
+ *     inference is not blocked.
+ *
+ * Memory model.  A pool is one serving instance's KV cache:
+ *
+ *     pool[layer][kv][block][slot][head][dim]       kv: 0 = K, 1 = V
+ *
+ * one dense allocation in that order, i.e. per layer and per K|V a row-major tensor
+ * [num_blocks, block_size, kv_heads, head_dim].  A "tile" is pool[layer][kv][block] —
+ * tile_bytes = block_size*kv_heads*head_dim*elem_bytes contiguous bytes — the paper's block.
+ * A "block id" names the same row index in every (layer, kv) slice; block_bytes =
+ * 2*layers*tile_bytes.  tile_bytes must be a multiple of 16 and the base 16-byte aligned.
+ *
+ * Conventions for every call.
+ *   - Pointers named *_ids / req_offsets are HOST int32 arrays owned by the caller; the
+ *     library copies them before returning, so they may be reused at once.
+ *   - Pointers named dev_* are DEVICE pointers.  `staging` may be a device pointer or a
+ *     pinned, mapped host pointer (UVA tells them apart).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Data calls only ENQUEUE work on it and return; completion is observed by the caller
+ *     through the stream.  Pools and staging buffers must outlive the enqueued work.
+ *   - Errors are return codes; nothing throws or aborts across this boundary.  Argument
+ *     errors are found on the host BEFORE anything is launched: a failed call changes no
+ *     byte of any pool.  An asynchronous CUDA fault surfaces as LLX_ERR_CUDA from a later
+ *     call.  n == 0 (or R == 0) is LLX_OK and launches nothing.
+ *   - The library never allocates or frees BLOCKS: reservation is the caller's job
+ *     (the paper's PRE-ALLOC).  An aborted migration needs no byte rollback.
+ *   - There is no CPU fallback: without a CUDA device every data call returns LLX_ERR_CUDA.
+ */
+#ifndef LLX_H_
+#define LLX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct llx_pool llx_pool; /* opaque */
+
+/* Only the element size matters to migration; decode attention requires LLX_F16. */
+typedef enum { LLX_F16 = 0, LLX_BF16 = 1, LLX_U8 = 2 } llx_dtype;
+
+typedef enum {
+    LLX_OK = 0,
+    LLX_ERR_INVALID_ARG = -1,       /* NULL pointer, negative size, unsupported shape */
+    LLX_ERR_GEOMETRY_MISMATCH = -2, /* src and dst pools differ in layers / tile_bytes */
+    LLX_ERR_BLOCK_OUT_OF_RANGE = -3,
+    LLX_ERR_DUPLICATE_DST = -4,     /* a destination block id appears twice in one call */
+    LLX_ERR_ALIAS = -5,             /* src and dst are the same pool / overlap */
+    LLX_ERR_STAGING_TOO_SMALL = -6,
+    LLX_ERR_OOM = -7,
+    LLX_ERR_CUDA = -8
+} llx_status;
+
+/* ---- pools (D1 in SURVEY.md; PagedAttention blocks) ------------------ */
+
+/* Allocates layers*2*num_blocks tiles with cudaMalloc on the current device; contents are
+ * undefined.  *out is owned by the caller and released with llx_pool_destroy. */
+llx_status llx_pool_create(int layers, int kv_heads, int head_dim, int block_size, llx_dtype dtype,
+                           int num_blocks, llx_pool** out);
+/* Describes caller-owned device memory (e.g. a torch tensor) of at least llx_pool_bytes;
+ * `bytes` is checked.  llx_pool_destroy of a wrapped pool frees only the handle. */
+llx_status llx_pool_wrap(void* dev_ptr, size_t bytes, int layers, int kv_heads, int head_dim, int block_size,
+                         llx_dtype dtype, int num_blocks, llx_pool** out);
+llx_status llx_pool_destroy(llx_pool* pool);
+
+void*  llx_pool_data(const llx_pool* pool, int layer, int kv); /* device address of pool[layer][kv][0]; NULL on bad args */
+size_t llx_pool_tile_bytes(const llx_pool* pool);              /* block_size*kv_heads*head_dim*elem_bytes */
+size_t llx_pool_block_bytes(const llx_pool* pool);             /* 2*layers*tile_bytes */
+size_t llx_pool_bytes(const llx_pool* pool);                   /* num_blocks*block_bytes */
+int    llx_pool_num_blocks(const llx_pool* pool);
+/* Bytes a pool of this geometry needs (for sizing memory passed to llx_pool_wrap); 0 on bad args. */
+size_t llx_pool_bytes_for(int layers, int kv_heads, int head_dim, int block_size, llx_dtype dtype, int num_blocks);
+
+/* Plain stream-ordered copies between HOST memory and n_blocks consecutive tiles
+ * pool[layer][kv][first_block ...]: how the owner of a library-allocated pool fills and
+ * inspects it.  `host` holds n_blocks*tile_bytes bytes; pinned memory makes them truly async. */
+llx_status llx_pool_upload(llx_pool* pool, int layer, int kv, int first_block, int n_blocks, const void* host,
+                           void* cuda_stream);
+llx_status llx_pool_download(const llx_pool* pool, int layer, int kv, int first_block, int n_blocks, void* host,
+                             void* cuda_stream);
+/* Sets every 16-bit word of the whole pool to `pattern` (the tests' sentinel). */
+llx_status llx_pool_fill_u16(llx_pool* pool, uint16_t pattern, void* cuda_stream);
+
+/* ---- S1: stage planning (host arithmetic, no device work) -------------------- */
+
+/* Which logical blocks [blocks_migrated, blocks_migrated + *n) of a request the NEXT stage takes.
+ * A non-final stage copies "the KV cache blocks of completed iterations" that can no longer
+ * change: the full blocks, never the one being appended to.  When at most
+ * last_stage_max_blocks blocks remain the stage is final (*is_final = 1): the caller stops the
+ * request first, and the stage takes everything left including the partly filled block.
+ * LLX_ERR_INVALID_ARG if blocks_migrated exceeds ceil(num_tokens/block_size) or a size is bad. */
+llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, int last_stage_max_blocks, int* n,
+                          int* is_final);
+
+/* ---- S3/S4: one migration stage (reserved dst blocks PAPER.md:142) -------- */
+
+/* for i<n, l<layers, kv<2:  dst[l][kv][dst_block_ids[i]][:] = src[l][kv][src_block_ids[i]][:]
+ * Whole tiles, including unused token slots of a partly filled last block.  One kernel
+ * launch on `cuda_stream`.  Checked: same geometry (num_blocks may differ), ids in range,
+ * no duplicate destination id (duplicate source ids are legal: prefix-shared blocks),
+ * src and dst distinct and non-overlapping.  src is never written. */
+llx_status llx_migrate_stage(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
+                             const int32_t* dst_block_ids, int n, void* cuda_stream);
+
+/* ---- S5: many requests in ONE launch (the source migrates its chosen
+ * requests one after another; batching them is this build's extension) -------------------- */
+
+/* Request r owns pairs [req_offsets[r], req_offsets[r+1]) of the flat id lists;
+ * req_offsets[0] == 0, non-decreasing, R+1 entries.  Result == R successive
+ * llx_migrate_stage calls.  Destination ids must be distinct across the whole batch. */
+llx_status llx_migrate_batch(const llx_pool* src, llx_pool* dst, const int32_t* req_offsets,
+                             const int32_t* src_block_ids, const int32_t* dst_block_ids, int R, void* cuda_stream);
+
+/* ---- S6: block fusion — gather into / scatter from ONE contiguous buffer -- */
+
+/* Staging layout: staging[i][layer][kv][tile_bytes], i = position in the id list, so the
+ * buffers of consecutive stages concatenate.  llx_staging_bytes = n*block_bytes. */
+size_t     llx_staging_bytes(const llx_pool* pool, int n);
+/* Pinned, mapped host memory for a staging buffer the kernels can address directly.
+ * *host_ptr is the CPU address, *dev_alias the address to pass as `staging` (equal under UVA). */
+llx_status llx_staging_alloc_pinned(size_t bytes, void** host_ptr, void** dev_alias);
+llx_status llx_staging_free_pinned(void* host_ptr);
+/* staging[i][l][kv][:] = src[l][kv][src_block_ids[i]][:] */
+llx_status llx_pack(const llx_pool* src, const int32_t* src_block_ids, int n, void* staging, size_t staging_bytes,
+                    void* cuda_stream);
+/* dst[l][kv][dst_block_ids[i]][:] = staging[i][l][kv][:]   (dst ids distinct) */
+llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, const int32_t* dst_block_ids, int n,
+                      void* cuda_stream);
+
+/* ---- S8: append-only growth while decoding continues --------------- */
+
+/* Writes the K and V vectors of tokens t0..t1-1 of one request into their slots: token t
+ * lives in block block_table[t / block_size], slot t % block_size.
+ * dev_values: DEVICE buffer [t1-t0][layers][2][kv_heads*head_dim] elements (token-major).
+ * block_table: HOST int32[table_len] with table_len > (t1-1)/block_size.  Nothing else is written. */
+llx_status llx_append_tokens(llx_pool* pool, const int32_t* block_table, int table_len, int t0, int t1,
+                             const void* dev_values, void* cuda_stream);
+
+/* ---- S7: stand-in paged decode attention (measurement only) ------------- */
+
+/* One query token per sequence, MHA (q heads = kv heads), fp16 in, fp32 accumulate, fp16 out:
+ *   o[b][h] = sum_t softmax_t(scale * q[b][h].k_t[h]) v_t[h],  t < dev_ctx_lens[b],
+ * K/V of token t read from block dev_block_tables[b*max_blocks + t/block_size], slot t%block_size.
+ * dev_q, dev_out: DEVICE fp16 [B, kv_heads, head_dim].  Requires LLX_F16, head_dim 64 or 128.
+ * ctx_len 0 gives zeros.  Uses a per-pool workspace that grows on demand (first call and
+ * growth synchronise the device); calls on one pool must be ordered on one stream. */
+llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* dev_q, void* dev_out,
+                                const int32_t* dev_block_tables, const int32_t* dev_ctx_lens, int B, int max_blocks,
+                                float scale, void* cuda_stream);
+
+/* ---- tuning, counters, errors ----------------------------------------------------------- */
+
+typedef enum {
+    LLX_OPT_COPY_KERNEL = 0,    /* 0 auto, 1 = 16-byte LDG/STG kernel, 2 = bulk-async (TMA) smem ring */
+    LLX_OPT_MAX_CTAS = 1,       /* cap on the copy grid (0 = auto: fill the GPU); the throttle of SURVEY NEXT-1 */
+    LLX_OPT_CHUNK_BYTES = 2,    /* bytes of one tile one CTA moves per step (multiple of 16; 0 = auto) */
+    LLX_OPT_RING_STAGES = 3,    /* smem stages per ring of the bulk-async kernel (0 = auto) */
+    LLX_OPT_IDS_BY_VALUE_MAX = 4, /* pairs up to which ids travel in the kernel parameters (<= 256) */
+    LLX_OPT_ATTN_SPLIT_TOKENS = 5 /* tokens per KV split of decode attention (multiple of 8; 0 = auto) */
+} llx_option;
+/* Process-wide; takes effect for later calls.  Returns LLX_ERR_INVALID_ARG for a bad value. */
+llx_status llx_set_option(llx_option opt, long long value);
+long long  llx_get_option(llx_option opt);
+
+typedef struct {
+    unsigned long long kernel_launches; /* kernels this library launched */
+    unsigned long long copy_launches;   /* of which gather/scatter copy kernels */
+    unsigned long long bytes_moved;     /* payload bytes those copies wrote */
+    unsigned long long id_uploads;      /* stages whose ids went through the pinned ring (not by value) */
+} llx_counters;
+void llx_get_counters(llx_counters* out);
+void llx_reset_counters(void);
+
+const char* llx_status_str(llx_status s);
+const char* llx_last_error(void); /* thread-local detail of this thread's last failed call */
+const char* llx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LLX_H_ */

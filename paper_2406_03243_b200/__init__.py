@@ -1,0 +1,15 @@
+"""paper_2406_03243_b200 — B200-native live migration of a paged KV cache (Llumnix §4.2/§5).
+
+Thin binding over the C-ABI library `libllx.so` (include/llx.h).  The functions here only
+marshal arguments; every step of the path runs in the library's CUDA kernels.  Importing this
+package needs the built library (`python -m paper_2406_03243_b200.build`); there is no CPU path.
+"""
+from .binding import (  # noqa: F401
+    LlxError, Pool, lib, load,
+    F16, BF16, U8,
+    OPT_COPY_KERNEL, OPT_MAX_CTAS, OPT_CHUNK_BYTES, OPT_RING_STAGES, OPT_IDS_BY_VALUE_MAX, OPT_ATTN_SPLIT_TOKENS,
+    pool_create, pool_wrap, pool_bytes_for,
+    plan_stage, migrate_stage, migrate_batch, staging_bytes, PinnedStaging, pack, unpack,
+    append_tokens, decode_attention,
+    set_option, get_option, options, counters, reset_counters, version, EXPORTS,
+)

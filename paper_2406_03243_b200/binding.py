@@ -1,0 +1,279 @@
+"""ctypes binding with the same names as include/llx.h.  Argument marshalling only.
+
+Block-id arguments are anything convertible to a contiguous int32 NumPy array (host memory, as the
+ABI requires); device buffers are passed as integer addresses (`tensor.data_ptr()`); streams as the
+integer `torch.cuda.Stream.cuda_stream` (0 / None = legacy default stream).
+"""
+from __future__ import annotations
+
+import contextlib
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libllx.so")
+
+F16, BF16, U8 = 0, 1, 2
+OPT_COPY_KERNEL, OPT_MAX_CTAS, OPT_CHUNK_BYTES, OPT_RING_STAGES, OPT_IDS_BY_VALUE_MAX, OPT_ATTN_SPLIT_TOKENS = range(6)
+
+_vp, _i, _sz, _i32p = C.c_void_p, C.c_int, C.c_size_t, C.POINTER(C.c_int32)
+
+
+class _Counters(C.Structure):
+    _fields_ = [("kernel_launches", C.c_ulonglong), ("copy_launches", C.c_ulonglong),
+                ("bytes_moved", C.c_ulonglong), ("id_uploads", C.c_ulonglong)]
+
+
+#: every symbol include/llx.h declares: name -> (restype, argtypes)
+EXPORTS = {
+    "llx_pool_create": (_i, [_i, _i, _i, _i, _i, _i, C.POINTER(_vp)]),
+    "llx_pool_wrap": (_i, [_vp, _sz, _i, _i, _i, _i, _i, _i, C.POINTER(_vp)]),
+    "llx_pool_destroy": (_i, [_vp]),
+    "llx_pool_data": (_vp, [_vp, _i, _i]),
+    "llx_pool_tile_bytes": (_sz, [_vp]),
+    "llx_pool_block_bytes": (_sz, [_vp]),
+    "llx_pool_bytes": (_sz, [_vp]),
+    "llx_pool_num_blocks": (_i, [_vp]),
+    "llx_pool_bytes_for": (_sz, [_i, _i, _i, _i, _i, _i]),
+    "llx_pool_upload": (_i, [_vp, _i, _i, _i, _i, _vp, _vp]),
+    "llx_pool_download": (_i, [_vp, _i, _i, _i, _i, _vp, _vp]),
+    "llx_pool_fill_u16": (_i, [_vp, C.c_uint16, _vp]),
+    "llx_plan_stage": (_i, [_i, _i, _i, _i, C.POINTER(_i), C.POINTER(_i)]),
+    "llx_migrate_stage": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp]),
+    "llx_migrate_batch": (_i, [_vp, _vp, _i32p, _i32p, _i32p, _i, _vp]),
+    "llx_staging_bytes": (_sz, [_vp, _i]),
+    "llx_staging_alloc_pinned": (_i, [_sz, C.POINTER(_vp), C.POINTER(_vp)]),
+    "llx_staging_free_pinned": (_i, [_vp]),
+    "llx_pack": (_i, [_vp, _i32p, _i, _vp, _sz, _vp]),
+    "llx_unpack": (_i, [_vp, _sz, _vp, _i32p, _i, _vp]),
+    "llx_append_tokens": (_i, [_vp, _i32p, _i, _i, _i, _vp, _vp]),
+    "llx_decode_attention": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _i, _i, C.c_float, _vp]),
+    "llx_set_option": (_i, [_i, C.c_longlong]),
+    "llx_get_option": (C.c_longlong, [_i]),
+    "llx_get_counters": (None, [C.POINTER(_Counters)]),
+    "llx_reset_counters": (None, []),
+    "llx_status_str": (C.c_char_p, [_i]),
+    "llx_last_error": (C.c_char_p, []),
+    "llx_version": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+class LlxError(RuntimeError):
+    def __init__(self, status: int, name: str, detail: str):
+        super().__init__(f"{name} ({status}): {detail}")
+        self.status, self.name, self.detail = status, name, detail
+
+
+def load():
+    """dlopen libllx.so and declare every prototype.  Fails loudly if the library is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2406_03243_b200.build` "
+                          "(the llx path has no CPU fallback)")
+    lib_ = C.CDLL(LIB_PATH)
+    for name, (res, args) in EXPORTS.items():
+        fn = getattr(lib_, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = lib_
+    return _lib
+
+
+def lib():
+    return load()
+
+
+def _check(rc: int):
+    if rc != 0:
+        l = load()
+        raise LlxError(rc, l.llx_status_str(rc).decode(), l.llx_last_error().decode())
+
+
+def _ids(x):
+    a = np.ascontiguousarray(np.asarray(x, dtype=np.int32).reshape(-1))
+    return a, a.ctypes.data_as(_i32p)
+
+
+def _stream(s) -> int:
+    if s is None:
+        return 0
+    return int(getattr(s, "cuda_stream", s))
+
+
+class Pool:
+    """Handle of one serving instance's KV pool (llx_pool*)."""
+
+    def __init__(self, handle: int, keepalive=None):
+        self._h = handle
+        self._keep = keepalive
+
+    @property
+    def handle(self) -> int:
+        if not self._h:
+            raise LlxError(-1, "LLX_ERR_INVALID_ARG", "pool already destroyed")
+        return self._h
+
+    tile_bytes = property(lambda self: load().llx_pool_tile_bytes(self.handle))
+    block_bytes = property(lambda self: load().llx_pool_block_bytes(self.handle))
+    nbytes = property(lambda self: load().llx_pool_bytes(self.handle))
+    num_blocks = property(lambda self: load().llx_pool_num_blocks(self.handle))
+
+    def data(self, layer: int, kv: int) -> int:
+        p = load().llx_pool_data(self.handle, layer, kv)
+        if not p:
+            raise LlxError(-1, "LLX_ERR_INVALID_ARG", f"bad (layer={layer}, kv={kv})")
+        return p
+
+    def upload(self, layer, kv, first_block, host: np.ndarray, stream=None):
+        host = np.ascontiguousarray(host)
+        nb, rem = divmod(host.nbytes, self.tile_bytes)
+        assert rem == 0, "host array must hold whole tiles"
+        _check(load().llx_pool_upload(self.handle, layer, kv, first_block, nb, host.ctypes.data, _stream(stream)))
+
+    def download(self, layer, kv, first_block, n_blocks, stream=None, dtype=np.uint16) -> np.ndarray:
+        out = np.empty((n_blocks, self.tile_bytes // np.dtype(dtype).itemsize), dtype=dtype)
+        _check(load().llx_pool_download(self.handle, layer, kv, first_block, n_blocks, out.ctypes.data, _stream(stream)))
+        return out
+
+    def fill_u16(self, pattern: int, stream=None):
+        _check(load().llx_pool_fill_u16(self.handle, pattern, _stream(stream)))
+
+    def destroy(self):
+        if self._h:
+            load().llx_pool_destroy(self._h)
+            self._h = 0
+            self._keep = None
+
+    def __del__(self):
+        with contextlib.suppress(Exception):
+            self.destroy()
+
+
+def pool_bytes_for(layers, kv_heads, head_dim, block_size, dtype, num_blocks) -> int:
+    return load().llx_pool_bytes_for(layers, kv_heads, head_dim, block_size, dtype, num_blocks)
+
+
+def pool_create(layers, kv_heads, head_dim, block_size, dtype, num_blocks) -> Pool:
+    h = _vp()
+    _check(load().llx_pool_create(layers, kv_heads, head_dim, block_size, dtype, num_blocks, C.byref(h)))
+    return Pool(h.value)
+
+
+def pool_wrap(dev_ptr: int, nbytes: int, layers, kv_heads, head_dim, block_size, dtype, num_blocks, keepalive=None) -> Pool:
+    h = _vp()
+    _check(load().llx_pool_wrap(dev_ptr, nbytes, layers, kv_heads, head_dim, block_size, dtype, num_blocks, C.byref(h)))
+    return Pool(h.value, keepalive)
+
+
+def plan_stage(num_tokens: int, blocks_migrated: int, block_size: int, last_stage_max_blocks: int):
+    """-> (n, is_final): the logical blocks [blocks_migrated, blocks_migrated+n) of the next stage."""
+    n, f = _i(), _i()
+    _check(load().llx_plan_stage(num_tokens, blocks_migrated, block_size, last_stage_max_blocks, C.byref(n), C.byref(f)))
+    return n.value, bool(f.value)
+
+
+def migrate_stage(src: Pool, src_block_ids, dst: Pool, dst_block_ids, stream=None):
+    s, sp = _ids(src_block_ids)
+    d, dp = _ids(dst_block_ids)
+    if s.size != d.size:
+        raise LlxError(-1, "LLX_ERR_INVALID_ARG", "src/dst id lists differ in length")
+    _check(load().llx_migrate_stage(src.handle, sp, dst.handle, dp, s.size, _stream(stream)))
+
+
+def migrate_batch(src: Pool, dst: Pool, req_offsets, src_block_ids, dst_block_ids, stream=None):
+    o, op = _ids(req_offsets)
+    s, sp = _ids(src_block_ids)
+    d, dp = _ids(dst_block_ids)
+    if o.size < 1 or s.size != d.size or int(o[-1]) != s.size:
+        raise LlxError(-1, "LLX_ERR_INVALID_ARG", "req_offsets[-1] must equal the number of id pairs")
+    _check(load().llx_migrate_batch(src.handle, dst.handle, op, sp, dp, o.size - 1, _stream(stream)))
+
+
+def staging_bytes(pool: Pool, n: int) -> int:
+    return load().llx_staging_bytes(pool.handle, n)
+
+
+class PinnedStaging:
+    """Pinned, mapped host staging buffer (llx_staging_alloc_pinned)."""
+
+    def __init__(self, nbytes: int):
+        h, d = _vp(), _vp()
+        _check(load().llx_staging_alloc_pinned(nbytes, C.byref(h), C.byref(d)))
+        self.host_ptr, self.dev_alias, self.nbytes = h.value, d.value, nbytes
+
+    def as_numpy(self, dtype=np.uint16) -> np.ndarray:
+        buf = (C.c_char * self.nbytes).from_address(self.host_ptr)
+        return np.frombuffer(buf, dtype=dtype)
+
+    def free(self):
+        if self.host_ptr:
+            load().llx_staging_free_pinned(self.host_ptr)
+            self.host_ptr = 0
+
+    def __del__(self):
+        with contextlib.suppress(Exception):
+            self.free()
+
+
+def pack(src: Pool, src_block_ids, staging_ptr: int, staging_nbytes: int, stream=None):
+    s, sp = _ids(src_block_ids)
+    _check(load().llx_pack(src.handle, sp, s.size, staging_ptr, staging_nbytes, _stream(stream)))
+
+
+def unpack(staging_ptr: int, staging_nbytes: int, dst: Pool, dst_block_ids, stream=None):
+    d, dp = _ids(dst_block_ids)
+    _check(load().llx_unpack(staging_ptr, staging_nbytes, dst.handle, dp, d.size, _stream(stream)))
+
+
+def append_tokens(pool: Pool, block_table, t0: int, t1: int, dev_values_ptr: int, stream=None):
+    t, tp = _ids(block_table)
+    _check(load().llx_append_tokens(pool.handle, tp, t.size, t0, t1, dev_values_ptr, _stream(stream)))
+
+
+def decode_attention(pool: Pool, layer: int, dev_q: int, dev_out: int, dev_block_tables: int, dev_ctx_lens: int,
+                     B: int, max_blocks: int, scale: float, stream=None):
+    _check(load().llx_decode_attention(pool.handle, layer, dev_q, dev_out, dev_block_tables, dev_ctx_lens,
+                                       B, max_blocks, scale, _stream(stream)))
+
+
+def set_option(opt: int, value: int):
+    _check(load().llx_set_option(opt, value))
+
+
+def get_option(opt: int) -> int:
+    return load().llx_get_option(opt)
+
+
+@contextlib.contextmanager
+def options(**kw):
+    """Temporarily set options by lower-case name, e.g. options(copy_kernel=1, max_ctas=16)."""
+    names = dict(copy_kernel=OPT_COPY_KERNEL, max_ctas=OPT_MAX_CTAS, chunk_bytes=OPT_CHUNK_BYTES,
+                 ring_stages=OPT_RING_STAGES, ids_by_value_max=OPT_IDS_BY_VALUE_MAX,
+                 attn_split_tokens=OPT_ATTN_SPLIT_TOKENS)
+    old = {k: get_option(names[k]) for k in kw}
+    try:
+        for k, v in kw.items():
+            set_option(names[k], v)
+        yield
+    finally:
+        for k, v in old.items():
+            set_option(names[k], v)
+
+
+def counters() -> dict:
+    c = _Counters()
+    load().llx_get_counters(C.byref(c))
+    return {f: int(getattr(c, f)) for f, _ in c._fields_}
+
+
+def reset_counters():
+    load().llx_reset_counters()
+
+
+def version() -> str:
+    return load().llx_version().decode()

@@ -1,0 +1,713 @@
+// C-ABI of the llx library (include/llx.h): pools, host-side validation, id hand-off and the
+// kernel launches.  Every data step runs in the kernels of llx_copy.cuh / llx_attention.cuh;
+// this file only checks arguments, stages the block ids and enqueues.  There is no CPU path.
+#include "../../include/llx.h"
+
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "llx_attention.cuh"
+#include "llx_copy.cuh"
+
+using namespace llx;
+
+struct llx_pool {
+    unsigned char* data = nullptr;
+    int layers = 0, kv_heads = 0, head_dim = 0, block_size = 0, num_blocks = 0;
+    llx_dtype dtype = LLX_F16;
+    int elem_bytes = 2;
+    long long tile_bytes = 0;
+    int device = 0;
+    bool owned = false;
+    // decode-attention workspace (grows on demand)
+    float* attn_ws = nullptr;
+    size_t attn_ws_bytes = 0;
+};
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+llx_status fail(llx_status s, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return s;
+}
+llx_status cuda_fail(cudaError_t e, const char* what) {
+    return fail(LLX_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+#define LLX_CUDA(call)                                   \
+    do {                                                 \
+        cudaError_t e_ = (call);                         \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+    } while (0)
+
+int elem_bytes_of(llx_dtype d) {
+    switch (d) {
+        case LLX_F16:
+        case LLX_BF16: return 2;
+        case LLX_U8: return 1;
+    }
+    return 0;
+}
+
+// ---- options / counters -------------------------------------------------------------------
+std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
+    g_opt_attn_split{0};
+std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
+
+// ---- device properties (cached per device) ------------------------------------------------
+struct DevInfo {
+    int sm_count = 0;
+    int max_smem_optin = 0;
+    bool ready = false;
+};
+std::mutex g_dev_mu;
+DevInfo g_dev[64];
+
+llx_status dev_info(int dev, DevInfo** out) {
+    if (dev < 0 || dev >= 64) return fail(LLX_ERR_INVALID_ARG, "device %d unsupported", dev);
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    DevInfo& d = g_dev[dev];
+    if (!d.ready) {
+        LLX_CUDA(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
+        LLX_CUDA(cudaDeviceGetAttribute(&d.max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        LLX_CUDA(cudaFuncSetAttribute(llx_copy_bulk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
+        LLX_CUDA(cudaFuncSetAttribute(llx_copy_bulk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
+        d.ready = true;
+    }
+    *out = &d;
+    return LLX_OK;
+}
+
+// ---- id ring: pinned host slots + device slots, reused in order, guarded by events ---------
+struct IdSlot {
+    int32_t* host = nullptr;
+    int32_t* dev = nullptr;
+    size_t cap = 0;  // int32 entries
+    cudaEvent_t ev = nullptr;
+    bool used = false;
+};
+constexpr int kIdSlots = 8;
+std::mutex g_ring_mu;
+IdSlot g_ring[kIdSlots];
+int g_ring_next = 0;
+
+// Copies `count` ids made of up to two host arrays (a then b) into a slot and enqueues the H2D
+// copy; returns the device address.  The caller records the slot's event after its launch.
+llx_status ring_stage(const int32_t* a, size_t na, const int32_t* b, size_t nb, cudaStream_t st, int32_t** dev_out,
+                      IdSlot** slot_out) {
+    std::lock_guard<std::mutex> lk(g_ring_mu);
+    IdSlot& s = g_ring[g_ring_next];
+    g_ring_next = (g_ring_next + 1) % kIdSlots;
+    if (s.used) LLX_CUDA(cudaEventSynchronize(s.ev));
+    const size_t need = na + nb;
+    if (need > s.cap) {
+        size_t cap = 1024;
+        while (cap < need) cap *= 2;
+        if (s.host) cudaFreeHost(s.host);
+        if (s.dev) cudaFree(s.dev);
+        s.host = nullptr;
+        s.dev = nullptr;
+        s.cap = 0;
+        if (cudaMallocHost(&s.host, cap * sizeof(int32_t)) != cudaSuccess ||
+            cudaMalloc(&s.dev, cap * sizeof(int32_t)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(LLX_ERR_OOM, "id ring: cannot allocate %zu ids", cap);
+        }
+        s.cap = cap;
+    }
+    if (!s.ev) LLX_CUDA(cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming));
+    if (na) memcpy(s.host, a, na * sizeof(int32_t));
+    if (nb) memcpy(s.host + na, b, nb * sizeof(int32_t));
+    LLX_CUDA(cudaMemcpyAsync(s.dev, s.host, need * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    s.used = true;
+    *dev_out = s.dev;
+    *slot_out = &s;
+    return LLX_OK;
+}
+
+// ---- validation ------------------------------------------------------------------------------
+llx_status check_pool(const llx_pool* p, const char* name) {
+    if (!p || !p->data) return fail(LLX_ERR_INVALID_ARG, "%s pool is NULL", name);
+    int dev = -1;
+    LLX_CUDA(cudaGetDevice(&dev));
+    if (dev != p->device) return fail(LLX_ERR_INVALID_ARG, "%s pool lives on device %d, current device is %d", name, p->device, dev);
+    return LLX_OK;
+}
+llx_status check_range(const int32_t* ids, long long n, int num_blocks, const char* name) {
+    for (long long i = 0; i < n; ++i)
+        if (ids[i] < 0 || ids[i] >= num_blocks)
+            return fail(LLX_ERR_BLOCK_OUT_OF_RANGE, "%s_block_ids[%lld] = %d not in [0,%d)", name, i, ids[i], num_blocks);
+    return LLX_OK;
+}
+llx_status check_unique(const int32_t* ids, long long n, int num_blocks) {
+    thread_local std::vector<unsigned char> seen;
+    seen.assign((size_t)num_blocks, 0);
+    for (long long i = 0; i < n; ++i) {
+        if (seen[ids[i]]) return fail(LLX_ERR_DUPLICATE_DST, "destination block id %d appears twice (second at %lld)", ids[i], i);
+        seen[ids[i]] = 1;
+    }
+    return LLX_OK;
+}
+size_t pool_bytes(const llx_pool* p) { return (size_t)p->num_blocks * 2 * p->layers * (size_t)p->tile_bytes; }
+
+// ---- copy launch -----------------------------------------------------------------------------
+struct Side {
+    const unsigned char* base;
+    const int32_t* ids;  // host ids or nullptr (contiguous side)
+    long long slice_stride, item_stride;
+    bool host_memory;  // staging in mapped host memory
+};
+
+llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers, long long tile_bytes, int device,
+                       cudaStream_t st) {
+    DevInfo* di = nullptr;
+    llx_status rc = dev_info(device, &di);
+    if (rc != LLX_OK) return rc;
+
+    // kernel choice: the bulk-async ring for device<->device, the LDG/STG kernel when a side is host memory
+    long long kern = g_opt_kernel.load();
+    if (kern == 0) kern = (src.host_memory || dst.host_memory) ? 1 : 2;
+
+    const long long total_bytes = n * 2 * layers * tile_bytes;
+    long long chunk = g_opt_chunk.load();
+    int nstages = (int)g_opt_stages.load();
+    int threads = 256, grid = 0;
+    size_t smem = 0;
+    const int slices = 2 * layers;
+
+    if (kern == 2) {
+        if (nstages <= 0) nstages = 4;
+        if (chunk <= 0) {
+            chunk = 16384;
+            // short stages (the final one): smaller chunks so that every SM gets several units
+            while (chunk > 4096 && total_bytes / chunk < (long long)di->sm_count * 8) chunk /= 2;
+        }
+        if (chunk > tile_bytes) chunk = tile_bytes;
+        chunk &= ~15ll;
+        threads = 32;
+        smem = 128 + (size_t)nstages * chunk;
+        if ((long long)smem > di->max_smem_optin) return fail(LLX_ERR_INVALID_ARG, "ring of %d x %lld bytes exceeds shared memory", nstages, chunk);
+    } else {
+        if (chunk <= 0) chunk = 256 * 16 * 4;
+        if (chunk > tile_bytes) chunk = tile_bytes;
+        chunk &= ~15ll;
+    }
+    const long long cpt = (tile_bytes + chunk - 1) / chunk;
+    const long long units = n * slices * cpt;
+    if (units >= (1ll << 31)) return fail(LLX_ERR_INVALID_ARG, "stage too large: %lld units", units);
+
+    if (kern == 2) {
+        int per_sm = (int)((size_t)di->max_smem_optin / (smem + 1024));  // 1 KiB per-CTA reservation
+        if (per_sm < 1) per_sm = 1;
+        if (per_sm > 16) per_sm = 16;
+        grid = di->sm_count * per_sm;
+    } else {
+        grid = di->sm_count * 8;
+    }
+    const long long cap = g_opt_max_ctas.load();
+    if (cap > 0 && grid > cap) grid = (int)cap;
+    if (grid > units) grid = (int)units;
+
+    CopyArgs a;
+    a.src_base = src.base;
+    a.dst_base = const_cast<unsigned char*>(dst.base);
+    a.src_slice_stride = src.slice_stride;
+    a.src_item_stride = src.item_stride;
+    a.dst_slice_stride = dst.slice_stride;
+    a.dst_item_stride = dst.item_stride;
+    a.src_indexed = src.ids != nullptr;
+    a.dst_indexed = dst.ids != nullptr;
+    a.src_ids = a.dst_ids = nullptr;
+    a.tile_bytes = (int)tile_bytes;
+    a.chunk_bytes = (int)chunk;
+    a.chunks_per_tile = (int)cpt;
+    a.slices = slices;
+    a.total_units = (int)units;
+
+    static thread_local IdPack pack;  // 2 KiB; only the first n entries are meaningful
+    const bool byval = n <= g_opt_byval.load();
+    IdSlot* slot = nullptr;
+    if (byval) {
+        if (src.ids) memcpy(pack.src, src.ids, n * sizeof(int32_t));
+        if (dst.ids) memcpy(pack.dst, dst.ids, n * sizeof(int32_t));
+    } else {
+        int32_t* dev_ids = nullptr;
+        rc = ring_stage(src.ids, src.ids ? n : 0, dst.ids, dst.ids ? n : 0, st, &dev_ids, &slot);
+        if (rc != LLX_OK) return rc;
+        if (src.ids) a.src_ids = dev_ids;
+        if (dst.ids) a.dst_ids = dev_ids + (src.ids ? n : 0);
+        g_id_uploads++;
+    }
+
+    if (kern == 2) {
+        if (byval)
+            llx_copy_bulk<true><<<grid, threads, smem, st>>>(a, pack, nstages);
+        else
+            llx_copy_bulk<false><<<grid, threads, smem, st>>>(a, pack, nstages);
+    } else {
+        if (byval)
+            llx_copy_vec16<true, 4><<<grid, 256, 0, st>>>(a, pack);
+        else
+            llx_copy_vec16<false, 4><<<grid, 256, 0, st>>>(a, pack);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (slot) cudaEventRecord(slot->ev, st);
+    if (e != cudaSuccess) return cuda_fail(e, "copy kernel launch");
+    g_launches++;
+    g_copy_launches++;
+    g_bytes += (unsigned long long)total_bytes;
+    return LLX_OK;
+}
+
+Side pool_side(const llx_pool* p, const int32_t* ids) {
+    return Side{p->data, ids, (long long)p->num_blocks * p->tile_bytes, p->tile_bytes, false};
+}
+llx_status staging_side(const void* staging, int layers, long long tile_bytes, Side* out) {
+    cudaPointerAttributes at;
+    LLX_CUDA(cudaPointerGetAttributes(&at, staging));
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged)
+        return fail(LLX_ERR_INVALID_ARG, "staging buffer is neither device nor pinned host memory");
+    const void* p = staging;
+    if (at.type == cudaMemoryTypeHost) p = at.devicePointer ? at.devicePointer : staging;
+    if (((uintptr_t)p & 15) != 0) return fail(LLX_ERR_INVALID_ARG, "staging buffer must be 16-byte aligned");
+    *out = Side{(const unsigned char*)p, nullptr, tile_bytes, 2ll * layers * tile_bytes, at.type == cudaMemoryTypeHost};
+    return LLX_OK;
+}
+
+llx_status check_pair(const llx_pool* src, const llx_pool* dst) {
+    llx_status rc = check_pool(src, "src");
+    if (rc != LLX_OK) return rc;
+    rc = check_pool(dst, "dst");
+    if (rc != LLX_OK) return rc;
+    if (src == dst) return fail(LLX_ERR_ALIAS, "src and dst are the same pool");
+    const unsigned char *a0 = src->data, *a1 = a0 + pool_bytes(src), *b0 = dst->data, *b1 = b0 + pool_bytes(dst);
+    if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "src and dst pools overlap in memory");
+    if (src->layers != dst->layers || src->tile_bytes != dst->tile_bytes || src->kv_heads != dst->kv_heads ||
+        src->head_dim != dst->head_dim || src->block_size != dst->block_size || src->elem_bytes != dst->elem_bytes)
+        return fail(LLX_ERR_GEOMETRY_MISMATCH, "src (L=%d,H=%d,D=%d,S=%d,e=%d) vs dst (L=%d,H=%d,D=%d,S=%d,e=%d)", src->layers,
+                    src->kv_heads, src->head_dim, src->block_size, src->elem_bytes, dst->layers, dst->kv_heads,
+                    dst->head_dim, dst->block_size, dst->elem_bytes);
+    return LLX_OK;
+}
+
+llx_status make_pool(void* ptr, size_t bytes, bool owned, int layers, int kv_heads, int head_dim, int block_size,
+                     llx_dtype dtype, int num_blocks, llx_pool** out) {
+    if (!out) return fail(LLX_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    const size_t need = llx_pool_bytes_for(layers, kv_heads, head_dim, block_size, dtype, num_blocks);
+    if (need == 0) return fail(LLX_ERR_INVALID_ARG, "bad geometry L=%d H=%d D=%d S=%d dtype=%d blocks=%d (tile must be a positive multiple of 16 bytes)",
+                               layers, kv_heads, head_dim, block_size, (int)dtype, num_blocks);
+    int dev = 0;
+    LLX_CUDA(cudaGetDevice(&dev));
+    if (owned) {
+        cudaError_t e = cudaMalloc(&ptr, need);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return e == cudaErrorMemoryAllocation ? fail(LLX_ERR_OOM, "cudaMalloc of %zu bytes failed", need)
+                                                  : cuda_fail(e, "cudaMalloc");
+        }
+    } else {
+        if (!ptr) return fail(LLX_ERR_INVALID_ARG, "dev_ptr is NULL");
+        if (((uintptr_t)ptr & 15) != 0) return fail(LLX_ERR_INVALID_ARG, "dev_ptr must be 16-byte aligned");
+        if (bytes < need) return fail(LLX_ERR_INVALID_ARG, "wrapped memory has %zu bytes, pool needs %zu", bytes, need);
+        cudaPointerAttributes at;
+        LLX_CUDA(cudaPointerGetAttributes(&at, ptr));
+        if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+            return fail(LLX_ERR_INVALID_ARG, "dev_ptr is not device memory");
+        dev = at.device;
+    }
+    llx_pool* p = new (std::nothrow) llx_pool();
+    if (!p) {
+        if (owned) cudaFree(ptr);
+        return fail(LLX_ERR_OOM, "host allocation failed");
+    }
+    p->data = (unsigned char*)ptr;
+    p->layers = layers;
+    p->kv_heads = kv_heads;
+    p->head_dim = head_dim;
+    p->block_size = block_size;
+    p->num_blocks = num_blocks;
+    p->dtype = dtype;
+    p->elem_bytes = elem_bytes_of(dtype);
+    p->tile_bytes = (long long)block_size * kv_heads * head_dim * p->elem_bytes;
+    p->device = dev;
+    p->owned = owned;
+    *out = p;
+    return LLX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t llx_pool_bytes_for(int layers, int kv_heads, int head_dim, int block_size, llx_dtype dtype, int num_blocks) {
+    const int e = elem_bytes_of(dtype);
+    if (layers <= 0 || kv_heads <= 0 || head_dim <= 0 || block_size <= 0 || num_blocks <= 0 || e == 0) return 0;
+    const unsigned long long tile = (unsigned long long)block_size * kv_heads * head_dim * e;
+    if (tile % 16 != 0 || tile > (1ull << 30)) return 0;
+    return (size_t)(tile * 2ull * layers * num_blocks);
+}
+
+llx_status llx_pool_create(int layers, int kv_heads, int head_dim, int block_size, llx_dtype dtype, int num_blocks,
+                           llx_pool** out) {
+    return make_pool(nullptr, 0, true, layers, kv_heads, head_dim, block_size, dtype, num_blocks, out);
+}
+llx_status llx_pool_wrap(void* dev_ptr, size_t bytes, int layers, int kv_heads, int head_dim, int block_size,
+                         llx_dtype dtype, int num_blocks, llx_pool** out) {
+    return make_pool(dev_ptr, bytes, false, layers, kv_heads, head_dim, block_size, dtype, num_blocks, out);
+}
+llx_status llx_pool_destroy(llx_pool* p) {
+    if (!p) return LLX_OK;
+    if (p->attn_ws) cudaFree(p->attn_ws);
+    if (p->owned && p->data) cudaFree(p->data);
+    delete p;
+    return LLX_OK;
+}
+void* llx_pool_data(const llx_pool* p, int layer, int kv) {
+    if (!p || layer < 0 || layer >= p->layers || kv < 0 || kv > 1) return nullptr;
+    return p->data + ((long long)layer * 2 + kv) * p->num_blocks * p->tile_bytes;
+}
+size_t llx_pool_tile_bytes(const llx_pool* p) { return p ? (size_t)p->tile_bytes : 0; }
+size_t llx_pool_block_bytes(const llx_pool* p) { return p ? (size_t)p->tile_bytes * 2 * p->layers : 0; }
+size_t llx_pool_bytes(const llx_pool* p) { return p ? pool_bytes(p) : 0; }
+int llx_pool_num_blocks(const llx_pool* p) { return p ? p->num_blocks : 0; }
+
+static llx_status pool_xfer(const llx_pool* p, int layer, int kv, int first, int nb, void* host, bool up, void* stream) {
+    llx_status rc = check_pool(p, "pool");
+    if (rc != LLX_OK) return rc;
+    if (layer < 0 || layer >= p->layers || kv < 0 || kv > 1) return fail(LLX_ERR_INVALID_ARG, "bad (layer=%d, kv=%d)", layer, kv);
+    if (nb < 0 || first < 0 || (long long)first + nb > p->num_blocks)
+        return fail(LLX_ERR_BLOCK_OUT_OF_RANGE, "blocks [%d,%d) not in [0,%d)", first, first + nb, p->num_blocks);
+    if (nb == 0) return LLX_OK;
+    if (!host) return fail(LLX_ERR_INVALID_ARG, "host pointer is NULL");
+    unsigned char* d = (unsigned char*)llx_pool_data(p, layer, kv) + (long long)first * p->tile_bytes;
+    const size_t bytes = (size_t)nb * p->tile_bytes;
+    if (up)
+        LLX_CUDA(cudaMemcpyAsync(d, host, bytes, cudaMemcpyHostToDevice, (cudaStream_t)stream));
+    else
+        LLX_CUDA(cudaMemcpyAsync(host, d, bytes, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    return LLX_OK;
+}
+llx_status llx_pool_upload(llx_pool* p, int layer, int kv, int first, int nb, const void* host, void* stream) {
+    return pool_xfer(p, layer, kv, first, nb, const_cast<void*>(host), true, stream);
+}
+llx_status llx_pool_download(const llx_pool* p, int layer, int kv, int first, int nb, void* host, void* stream) {
+    return pool_xfer(p, layer, kv, first, nb, host, false, stream);
+}
+llx_status llx_pool_fill_u16(llx_pool* p, uint16_t pattern, void* stream) {
+    llx_status rc = check_pool(p, "pool");
+    if (rc != LLX_OK) return rc;
+    const long long nvec = (long long)(pool_bytes(p) / 16);
+    const uint32_t w = (uint32_t)pattern | ((uint32_t)pattern << 16);
+    llx_fill_u16_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((uint4*)p->data, nvec, w);
+    LLX_CUDA(cudaGetLastError());
+    g_launches++;
+    return LLX_OK;
+}
+
+llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, int last_stage_max_blocks, int* n,
+                          int* is_final) {
+    if (!n || !is_final) return fail(LLX_ERR_INVALID_ARG, "NULL output");
+    if (num_tokens < 0 || blocks_migrated < 0 || block_size <= 0 || last_stage_max_blocks < 1)
+        return fail(LLX_ERR_INVALID_ARG, "bad arguments (tokens=%d, migrated=%d, S=%d, last=%d)", num_tokens, blocks_migrated, block_size, last_stage_max_blocks);
+    const int total = (int)(((long long)num_tokens + block_size - 1) / block_size);
+    const int full = num_tokens / block_size;
+    if (blocks_migrated > total) return fail(LLX_ERR_INVALID_ARG, "%d blocks migrated, request has %d", blocks_migrated, total);
+    const int remaining = total - blocks_migrated;
+    if (remaining <= last_stage_max_blocks) {
+        *n = remaining;
+        *is_final = 1;
+    } else {
+        *n = full - blocks_migrated;
+        *is_final = 0;
+    }
+    return LLX_OK;
+}
+
+llx_status llx_migrate_stage(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
+                             void* stream) {
+    llx_status rc = check_pair(src, dst);
+    if (rc != LLX_OK) return rc;
+    if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
+    if (n == 0) return LLX_OK;
+    if (!src_ids || !dst_ids) return fail(LLX_ERR_INVALID_ARG, "block id array is NULL");
+    if ((rc = check_range(src_ids, n, src->num_blocks, "src")) != LLX_OK) return rc;
+    if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
+    if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
+    return launch_copy(pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
+                       (cudaStream_t)stream);
+}
+
+llx_status llx_migrate_batch(const llx_pool* src, llx_pool* dst, const int32_t* off, const int32_t* src_ids,
+                             const int32_t* dst_ids, int R, void* stream) {
+    llx_status rc = check_pair(src, dst);
+    if (rc != LLX_OK) return rc;
+    if (R < 0) return fail(LLX_ERR_INVALID_ARG, "R = %d", R);
+    if (R == 0) return LLX_OK;
+    if (!off) return fail(LLX_ERR_INVALID_ARG, "req_offsets is NULL");
+    if (off[0] != 0) return fail(LLX_ERR_INVALID_ARG, "req_offsets[0] = %d, must be 0", off[0]);
+    for (int r = 0; r < R; ++r)
+        if (off[r + 1] < off[r]) return fail(LLX_ERR_INVALID_ARG, "req_offsets decreases at request %d", r);
+    const long long n = off[R];
+    if (n == 0) return LLX_OK;
+    if (!src_ids || !dst_ids) return fail(LLX_ERR_INVALID_ARG, "block id array is NULL");
+    if ((rc = check_range(src_ids, n, src->num_blocks, "src")) != LLX_OK) return rc;
+    if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
+    if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
+    // every (block, layer, K|V) tile is independent, so the requests are flattened into one grid
+    return launch_copy(pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
+                       (cudaStream_t)stream);
+}
+
+size_t llx_staging_bytes(const llx_pool* p, int n) { return (p && n > 0) ? (size_t)n * llx_pool_block_bytes(p) : 0; }
+
+llx_status llx_staging_alloc_pinned(size_t bytes, void** host_ptr, void** dev_alias) {
+    if (!host_ptr || !dev_alias || bytes == 0) return fail(LLX_ERR_INVALID_ARG, "bad arguments");
+    void* h = nullptr;
+    cudaError_t e = cudaHostAlloc(&h, bytes, cudaHostAllocMapped | cudaHostAllocPortable);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? fail(LLX_ERR_OOM, "cudaHostAlloc of %zu bytes failed", bytes)
+                                              : cuda_fail(e, "cudaHostAlloc");
+    }
+    void* d = nullptr;
+    e = cudaHostGetDevicePointer(&d, h, 0);
+    if (e != cudaSuccess) {
+        cudaFreeHost(h);
+        return cuda_fail(e, "cudaHostGetDevicePointer");
+    }
+    *host_ptr = h;
+    *dev_alias = d;
+    return LLX_OK;
+}
+llx_status llx_staging_free_pinned(void* host_ptr) {
+    if (!host_ptr) return LLX_OK;
+    LLX_CUDA(cudaFreeHost(host_ptr));
+    return LLX_OK;
+}
+
+llx_status llx_pack(const llx_pool* src, const int32_t* src_ids, int n, void* staging, size_t staging_bytes, void* stream) {
+    llx_status rc = check_pool(src, "src");
+    if (rc != LLX_OK) return rc;
+    if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
+    if (n == 0) return LLX_OK;
+    if (!src_ids || !staging) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
+    if (staging_bytes < llx_staging_bytes(src, n))
+        return fail(LLX_ERR_STAGING_TOO_SMALL, "staging has %zu bytes, %d blocks need %zu", staging_bytes, n, llx_staging_bytes(src, n));
+    if ((rc = check_range(src_ids, n, src->num_blocks, "src")) != LLX_OK) return rc;
+    Side stg;
+    if ((rc = staging_side(staging, src->layers, src->tile_bytes, &stg)) != LLX_OK) return rc;
+    const unsigned char *a0 = src->data, *a1 = a0 + pool_bytes(src), *b0 = stg.base, *b1 = b0 + llx_staging_bytes(src, n);
+    if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "staging buffer overlaps the pool");
+    return launch_copy(pool_side(src, src_ids), stg, n, src->layers, src->tile_bytes, src->device, (cudaStream_t)stream);
+}
+
+llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, const int32_t* dst_ids, int n, void* stream) {
+    llx_status rc = check_pool(dst, "dst");
+    if (rc != LLX_OK) return rc;
+    if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
+    if (n == 0) return LLX_OK;
+    if (!dst_ids || !staging) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
+    if (staging_bytes < llx_staging_bytes(dst, n))
+        return fail(LLX_ERR_STAGING_TOO_SMALL, "staging has %zu bytes, %d blocks need %zu", staging_bytes, n, llx_staging_bytes(dst, n));
+    if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
+    if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
+    Side stg;
+    if ((rc = staging_side(staging, dst->layers, dst->tile_bytes, &stg)) != LLX_OK) return rc;
+    const unsigned char *a0 = dst->data, *a1 = a0 + pool_bytes(dst), *b0 = stg.base, *b1 = b0 + llx_staging_bytes(dst, n);
+    if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "staging buffer overlaps the pool");
+    return launch_copy(stg, pool_side(dst, dst_ids), n, dst->layers, dst->tile_bytes, dst->device, (cudaStream_t)stream);
+}
+
+llx_status llx_append_tokens(llx_pool* p, const int32_t* table, int table_len, int t0, int t1, const void* dev_values,
+                             void* stream) {
+    llx_status rc = check_pool(p, "pool");
+    if (rc != LLX_OK) return rc;
+    if (t0 < 0 || t1 < t0) return fail(LLX_ERR_INVALID_ARG, "bad token range [%d,%d)", t0, t1);
+    if (t1 == t0) return LLX_OK;
+    if (!table || !dev_values) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
+    if ((t1 - 1) / p->block_size >= table_len) return fail(LLX_ERR_INVALID_ARG, "block table of %d entries too short for token %d", table_len, t1 - 1);
+    const int token_bytes = p->kv_heads * p->head_dim * p->elem_bytes;
+    if (token_bytes % 16 != 0 || ((uintptr_t)dev_values & 15) != 0) return fail(LLX_ERR_INVALID_ARG, "token vector must be a multiple of 16 bytes and 16-byte aligned");
+    const int ntok = t1 - t0;
+    std::vector<int32_t> tb((size_t)ntok);
+    for (int k = 0; k < ntok; ++k) tb[k] = table[(t0 + k) / p->block_size];
+    if ((rc = check_range(tb.data(), ntok, p->num_blocks, "table")) != LLX_OK) return rc;
+    AppendArgs a;
+    a.pool_base = p->data;
+    a.values = (const unsigned char*)dev_values;
+    a.tok_block = nullptr;
+    a.slice_stride = (long long)p->num_blocks * p->tile_bytes;
+    a.tile_bytes = (int)p->tile_bytes;
+    a.token_bytes = token_bytes;
+    a.block_size = p->block_size;
+    a.slices = 2 * p->layers;
+    a.t0 = t0;
+    a.ntok = ntok;
+    static thread_local IdPack pack;
+    cudaStream_t st = (cudaStream_t)stream;
+    IdSlot* slot = nullptr;
+    const int grid = ntok * a.slices;
+    if (ntok <= kIdsByValueCap) {
+        memcpy(pack.src, tb.data(), ntok * sizeof(int32_t));
+        llx_append_kernel<true><<<grid, 128, 0, st>>>(a, pack);
+    } else {
+        int32_t* dev_ids = nullptr;
+        if ((rc = ring_stage(tb.data(), ntok, nullptr, 0, st, &dev_ids, &slot)) != LLX_OK) return rc;
+        a.tok_block = dev_ids;
+        llx_append_kernel<false><<<grid, 128, 0, st>>>(a, pack);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (slot) cudaEventRecord(slot->ev, st);
+    if (e != cudaSuccess) return cuda_fail(e, "append kernel launch");
+    g_launches++;
+    return LLX_OK;
+}
+
+llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* q, void* out, const int32_t* block_tables,
+                                const int32_t* ctx_lens, int B, int max_blocks, float scale, void* stream) {
+    llx_status rc = check_pool(pool, "pool");
+    if (rc != LLX_OK) return rc;
+    if (pool->dtype != LLX_F16) return fail(LLX_ERR_INVALID_ARG, "decode attention needs an fp16 pool");
+    if (pool->head_dim != 64 && pool->head_dim != 128) return fail(LLX_ERR_INVALID_ARG, "head_dim %d unsupported (64 or 128)", pool->head_dim);
+    if (layer < 0 || layer >= pool->layers) return fail(LLX_ERR_INVALID_ARG, "layer %d not in [0,%d)", layer, pool->layers);
+    if (B < 0 || max_blocks < 0) return fail(LLX_ERR_INVALID_ARG, "B = %d, max_blocks = %d", B, max_blocks);
+    if (B == 0) return LLX_OK;
+    if (!q || !out || !block_tables || !ctx_lens) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
+    if ((((uintptr_t)q | (uintptr_t)out) & 15) != 0) return fail(LLX_ERR_INVALID_ARG, "q and out must be 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    llx_pool* p = const_cast<llx_pool*>(pool);
+
+    int split = (int)g_opt_attn_split.load();
+    if (split <= 0) split = 256;
+    const int D = pool->head_dim, H = pool->kv_heads;
+    const long long max_tokens = (long long)max_blocks * pool->block_size;
+    int max_splits = (int)((max_tokens + split - 1) / split);
+    if (max_splits < 1) max_splits = 1;
+    if (max_splits > 65535 || B > 65535) return fail(LLX_ERR_INVALID_ARG, "grid too large");
+    const size_t need = (size_t)B * H * max_splits * (D + 4) * sizeof(float);
+    if (need > p->attn_ws_bytes) {
+        if (p->attn_ws) {
+            LLX_CUDA(cudaDeviceSynchronize());
+            cudaFree(p->attn_ws);
+            p->attn_ws = nullptr;
+            p->attn_ws_bytes = 0;
+        }
+        cudaError_t e = cudaMalloc(&p->attn_ws, need);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return fail(LLX_ERR_OOM, "attention workspace of %zu bytes", need);
+        }
+        p->attn_ws_bytes = need;
+    }
+    AttnArgs a;
+    a.k_base = (const unsigned char*)llx_pool_data(pool, layer, 0);
+    a.v_base = (const unsigned char*)llx_pool_data(pool, layer, 1);
+    a.q = (const __half*)q;
+    a.out = (__half*)out;
+    a.block_tables = block_tables;
+    a.ctx_lens = ctx_lens;
+    a.part = p->attn_ws;
+    a.tile_bytes = pool->tile_bytes;
+    a.H = H;
+    a.S = pool->block_size;
+    a.max_blocks = max_blocks;
+    a.max_splits = max_splits;
+    a.split_tokens = split;
+    a.scale_log2 = scale * 1.4426950408889634f;
+    const int hpw = 32 / (D / 8);
+    const int head_groups = (H + kAttnWarps * hpw - 1) / (kAttnWarps * hpw);
+    dim3 grid1(max_splits, head_groups, B), grid2(H, B);
+    if (D == 128) {
+        llx_attn_partial<128><<<grid1, kAttnWarps * 32, 0, st>>>(a);
+        llx_attn_merge<128><<<grid2, 128, 0, st>>>(a);
+    } else {
+        llx_attn_partial<64><<<grid1, kAttnWarps * 32, 0, st>>>(a);
+        llx_attn_merge<64><<<grid2, 64, 0, st>>>(a);
+    }
+    LLX_CUDA(cudaGetLastError());
+    g_launches += 2;
+    return LLX_OK;
+}
+
+llx_status llx_set_option(llx_option opt, long long v) {
+    switch (opt) {
+        case LLX_OPT_COPY_KERNEL:
+            if (v < 0 || v > 2) break;
+            g_opt_kernel = v;
+            return LLX_OK;
+        case LLX_OPT_MAX_CTAS:
+            if (v < 0) break;
+            g_opt_max_ctas = v;
+            return LLX_OK;
+        case LLX_OPT_CHUNK_BYTES:
+            if (v < 0 || (v % 16) != 0 || v > (200 << 10)) break;
+            g_opt_chunk = v;
+            return LLX_OK;
+        case LLX_OPT_RING_STAGES:
+            if (v < 0 || v == 1 || v > 14) break;
+            g_opt_stages = v;
+            return LLX_OK;
+        case LLX_OPT_IDS_BY_VALUE_MAX:
+            if (v < 0 || v > kIdsByValueCap) break;
+            g_opt_byval = v;
+            return LLX_OK;
+        case LLX_OPT_ATTN_SPLIT_TOKENS:
+            if (v < 0 || (v % 8) != 0) break;
+            g_opt_attn_split = v;
+            return LLX_OK;
+    }
+    return fail(LLX_ERR_INVALID_ARG, "option %d: bad value %lld", (int)opt, v);
+}
+long long llx_get_option(llx_option opt) {
+    switch (opt) {
+        case LLX_OPT_COPY_KERNEL: return g_opt_kernel;
+        case LLX_OPT_MAX_CTAS: return g_opt_max_ctas;
+        case LLX_OPT_CHUNK_BYTES: return g_opt_chunk;
+        case LLX_OPT_RING_STAGES: return g_opt_stages;
+        case LLX_OPT_IDS_BY_VALUE_MAX: return g_opt_byval;
+        case LLX_OPT_ATTN_SPLIT_TOKENS: return g_opt_attn_split;
+    }
+    return -1;
+}
+
+void llx_get_counters(llx_counters* out) {
+    if (!out) return;
+    out->kernel_launches = g_launches;
+    out->copy_launches = g_copy_launches;
+    out->bytes_moved = g_bytes;
+    out->id_uploads = g_id_uploads;
+}
+void llx_reset_counters(void) {
+    g_launches = 0;
+    g_copy_launches = 0;
+    g_bytes = 0;
+    g_id_uploads = 0;
+}
+
+const char* llx_status_str(llx_status s) {
+    switch (s) {
+        case LLX_OK: return "LLX_OK";
+        case LLX_ERR_INVALID_ARG: return "LLX_ERR_INVALID_ARG";
+        case LLX_ERR_GEOMETRY_MISMATCH: return "LLX_ERR_GEOMETRY_MISMATCH";
+        case LLX_ERR_BLOCK_OUT_OF_RANGE: return "LLX_ERR_BLOCK_OUT_OF_RANGE";
+        case LLX_ERR_DUPLICATE_DST: return "LLX_ERR_DUPLICATE_DST";
+        case LLX_ERR_ALIAS: return "LLX_ERR_ALIAS";
+        case LLX_ERR_STAGING_TOO_SMALL: return "LLX_ERR_STAGING_TOO_SMALL";
+        case LLX_ERR_OOM: return "LLX_ERR_OOM";
+        case LLX_ERR_CUDA: return "LLX_ERR_CUDA";
+    }
+    return "LLX_ERR_UNKNOWN";
+}
+const char* llx_last_error(void) { return g_err; }
+const char* llx_version(void) { return "llx 0.1 (sm_100a)"; }
+
+}  // extern "C"

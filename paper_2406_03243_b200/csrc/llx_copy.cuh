@@ -1,0 +1,258 @@
+// Gather/scatter copy kernels for sm_100a: the data path of one migration stage
+// (§4.2; block = K or V of block_size tokens of one layer, §5).
+//
+// One work UNIT = one chunk (<= chunk_bytes) of one tile (block i, layer l, K|V).  Both sides
+// of a copy are addressed with the same affine form
+//
+//     addr(side, i, slice, c) = base + slice*slice_stride + item(side,i)*item_stride + c*chunk_bytes
+//
+// where slice = l*2+kv and item = ids[i] for a paged pool (slice_stride = num_blocks*tile_bytes,
+// item_stride = tile_bytes) or item = i for the contiguous fusion buffer of PAPER.md:237
+// (slice_stride = tile_bytes, item_stride = 2*layers*tile_bytes).  migrate = pool->pool,
+// pack = pool->buffer, unpack = buffer->pool: one kernel body serves S3, S4, S5 and S6.
+//
+// Two implementations, selected by the host (LLX_OPT_COPY_KERNEL):
+//   llx_copy_vec16 : 256-thread CTAs, 16-byte LDG/STG, UNROLL independent loads in flight per
+//                    thread before the first store; lane 0 fetches the pair's block ids and
+//                    broadcasts them with __shfl_sync.
+//   llx_copy_bulk  : one elected thread per warp drives a ring of shared-memory stages with the
+//                    bulk async-copy engine (cp.async.bulk global->shared completing on an
+//                    mbarrier, shared->global in bulk groups): no registers or LSU issue slots
+//                    per byte, 16 KiB per instruction.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace llx {
+
+constexpr int kIdsByValueCap = 256;
+
+struct IdPack {  // block ids carried in the kernel parameters (constant bank) for short stages
+    int32_t src[kIdsByValueCap];
+    int32_t dst[kIdsByValueCap];
+};
+
+struct CopyArgs {
+    const unsigned char* src_base;
+    unsigned char* dst_base;
+    long long src_slice_stride, src_item_stride;
+    long long dst_slice_stride, dst_item_stride;
+    const int32_t* src_ids;  // device; nullptr => item = i (contiguous side) or ids by value
+    const int32_t* dst_ids;
+    int src_indexed, dst_indexed;  // 1 => item = ids[i], 0 => item = i
+    int tile_bytes;
+    int chunk_bytes;
+    int chunks_per_tile;
+    int slices;       // 2*layers
+    int total_units;  // n * slices * chunks_per_tile
+};
+
+__device__ __forceinline__ uint4 ld_stream16(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream16(void* p, const uint4& v) {
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+                 "r"(v.w)
+                 : "memory");
+}
+
+struct UnitAddr {
+    const unsigned char* src;
+    unsigned char* dst;
+    int len;
+};
+
+// Decode unit u -> (i, slice, c) and form both addresses.  id_s/id_d are the items of pair i.
+__device__ __forceinline__ void unit_coords(const CopyArgs& a, int u, int& i, int& slice, int& c) {
+    c = u % a.chunks_per_tile;
+    int t = u / a.chunks_per_tile;
+    slice = t % a.slices;
+    i = t / a.slices;
+}
+__device__ __forceinline__ UnitAddr unit_addr(const CopyArgs& a, int slice, int c, int item_s, int item_d) {
+    UnitAddr r;
+    long long off = (long long)c * a.chunk_bytes;
+    r.src = a.src_base + slice * a.src_slice_stride + item_s * a.src_item_stride + off;
+    r.dst = a.dst_base + slice * a.dst_slice_stride + item_d * a.dst_item_stride + off;
+    int rem = a.tile_bytes - c * a.chunk_bytes;
+    r.len = rem < a.chunk_bytes ? rem : a.chunk_bytes;
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------
+// 16-byte vector kernel.  Persistent-style grid: CTA b handles units b, b+grid, b+2*grid, ...
+// ------------------------------------------------------------------------------------------
+template <bool BYVAL, int UNROLL>
+__global__ void __launch_bounds__(256, 8) llx_copy_vec16(const CopyArgs a, const __grid_constant__ IdPack ids) {
+    const int lane = threadIdx.x & 31;
+    for (int u = blockIdx.x; u < a.total_units; u += gridDim.x) {
+        int i, slice, c;
+        unit_coords(a, u, i, slice, c);
+        int item_s = i, item_d = i;
+        if (BYVAL) {
+            if (a.src_indexed) item_s = ids.src[i];
+            if (a.dst_indexed) item_d = ids.dst[i];
+        } else {
+            // warp-level index broadcast: one lane reads the pair's ids, the warp shares them
+            int vs = 0, vd = 0;
+            if (lane == 0) {
+                if (a.src_indexed) vs = __ldg(a.src_ids + i);
+                if (a.dst_indexed) vd = __ldg(a.dst_ids + i);
+            }
+            vs = __shfl_sync(0xffffffffu, vs, 0);
+            vd = __shfl_sync(0xffffffffu, vd, 0);
+            if (a.src_indexed) item_s = vs;
+            if (a.dst_indexed) item_d = vd;
+        }
+        const UnitAddr ua = unit_addr(a, slice, c, item_s, item_d);
+        const int nvec = ua.len >> 4;
+        const uint4* __restrict__ s = reinterpret_cast<const uint4*>(ua.src);
+        uint4* __restrict__ d = reinterpret_cast<uint4*>(ua.dst);
+        for (int v0 = threadIdx.x; v0 < nvec; v0 += 256 * UNROLL) {
+            uint4 r[UNROLL];
+#pragma unroll
+            for (int j = 0; j < UNROLL; ++j) {
+                int v = v0 + j * 256;
+                if (v < nvec) r[j] = ld_stream16(s + v);
+            }
+#pragma unroll
+            for (int j = 0; j < UNROLL; ++j) {
+                int v = v0 + j * 256;
+                if (v < nvec) st_stream16(d + v, r[j]);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Bulk async-copy (TMA, non-tensor form) ring kernel.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LLX_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LLX_DONE_%=;\n"
+        "bra LLX_WAIT_%=;\n"
+        "LLX_DONE_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     dst_smem),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src_smem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src_smem), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+// Shared memory: [rings_per_cta][nstages] mbarriers (8 B each, padded to 128 B per ring group),
+// then [rings_per_cta][nstages][chunk_bytes] data.  Ring r of the grid handles units
+// r, r+nrings, r+2*nrings, ...; lane 0 of each warp is the ring's only working thread.
+template <bool BYVAL>
+__global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack ids, int nstages) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int warp = threadIdx.x >> 5;
+    const int rings_per_cta = blockDim.x >> 5;
+    if ((threadIdx.x & 31) != 0) return;
+
+    const int bar_bytes = ((rings_per_cta * nstages * 8) + 127) & ~127;
+    const uint32_t bar0 = smem_u32(smem) + warp * nstages * 8;
+    const uint32_t buf0 = smem_u32(smem) + bar_bytes + warp * nstages * a.chunk_bytes;
+
+    for (int s = 0; s < nstages; ++s) mbar_init(bar0 + s * 8, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+
+    const int ring = blockIdx.x * rings_per_cta + warp;
+    const int nrings = gridDim.x * rings_per_cta;
+    if (ring >= a.total_units) return;
+    const int K = (a.total_units - ring + nrings - 1) / nrings;  // units of this ring
+
+    auto addr_of = [&](int k) -> UnitAddr {
+        int u = ring + k * nrings;
+        int i, slice, c;
+        unit_coords(a, u, i, slice, c);
+        int item_s = i, item_d = i;
+        if (a.src_indexed) item_s = BYVAL ? ids.src[i] : __ldg(a.src_ids + i);
+        if (a.dst_indexed) item_d = BYVAL ? ids.dst[i] : __ldg(a.dst_ids + i);
+        return unit_addr(a, slice, c, item_s, item_d);
+    };
+    auto issue_load = [&](int k) {
+        const int s = k % nstages;
+        UnitAddr ua = addr_of(k);
+        mbar_expect_tx(bar0 + s * 8, (uint32_t)ua.len);
+        bulk_g2s(buf0 + s * a.chunk_bytes, ua.src, (uint32_t)ua.len, bar0 + s * 8);
+    };
+
+    const int pre = K < nstages ? K : nstages;
+    for (int k = 0; k < pre; ++k) issue_load(k);
+    for (int k = 0; k < K; ++k) {
+        const int s = k % nstages;
+        mbar_wait(bar0 + s * 8, (uint32_t)((k / nstages) & 1));
+        UnitAddr ua = addr_of(k);
+        bulk_s2g(ua.dst, buf0 + s * a.chunk_bytes, (uint32_t)ua.len);
+        bulk_commit();
+        // refill the stage whose store was committed one iteration ago: allowing the newest
+        // group to stay pending keeps one store and nstages-1 loads in flight per ring
+        if (k >= 1 && k - 1 + nstages < K) {
+            bulk_wait_read<1>();
+            issue_load(k - 1 + nstages);
+        }
+    }
+    bulk_wait_all();
+}
+
+// ------------------------------------------------------------------------------------------
+// S8 append: values[t][l][kv][token_bytes] -> pool[l][kv][blk(t)][slot(t)]
+// One CTA per (token, layer, kv).  tok_block = block id of each token (by value or device).
+// ------------------------------------------------------------------------------------------
+struct AppendArgs {
+    unsigned char* pool_base;
+    const unsigned char* values;
+    const int32_t* tok_block;  // device, or nullptr when by value
+    long long slice_stride;    // num_blocks*tile_bytes
+    int tile_bytes, token_bytes, block_size, slices, t0, ntok;
+};
+template <bool BYVAL>
+__global__ void __launch_bounds__(128) llx_append_kernel(const AppendArgs a, const __grid_constant__ IdPack ids) {
+    const int u = blockIdx.x;  // (tok, slice)
+    const int slice = u % a.slices;
+    const int k = u / a.slices;
+    const int blk = BYVAL ? ids.src[k] : __ldg(a.tok_block + k);
+    const int slot = (a.t0 + k) % a.block_size;
+    const uint4* s = reinterpret_cast<const uint4*>(a.values + ((long long)k * a.slices + slice) * a.token_bytes);
+    uint4* d = reinterpret_cast<uint4*>(a.pool_base + slice * a.slice_stride + (long long)blk * a.tile_bytes +
+                                        (long long)slot * a.token_bytes);
+    for (int v = threadIdx.x; v < (a.token_bytes >> 4); v += blockDim.x) d[v] = s[v];
+}
+
+__global__ void __launch_bounds__(256) llx_fill_u16_kernel(uint4* p, long long nvec, uint32_t word) {
+    const uint4 v = make_uint4(word, word, word, word);
+    for (long long i = blockIdx.x * 256ll + threadIdx.x; i < nvec; i += (long long)gridDim.x * 256) p[i] = v;
+}
+
+}  // namespace llx

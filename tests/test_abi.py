@@ -1,0 +1,121 @@
+"""The C-ABI boundary without a GPU: the library builds for sm_100a, loads, exports every symbol
+include/llx.h declares, and its host-only entry points behave.  No compute calls here."""
+import ctypes
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "llx.h")
+
+
+@pytest.fixture(scope="module")
+def llx():
+    from paper_2406_03243_b200 import build
+    build.build()
+    import paper_2406_03243_b200 as m
+    m.load()
+    return m
+
+
+def declared_symbols():
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(llx_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_symbols_all_exported_and_bound(llx):
+    names = declared_symbols()
+    assert len(names) >= 25 and "llx_migrate_stage" in names and "llx_pack" in names
+    raw = ctypes.CDLL(os.path.join(ROOT, "paper_2406_03243_b200", "libllx.so"))
+    for n in names:
+        assert hasattr(raw, n), f"{n} declared in llx.h but not exported by libllx.so"
+    assert sorted(llx.EXPORTS) == names, "binding.EXPORTS and include/llx.h disagree"
+
+
+def test_library_is_sm100a_and_uses_bulk_async_copy():
+    lib = os.path.join(ROOT, "paper_2406_03243_b200", "libllx.so")
+    out = subprocess.run(["cuobjdump", "-lelf", lib], capture_output=True, text=True)
+    if out.returncode != 0:
+        pytest.skip("cuobjdump unavailable")
+    assert "sm_100a" in out.stdout
+    sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True).stdout
+    assert "UBLKCP" in sass and "LDG.E.128" in sass and "STG.E.128" in sass
+
+
+def test_geometry_arithmetic_matches_paper_example(llx):
+    # 16-bit LLaMA-7B: 128 KB per block (K or V, 16 tokens, one layer)
+    assert llx.pool_bytes_for(1, 32, 128, 16, llx.F16, 1) == 2 * 131072
+    assert llx.pool_bytes_for(32, 32, 128, 16, llx.F16, 2000) == 2000 * 8 * 2**20
+    assert llx.pool_bytes_for(60, 52, 128, 16, llx.F16, 3000) == 3000 * 120 * 208 * 1024
+    assert llx.pool_bytes_for(2, 4, 64, 16, llx.F16, 256) == 8 * 2**20
+    assert llx.pool_bytes_for(2, 4, 64, 16, llx.U8, 256) == 4 * 2**20
+    for bad in [(0, 4, 64, 16, 0, 1), (2, 4, 64, 16, 7, 1), (2, 1, 1, 1, 0, 4), (2, 4, 64, 16, 0, 0), (2, 4, 64, -1, 0, 1)]:
+        assert llx.pool_bytes_for(*bad) == 0
+
+
+def test_options_validate_and_roundtrip(llx):
+    old = llx.get_option(llx.OPT_CHUNK_BYTES)
+    llx.set_option(llx.OPT_CHUNK_BYTES, 8192)
+    assert llx.get_option(llx.OPT_CHUNK_BYTES) == 8192
+    with pytest.raises(llx.LlxError) as e:
+        llx.set_option(llx.OPT_CHUNK_BYTES, 100)          # not a multiple of 16
+    assert e.value.name == "LLX_ERR_INVALID_ARG"
+    with pytest.raises(llx.LlxError):
+        llx.set_option(llx.OPT_COPY_KERNEL, 9)
+    with pytest.raises(llx.LlxError):
+        llx.set_option(llx.OPT_IDS_BY_VALUE_MAX, 100000)
+    llx.set_option(llx.OPT_CHUNK_BYTES, old)
+    with llx.options(copy_kernel=1, max_ctas=3):
+        assert llx.get_option(llx.OPT_COPY_KERNEL) == 1 and llx.get_option(llx.OPT_MAX_CTAS) == 3
+    assert llx.get_option(llx.OPT_COPY_KERNEL) == 0 and llx.get_option(llx.OPT_MAX_CTAS) == 0
+
+
+def test_status_strings_and_counters(llx):
+    l = llx.lib()
+    assert l.llx_status_str(0) == b"LLX_OK" and l.llx_status_str(-4) == b"LLX_ERR_DUPLICATE_DST"
+    assert l.llx_status_str(-99) == b"LLX_ERR_UNKNOWN"
+    llx.reset_counters()
+    assert llx.counters() == dict(kernel_launches=0, copy_launches=0, bytes_moved=0, id_uploads=0)
+    assert "sm_100a" in llx.version()
+
+
+def test_no_cpu_fallback_without_a_device(llx):
+    """On a box without a GPU every data call must fail loudly (LLX_ERR_CUDA), never compute on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present; the no-device behaviour is checked on the CPU box")
+    with pytest.raises(llx.LlxError) as e:
+        llx.pool_create(2, 4, 64, 16, llx.F16, 256)
+    assert e.value.name == "LLX_ERR_CUDA"
+    host = np.zeros(1 << 16, dtype=np.uint8)
+    with pytest.raises(llx.LlxError):
+        llx.pool_wrap(host.ctypes.data, host.nbytes, 1, 1, 8, 1, llx.F16, 4)
+
+
+def test_null_and_trivial_arguments(llx):
+    l = llx.lib()
+    assert l.llx_pool_destroy(None) == 0
+    assert l.llx_pool_data(None, 0, 0) is None
+    assert l.llx_pool_tile_bytes(None) == 0 and l.llx_pool_bytes(None) == 0 and l.llx_pool_num_blocks(None) == 0
+    assert l.llx_staging_bytes(None, 4) == 0
+    assert l.llx_staging_free_pinned(None) == 0
+    rc = l.llx_migrate_stage(None, None, None, None, 0, None)
+    assert rc == -1 and b"NULL" in l.llx_last_error()
+
+
+def test_plan_stage_matches_oracle_on_every_state(llx):
+    """S1 is host arithmetic: the library's planner against oracle.plan_stage for every (tokens, migrated)."""
+    from oracle import kv_migration as om
+    for S, last in ((16, 2), (4, 1), (5, 3)):
+        for tokens in range(0, 150):
+            for m in range(0, -(-tokens // S) + 1):
+                assert llx.plan_stage(tokens, m, S, last) == om.plan_stage(tokens, m, S, last)
+    assert llx.plan_stage(2032, 0, 16, 2) == (127, False)
+    assert llx.plan_stage(2048, 126, 16, 2) == (2, True)
+    for bad in [(16, 2, 16, 2), (-1, 0, 16, 2), (16, 0, 0, 2), (16, 0, 16, 0)]:
+        with pytest.raises(llx.LlxError):
+            llx.plan_stage(*bad)

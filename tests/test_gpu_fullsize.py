@@ -1,0 +1,162 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default options).
+
+The pools are too large to mirror on the host (15.6 GiB / 71 GiB each), so — SURVEY.md §8(c) "verification
+at scale" — a SAMPLE of layers is generated on the host from the seeded recipe, replayed by the oracle one
+layer at a time and compared with a readback of the same destination layer (all blocks: mapping P1 and
+sentinel P2); the other layers are filled by a seeded device generator and checked by properties that
+hold at any size (destination rows equal source rows under an independent torch gather; every untouched
+destination block still holds the sentinel)."""
+import numpy as np
+import pytest
+import torch
+
+import synth
+from oracle import kv_migration as om
+
+pytestmark = pytest.mark.gpu
+SENT = synth.SENTINEL_U16
+SENT_I16 = int(np.array(SENT, dtype=np.uint16).view(np.int16))
+
+
+@pytest.fixture(scope="module")
+def env():
+    import gpu_harness as H
+    import paper_2406_03243_b200 as llx
+    llx.load()
+    return H, llx
+
+
+def free_gib():
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    return free / 2**30
+
+
+def check_untouched_and_mapping_on_device(src, dst, s_ids, d_ids, layers):
+    """Properties on the device with torch indexing (independent of the library's kernels)."""
+    s_idx = torch.from_numpy(np.asarray(s_ids, dtype=np.int64)).cuda()
+    d_idx = torch.from_numpy(np.asarray(d_ids, dtype=np.int64)).cuda()
+    mask = torch.ones(dst.nb, dtype=torch.bool, device="cuda")
+    mask[d_idx] = False
+    untouched = torch.nonzero(mask).flatten()
+    for l in layers:
+        for kv in range(2):
+            assert torch.equal(dst.view[l, kv].index_select(0, d_idx), src.view[l, kv].index_select(0, s_idx)), (l, kv)
+            assert bool((dst.view[l, kv].index_select(0, untouched) == SENT_I16).all()), (l, kv)
+
+
+def test_llama7b_2048_tokens_three_stages_with_appends(env):
+    """configs[1]: 2032 -> 2040 -> 2048 tokens, stages 112 / 14 / 2, 8-token appends between stages (A5)."""
+    H, llx = env
+    g = synth.CONFIGS["llama7b"]
+    if free_gib() < 34:
+        pytest.skip("needs two 15.6 GiB pools")
+    L, S, te = g["layers"], g["block_size"], H.tile_elems(g)
+    te_tok = g["kv_heads"] * g["head_dim"]
+    sample_layers = [0, 13, 31]
+    src, dst = H.DevPool(g), H.DevPool(g, fill=SENT)
+    src.fill_device_random(1234)
+    src.fill_from_synth(0, 0, layers=sample_layers)
+    s_tab = synth.block_permutation(1, g["num_blocks"])[:128]
+    d_tab = synth.block_permutation(2, g["num_blocks"])[:128]
+    schedule, appends, tokens = (112, 14, 2), (8, 8), 2032
+    values = lambda t, l, kv: synth.append_values_f16(3, t, l, kv, te_tok)
+
+    launches0 = llx.counters()["copy_launches"]
+    m = 0
+    for k, n in enumerate(schedule):
+        llx.migrate_stage(src.pool, s_tab[m:m + n], dst.pool, d_tab[m:m + n])
+        m += n
+        if k < len(appends):
+            vals = np.empty((appends[k], L, 2, te_tok), dtype=np.uint16)
+            for j in range(appends[k]):
+                for l in range(L):
+                    for kv in range(2):
+                        vals[j, l, kv] = values(tokens + j, l, kv)
+            dev_vals = torch.from_numpy(vals.view(np.int16)).cuda()
+            llx.append_tokens(src.pool, s_tab, tokens, tokens + appends[k], dev_vals.data_ptr())
+            tokens += appends[k]
+        # after EVERY stage: the blocks migrated so far equal their source blocks (device-side property, all layers)
+        torch.cuda.synchronize()
+        s_idx = torch.from_numpy(s_tab[:m].astype(np.int64)).cuda()
+        d_idx = torch.from_numpy(d_tab[:m].astype(np.int64)).cuda()
+        for l in (0, 17, 31):
+            assert torch.equal(dst.view[l, 1].index_select(0, d_idx), src.view[l, 1].index_select(0, s_idx))
+    assert tokens == 2048 and llx.counters()["copy_launches"] == launches0 + 3
+    torch.cuda.synchronize()
+
+    # oracle replay, one sampled layer at a time, compared on the WHOLE destination layer
+    for l in sample_layers:
+        h_src = H.host_pool_from_synth(g, 0, 0, layers=[l])
+        h_dst = om.new_pool(1, g["num_blocks"], te, fill=SENT)
+        om.staged_migration(h_src, s_tab, h_dst, d_tab, schedule, appends, S, 2032,
+                            lambda t, _l, kv, l=l: values(t, l, kv))
+        H.assert_pool_equal(dst.host_layer(l), h_dst)
+        H.assert_pool_equal(src.host_layer(l), h_src)          # appends landed where the oracle put them; src intact
+    check_untouched_and_mapping_on_device(src, dst, s_tab, d_tab, range(L))
+
+
+@pytest.mark.parametrize("tokens", [256, 8192])
+def test_llama7b_length_sweep_ends_single_shot_vs_two_stage(env, tokens):
+    """configs[2] end points: single-shot copy == (n-2, 2) staged copy == oracle on sampled layers."""
+    H, llx = env
+    g = synth.CONFIGS["llama7b"]
+    if free_gib() < 50:
+        pytest.skip("needs three 15.6 GiB pools")
+    n = tokens // g["block_size"]
+    te = H.tile_elems(g)
+    src, dst_a, dst_b = H.DevPool(g), H.DevPool(g, fill=SENT), H.DevPool(g, fill=SENT)
+    src.fill_device_random(99)
+    src.fill_from_synth(0, 0, layers=[5])
+    s_tab = synth.block_permutation(40 + n, g["num_blocks"])[:n]
+    d_tab = synth.block_permutation(50 + n, g["num_blocks"])[:n]
+    llx.migrate_stage(src.pool, s_tab, dst_a.pool, d_tab)
+    llx.migrate_stage(src.pool, s_tab[:n - 2], dst_b.pool, d_tab[:n - 2])
+    llx.migrate_stage(src.pool, s_tab[n - 2:], dst_b.pool, d_tab[n - 2:])
+    torch.cuda.synchronize()
+    h_src = H.host_pool_from_synth(g, 0, 0, layers=[5])
+    h_dst = om.new_pool(1, g["num_blocks"], te, fill=SENT)
+    om.migrate_stage(h_src, s_tab, h_dst, d_tab)
+    H.assert_pool_equal(dst_a.host_layer(5), h_dst)
+    H.assert_pool_equal(dst_b.host_layer(5), h_dst)
+    check_untouched_and_mapping_on_device(src, dst_a, s_tab, d_tab, range(0, g["layers"], 5))
+    for l in range(0, g["layers"], 7):
+        assert torch.equal(dst_a.view[l], dst_b.view[l])
+
+
+def test_llama30b_batch_of_64_requests(env):
+    """configs[3]: 64 requests, bounded-Pareto lengths (mean 512, [16, 8192]), one llx_migrate_batch launch."""
+    H, llx = env
+    g = dict(synth.CONFIGS["llama30b"])
+    lens, nblk, seed_used = synth.batch_request_blocks(0, 64, g["block_size"], g["num_blocks"])
+    total = int(nblk.sum())
+    block_gib = 2 * g["layers"] * H.tile_elems(g) * 2 / 2**30
+    # shrink both pools equally if two 3000-block pools (142.8 GiB) do not fit next to the workspace (recorded)
+    nb = g["num_blocks"]
+    while 2 * nb * block_gib > free_gib() - 6 and nb > total:
+        nb -= 100
+    if nb < total:
+        pytest.skip(f"not enough device memory for {total} blocks per pool")
+    g["num_blocks"] = nb
+    te = H.tile_elems(g)
+    src, dst = H.DevPool(g), H.DevPool(g, fill=SENT)
+    src.fill_device_random(7)
+    sample = [0, 59]
+    src.fill_from_synth(0, 0, layers=sample)
+    s_ids = synth.block_permutation(1, nb)[:total]
+    d_ids = synth.block_permutation(2, nb)[:total]
+    off = np.concatenate([[0], np.cumsum(nblk)]).astype(np.int32)
+    c0 = llx.counters()
+    llx.migrate_batch(src.pool, dst.pool, off, s_ids, d_ids)
+    torch.cuda.synchronize()
+    c1 = llx.counters()
+    assert c1["copy_launches"] == c0["copy_launches"] + 1
+    assert c1["bytes_moved"] - c0["bytes_moved"] == total * src.pool.block_bytes
+    for l in sample:
+        h_src = H.host_pool_from_synth(g, 0, 0, layers=[l])
+        h_dst = om.new_pool(1, nb, te, fill=SENT)
+        om.migrate_batch(h_src, h_dst, off, s_ids, d_ids)
+        H.assert_pool_equal(dst.host_layer(l), h_dst)
+    check_untouched_and_mapping_on_device(src, dst, s_ids, d_ids, range(0, g["layers"], 6))

@@ -1,0 +1,270 @@
+"""GPU-vs-oracle parity for the migration path (S3-S6, S8), bit-exact on uint16 views.  All calls go
+through the C-ABI (paper_2406_03243_b200.binding -> libllx.so).  SURVEY.md §8(c) P1-P8 on the device."""
+import numpy as np
+import pytest
+import torch
+
+import synth
+from oracle import kv_migration as om
+
+pytestmark = pytest.mark.gpu
+
+SENT = synth.SENTINEL_U16
+TINY = synth.CONFIGS["tiny"]
+# a tile of 34,560 bytes: two full 16 KiB chunks and a ragged 1,792-byte tail
+RAGGED = dict(layers=3, kv_heads=9, head_dim=120, block_size=16, elem_bytes=2, num_blocks=40)
+# a tile smaller than any chunk (1,008 bytes)
+SMALLTILE = dict(layers=2, kv_heads=7, head_dim=24, block_size=3, elem_bytes=2, num_blocks=64)
+
+KERNELS = [dict(copy_kernel=2), dict(copy_kernel=1), dict(copy_kernel=2, chunk_bytes=4096, ring_stages=2),
+           dict(copy_kernel=1, chunk_bytes=2048), dict(copy_kernel=2, ids_by_value_max=0),
+           dict(copy_kernel=1, ids_by_value_max=0), dict(copy_kernel=2, max_ctas=3), dict(copy_kernel=1, max_ctas=1)]
+
+
+@pytest.fixture(scope="module")
+def env():
+    import gpu_harness as H
+    import paper_2406_03243_b200 as llx
+    llx.load()
+    return H, llx
+
+
+def make(H, g, seed=0):
+    src = H.DevPool(g)
+    src.fill_from_synth(seed, 0)
+    dst = H.DevPool(g, fill=SENT)
+    h_src = H.host_pool_from_synth(g, seed, 0)
+    h_dst = om.new_pool(g["layers"], g["num_blocks"], H.tile_elems(g), fill=SENT)
+    return src, dst, h_src, h_dst
+
+
+# ---- configs[0] "Tiny": 100-token request, 7 blocks, 2 stages (5 then 2); everything compared after every stage
+@pytest.mark.parametrize("opts", KERNELS)
+def test_tiny_two_stage_migration_bit_exact(env, opts):
+    H, llx = env
+    src, dst, h_src, h_dst = make(H, TINY)
+    s_tab = synth.block_permutation(1, TINY["num_blocks"])[:7]
+    d_tab = synth.block_permutation(2, TINY["num_blocks"])[:7]
+    m = 0
+    with llx.options(**opts):
+        for n in (5, 2):
+            llx.migrate_stage(src.pool, s_tab[m:m + n], dst.pool, d_tab[m:m + n])
+            om.migrate_stage(h_src, s_tab[m:m + n], h_dst, d_tab[m:m + n])
+            m += n
+            H.assert_pool_equal(dst.host(), h_dst)      # P1 mapping + P2 sentinel on every other block
+            H.assert_pool_equal(src.host(), h_src)      # P3 source intact
+    untouched = np.setdiff1d(np.arange(TINY["num_blocks"]), d_tab)
+    assert np.all(dst.host()[:, :, untouched] == SENT)
+
+
+@pytest.mark.parametrize("g", [RAGGED, SMALLTILE])
+@pytest.mark.parametrize("opts", KERNELS)
+@pytest.mark.parametrize("n", [1, 13])
+def test_ragged_tiles_and_small_tiles(env, g, opts, n):
+    H, llx = env
+    src, dst, h_src, h_dst = make(H, g, seed=5)
+    s_ids = synth.block_permutation(11, g["num_blocks"])[:n]
+    d_ids = synth.block_permutation(12, g["num_blocks"])[:n]
+    with llx.options(**opts):
+        llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids)
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
+    H.assert_pool_equal(src.host(), h_src)
+
+
+def test_whole_pool_and_ids_through_the_ring(env):
+    """n = num_blocks > 256: ids go through the pinned ring, every block moves, twice in a row (slot reuse)."""
+    H, llx = env
+    g = dict(TINY, num_blocks=700)
+    src, dst, h_src, h_dst = make(H, g, seed=2)
+    for rep in range(3):
+        s_ids = synth.block_permutation(20 + rep, 700)
+        d_ids = synth.block_permutation(30 + rep, 700)
+        c0 = llx.counters()["id_uploads"]
+        llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids)
+        assert llx.counters()["id_uploads"] == c0 + 1
+        om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+        H.assert_pool_equal(dst.host(), h_dst)
+
+
+def test_duplicate_source_ids_are_legal(env):
+    H, llx = env
+    src, dst, h_src, h_dst = make(H, TINY)
+    llx.migrate_stage(src.pool, [9, 9, 9], dst.pool, [0, 100, 255])
+    om.migrate_stage(h_src, [9, 9, 9], h_dst, [0, 100, 255])
+    H.assert_pool_equal(dst.host(), h_dst)
+
+
+def test_order_and_partition_invariance(env):                       # P6
+    H, llx = env
+    g = RAGGED
+    src, dst_a, h_src, h_dst = make(H, g, seed=7)
+    dst_b, dst_c = H.DevPool(g, fill=SENT), H.DevPool(g, fill=SENT)
+    s_ids = synth.block_permutation(1, g["num_blocks"])[:17]
+    d_ids = synth.block_permutation(2, g["num_blocks"])[:17]
+    llx.migrate_stage(src.pool, s_ids, dst_a.pool, d_ids)
+    p = np.random.default_rng(3).permutation(17)
+    llx.migrate_stage(src.pool, s_ids[p], dst_b.pool, d_ids[p])
+    for a, b in [(0, 1), (1, 9), (9, 17)]:
+        llx.migrate_stage(src.pool, s_ids[a:b], dst_c.pool, d_ids[a:b])
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    for d in (dst_a, dst_b, dst_c):
+        H.assert_pool_equal(d.host(), h_dst)
+
+
+def test_batch_equals_sequential_and_oracle(env):                   # P7, S5
+    H, llx = env
+    g = RAGGED
+    src, dst, h_src, h_dst = make(H, g, seed=8)
+    dst_seq = H.DevPool(g, fill=SENT)
+    s_ids = synth.block_permutation(1, g["num_blocks"])[:30]
+    d_ids = synth.block_permutation(2, g["num_blocks"])[:30]
+    off = [0, 7, 7, 8, 21, 30]                                       # includes an empty request
+    llx.migrate_batch(src.pool, dst.pool, off, s_ids, d_ids)
+    for r in range(5):
+        llx.migrate_stage(src.pool, s_ids[off[r]:off[r + 1]], dst_seq.pool, d_ids[off[r]:off[r + 1]])
+    om.migrate_batch(h_src, h_dst, off, s_ids, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
+    H.assert_pool_equal(dst_seq.host(), h_dst)
+    llx.migrate_batch(src.pool, dst.pool, [0], [], [])               # R = 0
+    llx.migrate_batch(src.pool, dst.pool, [0, 0, 0], [], [])         # only empty requests
+    H.assert_pool_equal(dst.host(), h_dst)
+
+
+@pytest.mark.parametrize("where", ["device", "pinned"])
+@pytest.mark.parametrize("opts", [dict(), dict(copy_kernel=1), dict(copy_kernel=2)])
+def test_pack_unpack_block_fusion(env, where, opts):                 # P5, S6
+    H, llx = env
+    g = RAGGED
+    src, dst, h_src, h_dst = make(H, g, seed=9)
+    n = 11
+    s_ids = synth.block_permutation(1, g["num_blocks"])[:n]
+    d_ids = synth.block_permutation(2, g["num_blocks"])[:n]
+    nbytes = llx.staging_bytes(src.pool, n)
+    assert nbytes == n * 2 * g["layers"] * src.pool.tile_bytes
+    if where == "device":
+        stg = torch.full((nbytes // 2,), 0x1111, dtype=torch.int16, device="cuda")
+        ptr = stg.data_ptr()
+    else:
+        pin = llx.PinnedStaging(nbytes)
+        pin.as_numpy()[:] = 0x1111
+        ptr = pin.dev_alias
+    with llx.options(**opts):
+        llx.pack(src.pool, s_ids, ptr, nbytes)
+        torch.cuda.synchronize()
+        got = stg.cpu().numpy().view(np.uint16) if where == "device" else pin.as_numpy().copy()
+        want = om.pack(h_src, s_ids)
+        assert np.array_equal(got.reshape(want.shape), want)         # staging layout [i][l][kv][tile] (A6)
+        llx.unpack(ptr, nbytes, dst.pool, d_ids)
+    om.unpack(want, h_dst, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
+    direct = H.DevPool(g, fill=SENT)
+    llx.migrate_stage(src.pool, s_ids, direct.pool, d_ids)           # unpack(pack(.)) == migrate (P5)
+    H.assert_pool_equal(direct.host(), h_dst)
+    H.assert_pool_equal(src.host(), h_src)
+    if where == "pinned":
+        pin.free()
+
+
+def test_staged_with_appends_equals_oracle_and_single_shot(env):     # P4, S1, S8 on the Tiny shape
+    H, llx = env
+    g = TINY
+    S, te_tok = g["block_size"], g["kv_heads"] * g["head_dim"]
+    src, dst, h_src, h_dst = make(H, g)
+    s_tab = synth.block_permutation(1, g["num_blocks"])[:7]
+    d_tab = synth.block_permutation(2, g["num_blocks"])[:7]
+    values = lambda t, l, kv: synth.append_values_f16(3, t, l, kv, te_tok)
+    tokens, m = 97, 0
+    for k, (n, app) in enumerate([(5, 3), (2, 0)]):
+        plan_n, final = om.plan_stage(tokens, m, S, 2)
+        assert plan_n == n and final == (k == 1)
+        llx.migrate_stage(src.pool, s_tab[m:m + n], dst.pool, d_tab[m:m + n])
+        m += n
+        if app:
+            vals = np.stack([np.stack([np.stack([values(t, l, kv) for kv in range(2)]) for l in range(g["layers"])])
+                             for t in range(tokens, tokens + app)])          # [t][l][kv][H*D]
+            dev_vals = torch.from_numpy(vals.view(np.int16)).cuda()
+            llx.append_tokens(src.pool, s_tab, tokens, tokens + app, dev_vals.data_ptr())
+            tokens += app
+    final_tokens = om.staged_migration(h_src, s_tab, h_dst, d_tab, (5, 2), (3,), S, 97, values)
+    assert final_tokens == tokens == 100
+    H.assert_pool_equal(src.host(), h_src)                          # appends landed in exactly the oracle's slots
+    H.assert_pool_equal(dst.host(), h_dst)
+    single = om.new_pool(g["layers"], g["num_blocks"], H.tile_elems(g), SENT)
+    om.migrate_stage(h_src, s_tab, single, d_tab)
+    H.assert_pool_equal(dst.host(), single)                         # P4
+
+
+def test_library_owned_pool_upload_download_fill(env):
+    H, llx = env
+    g = SMALLTILE
+    te = H.tile_elems(g)
+    a = llx.pool_create(g["layers"], g["kv_heads"], g["head_dim"], g["block_size"], llx.F16, g["num_blocks"])
+    b = llx.pool_create(g["layers"], g["kv_heads"], g["head_dim"], g["block_size"], llx.F16, 80)   # other num_blocks: legal
+    assert a.tile_bytes == te * 2 and a.num_blocks == 64 and b.nbytes == 80 * a.block_bytes
+    h_src = H.host_pool_from_synth(g, 4, 0)
+    for l in range(g["layers"]):
+        for kv in range(2):
+            a.upload(l, kv, 0, h_src[l, kv])
+    b.fill_u16(SENT)
+    h_dst = om.new_pool(g["layers"], 80, te, fill=SENT)
+    s_ids, d_ids = [63, 0, 5, 17], [79, 64, 1, 0]
+    llx.migrate_stage(a, s_ids, b, d_ids)
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    torch.cuda.synchronize()
+    for l in range(g["layers"]):
+        for kv in range(2):
+            got = b.download(l, kv, 0, 80)
+            torch.cuda.synchronize()
+            assert np.array_equal(got, h_dst[l, kv])
+            assert np.array_equal(a.download(l, kv, 3, 5), h_src[l, kv, 3:8])
+    a.destroy()
+    b.destroy()
+
+
+def test_argument_errors_change_no_byte(env):
+    H, llx = env
+    src, dst, h_src, h_dst = make(H, TINY)
+    other = H.DevPool(RAGGED, fill=SENT)
+    launches = llx.counters()["kernel_launches"]
+
+    def err(name, fn):
+        with pytest.raises(llx.LlxError) as e:
+            fn()
+        assert e.value.name == name, e.value
+
+    err("LLX_ERR_BLOCK_OUT_OF_RANGE", lambda: llx.migrate_stage(src.pool, [0, 256], dst.pool, [1, 2]))
+    err("LLX_ERR_BLOCK_OUT_OF_RANGE", lambda: llx.migrate_stage(src.pool, [0, 1], dst.pool, [1, -1]))
+    err("LLX_ERR_DUPLICATE_DST", lambda: llx.migrate_stage(src.pool, [0, 1], dst.pool, [4, 4]))
+    err("LLX_ERR_ALIAS", lambda: llx.migrate_stage(src.pool, [0], src.pool, [1]))
+    err("LLX_ERR_GEOMETRY_MISMATCH", lambda: llx.migrate_stage(src.pool, [0], other.pool, [1]))
+    err("LLX_ERR_INVALID_ARG", lambda: llx.migrate_batch(src.pool, dst.pool, [0, 2, 1, 3], [0, 1, 2], [0, 1, 2]))
+    err("LLX_ERR_DUPLICATE_DST", lambda: llx.migrate_batch(src.pool, dst.pool, [0, 1, 2], [0, 1], [7, 7]))
+    stg = torch.empty(llx.staging_bytes(src.pool, 2), dtype=torch.uint8, device="cuda")
+    err("LLX_ERR_STAGING_TOO_SMALL", lambda: llx.pack(src.pool, [0, 1, 2], stg.data_ptr(), stg.numel()))
+    err("LLX_ERR_STAGING_TOO_SMALL", lambda: llx.unpack(stg.data_ptr(), stg.numel(), dst.pool, [0, 1, 2]))
+    err("LLX_ERR_ALIAS", lambda: llx.pack(src.pool, [0], src.raw.data_ptr(), src.raw.numel()))
+    err("LLX_ERR_INVALID_ARG", lambda: llx.append_tokens(src.pool, [1, 2], 30, 40, stg.data_ptr()))
+    alias = llx.pool_wrap(src.raw.data_ptr(), src.raw.numel(), TINY["layers"], TINY["kv_heads"], TINY["head_dim"],
+                          TINY["block_size"], llx.F16, TINY["num_blocks"])
+    err("LLX_ERR_ALIAS", lambda: llx.migrate_stage(src.pool, [0], alias, [1]))       # distinct handle, same memory
+    err("LLX_ERR_INVALID_ARG", lambda: llx.pool_wrap(src.raw.data_ptr(), 100, 2, 4, 64, 16, llx.F16, 256))
+    err("LLX_ERR_INVALID_ARG", lambda: llx.pool_wrap(src.raw.data_ptr() + 2, 1 << 20, 1, 1, 8, 1, llx.F16, 4))
+    llx.migrate_stage(src.pool, [], dst.pool, [])                                   # n == 0: OK, no launch
+    assert llx.counters()["kernel_launches"] == launches
+    H.assert_pool_equal(dst.host(), h_dst)
+    H.assert_pool_equal(src.host(), h_src)
+
+
+def test_migration_on_a_side_stream_concurrent_with_default_stream(env):
+    H, llx = env
+    src, dst, h_src, h_dst = make(H, TINY)
+    side = torch.cuda.Stream(priority=0)
+    side.wait_stream(torch.cuda.current_stream())
+    s_ids = synth.block_permutation(1, 256)[:100]
+    d_ids = synth.block_permutation(2, 256)[:100]
+    for a in range(0, 100, 10):
+        llx.migrate_stage(src.pool, s_ids[a:a + 10], dst.pool, d_ids[a:a + 10], stream=side)
+    side.synchronize()
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
