@@ -1,0 +1,457 @@
+#!/usr/bin/env python
+"""bench.py — KV-cache live-migration throughput on B200 (BASELINE.json metric).
+
+One STEP = one pass of the hot path over BASELINE.json configs[1] (LLaMA-7B shape): a 2048-token request
+(128 scattered blocks of 8 MiB) migrated between two 2000-block pools in 3 stages (112, 14, then the 2
+final blocks) with 8 new tokens appended to the source between stages — S1 planning check, S3 stages,
+S8 appends and the S4 final stage, all through the C-ABI (libllx.so).
+
+    value     GB/s, bytes read + written by the three stage copies / device time of the whole step
+              (pools resident in HBM; CUDA events on the launching stream; max over ranks)
+    e2e       the same request migrated THROUGH HOST BUFFERS: llx_pack into a pinned host staging buffer
+              (D2H) and llx_unpack from it (H2D) — the paper's GPU->CPU buffer->GPU route
+    roofline  the dominant kernel (stage 0: 112 blocks, 1.75 GiB of traffic) against the measured HBM peak
+    cpu_baseline / --impl reference   the NumPy oracle timed on the host cores on a bounded sample
+
+`--suite` adds the other BASELINE.json configs (length sweep, 30B batch, interference + staging) as
+extra JSON lines on stderr and in gpurun_out/suite.json; the ONE stdout line keeps the contract.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synth  # noqa: E402
+
+METRIC = "kv_migration_gbps_rd_plus_wr"
+UNIT = "GB/s"
+WORKLOAD = "llama7b_2048tok_3stage_112_14_2"
+SCHEDULE, APPENDS, START_TOKENS = (112, 14, 2), (8, 8), 2032
+NOMINAL_HBM_GBS = 8000.0
+FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+# --------------------------------------------------------------------------------------------
+# clocks: sampled with NVML in a thread DURING the timed regions
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index: int):
+        self.samples, self.windows, self._stop, self.ok = [], [], threading.Event(), False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:  # noqa: BLE001
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                self.samples.append((time.perf_counter(), mhz, r))
+            except Exception:  # noqa: BLE001
+                pass
+            time.sleep(0.01)
+
+    def start(self):
+        if self.ok:
+            self.t.start()
+
+    def window(self, t0, t1):
+        self.windows.append((t0, t1))
+
+    def stop(self) -> dict:
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "error": getattr(self, "err", "")}
+        self._stop.set()
+        self.t.join(timeout=2)
+        inside = [(m, r) for (t, m, r) in self.samples if any(a <= t <= b for a, b in self.windows)]
+        use = inside if inside else [(m, r) for (_, m, r) in self.samples]
+        bits = 0
+        for _, r in use:
+            bits |= r
+        reasons = sorted(n for b, n in self.REASONS.items() if bits & b)
+        return {"sm_mhz": statistics.median([m for m, _ in use]) if use else None, "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "samples_in_timed_regions": len(inside), "samples": len(self.samples)}
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_ rd+wr)"
+    except Exception:  # noqa: BLE001
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# --------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference)
+# --------------------------------------------------------------------------------------------
+def oracle_sample_setup(pool_blocks=160):
+    """configs[1]'s request (128 scattered blocks, LLaMA-7B tiles) inside two host pools shrunk to
+    `pool_blocks` blocks so that they fit host RAM (2 x 1.25 GiB); same schedule and appends."""
+    from oracle import kv_migration as om
+    g = synth.CONFIGS["llama7b"]
+    te = g["block_size"] * g["kv_heads"] * g["head_dim"]
+    rng = np.random.default_rng(0)
+    src = om.new_pool(g["layers"], pool_blocks, te)
+    for l in range(g["layers"]):
+        # seeded fp16 bit patterns; one slice generated and rolled per layer to keep the setup short
+        base = synth.slice_values_f16(0, 0, l, 0, pool_blocks, te)
+        src[l, 0] = base
+        src[l, 1] = np.roll(base, 1, axis=0)
+    dst = om.new_pool(g["layers"], pool_blocks, te, fill=synth.SENTINEL_U16)
+    s_tab = synth.block_permutation(1, pool_blocks)[:128]
+    d_tab = synth.block_permutation(2, pool_blocks)[:128]
+    te_tok = g["kv_heads"] * g["head_dim"]
+    vals = rng.integers(0, 0x3C00, size=(16, g["layers"], 2, te_tok), dtype=np.uint16)
+    values = lambda t, l, kv: vals[t - START_TOKENS, l, kv]
+    return om, g, src, dst, s_tab, d_tab, values
+
+
+def oracle_step(ctx):
+    om, g, src, dst, s_tab, d_tab, values = ctx
+    t0 = time.perf_counter()
+    om.staged_migration(src, s_tab, dst, d_tab, SCHEDULE, APPENDS, g["block_size"], START_TOKENS, values)
+    return time.perf_counter() - t0
+
+
+def step_bytes(g) -> int:
+    block_bytes = 2 * g["layers"] * g["block_size"] * g["kv_heads"] * g["head_dim"] * g["elem_bytes"]
+    return 2 * sum(SCHEDULE) * block_bytes          # read + written
+
+
+def cpu_baseline(budget_s=12.0) -> dict:
+    ctx = oracle_sample_setup()
+    g = ctx[1]
+    times = [oracle_step(ctx)]
+    while sum(times) < budget_s and len(times) < 50:
+        times.append(oracle_step(ctx))
+    t = statistics.median(times)
+    return {"value": step_bytes(g) / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "host_cores_available": len(os.sched_getaffinity(0)),
+            "sample": f"the whole configs[1] step (128 blocks, stages 112/14/2, 2 appends of 8 tokens) inside two "
+                      f"160-block host pools instead of 2000-block ones; {len(times)} repetitions, median; "
+                      f"oracle.kv_migration.staged_migration as it stands (NumPy row copies, single thread)",
+            "ms_per_step": t * 1e3}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    ctx = oracle_sample_setup()
+    g = ctx[1]
+    for _ in range(min(args.warmup, 2)):
+        oracle_step(ctx)
+    steps = min(args.steps, 40)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(ctx)
+    dt = (time.perf_counter() - t0) / steps
+    val = step_bytes(g) / dt / 1e9
+    sample = ("configs[1] step (128 blocks, stages 112/14/2, appends 8+8) inside two 160-block host pools; "
+              f"{steps} timed steps (capped at 40 to bound the run)")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": min(args.warmup, 2), "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u16", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "pools": "2 x 160 host blocks (sample)", "note": "CPU oracle, host memory"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+    return 0
+
+
+# --------------------------------------------------------------------------------------------
+# the llx arm
+# --------------------------------------------------------------------------------------------
+class Workload:
+    """Two LLaMA-7B-shaped pools on the current device and the configs[1] request."""
+
+    def __init__(self, torch, llx, cfg="llama7b", num_blocks=None, src_blocks=None):
+        g = dict(synth.CONFIGS[cfg])
+        if num_blocks:
+            g["num_blocks"] = num_blocks
+        self.g, self.torch, self.llx = g, torch, llx
+        L, H, D, S = g["layers"], g["kv_heads"], g["head_dim"], g["block_size"]
+        self.nb_dst = g["num_blocks"]
+        self.nb_src = src_blocks or g["num_blocks"]
+        self.te = S * H * D
+        self.src_raw, self.src = self._pool(self.nb_src)
+        self.dst_raw, self.dst = self._pool(self.nb_dst)
+        # seeded synthetic fill on the device: fp16 U[-1,1) (input generation, not part of the path)
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(0)
+        flat = self.src_raw.view(torch.float16)
+        step = 1 << 28
+        for a in range(0, flat.numel(), step):
+            b = min(flat.numel(), a + step)
+            flat[a:b] = (torch.rand(b - a, generator=gen, device="cuda", dtype=torch.float32) * 2 - 1).half()
+        self.dst_raw.view(torch.int16).fill_(int(np.array(synth.SENTINEL_U16, np.uint16).view(np.int16)))
+        self.s_tab = synth.block_permutation(1, self.nb_src)[:128]
+        self.d_tab = synth.block_permutation(2, self.nb_dst)[:128]
+        te_tok = H * D
+        vals = np.empty((16, L, 2, te_tok), dtype=np.uint16)
+        for t in range(16):
+            for l in range(L):
+                for kv in range(2):
+                    vals[t, l, kv] = synth.append_values_f16(3, START_TOKENS + t, l, kv, te_tok)
+        self.append_host = torch.from_numpy(vals.view(np.int16)).pin_memory()
+        self.append_dev = self.append_host.cuda()
+        torch.cuda.synchronize()
+
+    def _pool(self, nb):
+        g, torch, llx = self.g, self.torch, self.llx
+        nbytes = llx.pool_bytes_for(g["layers"], g["kv_heads"], g["head_dim"], g["block_size"], llx.F16, nb)
+        raw = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        return raw, llx.pool_wrap(raw.data_ptr(), nbytes, g["layers"], g["kv_heads"], g["head_dim"], g["block_size"],
+                                  llx.F16, nb, keepalive=raw)
+
+    def step(self, stream, ev=None):
+        """One pass of the path: stage 0, append, stage 1, append, final stage — all enqueued on `stream`."""
+        llx, g = self.llx, self.g
+        tokens, m = START_TOKENS, 0
+        vptr = self.append_dev.data_ptr()
+        tok_bytes = g["layers"] * 2 * g["kv_heads"] * g["head_dim"] * 2
+        for k, n in enumerate(SCHEDULE):
+            if ev is not None and k == 0:
+                ev[0].record(stream)
+            llx.migrate_stage(self.src, self.s_tab[m:m + n], self.dst, self.d_tab[m:m + n], stream=stream)
+            if ev is not None and k == 0:
+                ev[1].record(stream)
+            m += n
+            if k < len(APPENDS):
+                llx.append_tokens(self.src, self.s_tab, tokens, tokens + APPENDS[k],
+                                  vptr + (tokens - START_TOKENS) * tok_bytes, stream=stream)
+                tokens += APPENDS[k]
+        return tokens
+
+
+def dist_setup(torch, n_gpus):
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    return world, rank, local
+
+
+def run_llx(args):
+    import torch
+
+    import paper_2406_03243_b200 as llx
+    from paper_2406_03243_b200 import replicas
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the llx path has no CPU fallback")
+    llx.load()
+    world, rank, local = dist_setup(torch, args.gpus)
+    peak, peak_src = measured_peak()
+
+    w = Workload(torch, llx)
+    g = w.g
+    assert llx.plan_stage(START_TOKENS + sum(APPENDS), sum(SCHEDULE[:-1]), g["block_size"], 2) == (SCHEDULE[-1], True)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    sampler = ClockSampler(local)
+    sampler.start()
+
+    # ---- device-resident throughput -----------------------------------------------------
+    for _ in range(args.warmup):
+        w.step(stream)
+    stream.synchronize()
+    pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    replicas.barrier()
+    torch.cuda.synchronize()
+    c0 = llx.counters()
+    tw0 = time.perf_counter()
+    e0.record(stream)
+    for k in range(args.steps):
+        w.step(stream, pairs[k])
+    e1.record(stream)
+    stream.synchronize()
+    tw1 = time.perf_counter()
+    replicas.barrier()
+    torch.cuda.synchronize()
+    c1 = llx.counters()
+    sampler.window(tw0, tw1)
+    ms_local = e0.elapsed_time(e1) / args.steps
+    ms_step = replicas.max_over_ranks(ms_local)
+    total_bytes = replicas.sum_over_ranks(step_bytes(g))
+    value = total_bytes / (ms_step * 1e-3) / 1e9
+    stage0_ms = statistics.mean(a.elapsed_time(b) for a, b in pairs)
+    stage0_bytes = 2 * SCHEDULE[0] * w.src.block_bytes
+    achieved = stage0_bytes / (stage0_ms * 1e-3) / 1e9
+    launches = c1["kernel_launches"] - c0["kernel_launches"]
+
+    # ---- end to end through pinned host buffers (block fusion path) -----------------------
+    n = sum(SCHEDULE)
+    stg_bytes = llx.staging_bytes(w.src, n)
+    pin = llx.PinnedStaging(stg_bytes)
+    e2e_steps = max(3, min(args.steps, 10))
+    for _ in range(2):
+        llx.pack(w.src, w.s_tab, pin.dev_alias, stg_bytes, stream=stream)
+        llx.unpack(pin.dev_alias, stg_bytes, w.dst, w.d_tab, stream=stream)
+    stream.synchronize()
+    replicas.barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        llx.pack(w.src, w.s_tab, pin.dev_alias, stg_bytes, stream=stream)       # device -> pinned host
+        llx.unpack(pin.dev_alias, stg_bytes, w.dst, w.d_tab, stream=stream)     # pinned host -> device
+        stream.synchronize()
+    t1 = time.perf_counter()
+    sampler.window(t0, t1)
+    e2e_ms = replicas.max_over_ranks((t1 - t0) * 1e3 / e2e_steps)
+    e2e_val = replicas.sum_over_ranks(2 * n * w.src.block_bytes) / (e2e_ms * 1e-3) / 1e9
+    pin.free()
+
+    # ---- final-stage downtime (S4): host wall clock around the C-ABI call + stream sync ----
+    downtime = measure_downtime(torch, llx, w, stream, reps=args.downtime_reps)
+    clocks = sampler.stop()
+
+    suite = None
+    if args.suite and world == 1:
+        suite = run_suite(torch, llx, w, stream, args)
+
+    if rank != 0:
+        return 0
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u16", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "shape": "L32 H32 D128 S16 fp16, 2 pools x 2000 blocks (15.6 GiB each)",
+                   "request": "128 scattered blocks (2048 tokens), stages 112/14/2, 8-token appends between stages",
+                   "bytes_per_step_rd_plus_wr": step_bytes(g), "parallelism": f"replicas x{world} (no collective)",
+                   "l2": "inputs larger than L2 (2.1 GB of traffic per step vs 126 MB L2), no flush needed",
+                   "copy_kernel": "bulk-async smem ring (llx_copy_bulk)" if llx.get_option(llx.OPT_COPY_KERNEL) in (0, 2) else "vec16"},
+        "pct_of_nominal_8TBps": 100.0 * value / world / NOMINAL_HBM_GBS,
+        "pct_of_measured_copy_peak": 100.0 * value / world / peak,
+        "downtime_us": downtime,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "kernel": "llx_copy_bulk (stage 0: 112 blocks)", "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": stage0_bytes, "avg_launch_ms": stage0_ms,
+                     "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS},
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": n * w.src.block_bytes,
+                "d2h_bytes_per_step": n * w.src.block_bytes, "ms_per_step": e2e_ms, "steps": e2e_steps,
+                "path": "llx_pack -> pinned host staging buffer -> llx_unpack (host wall clock incl. stream sync)"},
+        "gpu_launches": launches,
+        "clocks": clocks,
+        "paper_context": "Llumnix reports 20-30 ms downtime on A10 + 64 Gb/s Gloo (PAPER.md:287); no GB/s figure",
+    }
+    if args.no_cpu_baseline:
+        out["cpu_baseline"] = None
+    else:
+        out["cpu_baseline"] = cpu_baseline()
+    if suite is not None:
+        out["suite_file"] = suite
+    print(json.dumps(out))
+    return 0
+
+
+def measure_downtime(torch, llx, w, stream, reps=100):
+    """SURVEY.md §8(d) protocol: stages 0..N-2 done and synchronised, last append done ("source stops the
+    request"), then t0 -> llx_migrate_stage(final) -> cudaStreamSynchronize -> t1."""
+    import ctypes as C
+    lib = llx.lib()
+    g = w.g
+    n_final = SCHEDULE[-1]
+    m = sum(SCHEDULE[:-1])
+    s_ids = np.ascontiguousarray(w.s_tab[m:m + n_final], dtype=np.int32)
+    d_ids = np.ascontiguousarray(w.d_tab[m:m + n_final], dtype=np.int32)
+    sp = s_ids.ctypes.data_as(C.POINTER(C.c_int32))
+    dp = d_ids.ctypes.data_as(C.POINTER(C.c_int32))
+    sh, dh, st = w.src.handle, w.dst.handle, stream.cuda_stream
+    tok_bytes = g["layers"] * 2 * g["kv_heads"] * g["head_dim"] * 2
+    host_us, gpu_us = [], []
+    ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for rep in range(reps + 5):
+        tokens, mm = START_TOKENS, 0
+        for k, n in enumerate(SCHEDULE[:-1]):
+            llx.migrate_stage(w.src, w.s_tab[mm:mm + n], w.dst, w.d_tab[mm:mm + n], stream=stream)
+            mm += n
+            llx.append_tokens(w.src, w.s_tab, tokens, tokens + APPENDS[k],
+                              w.append_dev.data_ptr() + (tokens - START_TOKENS) * tok_bytes, stream=stream)
+            tokens += APPENDS[k]
+        stream.synchronize()
+        ea.record(stream)
+        t0 = time.perf_counter_ns()
+        rc = lib.llx_migrate_stage(sh, sp, dh, dp, n_final, st)
+        stream.synchronize()
+        t1 = time.perf_counter_ns()
+        assert rc == 0
+        # GPU duration measured on a second, untimed-by-host launch so that the events do not sit inside t0..t1
+        ea.record(stream)
+        lib.llx_migrate_stage(sh, sp, dh, dp, n_final, st)
+        eb.record(stream)
+        stream.synchronize()
+        if rep >= 5:
+            host_us.append((t1 - t0) / 1e3)
+            gpu_us.append(ea.elapsed_time(eb) * 1e3)
+    host_us.sort()
+    gpu_us.sort()
+    q = lambda v, p: v[min(len(v) - 1, int(p * len(v)))]
+    return {"final_stage_blocks": n_final, "final_stage_bytes_rd_plus_wr": 2 * n_final * w.src.block_bytes,
+            "host_median": q(host_us, 0.5), "host_p99": q(host_us, 0.99), "host_min": host_us[0],
+            "gpu_median": q(gpu_us, 0.5), "gpu_min": gpu_us[0], "reps": reps,
+            "definition": "host wall clock from entering llx_migrate_stage(final) to return of the stream "
+                          "synchronize; gpu_* = CUDA-event duration of the same launch repeated (L2-warm)"}
+
+
+def run_suite(torch, llx, w, stream, args):
+    from paper_2406_03243_b200 import suite
+    res = suite.run(torch, llx, w, stream)
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    path = os.path.join("gpurun_out", "suite.json")
+    with open(os.path.join(ROOT, path), "w") as f:
+        json.dump(res, f, indent=1)
+    for k, v in res.items():
+        print(json.dumps({k: v}), file=sys.stderr)
+    return path
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", choices=["llx", "reference"], default="llx")
+    ap.add_argument("--suite", action="store_true", help="also run the length sweep, 30B batch and interference configs")
+    ap.add_argument("--downtime-reps", type=int, default=100)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_llx(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

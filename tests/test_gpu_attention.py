@@ -14,8 +14,8 @@ TOL = 2e-3          # BASELINE.json north_star: "decode attention must agree wit
 SENT = synth.SENTINEL_U16
 
 # D=128 with 20 heads (a ragged head group: 16 + 4) and D=64 (Tiny's head_dim) with 6 heads (ragged warp)
-G128 = dict(layers=2, kv_heads=20, head_dim=128, block_size=16, elem_bytes=2, num_blocks=96)
-G64 = dict(layers=2, kv_heads=6, head_dim=64, block_size=16, elem_bytes=2, num_blocks=96)
+G128 = dict(layers=2, kv_heads=20, head_dim=128, block_size=16, elem_bytes=2, num_blocks=128)
+G64 = dict(layers=2, kv_heads=6, head_dim=64, block_size=16, elem_bytes=2, num_blocks=128)
 G64S = dict(layers=1, kv_heads=4, head_dim=64, block_size=5, elem_bytes=2, num_blocks=200)    # odd block size
 
 

@@ -176,8 +176,8 @@ def test_staged_with_appends_equals_oracle_and_single_shot(env):     # P4, S1, S
     values = lambda t, l, kv: synth.append_values_f16(3, t, l, kv, te_tok)
     tokens, m = 97, 0
     for k, (n, app) in enumerate([(5, 3), (2, 0)]):
-        plan_n, final = om.plan_stage(tokens, m, S, 2)
-        assert plan_n == n and final == (k == 1)
+        if k == 1:                                                   # S1: the library's planner names the final stage
+            assert llx.plan_stage(tokens, m, S, 2) == om.plan_stage(tokens, m, S, 2) == (n, True)
         llx.migrate_stage(src.pool, s_tab[m:m + n], dst.pool, d_tab[m:m + n])
         m += n
         if app:
