@@ -336,9 +336,11 @@ def run_llx(args):
     downtime = measure_downtime(torch, llx, w, stream, reps=args.downtime_reps)
     clocks = sampler.stop()
 
+    block_bytes = w.src.block_bytes
     suite = None
     if args.suite and world == 1:
-        suite = run_suite(torch, llx, w, stream, args)
+        del w
+        suite = run_suite(torch, llx, stream)
 
     if rank != 0:
         return 0
@@ -358,8 +360,8 @@ def run_llx(args):
                      "traffic": None, "kernel": "llx_copy_bulk (stage 0: 112 blocks)", "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": stage0_bytes, "avg_launch_ms": stage0_ms,
                      "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS},
-        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": n * w.src.block_bytes,
-                "d2h_bytes_per_step": n * w.src.block_bytes, "ms_per_step": e2e_ms, "steps": e2e_steps,
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": n * block_bytes,
+                "d2h_bytes_per_step": n * block_bytes, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "path": "llx_pack -> pinned host staging buffer -> llx_unpack (host wall clock incl. stream sync)"},
         "gpu_launches": launches,
         "clocks": clocks,
@@ -424,9 +426,9 @@ def measure_downtime(torch, llx, w, stream, reps=100):
                           "synchronize; gpu_* = CUDA-event duration of the same launch repeated (L2-warm)"}
 
 
-def run_suite(torch, llx, w, stream, args):
+def run_suite(torch, llx, stream):
     from paper_2406_03243_b200 import suite
-    res = suite.run(torch, llx, w, stream)
+    res = suite.run(torch, llx, stream)
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     path = os.path.join("gpurun_out", "suite.json")
     with open(os.path.join(ROOT, path), "w") as f:

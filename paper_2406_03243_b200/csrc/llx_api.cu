@@ -59,7 +59,7 @@ int elem_bytes_of(llx_dtype d) {
 
 // ---- options / counters -------------------------------------------------------------------
 std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
-    g_opt_attn_split{0};
+    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
 // ---- device properties (cached per device) ------------------------------------------------
@@ -184,16 +184,16 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     const int slices = 2 * layers;
 
     if (kern == 2) {
+        // Tuned on B200 (profiles/r01_copy_sweep.md): 2 CTAs per SM, each one ring of 4 x 8 KiB, every ring
+        // streaming a CONTIGUOUS range of chunks.  More bytes in flight than ~64 KiB per SM lowers DRAM efficiency.
         if (nstages <= 0) nstages = 4;
-        if (chunk <= 0) {
-            chunk = 16384;
-            // short stages (the final one): smaller chunks so that every SM gets several units
-            while (chunk > 4096 && total_bytes / chunk < (long long)di->sm_count * 8) chunk /= 2;
-        }
+        if (chunk <= 0) chunk = 8192;
         if (chunk > tile_bytes) chunk = tile_bytes;
         chunk &= ~15ll;
-        threads = 32;
-        smem = 128 + (size_t)nstages * chunk;
+        int rings = (int)g_opt_rings.load();
+        if (rings <= 0) rings = 1;
+        threads = 32 * rings;
+        smem = (((size_t)rings * nstages * 8 + 127) & ~(size_t)127) + (size_t)rings * nstages * chunk;
         if ((long long)smem > di->max_smem_optin) return fail(LLX_ERR_INVALID_ARG, "ring of %d x %lld bytes exceeds shared memory", nstages, chunk);
     } else {
         if (chunk <= 0) chunk = 256 * 16 * 4;
@@ -206,14 +206,14 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
 
     if (kern == 2) {
         int per_sm = (int)((size_t)di->max_smem_optin / (smem + 1024));  // 1 KiB per-CTA reservation
+        if (per_sm > 2) per_sm = 2;
         if (per_sm < 1) per_sm = 1;
-        if (per_sm > 16) per_sm = 16;
         grid = di->sm_count * per_sm;
     } else {
         grid = di->sm_count * 8;
     }
     const long long cap = g_opt_max_ctas.load();
-    if (cap > 0 && grid > cap) grid = (int)cap;
+    if (cap > 0) grid = (int)cap;  // explicit grid: the throttle (fewer CTAs) or an experiment (more)
     if (grid > units) grid = (int)units;
 
     CopyArgs a;
@@ -231,6 +231,8 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     a.chunks_per_tile = (int)cpt;
     a.slices = slices;
     a.total_units = (int)units;
+    a.blocked_order = (int)g_opt_order.load();
+    a.l2_hint = (int)g_opt_l2hint.load();
 
     static thread_local IdPack pack;  // 2 KiB; only the first n entries are meaningful
     const bool byval = n <= g_opt_byval.load();
@@ -664,6 +666,18 @@ llx_status llx_set_option(llx_option opt, long long v) {
             if (v < 0 || (v % 8) != 0) break;
             g_opt_attn_split = v;
             return LLX_OK;
+        case LLX_OPT_UNIT_ORDER:
+            if (v < 0 || v > 1) break;
+            g_opt_order = v;
+            return LLX_OK;
+        case LLX_OPT_L2_HINT:
+            if (v < 0 || v > 3) break;
+            g_opt_l2hint = v;
+            return LLX_OK;
+        case LLX_OPT_RINGS_PER_CTA:
+            if (v < 0 || v > 8) break;
+            g_opt_rings = v;
+            return LLX_OK;
     }
     return fail(LLX_ERR_INVALID_ARG, "option %d: bad value %lld", (int)opt, v);
 }
@@ -675,6 +689,9 @@ long long llx_get_option(llx_option opt) {
         case LLX_OPT_RING_STAGES: return g_opt_stages;
         case LLX_OPT_IDS_BY_VALUE_MAX: return g_opt_byval;
         case LLX_OPT_ATTN_SPLIT_TOKENS: return g_opt_attn_split;
+        case LLX_OPT_UNIT_ORDER: return g_opt_order;
+        case LLX_OPT_L2_HINT: return g_opt_l2hint;
+        case LLX_OPT_RINGS_PER_CTA: return g_opt_rings;
     }
     return -1;
 }

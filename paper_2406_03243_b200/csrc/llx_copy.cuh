@@ -45,6 +45,8 @@ struct CopyArgs {
     int chunks_per_tile;
     int slices;       // 2*layers
     int total_units;  // n * slices * chunks_per_tile
+    int blocked_order;  // 0: worker w takes units w, w+W, ...; 1: worker w takes a contiguous range
+    int l2_hint;        // bit0: loads L2::evict_first, bit1: stores L2::evict_first (bulk kernel)
 };
 
 __device__ __forceinline__ uint4 ld_stream16(const void* p) {
@@ -89,7 +91,13 @@ __device__ __forceinline__ UnitAddr unit_addr(const CopyArgs& a, int slice, int 
 template <bool BYVAL, int UNROLL>
 __global__ void __launch_bounds__(256, 8) llx_copy_vec16(const CopyArgs a, const __grid_constant__ IdPack ids) {
     const int lane = threadIdx.x & 31;
-    for (int u = blockIdx.x; u < a.total_units; u += gridDim.x) {
+    int u_begin = blockIdx.x, u_end = a.total_units, u_step = gridDim.x;
+    if (a.blocked_order) {
+        u_begin = (int)((long long)blockIdx.x * a.total_units / gridDim.x);
+        u_end = (int)((long long)(blockIdx.x + 1) * a.total_units / gridDim.x);
+        u_step = 1;
+    }
+    for (int u = u_begin; u < u_end; u += u_step) {
         int i, slice, c;
         unit_coords(a, u, i, slice, c);
         int item_s = i, item_d = i;
@@ -162,6 +170,23 @@ __device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src_smem, uint32_t 
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src_smem), "r"(bytes)
                  : "memory");
 }
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            dst_smem),
+        "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_hint(void* dst, uint32_t src_smem, uint32_t bytes, uint64_t pol) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dst),
+                 "r"(src_smem), "r"(bytes), "l"(pol)
+                 : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void bulk_wait_read() {
@@ -190,10 +215,23 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
     const int ring = blockIdx.x * rings_per_cta + warp;
     const int nrings = gridDim.x * rings_per_cta;
     if (ring >= a.total_units) return;
-    const int K = (a.total_units - ring + nrings - 1) / nrings;  // units of this ring
+    int K, u0, ustep;  // this ring handles units u0, u0+ustep, ... (K of them)
+    if (a.blocked_order) {
+        // balanced contiguous ranges: ring r takes [r*T/W, (r+1)*T/W)
+        u0 = (int)((long long)ring * a.total_units / nrings);
+        ustep = 1;
+        K = (int)((long long)(ring + 1) * a.total_units / nrings) - u0;
+        if (K <= 0) return;
+    } else {
+        u0 = ring;
+        ustep = nrings;
+        K = (a.total_units - ring + nrings - 1) / nrings;
+    }
+    const uint64_t pol = policy_evict_first();
+    const bool hint_ld = a.l2_hint & 1, hint_st = a.l2_hint & 2;
 
     auto addr_of = [&](int k) -> UnitAddr {
-        int u = ring + k * nrings;
+        int u = u0 + k * ustep;
         int i, slice, c;
         unit_coords(a, u, i, slice, c);
         int item_s = i, item_d = i;
@@ -205,7 +243,10 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
         const int s = k % nstages;
         UnitAddr ua = addr_of(k);
         mbar_expect_tx(bar0 + s * 8, (uint32_t)ua.len);
-        bulk_g2s(buf0 + s * a.chunk_bytes, ua.src, (uint32_t)ua.len, bar0 + s * 8);
+        if (hint_ld)
+            bulk_g2s_hint(buf0 + s * a.chunk_bytes, ua.src, (uint32_t)ua.len, bar0 + s * 8, pol);
+        else
+            bulk_g2s(buf0 + s * a.chunk_bytes, ua.src, (uint32_t)ua.len, bar0 + s * 8);
     };
 
     const int pre = K < nstages ? K : nstages;
@@ -214,7 +255,10 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
         const int s = k % nstages;
         mbar_wait(bar0 + s * 8, (uint32_t)((k / nstages) & 1));
         UnitAddr ua = addr_of(k);
-        bulk_s2g(ua.dst, buf0 + s * a.chunk_bytes, (uint32_t)ua.len);
+        if (hint_st)
+            bulk_s2g_hint(ua.dst, buf0 + s * a.chunk_bytes, (uint32_t)ua.len, pol);
+        else
+            bulk_s2g(ua.dst, buf0 + s * a.chunk_bytes, (uint32_t)ua.len);
         bulk_commit();
         // refill the stage whose store was committed one iteration ago: allowing the newest
         // group to stay pending keeps one store and nstages-1 loads in flight per ring

@@ -1,0 +1,334 @@
+"""The other BASELINE.json configs, measured through the C-ABI: configs[2] length sweep, configs[3] 30B batch,
+configs[4] interference with a decode step + staging through pinned host memory.  Called by `bench.py --suite`.
+
+Everything here is measurement harness: pools are torch allocations (memory + streams only), inputs come
+from `synth`, all timing is CUDA events on the launching stream (or host wall clock where stated)."""
+from __future__ import annotations
+
+import gc
+import statistics
+import time
+
+import numpy as np
+
+import synth
+
+SENT_I16 = int(np.array(synth.SENTINEL_U16, np.uint16).view(np.int16))
+
+
+def _events(torch, n):
+    return [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+
+
+def _time_stream(torch, stream, fn, reps=10, warm=2, before=None):
+    for _ in range(warm):
+        fn()
+    stream.synchronize()
+    evs = _events(torch, reps)
+    for a, b in evs:
+        if before is not None:
+            before()
+        a.record(stream)
+        fn()
+        b.record(stream)
+    stream.synchronize()
+    ts = sorted(a.elapsed_time(b) for a, b in evs)
+    return {"median_ms": statistics.median(ts), "min_ms": ts[0]}
+
+
+def _free(torch):
+    gc.collect()
+    torch.cuda.empty_cache()
+    return torch.cuda.mem_get_info()[0]
+
+
+class Pools:
+    def __init__(self, torch, llx, g, nb_src, nb_dst, fill_src=True):
+        self.torch, self.llx, self.g = torch, llx, dict(g)
+        self.src_raw, self.src = self._pool(nb_src)
+        self.dst_raw, self.dst = self._pool(nb_dst)
+        if fill_src:
+            gen = torch.Generator(device="cuda")
+            gen.manual_seed(0)
+            flat = self.src_raw.view(torch.float16)
+            step = 1 << 28
+            for a in range(0, flat.numel(), step):
+                b = min(flat.numel(), a + step)
+                flat[a:b] = (torch.rand(b - a, generator=gen, device="cuda", dtype=torch.float32) * 2 - 1).half()
+        self.dst_raw.view(torch.int16).fill_(SENT_I16)
+        torch.cuda.synchronize()
+
+    def _pool(self, nb):
+        g, torch, llx = self.g, self.torch, self.llx
+        nbytes = llx.pool_bytes_for(g["layers"], g["kv_heads"], g["head_dim"], g["block_size"], llx.F16, nb)
+        raw = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        return raw, llx.pool_wrap(raw.data_ptr(), nbytes, g["layers"], g["kv_heads"], g["head_dim"], g["block_size"],
+                                  llx.F16, nb, keepalive=raw)
+
+    def view(self, raw, nb):
+        g = self.g
+        return raw.view(self.torch.int16).view(g["layers"], 2, nb, g["block_size"] * g["kv_heads"] * g["head_dim"])
+
+
+# ---- configs[2]: length sweep ------------------------------------------------------------------
+def length_sweep(torch, llx, p: Pools, stream, nb):
+    import ctypes as C
+    lib = llx.lib()
+    out = []
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    for tokens in (256, 512, 1024, 2048, 4096, 8192):
+        n = tokens // p.g["block_size"]
+        s_tab = synth.block_permutation(40 + n, nb)[:n]
+        d_tab = synth.block_permutation(50 + n, nb)[:n]
+        by = 2 * n * p.src.block_bytes
+        single = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=stream))
+        first = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab[:n - 2], p.dst, d_tab[:n - 2], stream=stream))
+        # final stage: cold (L2 flushed by a 512 MiB write on the same stream), GPU time by events, host time by wall clock
+        with torch.cuda.stream(stream):
+            fin = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab[n - 2:], p.dst, d_tab[n - 2:], stream=stream),
+                               reps=20, before=lambda: flush.fill_(1))
+        s_ids = np.ascontiguousarray(s_tab[n - 2:], dtype=np.int32)
+        d_ids = np.ascontiguousarray(d_tab[n - 2:], dtype=np.int32)
+        sp, dp = s_ids.ctypes.data_as(C.POINTER(C.c_int32)), d_ids.ctypes.data_as(C.POINTER(C.c_int32))
+        host = []
+        for _ in range(60):
+            llx.migrate_stage(p.src, s_tab[:n - 2], p.dst, d_tab[:n - 2], stream=stream)   # the long stage evicts L2
+            stream.synchronize()
+            t0 = time.perf_counter_ns()
+            lib.llx_migrate_stage(p.src.handle, sp, p.dst.handle, dp, 2, stream.cuda_stream)
+            stream.synchronize()
+            host.append((time.perf_counter_ns() - t0) / 1e3)
+        host.sort()
+        out.append({"tokens": tokens, "blocks": n, "payload_MiB": n * p.src.block_bytes / 2**20,
+                    "single_shot_GBps": by / single["median_ms"] / 1e6, "single_shot_ms": single["median_ms"],
+                    "stage0_GBps": 2 * (n - 2) * p.src.block_bytes / first["median_ms"] / 1e6,
+                    "final_stage_gpu_us_cold": fin["median_ms"] * 1e3,
+                    "final_stage_host_us_median": host[len(host) // 2], "final_stage_host_us_p99": host[-1],
+                    "blocking_copy_downtime_us": single["median_ms"] * 1e3})
+    return out
+
+
+# ---- reference points on the same data ---------------------------------------
+def reference_points(torch, llx, p: Pools, stream, nb):
+    n = 128
+    s_tab = synth.block_permutation(1, nb)[:n]
+    d_tab = synth.block_permutation(2, nb)[:n]
+    by = 2 * n * p.src.block_bytes
+    res = {}
+    a = torch.empty(n * p.src.block_bytes, dtype=torch.uint8, device="cuda")
+    b = torch.empty_like(a)
+    with torch.cuda.stream(stream):
+        t = _time_stream(torch, stream, lambda: b.copy_(a))
+        res["torch_contiguous_copy_GBps"] = by / t["median_ms"] / 1e6
+        sv, dv = p.view(p.src_raw, nb), p.view(p.dst_raw, nb)
+        si = torch.from_numpy(s_tab.astype(np.int64)).cuda()
+        di = torch.from_numpy(d_tab.astype(np.int64)).cuda()
+
+        def index_form():
+            for l in range(p.g["layers"]):
+                for kv in range(2):
+                    dv[l, kv].index_copy_(0, di, sv[l, kv].index_select(0, si))
+        t = _time_stream(torch, stream, index_form, reps=5, warm=1)
+        res["torch_index_select_index_copy_GBps"] = by / t["median_ms"] / 1e6
+
+        def per_tile_memcpy():     # "many small messages": one cudaMemcpyAsync per 128 KiB tile
+            for i in range(n):
+                for l in range(p.g["layers"]):
+                    for kv in range(2):
+                        dv[l, kv, int(d_tab[i])].copy_(sv[l, kv, int(s_tab[i])])
+        t = _time_stream(torch, stream, per_tile_memcpy, reps=2, warm=1)
+        res["per_tile_memcpy_loop_GBps"] = by / t["median_ms"] / 1e6
+        res["per_tile_memcpy_loop_ms"] = t["median_ms"]
+    t = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=stream))
+    res["llx_migrate_stage_GBps"] = by / t["median_ms"] / 1e6
+    for kern, name in ((1, "llx_vec16_kernel_GBps"), (2, "llx_bulk_kernel_GBps")):
+        with llx.options(copy_kernel=kern):
+            t = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=stream))
+        res[name] = by / t["median_ms"] / 1e6
+    # device-buffer block fusion (pack then unpack through HBM)
+    stg = torch.empty(llx.staging_bytes(p.src, n), dtype=torch.uint8, device="cuda")
+    t = _time_stream(torch, stream, lambda: llx.pack(p.src, s_tab, stg.data_ptr(), stg.numel(), stream=stream))
+    res["llx_pack_device_GBps"] = by / t["median_ms"] / 1e6
+    t = _time_stream(torch, stream, lambda: llx.unpack(stg.data_ptr(), stg.numel(), p.dst, d_tab, stream=stream))
+    res["llx_unpack_device_GBps"] = by / t["median_ms"] / 1e6
+    return res
+
+
+# ---- configs[4] second half: staging through pinned host memory --------------------------------
+def staging_host(torch, llx, p: Pools, stream, nb):
+    n = 128
+    s_tab = synth.block_permutation(1, nb)[:n]
+    d_tab = synth.block_permutation(2, nb)[:n]
+    nbytes = llx.staging_bytes(p.src, n)
+    pin = llx.PinnedStaging(nbytes)
+    res = {"payload_GiB": nbytes / 2**30}
+    # host-link peak: plain copy-engine transfers of the same size, each direction
+    dev = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    host = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    with torch.cuda.stream(stream):
+        t = _time_stream(torch, stream, lambda: host.copy_(dev, non_blocking=True), reps=5, warm=1)
+        res["link_peak_d2h_GBps"] = nbytes / t["min_ms"] / 1e6
+        t = _time_stream(torch, stream, lambda: dev.copy_(host, non_blocking=True), reps=5, warm=1)
+        res["link_peak_h2d_GBps"] = nbytes / t["min_ms"] / 1e6
+    del host
+    t = _time_stream(torch, stream, lambda: llx.pack(p.src, s_tab, pin.dev_alias, nbytes, stream=stream), reps=5, warm=1)
+    res["llx_pack_to_pinned_host_GBps"] = nbytes / t["median_ms"] / 1e6
+    t = _time_stream(torch, stream, lambda: llx.unpack(pin.dev_alias, nbytes, p.dst, d_tab, stream=stream), reps=5, warm=1)
+    res["llx_unpack_from_pinned_host_GBps"] = nbytes / t["median_ms"] / 1e6
+    res["pack_frac_of_link_peak"] = res["llx_pack_to_pinned_host_GBps"] / res["link_peak_d2h_GBps"]
+    res["unpack_frac_of_link_peak"] = res["llx_unpack_from_pinned_host_GBps"] / res["link_peak_h2d_GBps"]
+    # alternative: pack into a DEVICE buffer, then one copy-engine transfer (and back)
+    stg = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    hbuf = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+
+    def via_ce():
+        llx.pack(p.src, s_tab, stg.data_ptr(), nbytes, stream=stream)
+        with torch.cuda.stream(stream):
+            hbuf.copy_(stg, non_blocking=True)
+            stg.copy_(hbuf, non_blocking=True)
+        llx.unpack(stg.data_ptr(), nbytes, p.dst, d_tab, stream=stream)
+    t = _time_stream(torch, stream, via_ce, reps=5, warm=1)
+    res["device_pack_plus_copy_engine_roundtrip_ms"] = t["median_ms"]
+
+    def direct():
+        llx.pack(p.src, s_tab, pin.dev_alias, nbytes, stream=stream)
+        llx.unpack(pin.dev_alias, nbytes, p.dst, d_tab, stream=stream)
+    t = _time_stream(torch, stream, direct, reps=5, warm=1)
+    res["zero_copy_pack_unpack_roundtrip_ms"] = t["median_ms"]
+    pin.free()
+    return res
+
+
+# ---- configs[3]: LLaMA-30B batch --------------------------------------------------------------
+def batch_30b(torch, llx, stream):
+    g = dict(synth.CONFIGS["llama30b"])
+    lens, nblk, seed_used = synth.batch_request_blocks(0, 64, g["block_size"], g["num_blocks"])
+    total = int(nblk.sum())
+    block_bytes = 2 * g["layers"] * g["block_size"] * g["kv_heads"] * g["head_dim"] * 2
+    nb = g["num_blocks"]
+    free = _free(torch)
+    while 2 * nb * block_bytes > free - (6 << 30) and nb > total:
+        nb -= 100
+    if nb < total:
+        return {"skipped": f"not enough device memory for {total} blocks per pool"}
+    p = Pools(torch, llx, g, nb, nb)
+    s_ids = synth.block_permutation(1, nb)[:total]
+    d_ids = synth.block_permutation(2, nb)[:total]
+    off = np.concatenate([[0], np.cumsum(nblk)]).astype(np.int32)
+    by = 2 * total * block_bytes
+    t = _time_stream(torch, stream, lambda: llx.migrate_batch(p.src, p.dst, off, s_ids, d_ids, stream=stream), reps=5, warm=1)
+
+    def sequential():
+        for r in range(64):
+            llx.migrate_stage(p.src, s_ids[off[r]:off[r + 1]], p.dst, d_ids[off[r]:off[r + 1]], stream=stream)
+    ts = _time_stream(torch, stream, sequential, reps=3, warm=1)
+    res = {"requests": 64, "length_seed_used": int(seed_used), "total_blocks": total, "pool_blocks_used": nb,
+           "pool_blocks_config": g["num_blocks"], "payload_GiB": total * block_bytes / 2**30,
+           "mean_tokens": float(lens.mean()), "max_tokens": int(lens.max()), "min_tokens": int(lens.min()),
+           "one_launch_ms": t["median_ms"], "one_launch_GBps": by / t["median_ms"] / 1e6,
+           "sequential_64_launches_ms": ts["median_ms"], "sequential_GBps": by / ts["median_ms"] / 1e6}
+    del p
+    _free(torch)
+    return res
+
+
+# ---- configs[4] first half: interference with a decode step -----------------------------------
+def interference(torch, llx, stream_mig_unused):
+    g = dict(synth.CONFIGS["llama7b"])
+    L, H, D, S = g["layers"], g["kv_heads"], g["head_dim"], g["block_size"]
+    B = 32
+    ctx = synth.context_lengths(4, B, 128, 4096)
+    need = [-(-int(c) // S) for c in ctx]
+    nb_src = B * 256 + 128 + 128          # reading A12: worst case for any seed, + the migrating request + slack
+    nb_dst = g["num_blocks"]
+    block_bytes = 2 * L * S * H * D * 2
+    if (nb_src + nb_dst) * block_bytes > _free(torch) - (4 << 30):
+        return {"skipped": "not enough device memory"}
+    p = Pools(torch, llx, g, nb_src, nb_dst)
+    perm = synth.block_permutation(6, nb_src)
+    MB = 256
+    bt = np.zeros((B, MB), dtype=np.int32)
+    pos = 0
+    for b, n in enumerate(need):
+        bt[b, :n] = perm[pos:pos + n]
+        pos += n
+    mig_src = perm[pos:pos + 128]
+    mig_dst = synth.block_permutation(2, nb_dst)[:128]
+    q = torch.from_numpy(synth.queries_f16(5, B, H, D).view(np.int16)).cuda()
+    o = torch.zeros_like(q)
+    d_bt = torch.from_numpy(bt).cuda()
+    d_ctx = torch.from_numpy(ctx).cuda()
+    scale = 1.0 / float(np.sqrt(D))
+    lo, hi = torch.cuda.Stream.priority_range()            # (least, greatest) = (0, -N)
+    s_dec = torch.cuda.Stream(priority=hi)
+    s_mig = torch.cuda.Stream(priority=lo)
+    kv_bytes_step = int(ctx.sum()) * 2 * H * D * 2 * L
+
+    def decode_step():
+        for l in range(L):
+            llx.decode_attention(p.src, l, q.data_ptr(), o.data_ptr(), d_bt.data_ptr(), d_ctx.data_ptr(), B, MB, scale,
+                                 stream=s_dec)
+
+    def migrate():
+        llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig)
+
+    decode_step()
+    torch.cuda.synchronize()
+    alone = _time_stream(torch, s_dec, decode_step, reps=10, warm=2)
+    mig_alone = _time_stream(torch, s_mig, migrate, reps=10, warm=2)
+    mig_bytes = 2 * 128 * block_bytes
+
+    def with_migration(n_mig, max_ctas):
+        times, mig_ms = [], []
+        for _ in range(8):
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ma, mb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with llx.options(max_ctas=max_ctas):
+                a.record(s_dec)
+                ma.record(s_mig)
+                for _ in range(n_mig):
+                    migrate()
+                mb.record(s_mig)
+                decode_step()
+                b.record(s_dec)
+            torch.cuda.synchronize()
+            times.append(a.elapsed_time(b))
+            mig_ms.append(ma.elapsed_time(mb))
+        return statistics.median(times), statistics.median(mig_ms)
+
+    res = {"batch": B, "ctx_tokens_total": int(ctx.sum()), "src_pool_blocks": nb_src, "dst_pool_blocks": nb_dst,
+           "decode_step_alone_ms": alone["median_ms"],
+           "decode_attention_GBps": kv_bytes_step / alone["median_ms"] / 1e6,
+           "migration_alone_ms": mig_alone["median_ms"], "migration_alone_GBps": mig_bytes / mig_alone["median_ms"] / 1e6,
+           "cases": []}
+    loop_n = max(2, int(alone["median_ms"] / mig_alone["median_ms"]) + 2)
+    for label, n_mig, cap in [("one 2048-token migration at step start, full width", 1, 0),
+                              ("migration looped for the whole step, full width", loop_n, 0),
+                              ("looped, throttled to 64 CTAs", loop_n, 64),
+                              ("looped, throttled to 32 CTAs", max(2, loop_n // 2), 32),
+                              ("looped, throttled to 16 CTAs", max(2, loop_n // 4), 16),
+                              ("looped, throttled to 8 CTAs", max(2, loop_n // 8), 8),
+                              ("looped, throttled to 4 CTAs", max(2, loop_n // 16), 4)]:
+        t, m = with_migration(n_mig, cap)
+        res["cases"].append({"case": label, "migrations": n_mig, "max_ctas": cap, "decode_step_ms": t,
+                             "slowdown_pct": 100.0 * (t / alone["median_ms"] - 1.0),
+                             "migration_GBps_while_overlapped": n_mig * mig_bytes / m / 1e6})
+    del p
+    _free(torch)
+    return res
+
+
+def run(torch, llx, stream):
+    res = {}
+    g = synth.CONFIGS["llama7b"]
+    nb = g["num_blocks"]
+    p = Pools(torch, llx, g, nb, nb)
+    res["length_sweep_llama7b"] = length_sweep(torch, llx, p, stream, nb)
+    res["reference_points_2048tok"] = reference_points(torch, llx, p, stream, nb)
+    res["staging_pinned_host_2048tok"] = staging_host(torch, llx, p, stream, nb)
+    del p
+    _free(torch)
+    res["interference_decode_batch32"] = interference(torch, llx, stream)
+    res["batch_llama30b_64req"] = batch_30b(torch, llx, stream)
+    return res
