@@ -176,7 +176,9 @@ typedef enum {
     LLX_OPT_ATTN_SPLIT_TOKENS = 5, /* tokens per KV split of decode attention (multiple of 8; 0 = auto) */
     LLX_OPT_UNIT_ORDER = 6,     /* 0: worker w copies chunks w, w+W, w+2W, ... (striped); 1: a contiguous range each */
     LLX_OPT_L2_HINT = 7,        /* bulk kernel: bit0 loads, bit1 stores carry an L2::evict_first policy */
-    LLX_OPT_RINGS_PER_CTA = 8   /* bulk kernel: independent smem rings (warps) per CTA (0 = auto) */
+    LLX_OPT_RINGS_PER_CTA = 8,  /* bulk kernel: independent smem rings (warps) per CTA (0 = auto) */
+    LLX_OPT_PDL = 9             /* 1 (default): launch copy/append kernels with programmatic stream serialization so that
+                                   a kernel's prologue overlaps the previous kernel's tail; results are unchanged */
 } llx_option;
 /* Process-wide; takes effect for later calls.  Returns LLX_ERR_INVALID_ARG for a bad value. */
 llx_status llx_set_option(llx_option opt, long long value);

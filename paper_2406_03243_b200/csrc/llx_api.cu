@@ -59,7 +59,7 @@ int elem_bytes_of(llx_dtype d) {
 
 // ---- options / counters -------------------------------------------------------------------
 std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
-    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0};
+    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
 // ---- device properties (cached per device) ------------------------------------------------
@@ -158,6 +158,24 @@ llx_status check_unique(const int32_t* ids, long long n, int num_blocks) {
 }
 size_t pool_bytes(const llx_pool* p) { return (size_t)p->num_blocks * 2 * p->layers * (size_t)p->tile_bytes; }
 
+// ---- launch helper: programmatic dependent launch (PDL) lets the next kernel of the stream become
+// resident and run its prologue while the previous one drains; the kernels order their memory
+// accesses themselves with griddepcontrol.wait, so stream semantics are unchanged. ----------------
+template <typename... KArgs, typename... Args>
+cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = g_opt_pdl.load() ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ---- copy launch -----------------------------------------------------------------------------
 struct Side {
     const unsigned char* base;
@@ -249,18 +267,19 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         g_id_uploads++;
     }
 
+    cudaError_t e;
     if (kern == 2) {
         if (byval)
-            llx_copy_bulk<true><<<grid, threads, smem, st>>>(a, pack, nstages);
+            e = launch_k(llx_copy_bulk<true>, grid, threads, smem, st, a, pack, nstages);
         else
-            llx_copy_bulk<false><<<grid, threads, smem, st>>>(a, pack, nstages);
+            e = launch_k(llx_copy_bulk<false>, grid, threads, smem, st, a, pack, nstages);
     } else {
         if (byval)
-            llx_copy_vec16<true, 4><<<grid, 256, 0, st>>>(a, pack);
+            e = launch_k(llx_copy_vec16<true, 4>, grid, 256, 0, st, a, pack);
         else
-            llx_copy_vec16<false, 4><<<grid, 256, 0, st>>>(a, pack);
+            e = launch_k(llx_copy_vec16<false, 4>, grid, 256, 0, st, a, pack);
     }
-    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaGetLastError();
     if (slot) cudaEventRecord(slot->ev, st);
     if (e != cudaSuccess) return cuda_fail(e, "copy kernel launch");
     g_launches++;
@@ -558,16 +577,17 @@ llx_status llx_append_tokens(llx_pool* p, const int32_t* table, int table_len, i
     cudaStream_t st = (cudaStream_t)stream;
     IdSlot* slot = nullptr;
     const int grid = ntok * a.slices;
+    cudaError_t e;
     if (ntok <= kIdsByValueCap) {
         memcpy(pack.src, tb.data(), ntok * sizeof(int32_t));
-        llx_append_kernel<true><<<grid, 128, 0, st>>>(a, pack);
+        e = launch_k(llx_append_kernel<true>, grid, 128, 0, st, a, pack);
     } else {
         int32_t* dev_ids = nullptr;
         if ((rc = ring_stage(tb.data(), ntok, nullptr, 0, st, &dev_ids, &slot)) != LLX_OK) return rc;
         a.tok_block = dev_ids;
-        llx_append_kernel<false><<<grid, 128, 0, st>>>(a, pack);
+        e = launch_k(llx_append_kernel<false>, grid, 128, 0, st, a, pack);
     }
-    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaGetLastError();
     if (slot) cudaEventRecord(slot->ev, st);
     if (e != cudaSuccess) return cuda_fail(e, "append kernel launch");
     g_launches++;
@@ -678,6 +698,10 @@ llx_status llx_set_option(llx_option opt, long long v) {
             if (v < 0 || v > 8) break;
             g_opt_rings = v;
             return LLX_OK;
+        case LLX_OPT_PDL:
+            if (v < 0 || v > 1) break;
+            g_opt_pdl = v;
+            return LLX_OK;
     }
     return fail(LLX_ERR_INVALID_ARG, "option %d: bad value %lld", (int)opt, v);
 }
@@ -692,6 +716,7 @@ long long llx_get_option(llx_option opt) {
         case LLX_OPT_UNIT_ORDER: return g_opt_order;
         case LLX_OPT_L2_HINT: return g_opt_l2hint;
         case LLX_OPT_RINGS_PER_CTA: return g_opt_rings;
+        case LLX_OPT_PDL: return g_opt_pdl;
     }
     return -1;
 }

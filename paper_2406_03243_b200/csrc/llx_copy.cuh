@@ -62,6 +62,11 @@ __device__ __forceinline__ void st_stream16(void* p, const uint4& v) {
                  : "memory");
 }
 
+// Programmatic dependent launch: let the next kernel of the stream start its prologue now, and
+// wait for the previous kernel's memory before touching global memory.  No-ops without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait_prior_grids() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 struct UnitAddr {
     const unsigned char* src;
     unsigned char* dst;
@@ -91,6 +96,8 @@ __device__ __forceinline__ UnitAddr unit_addr(const CopyArgs& a, int slice, int 
 template <bool BYVAL, int UNROLL>
 __global__ void __launch_bounds__(256, 8) llx_copy_vec16(const CopyArgs a, const __grid_constant__ IdPack ids) {
     const int lane = threadIdx.x & 31;
+    pdl_launch_dependents();
+    pdl_wait_prior_grids();
     int u_begin = blockIdx.x, u_end = a.total_units, u_step = gridDim.x;
     if (a.blocked_order) {
         u_begin = (int)((long long)blockIdx.x * a.total_units / gridDim.x);
@@ -211,6 +218,8 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
     for (int s = 0; s < nstages; ++s) mbar_init(bar0 + s * 8, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    pdl_launch_dependents();
+    pdl_wait_prior_grids();
 
     const int ring = blockIdx.x * rings_per_cta + warp;
     const int nrings = gridDim.x * rings_per_cta;
@@ -283,6 +292,8 @@ struct AppendArgs {
 };
 template <bool BYVAL>
 __global__ void __launch_bounds__(128) llx_append_kernel(const AppendArgs a, const __grid_constant__ IdPack ids) {
+    pdl_launch_dependents();
+    pdl_wait_prior_grids();
     const int u = blockIdx.x;  // (tok, slice)
     const int slice = u % a.slices;
     const int k = u / a.slices;
@@ -291,7 +302,16 @@ __global__ void __launch_bounds__(128) llx_append_kernel(const AppendArgs a, con
     const uint4* s = reinterpret_cast<const uint4*>(a.values + ((long long)k * a.slices + slice) * a.token_bytes);
     uint4* d = reinterpret_cast<uint4*>(a.pool_base + slice * a.slice_stride + (long long)blk * a.tile_bytes +
                                         (long long)slot * a.token_bytes);
-    for (int v = threadIdx.x; v < (a.token_bytes >> 4); v += blockDim.x) d[v] = s[v];
+    const int nvec = a.token_bytes >> 4;
+    for (int v0 = threadIdx.x; v0 < nvec; v0 += 128 * 4) {  // 4 independent 16-byte loads in flight per thread
+        uint4 r[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (v0 + j * 128 < nvec) r[j] = ld_stream16(s + v0 + j * 128);
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (v0 + j * 128 < nvec) d[v0 + j * 128] = r[j];
+    }
 }
 
 __global__ void __launch_bounds__(256) llx_fill_u16_kernel(uint4* p, long long nvec, uint32_t word) {
