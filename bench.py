@@ -100,6 +100,19 @@ class ClockSampler:
                 "reasons": reasons, "samples_in_timed_regions": len(inside), "samples": len(self.samples)}
 
 
+def profiled_traffic(launch="stage0_112_blocks"):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed ncu capture."""
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "r01_copy_bulk_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["launch"] == launch:
+                    return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+    except Exception:  # noqa: BLE001
+        pass
+    return None
+
+
 def measured_peak():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -366,7 +379,7 @@ def run_llx(args):
         "pct_of_measured_copy_peak": 100.0 * value / world / peak,
         "downtime_us": downtime,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": "llx_copy_bulk (stage 0: 112 blocks)", "peak_source": peak_src,
+                     "traffic": profiled_traffic(), "traffic_source": "profiles/r01_copy_bulk_traffic.csv (ncu --set full)", "kernel": "llx_copy_bulk (stage 0: 112 blocks)", "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": stage0_bytes, "avg_launch_ms": stage0_ms,
                      "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS},
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": n * block_bytes,
