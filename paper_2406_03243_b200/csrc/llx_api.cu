@@ -648,13 +648,15 @@ llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* q, 
     const int hpw = 32 / (D / 8);
     const int head_groups = (H + kAttnWarps * hpw - 1) / (kAttnWarps * hpw);
     dim3 grid1(max_splits, head_groups, B), grid2(H, B);
+    cudaError_t e;
     if (D == 128) {
-        llx_attn_partial<128><<<grid1, kAttnWarps * 32, 0, st>>>(a);
-        llx_attn_merge<128><<<grid2, 128, 0, st>>>(a);
+        e = launch_k(llx_attn_partial<128>, grid1, kAttnWarps * 32, 0, st, a);
+        if (e == cudaSuccess) e = launch_k(llx_attn_merge<128>, grid2, 128, 0, st, a);
     } else {
-        llx_attn_partial<64><<<grid1, kAttnWarps * 32, 0, st>>>(a);
-        llx_attn_merge<64><<<grid2, 64, 0, st>>>(a);
+        e = launch_k(llx_attn_partial<64>, grid1, kAttnWarps * 32, 0, st, a);
+        if (e == cudaSuccess) e = launch_k(llx_attn_merge<64>, grid2, 64, 0, st, a);
     }
+    if (e != cudaSuccess) return cuda_fail(e, "attention kernel launch");
     LLX_CUDA(cudaGetLastError());
     g_launches += 2;
     return LLX_OK;

@@ -55,10 +55,27 @@ __device__ __forceinline__ void unpack8(const uint4& u, float* f) {
     }
 }
 
+// two fp32 FMAs per instruction (sm_100 FFMA2): c += a * b on float2
+__device__ __forceinline__ void ffma2(float2& c, const float2 a, const float2 b) {
+    unsigned long long ra, rb, rc;
+    asm("mov.b64 %0, {%1,%2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(rc) : "f"(c.x), "f"(c.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(rc) : "l"(ra), "l"(rb));
+    asm("mov.b64 {%0,%1}, %2;" : "=f"(c.x), "=f"(c.y) : "l"(rc));
+}
+
+__device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 template <int D>
-__global__ void __launch_bounds__(kAttnWarps * 32) llx_attn_partial(const AttnArgs a) {
-    constexpr int LPH = D / 8;    // lanes per head
-    constexpr int HPW = 32 / LPH; // heads per warp
+__global__ void __launch_bounds__(kAttnWarps * 32, 2) llx_attn_partial(const AttnArgs a) {
+    constexpr int LPH = D / 8;     // lanes per head
+    constexpr int HPW = 32 / LPH;  // heads per warp
+    constexpr int G = kAttnGroup;  // 8 tokens per group
+    static_assert(G == 8 && LPH >= 8, "the transposed reduction below assumes 8 tokens and >= 8 lanes per head");
+    griddep_launch();
+    griddep_wait();
     const int b = blockIdx.z;
     const int split = blockIdx.x;
     const int ctx = a.ctx_lens[b];
@@ -67,74 +84,124 @@ __global__ void __launch_bounds__(kAttnWarps * 32) llx_attn_partial(const AttnAr
     const int t1 = min(ctx, t0 + a.split_tokens);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int li = lane % LPH;  // lane within its head
     const int h = (blockIdx.y * kAttnWarps + warp) * HPW + lane / LPH;
-    const int dl = (lane % LPH) * 8;  // first dim owned by this lane
+    const int dl = li * 8;  // first dim owned by this lane
     const bool head_ok = h < a.H;
     const int hc = head_ok ? h : a.H - 1;  // clamp: idle lanes still take part in the shuffles
 
-    float qf[8];
-    unpack8(*reinterpret_cast<const uint4*>(a.q + ((long long)b * a.H + hc) * D + dl), qf);
+    float2 q2[4];
+    {
+        const uint4 qu = *reinterpret_cast<const uint4*>(a.q + ((long long)b * a.H + hc) * D + dl);
+        const __half2* qh = reinterpret_cast<const __half2*>(&qu);
 #pragma unroll
-    for (int j = 0; j < 8; ++j) qf[j] *= a.scale_log2;
-
+        for (int j = 0; j < 4; ++j) {
+            q2[j] = __half22float2(qh[j]);
+            q2[j].x *= a.scale_log2;
+            q2[j].y *= a.scale_log2;
+        }
+    }
     const long long row_bytes = (long long)a.H * D * 2;  // one token, all heads
     const long long lane_off = ((long long)hc * D + dl) * 2;
     const int32_t* bt = a.block_tables + (long long)b * a.max_blocks;
 
-    float m = -INFINITY, l = 0.f, acc[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+    // halving offsets of the transposed reduction: after them this lane owns the score of token g_own
+    constexpr int O1 = LPH / 2, O2 = LPH / 4, O3 = LPH / 8;
+    const bool b1 = li & O1, b2 = li & O2, b3 = li & O3;
+    const int g_own = (b1 ? 4 : 0) + (b2 ? 2 : 0) + (b3 ? 1 : 0);
 
-    for (int t = t0; t < t1; t += kAttnGroup) {
-        uint4 kq[kAttnGroup], vq[kAttnGroup];
+    float m = -INFINITY, l = 0.f;  // l: partial over the tokens this lane owned
+    float2 acc[4];
 #pragma unroll
-        for (int g = 0; g < kAttnGroup; ++g) {
-            const int tt = t + g;
-            if (tt < t1) {
-                const int blk = __ldg(bt + tt / a.S);
-                const long long off = blk * a.tile_bytes + (long long)(tt % a.S) * row_bytes + lane_off;
-                kq[g] = ld_kv16(a.k_base + off);
-                vq[g] = ld_kv16(a.v_base + off);
-            } else {
-                kq[g] = make_uint4(0, 0, 0, 0);
-                vq[g] = make_uint4(0, 0, 0, 0);
+    for (int j = 0; j < 4; ++j) acc[j] = make_float2(0.f, 0.f);
+
+    int bi = t0 / a.S;
+    int blk_first = bi * a.S;  // token index of slot 0 of block bi
+    for (; blk_first < t1; ++bi, blk_first += a.S) {
+        const int blk = __ldg(bt + bi);
+        const int s_lo = max(t0 - blk_first, 0);
+        const int s_hi = min(t1 - blk_first, a.S);
+        const unsigned char* kb = a.k_base + blk * a.tile_bytes + lane_off;
+        const unsigned char* vb = a.v_base + blk * a.tile_bytes + lane_off;
+        for (int s0 = s_lo; s0 < s_hi; s0 += G) {
+            const int nvalid = s_hi - s0;  // >= 1; tokens g >= nvalid are masked
+            uint4 kq[G], vq[G];
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                if (g < nvalid) {
+                    const long long off = (long long)(s0 + g) * row_bytes;
+                    kq[g] = ld_kv16(kb + off);
+                    vq[g] = ld_kv16(vb + off);
+                } else {
+                    kq[g] = make_uint4(0, 0, 0, 0);
+                    vq[g] = make_uint4(0, 0, 0, 0);
+                }
+            }
+            // partial dot products of this lane's 8 dims with each of the 8 tokens
+            float d[G];
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                const __half2* kh = reinterpret_cast<const __half2*>(&kq[g]);
+                float2 s2 = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) ffma2(s2, q2[j], __half22float2(kh[j]));
+                d[g] = s2.x + s2.y;
+            }
+            // transposed reduction over the LPH lanes: 4 + 2 + 1 shuffles instead of 8 * log2(LPH)
+            float k4[4], k2[2], sc;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float mine = b1 ? d[4 + j] : d[j], other = b1 ? d[j] : d[4 + j];
+                k4[j] = mine + __shfl_xor_sync(0xffffffffu, other, O1);
+            }
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const float mine = b2 ? k4[2 + j] : k4[j], other = b2 ? k4[j] : k4[2 + j];
+                k2[j] = mine + __shfl_xor_sync(0xffffffffu, other, O2);
+            }
+            {
+                const float mine = b3 ? k2[1] : k2[0], other = b3 ? k2[0] : k2[1];
+                sc = mine + __shfl_xor_sync(0xffffffffu, other, O3);
+            }
+#pragma unroll
+            for (int o = O3 / 2; o >= 1; o >>= 1) sc += __shfl_xor_sync(0xffffffffu, sc, o);
+            if (g_own >= nvalid) sc = -INFINITY;
+            // online softmax: group max over the head's lanes, one exp2 per lane
+            float gmax = sc;
+            gmax = fmaxf(gmax, __shfl_xor_sync(0xffffffffu, gmax, O1));
+            gmax = fmaxf(gmax, __shfl_xor_sync(0xffffffffu, gmax, O2));
+            gmax = fmaxf(gmax, __shfl_xor_sync(0xffffffffu, gmax, O3));
+            const float m_new = fmaxf(m, gmax);  // finite: token s0 is valid
+            const float corr = exp2f(m - m_new);
+            const float p_own = exp2f(sc - m_new);
+            l = l * corr + p_own;
+            m = m_new;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                acc[j].x *= corr;
+                acc[j].y *= corr;
+            }
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                // the lane (within the head) that owns token g: bits of g placed at O1, O2, O3
+                const int src = ((g & 4) ? O1 : 0) + ((g & 2) ? O2 : 0) + ((g & 1) ? O3 : 0);
+                const float p = __shfl_sync(0xffffffffu, p_own, src, LPH);
+                const float2 p2 = make_float2(p, p);
+                const __half2* vh = reinterpret_cast<const __half2*>(&vq[g]);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) ffma2(acc[j], p2, __half22float2(vh[j]));
             }
         }
-        float s[kAttnGroup];
-        float gmax = -INFINITY;
-#pragma unroll
-        for (int g = 0; g < kAttnGroup; ++g) {
-            float kf[8];
-            unpack8(kq[g], kf);
-            float d = 0.f;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) d = fmaf(qf[j], kf[j], d);
-#pragma unroll
-            for (int o = LPH / 2; o >= 1; o >>= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
-            s[g] = (t + g < t1) ? d : -INFINITY;
-            gmax = fmaxf(gmax, s[g]);
-        }
-        const float m_new = fmaxf(m, gmax);  // finite: the group holds at least one valid token
-        const float corr = exp2f(m - m_new);
-        l *= corr;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) acc[j] *= corr;
-#pragma unroll
-        for (int g = 0; g < kAttnGroup; ++g) {
-            const float p = exp2f(s[g] - m_new);
-            float vf[8];
-            unpack8(vq[g], vf);
-            l += p;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) acc[j] = fmaf(p, vf[j], acc[j]);
-        }
-        m = m_new;
     }
+    // l: sum over the distinct token owners (lanes differing in the O1, O2, O3 bits)
+    l += __shfl_xor_sync(0xffffffffu, l, O1);
+    l += __shfl_xor_sync(0xffffffffu, l, O2);
+    l += __shfl_xor_sync(0xffffffffu, l, O3);
     if (!head_ok) return;
     float* o = a.part + (((long long)b * a.H + h) * a.max_splits + split) * (D + 4);
-    *reinterpret_cast<float4*>(o + dl) = make_float4(acc[0], acc[1], acc[2], acc[3]);
-    *reinterpret_cast<float4*>(o + dl + 4) = make_float4(acc[4], acc[5], acc[6], acc[7]);
-    if ((lane % LPH) == 0) {
+    *reinterpret_cast<float4*>(o + dl) = make_float4(acc[0].x, acc[0].y, acc[1].x, acc[1].y);
+    *reinterpret_cast<float4*>(o + dl + 4) = make_float4(acc[2].x, acc[2].y, acc[3].x, acc[3].y);
+    if (li == 0) {
         o[D] = m;
         o[D + 1] = l;
     }
@@ -143,6 +210,8 @@ __global__ void __launch_bounds__(kAttnWarps * 32) llx_attn_partial(const AttnAr
 // grid (H, B), D threads: out[b][h][d] = sum_s 2^(m_s-M) acc_s[d] / sum_s 2^(m_s-M) l_s
 template <int D>
 __global__ void __launch_bounds__(D) llx_attn_merge(const AttnArgs a) {
+    griddep_launch();
+    griddep_wait();
     const int h = blockIdx.x, b = blockIdx.y, d = threadIdx.x;
     const int ctx = a.ctx_lens[b];
     const int ns = (ctx + a.split_tokens - 1) / a.split_tokens;

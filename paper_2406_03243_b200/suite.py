@@ -332,3 +332,38 @@ def run(torch, llx, stream):
     res["interference_decode_batch32"] = interference(torch, llx, stream)
     res["batch_llama30b_64req"] = batch_30b(torch, llx, stream)
     return res
+
+
+def main():
+    """python -m paper_2406_03243_b200.suite [--only NAME]   (NAME: sweep | refs | staging | interference | batch)"""
+    import argparse
+    import json
+
+    import torch
+
+    import paper_2406_03243_b200 as llx
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--only", default="")
+    args = ap.parse_args()
+    llx.load()
+    stream = torch.cuda.Stream()
+    if not args.only:
+        print(json.dumps(run(torch, llx, stream), indent=1))
+        return 0
+    g = synth.CONFIGS["llama7b"]
+    nb = g["num_blocks"]
+    if args.only == "interference":
+        res = interference(torch, llx, stream)
+    elif args.only == "batch":
+        res = batch_30b(torch, llx, stream)
+    else:
+        p = Pools(torch, llx, g, nb, nb)
+        fn = {"sweep": length_sweep, "refs": reference_points, "staging": staging_host}[args.only]
+        res = fn(torch, llx, p, stream, nb)
+    print(json.dumps(res, indent=1))
+    return 0
+
+
+if __name__ == "__main__":
+    import sys
+    sys.exit(main())
