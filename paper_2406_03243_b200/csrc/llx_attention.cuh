@@ -69,12 +69,11 @@ __device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 template <int D>
-__global__ void __launch_bounds__(kAttnWarps * 32, 2) llx_attn_partial(const AttnArgs a) {
+__global__ void __maxnreg__(112) llx_attn_partial(const AttnArgs a) {
     constexpr int LPH = D / 8;     // lanes per head
     constexpr int HPW = 32 / LPH;  // heads per warp
     constexpr int G = kAttnGroup;  // 8 tokens per group
     static_assert(G == 8 && LPH >= 8, "the transposed reduction below assumes 8 tokens and >= 8 lanes per head");
-    griddep_launch();
     griddep_wait();
     const int b = blockIdx.z;
     const int split = blockIdx.x;
@@ -193,6 +192,10 @@ __global__ void __launch_bounds__(kAttnWarps * 32, 2) llx_attn_partial(const Att
             }
         }
     }
+    // dependents may start launching now: triggering only after the main loop keeps waiting CTAs of the next
+    // kernel from occupying registers while this kernel still needs both of its CTAs per SM (measured: an early
+    // trigger costs +25 % under a concurrent full-width migration)
+    griddep_launch();
     // l: sum over the distinct token owners (lanes differing in the O1, O2, O3 bits)
     l += __shfl_xor_sync(0xffffffffu, l, O1);
     l += __shfl_xor_sync(0xffffffffu, l, O2);

@@ -295,10 +295,11 @@ def interference(torch, llx, stream_mig_unused):
             torch.cuda.synchronize()
             times.append(a.elapsed_time(b))
             mig_ms.append(ma.elapsed_time(mb))
-        return statistics.median(times), statistics.median(mig_ms)
+        return statistics.median(times), statistics.median(mig_ms), times
 
+    iso_ms, _, _ = with_migration(0, 0)      # the baseline of every case: one isolated step, measured the same way
     res = {"batch": B, "ctx_tokens_total": int(ctx.sum()), "src_pool_blocks": nb_src, "dst_pool_blocks": nb_dst,
-           "decode_step_alone_ms": alone["median_ms"],
+           "decode_step_alone_ms": alone["median_ms"], "decode_step_alone_isolated_ms": iso_ms,
            "decode_attention_GBps": kv_bytes_step / alone["median_ms"] / 1e6,
            "migration_alone_ms": mig_alone["median_ms"], "migration_alone_GBps": mig_bytes / mig_alone["median_ms"] / 1e6,
            "cases": []}
@@ -310,10 +311,11 @@ def interference(torch, llx, stream_mig_unused):
                               ("looped, throttled to 16 CTAs", max(2, loop_n // 4), 16),
                               ("looped, throttled to 8 CTAs", max(2, loop_n // 8), 8),
                               ("looped, throttled to 4 CTAs", max(2, loop_n // 16), 4)]:
-        t, m = with_migration(n_mig, cap)
-        res["cases"].append({"case": label, "migrations": n_mig, "max_ctas": cap, "decode_step_ms": t,
-                             "slowdown_pct": 100.0 * (t / alone["median_ms"] - 1.0),
-                             "migration_GBps_while_overlapped": n_mig * mig_bytes / m / 1e6})
+        t, m, all_t = with_migration(n_mig, cap)
+        res["cases"].append({"case": label, "migrations": n_mig, "max_ctas": cap, "decode_step_ms": t, "decode_step_ms_all_reps": all_t,
+                             "slowdown_pct": 100.0 * (t / iso_ms - 1.0),
+                             "migration_GBps_while_overlapped": n_mig * mig_bytes / m / 1e6,
+                             "ideal_shared_bandwidth_slowdown_pct": 100.0 * min(n_mig * mig_bytes, mig_bytes * t / max(m, 1e-9) * n_mig) / kv_bytes_step})
     del p
     _free(torch)
     return res
