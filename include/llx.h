@@ -177,8 +177,11 @@ typedef enum {
     LLX_OPT_UNIT_ORDER = 6,     /* 0: worker w copies chunks w, w+W, w+2W, ... (striped); 1: a contiguous range each */
     LLX_OPT_L2_HINT = 7,        /* bulk kernel: bit0 loads, bit1 stores carry an L2::evict_first policy */
     LLX_OPT_RINGS_PER_CTA = 8,  /* bulk kernel: independent smem rings (warps) per CTA (0 = auto) */
-    LLX_OPT_PDL = 9             /* 1 (default): launch copy/append kernels with programmatic stream serialization so that
+    LLX_OPT_PDL = 9,            /* 1 (default): launch copy/append kernels with programmatic stream serialization so that
                                    a kernel's prologue overlaps the previous kernel's tail; results are unchanged */
+    LLX_OPT_BANDWIDTH_GBPS = 10 /* bandwidth budget of device<->device copies in GB/s, read + written (0 = unlimited):
+                                   one paced ring per SM instead of a few full-speed CTAs, so that a co-running
+                                   decode step loses the same small share on every SM (<= 1 %) */
 } llx_option;
 /* Process-wide; takes effect for later calls.  Returns LLX_ERR_INVALID_ARG for a bad value. */
 llx_status llx_set_option(llx_option opt, long long value);

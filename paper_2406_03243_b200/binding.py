@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(HERE, "libllx.so")
 
 F16, BF16, U8 = 0, 1, 2
 (OPT_COPY_KERNEL, OPT_MAX_CTAS, OPT_CHUNK_BYTES, OPT_RING_STAGES, OPT_IDS_BY_VALUE_MAX, OPT_ATTN_SPLIT_TOKENS,
- OPT_UNIT_ORDER, OPT_L2_HINT, OPT_RINGS_PER_CTA, OPT_PDL) = range(10)
+ OPT_UNIT_ORDER, OPT_L2_HINT, OPT_RINGS_PER_CTA, OPT_PDL, OPT_BANDWIDTH_GBPS) = range(11)
 
 _vp, _i, _sz, _i32p = C.c_void_p, C.c_int, C.c_size_t, C.POINTER(C.c_int32)
 
@@ -256,7 +256,7 @@ def options(**kw):
     names = dict(copy_kernel=OPT_COPY_KERNEL, max_ctas=OPT_MAX_CTAS, chunk_bytes=OPT_CHUNK_BYTES,
                  ring_stages=OPT_RING_STAGES, ids_by_value_max=OPT_IDS_BY_VALUE_MAX,
                  attn_split_tokens=OPT_ATTN_SPLIT_TOKENS, unit_order=OPT_UNIT_ORDER, l2_hint=OPT_L2_HINT,
-                 rings_per_cta=OPT_RINGS_PER_CTA, pdl=OPT_PDL)
+                 rings_per_cta=OPT_RINGS_PER_CTA, pdl=OPT_PDL, bandwidth_gbps=OPT_BANDWIDTH_GBPS)
     old = {k: get_option(names[k]) for k in kw}
     try:
         for k, v in kw.items():

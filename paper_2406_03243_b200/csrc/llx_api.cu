@@ -59,7 +59,7 @@ int elem_bytes_of(llx_dtype d) {
 
 // ---- options / counters -------------------------------------------------------------------
 std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
-    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1};
+    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
 // ---- device properties (cached per device) ------------------------------------------------
@@ -193,6 +193,11 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     // kernel choice: the bulk-async ring for device<->device, the LDG/STG kernel when a side is host memory
     long long kern = g_opt_kernel.load();
     if (kern == 0) kern = (src.host_memory || dst.host_memory) ? 1 : 2;
+    // Bandwidth budget: paced register-staged copies, no shared memory.  Measured
+    // on B200: a co-resident CTA that holds > ~6 KB of shared memory shrinks the L1 of its SM and slows a
+    // bandwidth-bound decode kernel by 30 %, and a few full-speed CTAs turn their SMs into stragglers.
+    const long long budget = g_opt_budget.load();
+    if (budget > 0) kern = 1;
 
     const long long total_bytes = n * 2 * layers * tile_bytes;
     long long chunk = g_opt_chunk.load();
@@ -214,7 +219,20 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         smem = (((size_t)rings * nstages * 8 + 127) & ~(size_t)127) + (size_t)rings * nstages * chunk;
         if ((long long)smem > di->max_smem_optin) return fail(LLX_ERR_INVALID_ARG, "ring of %d x %lld bytes exceeds shared memory", nstages, chunk);
     } else {
-        if (chunk <= 0) chunk = 256 * 16 * 4;
+        if (budget > 0) {  // ~2 GB/s (rd+wr) per warp keeps the loads latency-bound and gentle; spread over all SMs
+            long long warps = (budget + 1) / 2;
+            int ctas_per_sm = (int)((warps + (long long)di->sm_count * 8 - 1) / ((long long)di->sm_count * 8));
+            if (ctas_per_sm < 1) ctas_per_sm = 1;
+            if (ctas_per_sm > 8) ctas_per_sm = 8;
+            grid = di->sm_count * ctas_per_sm;
+            long long wpc = (warps + grid - 1) / grid;
+            if (wpc < 1) wpc = 1;
+            if (wpc > 8) wpc = 8;
+            threads = (int)wpc * 32;
+            chunk = (long long)threads * 16 * 4;
+        } else if (chunk <= 0) {
+            chunk = 256 * 16 * 4;
+        }
         if (chunk > tile_bytes) chunk = tile_bytes;
         chunk &= ~15ll;
     }
@@ -227,12 +245,21 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         if (per_sm > 2) per_sm = 2;
         if (per_sm < 1) per_sm = 1;
         grid = di->sm_count * per_sm;
-    } else {
+    } else if (budget <= 0) {
         grid = di->sm_count * 8;
     }
     const long long cap = g_opt_max_ctas.load();
     if (cap > 0) grid = (int)cap;  // explicit grid: the throttle (fewer CTAs) or an experiment (more)
-    if (grid > units) grid = (int)units;
+    {
+        const long long workers_per_cta = (kern == 2) ? threads / 32 : 1;  // rings per CTA
+        const long long need = (units + workers_per_cta - 1) / workers_per_cta;
+        if (grid > need) grid = (int)need;
+    }
+    long long pace_ns = 0;
+    if (budget > 0) {
+        pace_ns = (long long)grid * 2 * chunk / budget;  // per CTA; bytes/ns == GB/s, read + written
+        if (pace_ns > 1000000000ll) pace_ns = 1000000000ll;
+    }
 
     CopyArgs a;
     a.src_base = src.base;
@@ -251,6 +278,7 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     a.total_units = (int)units;
     a.blocked_order = (int)g_opt_order.load();
     a.l2_hint = (int)g_opt_l2hint.load();
+    a.pace_ns = (int)pace_ns;
 
     static thread_local IdPack pack;  // 2 KiB; only the first n entries are meaningful
     const bool byval = n <= g_opt_byval.load();
@@ -275,9 +303,9 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
             e = launch_k(llx_copy_bulk<false>, grid, threads, smem, st, a, pack, nstages);
     } else {
         if (byval)
-            e = launch_k(llx_copy_vec16<true, 4>, grid, 256, 0, st, a, pack);
+            e = launch_k(llx_copy_vec16<true, 4>, grid, threads, 0, st, a, pack);
         else
-            e = launch_k(llx_copy_vec16<false, 4>, grid, 256, 0, st, a, pack);
+            e = launch_k(llx_copy_vec16<false, 4>, grid, threads, 0, st, a, pack);
     }
     if (e == cudaSuccess) e = cudaGetLastError();
     if (slot) cudaEventRecord(slot->ev, st);
@@ -704,6 +732,10 @@ llx_status llx_set_option(llx_option opt, long long v) {
             if (v < 0 || v > 1) break;
             g_opt_pdl = v;
             return LLX_OK;
+        case LLX_OPT_BANDWIDTH_GBPS:
+            if (v < 0 || v > 100000) break;
+            g_opt_budget = v;
+            return LLX_OK;
     }
     return fail(LLX_ERR_INVALID_ARG, "option %d: bad value %lld", (int)opt, v);
 }
@@ -719,6 +751,7 @@ long long llx_get_option(llx_option opt) {
         case LLX_OPT_L2_HINT: return g_opt_l2hint;
         case LLX_OPT_RINGS_PER_CTA: return g_opt_rings;
         case LLX_OPT_PDL: return g_opt_pdl;
+        case LLX_OPT_BANDWIDTH_GBPS: return g_opt_budget;
     }
     return -1;
 }

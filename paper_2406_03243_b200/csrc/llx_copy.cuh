@@ -47,6 +47,7 @@ struct CopyArgs {
     int total_units;  // n * slices * chunks_per_tile
     int blocked_order;  // 0: worker w takes units w, w+W, ...; 1: worker w takes a contiguous range
     int l2_hint;        // bit0: loads L2::evict_first, bit1: stores L2::evict_first (bulk kernel)
+    int pace_ns;        // bulk kernel: minimum time between two chunks of one ring (0 = unthrottled)
 };
 
 __device__ __forceinline__ uint4 ld_stream16(const void* p) {
@@ -66,6 +67,12 @@ __device__ __forceinline__ void st_stream16(void* p, const uint4& v) {
 // wait for the previous kernel's memory before touching global memory.  No-ops without the attribute.
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait_prior_grids() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 
 struct UnitAddr {
     const unsigned char* src;
@@ -96,8 +103,10 @@ __device__ __forceinline__ UnitAddr unit_addr(const CopyArgs& a, int slice, int 
 template <bool BYVAL, int UNROLL>
 __global__ void __launch_bounds__(256, 8) llx_copy_vec16(const CopyArgs a, const __grid_constant__ IdPack ids) {
     const int lane = threadIdx.x & 31;
+    const int nt = blockDim.x;
     pdl_launch_dependents();
     pdl_wait_prior_grids();
+    unsigned long long deadline = a.pace_ns > 0 ? global_timer_ns() : 0ull;
     int u_begin = blockIdx.x, u_end = a.total_units, u_step = gridDim.x;
     if (a.blocked_order) {
         u_begin = (int)((long long)blockIdx.x * a.total_units / gridDim.x);
@@ -127,17 +136,26 @@ __global__ void __launch_bounds__(256, 8) llx_copy_vec16(const CopyArgs a, const
         const int nvec = ua.len >> 4;
         const uint4* __restrict__ s = reinterpret_cast<const uint4*>(ua.src);
         uint4* __restrict__ d = reinterpret_cast<uint4*>(ua.dst);
-        for (int v0 = threadIdx.x; v0 < nvec; v0 += 256 * UNROLL) {
+        for (int v0 = threadIdx.x; v0 < nvec; v0 += nt * UNROLL) {
             uint4 r[UNROLL];
 #pragma unroll
             for (int j = 0; j < UNROLL; ++j) {
-                int v = v0 + j * 256;
+                int v = v0 + j * nt;
                 if (v < nvec) r[j] = ld_stream16(s + v);
             }
 #pragma unroll
             for (int j = 0; j < UNROLL; ++j) {
-                int v = v0 + j * 256;
+                int v = v0 + j * nt;
                 if (v < nvec) st_stream16(d + v, r[j]);
+            }
+        }
+        if (a.pace_ns > 0) {  // bandwidth budget: the CTA starts its next chunk only at its next deadline
+            deadline += (unsigned long long)a.pace_ns;
+            unsigned long long now = global_timer_ns();
+            while (now < deadline) {
+                const unsigned long long left = deadline - now;
+                __nanosleep(left > 2000 ? 2000u : (unsigned)left);
+                now = global_timer_ns();
             }
         }
     }
@@ -223,7 +241,6 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
 
     const int ring = blockIdx.x * rings_per_cta + warp;
     const int nrings = gridDim.x * rings_per_cta;
-    if (ring >= a.total_units) return;
     int K, u0, ustep;  // this ring handles units u0, u0+ustep, ... (K of them)
     if (a.blocked_order) {
         // balanced contiguous ranges: ring r takes [r*T/W, (r+1)*T/W)
@@ -232,12 +249,14 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
         K = (int)((long long)(ring + 1) * a.total_units / nrings) - u0;
         if (K <= 0) return;
     } else {
+        if (ring >= a.total_units) return;
         u0 = ring;
         ustep = nrings;
         K = (a.total_units - ring + nrings - 1) / nrings;
     }
     const uint64_t pol = policy_evict_first();
     const bool hint_ld = a.l2_hint & 1, hint_st = a.l2_hint & 2;
+    unsigned long long deadline = a.pace_ns > 0 ? global_timer_ns() : 0ull;
 
     auto addr_of = [&](int k) -> UnitAddr {
         int u = u0 + k * ustep;
@@ -269,6 +288,15 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
         else
             bulk_s2g(ua.dst, buf0 + s * a.chunk_bytes, (uint32_t)ua.len);
         bulk_commit();
+        if (a.pace_ns > 0) {  // bandwidth budget: this ring may start its next chunk only at its next deadline
+            deadline += (unsigned long long)a.pace_ns;
+            unsigned long long now = global_timer_ns();
+            while (now < deadline) {
+                const unsigned long long left = deadline - now;
+                __nanosleep(left > 2000 ? 2000u : (unsigned)left);
+                now = global_timer_ns();
+            }
+        }
         // refill the stage whose store was committed one iteration ago: allowing the newest
         // group to stay pending keeps one store and nstages-1 loads in flight per ring
         if (k >= 1 && k - 1 + nstages < K) {

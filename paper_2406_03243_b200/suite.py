@@ -278,13 +278,13 @@ def interference(torch, llx, stream_mig_unused):
     mig_alone = _time_stream(torch, s_mig, migrate, reps=10, warm=2)
     mig_bytes = 2 * 128 * block_bytes
 
-    def with_migration(n_mig, max_ctas):
+    def with_migration(n_mig, max_ctas, budget=0):
         times, mig_ms = [], []
         for _ in range(8):
             torch.cuda.synchronize()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ma, mb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            with llx.options(max_ctas=max_ctas):
+            with llx.options(max_ctas=max_ctas, bandwidth_gbps=budget):
                 a.record(s_dec)
                 ma.record(s_mig)
                 for _ in range(n_mig):
@@ -304,18 +304,25 @@ def interference(torch, llx, stream_mig_unused):
            "migration_alone_ms": mig_alone["median_ms"], "migration_alone_GBps": mig_bytes / mig_alone["median_ms"] / 1e6,
            "cases": []}
     loop_n = max(2, int(alone["median_ms"] / mig_alone["median_ms"]) + 2)
-    for label, n_mig, cap in [("one 2048-token migration at step start, full width", 1, 0),
-                              ("migration looped for the whole step, full width", loop_n, 0),
-                              ("looped, throttled to 64 CTAs", loop_n, 64),
-                              ("looped, throttled to 32 CTAs", max(2, loop_n // 2), 32),
-                              ("looped, throttled to 16 CTAs", max(2, loop_n // 4), 16),
-                              ("looped, throttled to 8 CTAs", max(2, loop_n // 8), 8),
-                              ("looped, throttled to 4 CTAs", max(2, loop_n // 16), 4)]:
-        t, m, all_t = with_migration(n_mig, cap)
-        res["cases"].append({"case": label, "migrations": n_mig, "max_ctas": cap, "decode_step_ms": t, "decode_step_ms_all_reps": all_t,
-                             "slowdown_pct": 100.0 * (t / iso_ms - 1.0),
+    step_s = alone["median_ms"] * 1e-3
+
+    def n_for(gbps):      # migrations needed to keep the copy stream busy for the whole decode step
+        return max(1, int(gbps * 1e9 * step_s * 1.6 / mig_bytes) + 1)
+    cases = [("one 2048-token migration at step start, full speed", 1, 0, 0),
+             ("migration looped for the whole step, full speed", loop_n, 0, 0)]
+    cases += [(f"looped, {c} full-speed CTAs (LLX_OPT_MAX_CTAS)", n_for(c * 33), c, 0) for c in (32, 16, 8, 4)]
+    cases += [(f"looped, paced to {bw} GB/s over all SMs (LLX_OPT_BANDWIDTH_GBPS)", n_for(bw), 0, bw)
+              for bw in (1600, 800, 400, 200, 100, 65, 20)]
+    for label, n_mig, cap, bw in cases:
+        t, m, all_t = with_migration(n_mig, cap, bw)
+        res["cases"].append({"case": label, "migrations": n_mig, "max_ctas": cap, "bandwidth_budget_GBps": bw,
+                             "decode_step_ms": t, "slowdown_pct": 100.0 * (t / iso_ms - 1.0),
                              "migration_GBps_while_overlapped": n_mig * mig_bytes / m / 1e6,
-                             "ideal_shared_bandwidth_slowdown_pct": 100.0 * min(n_mig * mig_bytes, mig_bytes * t / max(m, 1e-9) * n_mig) / kv_bytes_step})
+                             "bandwidth_share_pct": 100.0 * min(1.0, t / m) * n_mig * mig_bytes / (kv_bytes_step + min(1.0, t / m) * n_mig * mig_bytes)})
+    res["note"] = ("slowdown is relative to one isolated decode step measured the same way; any concurrent kernel of another "
+                   "stream costs ~3.5 % (floor, independent of its rate: launch gaps of the 64-launch step grow), a co-resident "
+                   "CTA holding > ~6 KB shared memory costs +30 % (L1 carve-out), and a few full-speed CTAs make their SMs "
+                   "stragglers; the paced mode therefore copies through registers with one small CTA per SM")
     del p
     _free(torch)
     return res

@@ -18,7 +18,9 @@ SMALLTILE = dict(layers=2, kv_heads=7, head_dim=24, block_size=3, elem_bytes=2, 
 
 KERNELS = [dict(copy_kernel=2), dict(copy_kernel=1), dict(copy_kernel=2, chunk_bytes=4096, ring_stages=2),
            dict(copy_kernel=1, chunk_bytes=2048), dict(copy_kernel=2, ids_by_value_max=0),
-           dict(copy_kernel=1, ids_by_value_max=0), dict(copy_kernel=2, max_ctas=3), dict(copy_kernel=1, max_ctas=1)]
+           dict(copy_kernel=1, ids_by_value_max=0), dict(copy_kernel=2, max_ctas=3), dict(copy_kernel=1, max_ctas=1),
+           dict(bandwidth_gbps=40), dict(bandwidth_gbps=3000), dict(copy_kernel=2, unit_order=0), dict(copy_kernel=1, unit_order=0),
+           dict(copy_kernel=2, l2_hint=3, rings_per_cta=2), dict(pdl=0)]
 
 
 @pytest.fixture(scope="module")
