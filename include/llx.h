@@ -144,6 +144,19 @@ llx_status llx_pack(const llx_pool* src, const int32_t* src_block_ids, int n, vo
 llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, const int32_t* dst_block_ids, int n,
                       void* cuda_stream);
 
+/* The paper's whole transfer route in one call: gather into the contiguous buffer, then scatter
+ * from it into the destination's reserved blocks.  Result: dst as after llx_migrate_stage, staging as after llx_pack.
+ * The request is cut into chunks of `chunk_blocks` blocks (<= 0: auto, ~64 MiB); chunk k is scattered on an internal
+ * stream while chunk k+1 is gathered on `cuda_stream`.  With a pinned-host buffer the chunks cross the host link on the
+ * copy engines, device->host and host->device at the same time (the source and destination machines of the paper work
+ * concurrently in the same way), through library-owned device bounce buffers (4 x chunk bytes, allocated on first use:
+ * that call synchronises the device).  `cuda_stream` is joined with the internal streams before the call returns: work
+ * enqueued on it afterwards sees the complete migration.  Checks as llx_migrate_stage + llx_pack; nothing is launched
+ * when a check fails.  Calls are serialised per process (they share the internal streams). */
+llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
+                                const int32_t* dst_block_ids, int n, void* staging, size_t staging_bytes,
+                                int chunk_blocks, void* cuda_stream);
+
 /* ---- S8: append-only growth while decoding continues --------------- */
 
 /* Writes the K and V vectors of tokens t0..t1-1 of one request into their slots: token t
@@ -179,9 +192,11 @@ typedef enum {
     LLX_OPT_RINGS_PER_CTA = 8,  /* bulk kernel: independent smem rings (warps) per CTA (0 = auto) */
     LLX_OPT_PDL = 9,            /* 1 (default): launch copy/append kernels with programmatic stream serialization so that
                                    a kernel's prologue overlaps the previous kernel's tail; results are unchanged */
-    LLX_OPT_BANDWIDTH_GBPS = 10 /* bandwidth budget of device<->device copies in GB/s, read + written (0 = unlimited):
+    LLX_OPT_BANDWIDTH_GBPS = 10,/* bandwidth budget of device<->device copies in GB/s, read + written (0 = unlimited):
                                    one paced ring per SM instead of a few full-speed CTAs, so that a co-running
                                    decode step loses the same small share on every SM (<= 1 %) */
+    LLX_OPT_VIA_HOST_MODE = 11  /* llx_migrate_via_host with a pinned-host buffer: 0 (default) copy engines through device
+                                   bounce buffers, both link directions at once; 1 the kernels address the host buffer directly */
 } llx_option;
 /* Process-wide; takes effect for later calls.  Returns LLX_ERR_INVALID_ARG for a bad value. */
 llx_status llx_set_option(llx_option opt, long long value);

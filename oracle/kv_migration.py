@@ -158,6 +158,23 @@ def staged_migration(src, src_table, dst, dst_table, schedule, appends, block_si
     return num_tokens
 
 
+def migrate_via_buffer(src: np.ndarray, src_block_ids, dst: np.ndarray, dst_block_ids) -> np.ndarray:
+    """The paper's transfer route written out: the request's blocks are fused into one
+    contiguous buffer (`pack`), the buffer is what travels, and the destination scatters it into its reserved
+    blocks (`unpack`).  Returns the buffer.  The final DST equals `migrate_stage` (pin P5)."""
+    if src is dst:
+        raise ValueError("source and destination are the same pool")
+    s_ids = _check_ids(src_block_ids, src.shape[2], "src")
+    d_ids = _check_ids(dst_block_ids, dst.shape[2], "dst")
+    if s_ids.size != d_ids.size:
+        raise ValueError("src/dst id lists differ in length")
+    if np.unique(d_ids).size != d_ids.size:
+        raise ValueError("duplicate destination block id")
+    buf = pack(src, s_ids)
+    unpack(buf, dst, d_ids)
+    return buf
+
+
 # --------------------------------------------------------------------------
 # Stage planning (PAPER.md:134; readings A3, A4 in DESIGN.md)
 # --------------------------------------------------------------------------

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(HERE, "libllx.so")
 
 F16, BF16, U8 = 0, 1, 2
 (OPT_COPY_KERNEL, OPT_MAX_CTAS, OPT_CHUNK_BYTES, OPT_RING_STAGES, OPT_IDS_BY_VALUE_MAX, OPT_ATTN_SPLIT_TOKENS,
- OPT_UNIT_ORDER, OPT_L2_HINT, OPT_RINGS_PER_CTA, OPT_PDL, OPT_BANDWIDTH_GBPS) = range(11)
+ OPT_UNIT_ORDER, OPT_L2_HINT, OPT_RINGS_PER_CTA, OPT_PDL, OPT_BANDWIDTH_GBPS, OPT_VIA_HOST_MODE) = range(12)
 
 _vp, _i, _sz, _i32p = C.c_void_p, C.c_int, C.c_size_t, C.POINTER(C.c_int32)
 
@@ -49,6 +49,7 @@ EXPORTS = {
     "llx_staging_free_pinned": (_i, [_vp]),
     "llx_pack": (_i, [_vp, _i32p, _i, _vp, _sz, _vp]),
     "llx_unpack": (_i, [_vp, _sz, _vp, _i32p, _i, _vp]),
+    "llx_migrate_via_host": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp, _sz, _i, _vp]),
     "llx_append_tokens": (_i, [_vp, _i32p, _i, _i, _i, _vp, _vp]),
     "llx_decode_attention": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _i, _i, C.c_float, _vp]),
     "llx_set_option": (_i, [_i, C.c_longlong]),
@@ -231,6 +232,16 @@ def unpack(staging_ptr: int, staging_nbytes: int, dst: Pool, dst_block_ids, stre
     _check(load().llx_unpack(staging_ptr, staging_nbytes, dst.handle, dp, d.size, _stream(stream)))
 
 
+def migrate_via_host(src: Pool, src_block_ids, dst: Pool, dst_block_ids, staging_ptr: int, staging_nbytes: int,
+                     chunk_blocks: int = 0, stream=None):
+    s, sp = _ids(src_block_ids)
+    d, dp = _ids(dst_block_ids)
+    if s.size != d.size:
+        raise LlxError(-1, "LLX_ERR_INVALID_ARG", "src/dst id lists differ in length")
+    _check(load().llx_migrate_via_host(src.handle, sp, dst.handle, dp, s.size, staging_ptr, staging_nbytes,
+                                       chunk_blocks, _stream(stream)))
+
+
 def append_tokens(pool: Pool, block_table, t0: int, t1: int, dev_values_ptr: int, stream=None):
     t, tp = _ids(block_table)
     _check(load().llx_append_tokens(pool.handle, tp, t.size, t0, t1, dev_values_ptr, _stream(stream)))
@@ -256,7 +267,8 @@ def options(**kw):
     names = dict(copy_kernel=OPT_COPY_KERNEL, max_ctas=OPT_MAX_CTAS, chunk_bytes=OPT_CHUNK_BYTES,
                  ring_stages=OPT_RING_STAGES, ids_by_value_max=OPT_IDS_BY_VALUE_MAX,
                  attn_split_tokens=OPT_ATTN_SPLIT_TOKENS, unit_order=OPT_UNIT_ORDER, l2_hint=OPT_L2_HINT,
-                 rings_per_cta=OPT_RINGS_PER_CTA, pdl=OPT_PDL, bandwidth_gbps=OPT_BANDWIDTH_GBPS)
+                 rings_per_cta=OPT_RINGS_PER_CTA, pdl=OPT_PDL, bandwidth_gbps=OPT_BANDWIDTH_GBPS,
+                 via_host_mode=OPT_VIA_HOST_MODE)
     old = {k: get_option(names[k]) for k in kw}
     try:
         for k, v in kw.items():

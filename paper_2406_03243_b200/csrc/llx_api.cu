@@ -59,7 +59,7 @@ int elem_bytes_of(llx_dtype d) {
 
 // ---- options / counters -------------------------------------------------------------------
 std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
-    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0};
+    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
 // ---- device properties (cached per device) ------------------------------------------------
@@ -197,7 +197,7 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     // on B200: a co-resident CTA that holds > ~6 KB of shared memory shrinks the L1 of its SM and slows a
     // bandwidth-bound decode kernel by 30 %, and a few full-speed CTAs turn their SMs into stragglers.
     const long long budget = g_opt_budget.load();
-    if (budget > 0) kern = 1;
+    if (budget > 0 && g_opt_kernel.load() != 2) kern = 1;
 
     const long long total_bytes = n * 2 * layers * tile_bytes;
     long long chunk = g_opt_chunk.load();
@@ -209,8 +209,8 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     if (kern == 2) {
         // Tuned on B200 (profiles/r01_copy_sweep.md): 2 CTAs per SM, each one ring of 4 x 8 KiB, every ring
         // streaming a CONTIGUOUS range of chunks.  More bytes in flight than ~64 KiB per SM lowers DRAM efficiency.
-        if (nstages <= 0) nstages = 4;
-        if (chunk <= 0) chunk = 8192;
+        if (nstages <= 0) nstages = budget > 0 ? 2 : 4;
+        if (chunk <= 0) chunk = budget > 0 ? 2048 : 8192;  // paced: a 4 KiB ring stays below the L1 carve-out step
         if (chunk > tile_bytes) chunk = tile_bytes;
         chunk &= ~15ll;
         int rings = (int)g_opt_rings.load();
@@ -243,10 +243,12 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     if (kern == 2) {
         int per_sm = (int)((size_t)di->max_smem_optin / (smem + 1024));  // 1 KiB per-CTA reservation
         if (per_sm > 2) per_sm = 2;
-        if (per_sm < 1) per_sm = 1;
+        if (per_sm < 1 || budget > 0) per_sm = 1;
         grid = di->sm_count * per_sm;
     } else if (budget <= 0) {
-        grid = di->sm_count * 8;
+        // A side in host memory is bound by the host link (~52 GB/s): one CTA per SM already saturates it
+        // (measured: 52.7 GB/s with 74..296 CTAs, 51.5 with 1184) and leaves the SMs to whatever else is running.
+        grid = (src.host_memory || dst.host_memory) ? di->sm_count : di->sm_count * 8;
     }
     const long long cap = g_opt_max_ctas.load();
     if (cap > 0) grid = (int)cap;  // explicit grid: the throttle (fewer CTAs) or an experiment (more)
@@ -257,7 +259,8 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     }
     long long pace_ns = 0;
     if (budget > 0) {
-        pace_ns = (long long)grid * 2 * chunk / budget;  // per CTA; bytes/ns == GB/s, read + written
+        const long long workers = (kern == 2) ? (long long)grid * (threads / 32) : grid;  // rings or CTAs
+        pace_ns = workers * 2 * chunk / budget;  // per worker; bytes/ns == GB/s, read + written
         if (pace_ns > 1000000000ll) pace_ns = 1000000000ll;
     }
 
@@ -344,6 +347,48 @@ llx_status check_pair(const llx_pool* src, const llx_pool* dst) {
         return fail(LLX_ERR_GEOMETRY_MISMATCH, "src (L=%d,H=%d,D=%d,S=%d,e=%d) vs dst (L=%d,H=%d,D=%d,S=%d,e=%d)", src->layers,
                     src->kv_heads, src->head_dim, src->block_size, src->elem_bytes, dst->layers, dst->kv_heads,
                     dst->head_dim, dst->block_size, dst->elem_bytes);
+    return LLX_OK;
+}
+
+// ---- the pipelined host route (llx_migrate_via_host): two internal streams, a ring of events and four
+// device bounce buffers per device ------------------------------------------------------------------------
+struct Pipe {
+    cudaStream_t d2h = nullptr, h2d = nullptr;
+    cudaEvent_t ev[64] = {};
+    int next = 0;
+    unsigned char* bounce[4] = {};  // [0,1] gather side, [2,3] scatter side
+    size_t bounce_bytes = 0;        // of each
+    cudaEvent_t take() {
+        cudaEvent_t e = ev[next];
+        next = (next + 1) % 64;
+        return e;
+    }
+};
+std::mutex g_pipe_mu;
+Pipe g_pipe[64];
+
+llx_status pipe_get(int dev, size_t bounce_bytes, Pipe** out) {
+    Pipe& p = g_pipe[dev];
+    if (!p.d2h) {
+        LLX_CUDA(cudaStreamCreateWithFlags(&p.d2h, cudaStreamNonBlocking));
+        LLX_CUDA(cudaStreamCreateWithFlags(&p.h2d, cudaStreamNonBlocking));
+        for (auto& e : p.ev) LLX_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    if (bounce_bytes > p.bounce_bytes) {  // first use or growth: synchronises the device
+        LLX_CUDA(cudaDeviceSynchronize());
+        for (auto& b : p.bounce) {
+            if (b) cudaFree(b);
+            b = nullptr;
+        }
+        p.bounce_bytes = 0;
+        for (auto& b : p.bounce)
+            if (cudaMalloc(&b, bounce_bytes) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(LLX_ERR_OOM, "bounce buffers of %zu bytes", bounce_bytes);
+            }
+        p.bounce_bytes = bounce_bytes;
+    }
+    *out = &p;
     return LLX_OK;
 }
 
@@ -576,6 +621,82 @@ llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, 
     return launch_copy(stg, pool_side(dst, dst_ids), n, dst->layers, dst->tile_bytes, dst->device, (cudaStream_t)stream);
 }
 
+llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
+                                void* staging, size_t staging_bytes, int chunk_blocks, void* stream) {
+    llx_status rc = check_pair(src, dst);
+    if (rc != LLX_OK) return rc;
+    if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
+    if (n == 0) return LLX_OK;
+    if (!src_ids || !dst_ids || !staging) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
+    if (staging_bytes < llx_staging_bytes(src, n))
+        return fail(LLX_ERR_STAGING_TOO_SMALL, "staging has %zu bytes, %d blocks need %zu", staging_bytes, n, llx_staging_bytes(src, n));
+    if ((rc = check_range(src_ids, n, src->num_blocks, "src")) != LLX_OK) return rc;
+    if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
+    if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
+    Side stg;
+    if ((rc = staging_side(staging, src->layers, src->tile_bytes, &stg)) != LLX_OK) return rc;
+    const unsigned char *b0 = stg.base, *b1 = b0 + llx_staging_bytes(src, n);
+    for (const llx_pool* p : {src, (const llx_pool*)dst}) {
+        const unsigned char *a0 = p->data, *a1 = a0 + pool_bytes(p);
+        if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "staging buffer overlaps a pool");
+    }
+    const long long block_bytes = 2ll * src->layers * src->tile_bytes;
+    // Route.  Pinned-host buffer: gather into a device bounce buffer with the copy kernel, move the chunk over
+    // the host link with the copy engines (D2H on one internal stream, H2D on another: the link is full duplex,
+    // 2 x 1 GiB in 21.6 ms vs 41 ms one after the other), scatter from a second bounce buffer.  Measured on
+    // B200: kernels that address the pinned buffer directly reach 52 GB/s per direction but share ~60 GB/s when
+    // both directions run at once, so the zero-copy form (LLX_OPT_VIA_HOST_MODE=1) is kept for comparison only.
+    // Device buffer: nothing crosses the link; the two kernels of a chunk simply run on two streams.
+    const bool bounce = stg.host_memory && g_opt_via_host.load() == 0;
+    if (chunk_blocks <= 0) {  // ~64 MiB per chunk (measured best on B200: 24.6 ms per GiB each way; 32 MiB 24.9, 128 MiB 25.5)
+        chunk_blocks = (int)((64ll << 20) / block_bytes);
+        if (chunk_blocks < 1) chunk_blocks = 1;
+    }
+    if (chunk_blocks > n) chunk_blocks = n;
+    if (chunk_blocks > kIdsByValueCap) chunk_blocks = kIdsByValueCap;
+
+    std::lock_guard<std::mutex> lk(g_pipe_mu);  // the internal streams, events and bounce buffers are shared per device
+    Pipe* pipe = nullptr;
+    if ((rc = pipe_get(src->device, bounce ? (size_t)chunk_blocks * block_bytes : 0, &pipe)) != LLX_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaEvent_t d2h_done[2] = {nullptr, nullptr};
+    int idx = 0;
+    for (int k = 0; k < n; k += chunk_blocks, ++idx) {
+        const int m = (n - k < chunk_blocks) ? n - k : chunk_blocks;
+        const long long off = (long long)k * block_bytes;
+        Side part = stg;  // chunk k's slice of the caller's buffer
+        part.base = stg.base + off;
+        if (!bounce) {
+            if ((rc = launch_copy(pool_side(src, src_ids + k), part, m, src->layers, src->tile_bytes, src->device, st)) != LLX_OK) return rc;
+            cudaEvent_t ev = pipe->take();
+            LLX_CUDA(cudaEventRecord(ev, st));
+            LLX_CUDA(cudaStreamWaitEvent(pipe->h2d, ev, 0));
+            if ((rc = launch_copy(part, pool_side(dst, dst_ids + k), m, dst->layers, dst->tile_bytes, dst->device, pipe->h2d)) != LLX_OK) return rc;
+            continue;
+        }
+        const int slot = idx & 1;
+        Side ga = Side{pipe->bounce[slot], nullptr, stg.slice_stride, stg.item_stride, false};
+        Side sc = Side{pipe->bounce[2 + slot], nullptr, stg.slice_stride, stg.item_stride, false};
+        const size_t bytes = (size_t)m * block_bytes;
+        if (d2h_done[slot]) LLX_CUDA(cudaStreamWaitEvent(st, d2h_done[slot], 0));  // bounce buffer free again
+        if ((rc = launch_copy(pool_side(src, src_ids + k), ga, m, src->layers, src->tile_bytes, src->device, st)) != LLX_OK) return rc;
+        cudaEvent_t packed = pipe->take();
+        LLX_CUDA(cudaEventRecord(packed, st));
+        LLX_CUDA(cudaStreamWaitEvent(pipe->d2h, packed, 0));
+        LLX_CUDA(cudaMemcpyAsync(const_cast<unsigned char*>(part.base), ga.base, bytes, cudaMemcpyDefault, pipe->d2h));
+        cudaEvent_t landed = pipe->take();
+        LLX_CUDA(cudaEventRecord(landed, pipe->d2h));
+        d2h_done[slot] = landed;
+        LLX_CUDA(cudaStreamWaitEvent(pipe->h2d, landed, 0));
+        LLX_CUDA(cudaMemcpyAsync(const_cast<unsigned char*>(sc.base), part.base, bytes, cudaMemcpyDefault, pipe->h2d));
+        if ((rc = launch_copy(sc, pool_side(dst, dst_ids + k), m, dst->layers, dst->tile_bytes, dst->device, pipe->h2d)) != LLX_OK) return rc;
+    }
+    cudaEvent_t done = pipe->take();
+    LLX_CUDA(cudaEventRecord(done, pipe->h2d));
+    LLX_CUDA(cudaStreamWaitEvent(st, done, 0));  // join: later work on the caller's stream sees the whole migration
+    return LLX_OK;
+}
+
 llx_status llx_append_tokens(llx_pool* p, const int32_t* table, int table_len, int t0, int t1, const void* dev_values,
                              void* stream) {
     llx_status rc = check_pool(p, "pool");
@@ -736,6 +857,10 @@ llx_status llx_set_option(llx_option opt, long long v) {
             if (v < 0 || v > 100000) break;
             g_opt_budget = v;
             return LLX_OK;
+        case LLX_OPT_VIA_HOST_MODE:
+            if (v < 0 || v > 1) break;
+            g_opt_via_host = v;
+            return LLX_OK;
     }
     return fail(LLX_ERR_INVALID_ARG, "option %d: bad value %lld", (int)opt, v);
 }
@@ -752,6 +877,7 @@ long long llx_get_option(llx_option opt) {
         case LLX_OPT_RINGS_PER_CTA: return g_opt_rings;
         case LLX_OPT_PDL: return g_opt_pdl;
         case LLX_OPT_BANDWIDTH_GBPS: return g_opt_budget;
+        case LLX_OPT_VIA_HOST_MODE: return g_opt_via_host;
     }
     return -1;
 }

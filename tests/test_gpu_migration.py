@@ -168,6 +168,64 @@ def test_pack_unpack_block_fusion(env, where, opts):                 # P5, S6
         pin.free()
 
 
+@pytest.mark.parametrize("where", ["device", "pinned", "pinned_zero_copy"])
+@pytest.mark.parametrize("n,chunk", [(1, 0), (11, 0), (11, 1), (13, 4), (37, 5), (40, 64)])
+def test_migrate_via_host_pipelined_route(env, where, n, chunk):    # S6: PAPER.md:235-237 in one call
+    H, llx = env
+    mode = 1 if where == "pinned_zero_copy" else 0
+    where = where.split("_")[0]
+    g = RAGGED
+    src, dst, h_src, h_dst = make(H, g, seed=10)
+    s_ids = synth.block_permutation(5, g["num_blocks"])[:n]
+    d_ids = synth.block_permutation(6, g["num_blocks"])[:n]
+    nbytes = llx.staging_bytes(src.pool, n)
+    if where == "device":
+        stg = torch.full((nbytes // 2,), 0x2222, dtype=torch.int16, device="cuda")
+        ptr = stg.data_ptr()
+    else:
+        pin = llx.PinnedStaging(nbytes)
+        pin.as_numpy()[:] = 0x2222
+        ptr = pin.dev_alias
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with llx.options(via_host_mode=mode):
+        llx.migrate_via_host(src.pool, s_ids, dst.pool, d_ids, ptr, nbytes, chunk_blocks=chunk, stream=st)
+        if n == 37:      # a second migration right behind the first reuses the bounce buffers and events
+            llx.migrate_via_host(src.pool, s_ids[::-1], dst.pool, d_ids[::-1], ptr, nbytes, chunk_blocks=chunk + 1, stream=st)
+            llx.migrate_via_host(src.pool, s_ids, dst.pool, d_ids, ptr, nbytes, chunk_blocks=chunk, stream=st)
+    # work enqueued on the caller's stream afterwards must see the complete migration (the call joins its side stream)
+    with torch.cuda.stream(st):
+        after = dst.view.clone()
+    st.synchronize()
+    want_buf = om.migrate_via_buffer(h_src, s_ids, h_dst, d_ids)
+    H.assert_pool_equal(after.cpu().numpy().view(np.uint16), h_dst)
+    got = stg.cpu().numpy().view(np.uint16) if where == "device" else pin.as_numpy().copy()
+    assert np.array_equal(got.reshape(want_buf.shape), want_buf)
+    H.assert_pool_equal(src.host(), h_src)
+    if where == "pinned":
+        pin.free()
+
+
+def test_migrate_via_host_argument_errors(env):
+    H, llx = env
+    src, dst, h_src, h_dst = make(H, TINY)
+    stg = torch.empty(llx.staging_bytes(src.pool, 2), dtype=torch.uint8, device="cuda")
+    launches = llx.counters()["kernel_launches"]
+    for name, fn in [
+        ("LLX_ERR_STAGING_TOO_SMALL", lambda: llx.migrate_via_host(src.pool, [0, 1, 2], dst.pool, [0, 1, 2], stg.data_ptr(), stg.numel())),
+        ("LLX_ERR_DUPLICATE_DST", lambda: llx.migrate_via_host(src.pool, [0, 1], dst.pool, [3, 3], stg.data_ptr(), stg.numel())),
+        ("LLX_ERR_BLOCK_OUT_OF_RANGE", lambda: llx.migrate_via_host(src.pool, [0, 999], dst.pool, [3, 4], stg.data_ptr(), stg.numel())),
+        ("LLX_ERR_ALIAS", lambda: llx.migrate_via_host(src.pool, [0], dst.pool, [3], dst.raw.data_ptr(), dst.raw.numel())),
+        ("LLX_ERR_ALIAS", lambda: llx.migrate_via_host(src.pool, [0], src.pool, [3], stg.data_ptr(), stg.numel())),
+    ]:
+        with pytest.raises(llx.LlxError) as e:
+            fn()
+        assert e.value.name == name, e.value
+    llx.migrate_via_host(src.pool, [], dst.pool, [], stg.data_ptr(), stg.numel())
+    assert llx.counters()["kernel_launches"] == launches
+    H.assert_pool_equal(dst.host(), h_dst)
+
+
 def test_staged_with_appends_equals_oracle_and_single_shot(env):     # P4, S1, S8 on the Tiny shape
     H, llx = env
     g = TINY

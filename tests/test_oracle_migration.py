@@ -156,6 +156,22 @@ def test_pack_unpack_roundtrip_and_layout():
     assert np.array_equal(om.pack(src, s_ids[:2]), buf[:2])
 
 
+def test_migrate_via_buffer_equals_bruteforce_stage():
+    """PAPER.md:235-237 route (fuse -> send buffer -> scatter) against the brute-force stage and brute-force pack."""
+    for g in (MICRO, SMALL):
+        src, dst = make_pools(g)
+        s_ids = synth.block_permutation(3, g["num_blocks"])[:6]
+        d_ids = synth.block_permutation(4, g["num_blocks"])[:6]
+        bs = brute.pool_from_numpy(src)
+        bd = brute.pool_from_numpy(dst)
+        brute.migrate_stage(bs, s_ids, bd, d_ids)
+        buf = om.migrate_via_buffer(src, s_ids, dst, d_ids)
+        assert dst.tolist() == bd
+        assert buf.reshape(-1).tolist() == brute.pack(bs, s_ids)
+        with pytest.raises(ValueError):
+            om.migrate_via_buffer(src, [0, 1], dst, [2, 2])
+
+
 # ---- P4: append-only => staged migration == single-shot copy of the FINAL state ----------
 def _values(seed, te_tok):
     return lambda t, l, kv: synth.append_values_f16(seed, t, l, kv, te_tok)
