@@ -65,7 +65,9 @@ typedef enum {
     LLX_ERR_ALIAS = -5,             /* src and dst are the same pool / overlap */
     LLX_ERR_STAGING_TOO_SMALL = -6,
     LLX_ERR_OOM = -7,
-    LLX_ERR_CUDA = -8
+    LLX_ERR_CUDA = -8,
+    LLX_ERR_NO_SPACE = -9,          /* the block manager has fewer free blocks than asked for */
+    LLX_ERR_STATE = -10             /* call not allowed in the migration's current state */
 } llx_status;
 
 /* ---- pools (D1 in SURVEY.md; PagedAttention blocks) ------------------ */
@@ -156,6 +158,64 @@ llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, 
 llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
                                 const int32_t* dst_block_ids, int n, void* staging, size_t staging_bytes,
                                 int chunk_blocks, void* cuda_stream);
+
+/* ---- NEXT-3: block manager + migration handshake (Fig. 7) -- host logic only ------------------
+ *
+ * llx_blockmgr is one instance's free list of block ids.  Policy (A23): a stack; a fresh manager hands
+ * out 0,1,2,...; released ids are pushed in the order given and handed out again last-in-first-out.
+ * llx_migration drives ONE request's migration through the handshake of PAPER.md:142:
+ *   before each stage  PRE-ALLOC n blocks on the destination (all or nothing, A24) -> proceed | abort
+ *   after each stage   the source checks the request: finished / preempted / peer failed -> abort, the destination
+ *                      releases everything reserved for this migration (A25); no byte is rolled back
+ *   after the final stage  the source releases its blocks, the destination commits: the request resumes there.
+ * Not thread-safe per object; distinct objects are independent. */
+typedef struct llx_blockmgr llx_blockmgr;
+typedef struct llx_migration llx_migration;
+typedef enum { LLX_REQ_RUNNING = 0, LLX_REQ_FINISHED = 1, LLX_REQ_PREEMPTED = 2, LLX_REQ_PEER_FAILED = 3 } llx_req_status;
+typedef enum {
+    LLX_MIG_READY = 0,         /* no stage issued yet */
+    LLX_MIG_COPYING = 1,       /* a non-final stage was issued; the request keeps decoding on the source */
+    LLX_MIG_FINAL_COPYING = 2, /* the final stage was issued; the request is stopped (downtime) */
+    LLX_MIG_COMMITTED = 3,
+    LLX_MIG_ABORTED = 4
+} llx_mig_state;
+typedef enum { LLX_ABORT_NONE = 0, LLX_ABORT_FINISHED = 1, LLX_ABORT_PREEMPTED = 2, LLX_ABORT_PEER_FAILED = 3,
+               LLX_ABORT_NO_SPACE = 4 } llx_abort_reason;
+
+llx_status llx_blockmgr_create(int num_blocks, llx_blockmgr** out);
+llx_status llx_blockmgr_destroy(llx_blockmgr* mgr);
+int        llx_blockmgr_num_free(const llx_blockmgr* mgr);   /* -1 on NULL */
+int        llx_blockmgr_num_blocks(const llx_blockmgr* mgr); /* -1 on NULL */
+/* n ids into ids_out (HOST int32[n]); LLX_ERR_NO_SPACE when fewer than n are free: nothing is allocated. */
+llx_status llx_blockmgr_alloc(llx_blockmgr* mgr, int n, int32_t* ids_out);
+/* Returns ids to the free list; LLX_ERR_BLOCK_OUT_OF_RANGE / LLX_ERR_INVALID_ARG (already free, or twice in the
+ * list): nothing is released. */
+llx_status llx_blockmgr_release(llx_blockmgr* mgr, const int32_t* ids, int n);
+
+/* src / dst may both be NULL: the session then only coordinates (no copy is enqueued) — how the handshake is
+ * tested without a device.  The managers are borrowed, not owned. */
+llx_status llx_migration_begin(const llx_pool* src, llx_blockmgr* src_mgr, llx_pool* dst, llx_blockmgr* dst_mgr,
+                               int block_size, int last_stage_max_blocks, llx_migration** out);
+/* One round.  (1) the source's check: status != RUNNING aborts (reserved destination blocks are released).
+ * (2) llx_plan_stage(num_tokens, blocks migrated so far).  (3) PRE-ALLOC of *n blocks on the destination manager;
+ * LLX_ERR_NO_SPACE aborts likewise.  (4) with pools: llx_migrate_stage of src_block_table[m .. m+*n) into the
+ * reserved ids is enqueued on cuda_stream.  src_block_table: HOST int32[table_len], the request's logical->physical
+ * table on the source, table_len >= ceil(num_tokens/block_size).  dst_ids_out (may be NULL): the *n reserved ids.
+ * Returns LLX_OK also when the round ended in an abort: read llx_migration_state(). */
+llx_status llx_migration_stage(llx_migration* mig, const int32_t* src_block_table, int table_len, int num_tokens,
+                               llx_req_status status, void* cuda_stream, int* n, int* is_final, int32_t* dst_ids_out);
+/* After the final stage's copy has completed (the caller synchronised its stream).  status != RUNNING aborts (A26).
+ * Otherwise the source's blocks src_block_table[0 .. blocks migrated) go back to src_mgr and the request's
+ * destination table is written to dst_table_out (HOST int32[cap], cap >= blocks migrated); state COMMITTED. */
+llx_status llx_migration_commit(llx_migration* mig, const int32_t* src_block_table, int table_len, llx_req_status status,
+                                int32_t* dst_table_out, int cap, int* n_out);
+/* Either side may abort before the commit ("if the other side fails"). */
+llx_status llx_migration_abort(llx_migration* mig, llx_abort_reason reason);
+llx_mig_state    llx_migration_state(const llx_migration* mig);
+llx_abort_reason llx_migration_abort_reason(const llx_migration* mig);
+int              llx_migration_blocks_migrated(const llx_migration* mig);
+int              llx_migration_stages(const llx_migration* mig); /* stages issued so far */
+llx_status       llx_migration_destroy(llx_migration* mig);     /* an uncommitted session is aborted first */
 
 /* ---- S8: append-only growth while decoding continues --------------- */
 

@@ -25,6 +25,9 @@ What it computes, and the passage each part follows (all `PAPER.md:<line>`):
 * `kv_migration.plan_stage`, `stage_sizes` — which logical blocks a stage takes
    and the shrinking-stage recurrence behind "only takes two
   stages" (§6.2).
+* `handshake.BlockManager`, `handshake.Migration`, `handshake.run_script` — the migration
+  handshake of Figure 7 (§4.2): PRE-ALLOC before each stage, the source's
+  check after each stage, abort and release, commit.
 * `decode_attention.decode_attention_fp64` — standard KV-cache attention for one
   decode token per sequence, read through the block table (§2).
 
@@ -33,5 +36,8 @@ pinned to something other than itself — pure-Python element-loop brute force o
 micro pools (P1–P8), the paper's printed block arithmetic (P12,
 tests/golden/paper_block_arithmetic.txt), closed-form special cases and
 `torch.nn.functional.scaled_dot_product_attention` in float64 (P11), and the
-closed form of the stage recurrence (P9).  Nothing here is "parity unpinned".
+closed form of the stage recurrence (P9); the handshake is pinned to the message
+sequence the paper narrates (tests/golden/paper_handshake_fig7.txt), block conservation,
+leak freedom at every abort point and the commit bookkeeping in closed form
+(tests/test_oracle_handshake.py).  Nothing here is "parity unpinned".
 """

@@ -12,5 +12,8 @@ from .binding import (  # noqa: F401
     pool_create, pool_wrap, pool_bytes_for,
     plan_stage, migrate_stage, migrate_batch, staging_bytes, PinnedStaging, pack, unpack, migrate_via_host,
     append_tokens, decode_attention,
+    BlockManager, Migration, REQ_RUNNING, REQ_FINISHED, REQ_PREEMPTED, REQ_PEER_FAILED,
+    MIG_READY, MIG_COPYING, MIG_FINAL_COPYING, MIG_COMMITTED, MIG_ABORTED,
+    ABORT_NONE, ABORT_FINISHED, ABORT_PREEMPTED, ABORT_PEER_FAILED, ABORT_NO_SPACE,
     set_option, get_option, options, counters, reset_counters, version, EXPORTS,
 )

@@ -50,6 +50,21 @@ EXPORTS = {
     "llx_pack": (_i, [_vp, _i32p, _i, _vp, _sz, _vp]),
     "llx_unpack": (_i, [_vp, _sz, _vp, _i32p, _i, _vp]),
     "llx_migrate_via_host": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp, _sz, _i, _vp]),
+    "llx_blockmgr_create": (_i, [_i, C.POINTER(_vp)]),
+    "llx_blockmgr_destroy": (_i, [_vp]),
+    "llx_blockmgr_num_free": (_i, [_vp]),
+    "llx_blockmgr_num_blocks": (_i, [_vp]),
+    "llx_blockmgr_alloc": (_i, [_vp, _i, _i32p]),
+    "llx_blockmgr_release": (_i, [_vp, _i32p, _i]),
+    "llx_migration_begin": (_i, [_vp, _vp, _vp, _vp, _i, _i, C.POINTER(_vp)]),
+    "llx_migration_stage": (_i, [_vp, _i32p, _i, _i, _i, _vp, C.POINTER(_i), C.POINTER(_i), _i32p]),
+    "llx_migration_commit": (_i, [_vp, _i32p, _i, _i, _i32p, _i, C.POINTER(_i)]),
+    "llx_migration_abort": (_i, [_vp, _i]),
+    "llx_migration_state": (_i, [_vp]),
+    "llx_migration_abort_reason": (_i, [_vp]),
+    "llx_migration_blocks_migrated": (_i, [_vp]),
+    "llx_migration_stages": (_i, [_vp]),
+    "llx_migration_destroy": (_i, [_vp]),
     "llx_append_tokens": (_i, [_vp, _i32p, _i, _i, _i, _vp, _vp]),
     "llx_decode_attention": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _i, _i, C.c_float, _vp]),
     "llx_set_option": (_i, [_i, C.c_longlong]),
@@ -240,6 +255,82 @@ def migrate_via_host(src: Pool, src_block_ids, dst: Pool, dst_block_ids, staging
         raise LlxError(-1, "LLX_ERR_INVALID_ARG", "src/dst id lists differ in length")
     _check(load().llx_migrate_via_host(src.handle, sp, dst.handle, dp, s.size, staging_ptr, staging_nbytes,
                                        chunk_blocks, _stream(stream)))
+
+
+REQ_RUNNING, REQ_FINISHED, REQ_PREEMPTED, REQ_PEER_FAILED = range(4)
+MIG_READY, MIG_COPYING, MIG_FINAL_COPYING, MIG_COMMITTED, MIG_ABORTED = range(5)
+ABORT_NONE, ABORT_FINISHED, ABORT_PREEMPTED, ABORT_PEER_FAILED, ABORT_NO_SPACE = range(5)
+
+
+class BlockManager:
+    """One instance's free list of block ids (llx_blockmgr*)."""
+
+    def __init__(self, num_blocks: int):
+        h = _vp()
+        _check(load().llx_blockmgr_create(num_blocks, C.byref(h)))
+        self._h = h.value
+
+    handle = property(lambda self: self._h)
+    num_free = property(lambda self: load().llx_blockmgr_num_free(self._h))
+    num_blocks = property(lambda self: load().llx_blockmgr_num_blocks(self._h))
+
+    def alloc(self, n: int) -> np.ndarray:
+        out = np.empty(max(n, 0), dtype=np.int32)
+        _check(load().llx_blockmgr_alloc(self._h, n, out.ctypes.data_as(_i32p)))
+        return out
+
+    def release(self, ids):
+        a, ap = _ids(ids)
+        _check(load().llx_blockmgr_release(self._h, ap, a.size))
+
+    def __del__(self):
+        with contextlib.suppress(Exception):
+            if self._h:
+                load().llx_blockmgr_destroy(self._h)
+                self._h = 0
+
+
+class Migration:
+    """One request's migration through the handshake of PAPER.md:142 (llx_migration*)."""
+
+    def __init__(self, src, src_mgr: BlockManager, dst, dst_mgr: BlockManager, block_size: int,
+                 last_stage_max_blocks: int):
+        h = _vp()
+        _check(load().llx_migration_begin(src.handle if src is not None else None, src_mgr.handle,
+                                          dst.handle if dst is not None else None, dst_mgr.handle,
+                                          block_size, last_stage_max_blocks, C.byref(h)))
+        self._h, self._keep = h.value, (src, src_mgr, dst, dst_mgr)
+
+    state = property(lambda self: load().llx_migration_state(self._h))
+    abort_reason = property(lambda self: load().llx_migration_abort_reason(self._h))
+    blocks_migrated = property(lambda self: load().llx_migration_blocks_migrated(self._h))
+    stages = property(lambda self: load().llx_migration_stages(self._h))
+
+    def stage(self, src_block_table, num_tokens: int, status: int = REQ_RUNNING, stream=None):
+        """-> (n, is_final, dst_ids) of the stage just issued; n == 0 and state MIG_ABORTED after an abort."""
+        t, tp = _ids(src_block_table)
+        n, f = _i(), _i()
+        out = np.empty(max(t.size, 1), dtype=np.int32)
+        _check(load().llx_migration_stage(self._h, tp, t.size, num_tokens, status, _stream(stream), C.byref(n),
+                                          C.byref(f), out.ctypes.data_as(_i32p)))
+        return n.value, bool(f.value), out[:n.value].copy()
+
+    def commit(self, src_block_table, status: int = REQ_RUNNING):
+        """-> the request's block table on the destination, or None when the commit turned into an abort."""
+        t, tp = _ids(src_block_table)
+        out = np.empty(max(t.size, 1), dtype=np.int32)
+        n = _i()
+        _check(load().llx_migration_commit(self._h, tp, t.size, status, out.ctypes.data_as(_i32p), out.size, C.byref(n)))
+        return out[:n.value].copy() if self.state == MIG_COMMITTED else None
+
+    def abort(self, reason: int = ABORT_PEER_FAILED):
+        _check(load().llx_migration_abort(self._h, reason))
+
+    def __del__(self):
+        with contextlib.suppress(Exception):
+            if self._h:
+                load().llx_migration_destroy(self._h)
+                self._h = 0
 
 
 def append_tokens(pool: Pool, block_table, t0: int, t1: int, dev_values_ptr: int, stream=None):

@@ -8,8 +8,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libllx.so")
-SOURCES = [os.path.join(CSRC, "llx_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("llx_copy.cuh", "llx_attention.cuh")] + \
+SOURCES = [os.path.join(CSRC, "llx_api.cu"), os.path.join(CSRC, "llx_coord.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("llx_copy.cuh", "llx_attention.cuh", "llx_internal.h")] + \
     [os.path.join(os.path.dirname(HERE), "include", "llx.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -12,6 +12,7 @@
 
 #include "llx_attention.cuh"
 #include "llx_copy.cuh"
+#include "llx_internal.h"
 
 using namespace llx;
 
@@ -28,8 +29,7 @@ struct llx_pool {
     size_t attn_ws_bytes = 0;
 };
 
-namespace {
-
+namespace llx {
 thread_local char g_err[512] = "";
 
 llx_status fail(llx_status s, const char* fmt, ...) {
@@ -39,6 +39,10 @@ llx_status fail(llx_status s, const char* fmt, ...) {
     va_end(ap);
     return s;
 }
+}  // namespace llx
+
+namespace {
+
 llx_status cuda_fail(cudaError_t e, const char* what) {
     return fail(LLX_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
@@ -907,6 +911,8 @@ const char* llx_status_str(llx_status s) {
         case LLX_ERR_STAGING_TOO_SMALL: return "LLX_ERR_STAGING_TOO_SMALL";
         case LLX_ERR_OOM: return "LLX_ERR_OOM";
         case LLX_ERR_CUDA: return "LLX_ERR_CUDA";
+        case LLX_ERR_NO_SPACE: return "LLX_ERR_NO_SPACE";
+        case LLX_ERR_STATE: return "LLX_ERR_STATE";
     }
     return "LLX_ERR_UNKNOWN";
 }

@@ -1,0 +1,243 @@
+// Host-side coordination around the copy path: an instance's block manager and the
+// migration handshake of Llumnix §4.2 (Figure 7).  No device code here; the only CUDA
+// work a session causes is the llx_migrate_stage it enqueues for each stage.
+//
+//   PRE-ALLOC before each stage ("issues a pre-allocate request with the number of blocks")
+//   proceed | abort from the destination ("try to allocate and reserve the blocks")
+//   the source's check after each stage ("has completed or been preempted")
+//   abort when the other side fails
+//   release on the source + commit on the destination after the final stage
+#include <new>
+#include <vector>
+
+#include "llx_internal.h"
+
+using llx::fail;
+
+// ---- block manager: a stack of free ids (A23) ---------------------------------------------
+struct llx_blockmgr {
+    int num_blocks = 0;
+    std::vector<int32_t> free_stack;     // back() is handed out next
+    std::vector<unsigned char> is_free;  // per id
+};
+
+struct llx_migration {
+    const llx_pool* src = nullptr;
+    llx_pool* dst = nullptr;
+    llx_blockmgr* src_mgr = nullptr;
+    llx_blockmgr* dst_mgr = nullptr;
+    int block_size = 0, last_stage_max_blocks = 0;
+    llx_mig_state state = LLX_MIG_READY;
+    llx_abort_reason reason = LLX_ABORT_NONE;
+    int blocks_migrated = 0, stages = 0;
+    std::vector<int32_t> dst_table;  // blocks reserved on the destination so far, in logical order
+};
+
+extern "C" {
+
+llx_status llx_blockmgr_create(int num_blocks, llx_blockmgr** out) {
+    if (!out) return fail(LLX_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (num_blocks <= 0) return fail(LLX_ERR_INVALID_ARG, "num_blocks = %d", num_blocks);
+    llx_blockmgr* m = new (std::nothrow) llx_blockmgr();
+    if (!m) return fail(LLX_ERR_OOM, "host allocation failed");
+    m->num_blocks = num_blocks;
+    m->free_stack.resize((size_t)num_blocks);
+    for (int i = 0; i < num_blocks; ++i) m->free_stack[(size_t)i] = num_blocks - 1 - i;  // pops give 0, 1, 2, ...
+    m->is_free.assign((size_t)num_blocks, 1);
+    *out = m;
+    return LLX_OK;
+}
+
+llx_status llx_blockmgr_destroy(llx_blockmgr* m) {
+    delete m;
+    return LLX_OK;
+}
+
+int llx_blockmgr_num_free(const llx_blockmgr* m) { return m ? (int)m->free_stack.size() : -1; }
+int llx_blockmgr_num_blocks(const llx_blockmgr* m) { return m ? m->num_blocks : -1; }
+
+llx_status llx_blockmgr_alloc(llx_blockmgr* m, int n, int32_t* ids_out) {
+    if (!m) return fail(LLX_ERR_INVALID_ARG, "block manager is NULL");
+    if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
+    if (n == 0) return LLX_OK;
+    if (!ids_out) return fail(LLX_ERR_INVALID_ARG, "ids_out is NULL");
+    if ((size_t)n > m->free_stack.size())
+        return fail(LLX_ERR_NO_SPACE, "%d blocks asked for, %zu free", n, m->free_stack.size());
+    for (int i = 0; i < n; ++i) {
+        const int32_t b = m->free_stack.back();
+        m->free_stack.pop_back();
+        m->is_free[(size_t)b] = 0;
+        ids_out[i] = b;
+    }
+    return LLX_OK;
+}
+
+llx_status llx_blockmgr_release(llx_blockmgr* m, const int32_t* ids, int n) {
+    if (!m) return fail(LLX_ERR_INVALID_ARG, "block manager is NULL");
+    if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
+    if (n == 0) return LLX_OK;
+    if (!ids) return fail(LLX_ERR_INVALID_ARG, "ids is NULL");
+    // validate everything first: a failed release changes nothing
+    for (int i = 0; i < n; ++i) {
+        if (ids[i] < 0 || ids[i] >= m->num_blocks)
+            return fail(LLX_ERR_BLOCK_OUT_OF_RANGE, "ids[%d] = %d not in [0,%d)", i, ids[i], m->num_blocks);
+        if (m->is_free[(size_t)ids[i]]) return fail(LLX_ERR_INVALID_ARG, "block %d is already free", ids[i]);
+    }
+    for (int i = 0; i < n; ++i) {  // a duplicate inside the list shows up as "already free" on its second visit
+        if (m->is_free[(size_t)ids[i]]) {
+            for (int j = 0; j < i; ++j) {  // undo
+                m->is_free[(size_t)ids[j]] = 0;
+                m->free_stack.pop_back();
+            }
+            return fail(LLX_ERR_INVALID_ARG, "block %d appears twice in the list", ids[i]);
+        }
+        m->is_free[(size_t)ids[i]] = 1;
+        m->free_stack.push_back(ids[i]);
+    }
+    return LLX_OK;
+}
+
+}  // extern "C"
+
+// ---- migration session: the handshake -----------------------------------------------------------------
+namespace {
+
+// destination side of an abort ("abort the migration and clean the states"; A25): every block
+// reserved for this migration goes back to the destination's free list; the source is untouched
+void do_abort(llx_migration* g, llx_abort_reason why) {
+    if (!g->dst_table.empty()) llx_blockmgr_release(g->dst_mgr, g->dst_table.data(), (int)g->dst_table.size());
+    g->dst_table.clear();
+    g->reason = why;
+    g->state = LLX_MIG_ABORTED;
+}
+
+llx_abort_reason reason_of(llx_req_status s) {
+    switch (s) {
+        case LLX_REQ_FINISHED: return LLX_ABORT_FINISHED;
+        case LLX_REQ_PREEMPTED: return LLX_ABORT_PREEMPTED;
+        case LLX_REQ_PEER_FAILED: return LLX_ABORT_PEER_FAILED;
+        default: return LLX_ABORT_NONE;
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+llx_status llx_migration_begin(const llx_pool* src, llx_blockmgr* src_mgr, llx_pool* dst, llx_blockmgr* dst_mgr,
+                               int block_size, int last_stage_max_blocks, llx_migration** out) {
+    if (!out) return fail(LLX_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!src_mgr || !dst_mgr) return fail(LLX_ERR_INVALID_ARG, "block manager is NULL");
+    if (src_mgr == dst_mgr) return fail(LLX_ERR_ALIAS, "source and destination share one block manager");
+    if ((src == nullptr) != (dst == nullptr)) return fail(LLX_ERR_INVALID_ARG, "pass both pools or neither");
+    if (block_size <= 0 || last_stage_max_blocks < 1)
+        return fail(LLX_ERR_INVALID_ARG, "block_size = %d, last_stage_max_blocks = %d", block_size, last_stage_max_blocks);
+    if (src) {
+        if (llx_pool_num_blocks(src) != src_mgr->num_blocks || llx_pool_num_blocks(dst) != dst_mgr->num_blocks)
+            return fail(LLX_ERR_GEOMETRY_MISMATCH, "a block manager does not match its pool's num_blocks");
+    }
+    llx_migration* g = new (std::nothrow) llx_migration();
+    if (!g) return fail(LLX_ERR_OOM, "host allocation failed");
+    g->src = src;
+    g->dst = dst;
+    g->src_mgr = src_mgr;
+    g->dst_mgr = dst_mgr;
+    g->block_size = block_size;
+    g->last_stage_max_blocks = last_stage_max_blocks;
+    *out = g;
+    return LLX_OK;
+}
+
+llx_status llx_migration_stage(llx_migration* g, const int32_t* table, int table_len, int num_tokens, llx_req_status status,
+                               void* stream, int* n_out, int* is_final_out, int32_t* dst_ids_out) {
+    if (!g || !n_out || !is_final_out) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
+    *n_out = 0;
+    *is_final_out = 0;
+    if (g->state != LLX_MIG_READY && g->state != LLX_MIG_COPYING)
+        return fail(LLX_ERR_STATE, "llx_migration_stage in state %d", (int)g->state);
+    // (1) the source's check (A26: also before the first stage)
+    if (status != LLX_REQ_RUNNING) {
+        do_abort(g, reason_of(status));
+        return LLX_OK;
+    }
+    // (2) which blocks
+    int n = 0, fin = 0;
+    llx_status rc = llx_plan_stage(num_tokens, g->blocks_migrated, g->block_size, g->last_stage_max_blocks, &n, &fin);
+    if (rc != LLX_OK) return rc;
+    const int m = g->blocks_migrated;
+    if (n > 0 && (!table || table_len < m + n))
+        return fail(LLX_ERR_INVALID_ARG, "source block table of %d entries, stage needs [%d,%d)", table_len, m, m + n);
+    // (3) PRE-ALLOC on the destination: all or nothing
+    std::vector<int32_t> ids((size_t)n);
+    rc = llx_blockmgr_alloc(g->dst_mgr, n, ids.data());
+    if (rc == LLX_ERR_NO_SPACE) {
+        do_abort(g, LLX_ABORT_NO_SPACE);
+        return LLX_OK;
+    }
+    if (rc != LLX_OK) return rc;
+    // (4) the stage's copy
+    if (g->src && n > 0) {
+        rc = llx_migrate_stage(g->src, table + m, g->dst, ids.data(), n, stream);
+        if (rc != LLX_OK) {  // nothing was launched: give the reservation back, the session stays where it was
+            llx_blockmgr_release(g->dst_mgr, ids.data(), n);
+            return rc;
+        }
+    }
+    g->dst_table.insert(g->dst_table.end(), ids.begin(), ids.end());
+    g->blocks_migrated += n;
+    g->stages += 1;
+    g->state = fin ? LLX_MIG_FINAL_COPYING : LLX_MIG_COPYING;
+    if (dst_ids_out)
+        for (int i = 0; i < n; ++i) dst_ids_out[i] = ids[(size_t)i];
+    *n_out = n;
+    *is_final_out = fin;
+    return LLX_OK;
+}
+
+llx_status llx_migration_commit(llx_migration* g, const int32_t* table, int table_len, llx_req_status status,
+                                int32_t* dst_table_out, int cap, int* n_out) {
+    if (!g) return fail(LLX_ERR_INVALID_ARG, "migration is NULL");
+    if (n_out) *n_out = 0;
+    if (g->state != LLX_MIG_FINAL_COPYING) return fail(LLX_ERR_STATE, "llx_migration_commit in state %d", (int)g->state);
+    if (status != LLX_REQ_RUNNING) {  // A26: a request that ended during the final copy is not committed
+        do_abort(g, reason_of(status));
+        return LLX_OK;
+    }
+    const int n = g->blocks_migrated;
+    if (n > 0 && (!table || table_len < n)) return fail(LLX_ERR_INVALID_ARG, "source block table of %d entries, %d blocks migrated", table_len, n);
+    if (n > 0 && (!dst_table_out || cap < n)) return fail(LLX_ERR_INVALID_ARG, "dst_table_out holds %d entries, %d needed", cap, n);
+    // the source releases its local blocks ...
+    llx_status rc = llx_blockmgr_release(g->src_mgr, table, n);
+    if (rc != LLX_OK) return rc;
+    // ... and the destination commits: the reserved blocks now belong to the request there
+    for (int i = 0; i < n; ++i) dst_table_out[i] = g->dst_table[(size_t)i];
+    if (n_out) *n_out = n;
+    g->dst_table.clear();
+    g->state = LLX_MIG_COMMITTED;
+    return LLX_OK;
+}
+
+llx_status llx_migration_abort(llx_migration* g, llx_abort_reason reason) {
+    if (!g) return fail(LLX_ERR_INVALID_ARG, "migration is NULL");
+    if (g->state == LLX_MIG_COMMITTED || g->state == LLX_MIG_ABORTED)
+        return fail(LLX_ERR_STATE, "llx_migration_abort in state %d", (int)g->state);
+    if (reason <= LLX_ABORT_NONE || reason > LLX_ABORT_NO_SPACE) return fail(LLX_ERR_INVALID_ARG, "reason = %d", (int)reason);
+    do_abort(g, reason);
+    return LLX_OK;
+}
+
+llx_mig_state llx_migration_state(const llx_migration* g) { return g ? g->state : LLX_MIG_ABORTED; }
+llx_abort_reason llx_migration_abort_reason(const llx_migration* g) { return g ? g->reason : LLX_ABORT_NONE; }
+int llx_migration_blocks_migrated(const llx_migration* g) { return g ? g->blocks_migrated : -1; }
+int llx_migration_stages(const llx_migration* g) { return g ? g->stages : -1; }
+
+llx_status llx_migration_destroy(llx_migration* g) {
+    if (!g) return LLX_OK;
+    if (g->state != LLX_MIG_COMMITTED && g->state != LLX_MIG_ABORTED) do_abort(g, LLX_ABORT_PEER_FAILED);
+    delete g;
+    return LLX_OK;
+}
+
+}  // extern "C"

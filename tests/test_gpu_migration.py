@@ -328,3 +328,73 @@ def test_migration_on_a_side_stream_concurrent_with_default_stream(env):        
     side.synchronize()
     om.migrate_stage(h_src, s_ids, h_dst, d_ids)
     H.assert_pool_equal(dst.host(), h_dst)
+
+
+def test_migration_session_handshake_drives_the_copies(env):        # NEXT-3: PAPER.md:142 around S1/S3/S4/S8
+    """A whole live migration through llx_migration_*: planner + PRE-ALLOC + copy per stage, appends in between,
+    commit; destination content equals the oracle's staged migration, block bookkeeping equals oracle.handshake."""
+    from oracle import handshake as oh
+    H, llx = env
+    g = TINY
+    S, te_tok, nb = g["block_size"], g["kv_heads"] * g["head_dim"], g["num_blocks"]
+    src, dst, h_src, h_dst = make(H, g)
+    values = lambda t, l, kv: synth.append_values_f16(3, t, l, kv, te_tok)
+    src_mgr, dst_mgr = llx.BlockManager(nb), llx.BlockManager(nb)
+    o_src, o_dst = oh.BlockManager(nb), oh.BlockManager(nb)
+    dst_mgr.alloc(9), o_dst.allocate(9)                              # the destination already serves other requests
+    table = src_mgr.alloc(7)
+    o_table = o_src.allocate(7)
+    assert list(table) == o_table
+    mig = llx.Migration(src.pool, src_mgr, dst.pool, dst_mgr, S, 2)
+    o_mig = oh.Migration(o_src, o_dst, S, 2)
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    tokens, schedule = 97, []
+    while mig.state not in (llx.MIG_FINAL_COPYING,):
+        n, fin, ids = mig.stage(table, tokens, stream=st)
+        o = o_mig.stage(tokens)
+        assert (n, fin, list(ids)) == (o[0], o[1], o[3])
+        schedule.append(n)
+        if not fin:                                                  # decoding continues: 3 more tokens
+            vals = np.stack([np.stack([np.stack([values(t, l, kv) for kv in range(2)]) for l in range(g["layers"])])
+                             for t in range(tokens, tokens + 3)])
+            dev_vals = torch.from_numpy(vals.view(np.int16)).cuda()
+            st.wait_stream(torch.cuda.current_stream())
+            llx.append_tokens(src.pool, table, tokens, tokens + 3, dev_vals.data_ptr(), stream=st)
+            tokens += 3
+    st.synchronize()
+    d_table = mig.commit(table)
+    assert list(d_table) == o_mig.commit(o_table) and mig.state == llx.MIG_COMMITTED
+    assert (src_mgr.num_free, dst_mgr.num_free) == (o_src.num_free(), o_dst.num_free()) == (nb, nb - 9 - 7)
+    assert schedule == [6, 1] and tokens == 100
+    om.staged_migration(h_src, np.array(o_table), h_dst, np.array(d_table), schedule, (3,), S, 97, values)
+    H.assert_pool_equal(dst.host(), h_dst)
+    H.assert_pool_equal(src.host(), h_src)
+
+
+def test_migration_session_abort_releases_reservation_and_touches_nothing_else(env):
+    H, llx = env
+    g = TINY
+    nb = g["num_blocks"]
+    src, dst, h_src, h_dst = make(H, g)
+    src_mgr, dst_mgr = llx.BlockManager(nb), llx.BlockManager(nb)
+    table = src_mgr.alloc(7)
+    mig = llx.Migration(src.pool, src_mgr, dst.pool, dst_mgr, g["block_size"], 2)
+    n, fin, ids = mig.stage(table, 97)
+    assert (n, fin) == (6, False) and dst_mgr.num_free == nb - 6
+    n2, _, _ = mig.stage(table, 100, llx.REQ_FINISHED)              # the request produced EOS during stage 0
+    assert n2 == 0 and mig.state == llx.MIG_ABORTED and mig.abort_reason == llx.ABORT_FINISHED
+    assert dst_mgr.num_free == nb and src_mgr.num_free == nb - 7     # reservation released, source keeps its blocks
+    om.migrate_stage(h_src, table[:6], h_dst, ids)                   # A10/A25: no byte rollback
+    H.assert_pool_equal(dst.host(), h_dst)
+    # destination out of space: PRE-ALLOC fails, nothing is copied
+    small = llx.BlockManager(nb)
+    small.alloc(nb - 3)
+    launches = llx.counters()["kernel_launches"]
+    mig2 = llx.Migration(src.pool, src_mgr, dst.pool, small, g["block_size"], 2)
+    assert mig2.stage(table, 97)[0] == 0 and mig2.abort_reason == llx.ABORT_NO_SPACE and small.num_free == 3
+    assert llx.counters()["kernel_launches"] == launches
+    wrong = llx.BlockManager(nb + 1)
+    with pytest.raises(llx.LlxError) as e:
+        llx.Migration(src.pool, src_mgr, dst.pool, wrong, g["block_size"], 2)
+    assert e.value.name == "LLX_ERR_GEOMETRY_MISMATCH"
