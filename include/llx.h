@@ -217,6 +217,30 @@ int              llx_migration_blocks_migrated(const llx_migration* mig);
 int              llx_migration_stages(const llx_migration* mig); /* stages issued so far */
 llx_status       llx_migration_destroy(llx_migration* mig);     /* an uncommitted session is aborted first */
 
+/* ---- NEXT-4: virtual usage, freeness, pairing (Algorithm 1; §4.4.3) -- host arithmetic
+ *
+ * The step before the hot path: which instances migrate to which, and which requests go first.  Usages, demands,
+ * headrooms and M share one unit (tokens or blocks).  Readings A27-A30 in DESIGN.md. */
+typedef struct {
+    int32_t is_queuing;      /* not yet running on the instance */
+    int32_t is_head_of_line; /* first in the instance's queue (only read when is_queuing) */
+    int32_t is_fake;         /* the infinite-usage request of a terminating instance */
+    int32_t priority;        /* 0 = normal ... num_priorities-1 = highest */
+    double demand;           /* memory the queuing request needs to start */
+    double physical_usage;   /* memory the running request occupies */
+} llx_req_info;
+/* CalcFreeness: *freeness = (M - sum of CalcVirtualUsage) / B, B = running requests (1 if none).  A terminating
+ * instance gets the fake request: -inf.  *total_virtual_usage may be NULL. */
+llx_status llx_calc_freeness(const llx_req_info* reqs, int n, double M, const double* headroom_for_priority,
+                             int num_priorities, int is_terminating, double* freeness, double* total_virtual_usage);
+/* Sources: freeness < src_below; destinations: freeness > dst_above (src_below <= dst_above).  Pairs the lowest
+ * source with the highest destination repeatedly (ties: lower index first).  *n_pairs = min(#src, #dst); the pairs
+ * are written to src_out / dst_out (HOST int32[cap]); LLX_ERR_INVALID_ARG if cap is too small (*n_pairs still set). */
+llx_status llx_pair_instances(const double* freeness, int n, double src_below, double dst_above, int32_t* src_out,
+                              int32_t* dst_out, int cap, int* n_pairs);
+/* The order in which a source offers its requests: lower priority first, then shorter sequence, then lower index. */
+llx_status llx_migration_order(const int32_t* priority, const int32_t* seq_len, int n, int32_t* order_out);
+
 /* ---- S8: append-only growth while decoding continues --------------- */
 
 /* Writes the K and V vectors of tokens t0..t1-1 of one request into their slots: token t

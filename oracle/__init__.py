@@ -28,6 +28,8 @@ What it computes, and the passage each part follows (all `PAPER.md:<line>`):
 * `handshake.BlockManager`, `handshake.Migration`, `handshake.run_script` — the migration
   handshake of Figure 7 (§4.2): PRE-ALLOC before each stage, the source's
   check after each stage, abort and release, commit.
+* `policy.calc_freeness`, `policy.pair_instances`, `policy.migration_order` — Algorithm 1
+  (virtual usage and freeness) and the pairing rule of §4.4.3.
 * `decode_attention.decode_attention_fp64` — standard KV-cache attention for one
   decode token per sequence, read through the block table (§2).
 
@@ -39,5 +41,8 @@ tests/golden/paper_block_arithmetic.txt), closed-form special cases and
 closed form of the stage recurrence (P9); the handshake is pinned to the message
 sequence the paper narrates (tests/golden/paper_handshake_fig7.txt), block conservation,
 leak freedom at every abort point and the commit bookkeeping in closed form
-(tests/test_oracle_handshake.py).  Nothing here is "parity unpinned".
+(tests/test_oracle_handshake.py); Algorithm 1 is pinned to the meaning the paper gives
+freeness (decode iterations left, by brute-force simulation), to the printed capacity
+13,616 tokens / target load 1,600 tokens (tests/golden/paper_priority_headroom.txt) and to
+the rule-by-rule special cases (tests/test_oracle_policy.py).  Nothing here is "parity unpinned".
 """

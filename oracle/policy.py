@@ -1,0 +1,107 @@
+"""Oracle: Llumnix's virtual usage / freeness calculation (Algorithm 1) and the
+migration pairing policy built on it (§4.4.3).  TEST INFRASTRUCTURE ONLY — the
+algorithm in the paper's order and notation, plain Python, fp64.  Shares no code with
+paper_2406_03243_b200/csrc/llx_coord.cu.
+
+Algorithm 1 as printed (line numbers are the paper's; the extracted text lost lines 2-5's layout,
+the prose fixes them: "directly uses its real demand (line 4)", "a fake request with a virtual usage
+of infinity (line 7)", "adding such a headroom on the physical usage (line 8)", "this headroom is
+divided among them (line 10)"):
+
+     1  Function CalcVirtualUsage(req, instance):
+     2    if req.isQueuing then
+     3      if req.isHeadOfLine then
+     4        return req.demand
+     5      return 0
+     6    if req.isFake then
+     7      return inf
+     8    return req.physicalUsage + GetHeadroom(req.priority, instance)
+     9  Function GetHeadroom(p, instance):
+    10    return headroomForPriority[p] / instance.numRequests[p]
+    11  Function CalcFreeness(instance):
+    12    if instance.isTerminating then
+    13      AddFakeReq(instance.requests)
+    14    totalVirtualUsages = 0
+    15    for req in instance.requests do
+    16      totalVirtualUsages += CalcVirtualUsage(req, instance)
+    17    freeness = (instance.M - totalVirtualUsages) / instance.B
+    18    return freeness
+
+Readings (A27-A30):
+  A27  line 5 (lost in extraction): a queuing request that is not head-of-line has virtual usage 0
+       ("For the head-of-line queuing request ... we assign a positive virtual usage").
+  A28  B = number of running requests ("the batch size ... the number of new tokens per iteration",
+       PAPER.md:223); an instance with no running request uses B = 1 so that F stays finite.
+  A29  numRequests[p] counts the RUNNING requests of priority p (the ones that receive headroom).
+  A30  pairing: sources are instances with F < src_below, destinations those with F > dst_above; the
+       lowest-F source is paired with the highest-F destination, repeatedly, until one set is empty
+       (PAPER.md:225); ties broken by the lower instance index.  Requests to migrate: lower priority
+       first, then shorter sequence, then lower index ("prefers the requests with lower
+       priorities and shorter sequence lengths").
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass
+
+
+@dataclass
+class Req:
+    is_queuing: bool = False
+    is_head_of_line: bool = False
+    is_fake: bool = False
+    priority: int = 0
+    demand: float = 0.0
+    physical_usage: float = 0.0
+
+
+@dataclass
+class Instance:
+    M: float                                # total memory, in the unit of the usages (tokens or blocks)
+    requests: list
+    headroom_for_priority: list             # per priority class; 0 for the normal class
+    is_terminating: bool = False
+
+
+def num_requests(instance: Instance, p: int) -> int:
+    return sum(1 for r in instance.requests if not r.is_queuing and not r.is_fake and r.priority == p)   # A29
+
+
+def get_headroom(p: int, instance: Instance) -> float:                      # lines 9-10
+    return instance.headroom_for_priority[p] / num_requests(instance, p)
+
+
+def calc_virtual_usage(req: Req, instance: Instance) -> float:             # lines 1-8
+    if req.is_queuing:
+        if req.is_head_of_line:
+            return req.demand
+        return 0.0
+    if req.is_fake:
+        return math.inf
+    return req.physical_usage + get_headroom(req.priority, instance)
+
+
+def calc_freeness(instance: Instance):                                      # lines 11-18
+    """-> (freeness, total virtual usage)"""
+    requests = list(instance.requests)
+    if instance.is_terminating:
+        requests.append(Req(is_fake=True))
+    total = 0.0
+    for req in requests:
+        total += calc_virtual_usage(req, instance)
+    B = sum(1 for r in instance.requests if not r.is_queuing and not r.is_fake)
+    if B == 0:
+        B = 1                                                               # A28
+    return (instance.M - total) / B, total
+
+
+def pair_instances(freeness, src_below: float, dst_above: float):
+    """list of (source index, destination index)."""
+    src = sorted((i for i, f in enumerate(freeness) if f < src_below), key=lambda i: (freeness[i], i))
+    dst = sorted((i for i, f in enumerate(freeness) if f > dst_above), key=lambda i: (-freeness[i], i))
+    return list(zip(src, dst))
+
+
+def migration_order(priority, seq_len):
+    """request indices in the order the source llumlet offers them for migration."""
+    return sorted(range(len(priority)), key=lambda i: (priority[i], seq_len[i], i))

@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     pool_create, pool_wrap, pool_bytes_for,
     plan_stage, migrate_stage, migrate_batch, staging_bytes, PinnedStaging, pack, unpack, migrate_via_host,
     append_tokens, decode_attention,
+    calc_freeness, pair_instances, migration_order,
     BlockManager, Migration, REQ_RUNNING, REQ_FINISHED, REQ_PREEMPTED, REQ_PEER_FAILED,
     MIG_READY, MIG_COPYING, MIG_FINAL_COPYING, MIG_COMMITTED, MIG_ABORTED,
     ABORT_NONE, ABORT_FINISHED, ABORT_PREEMPTED, ABORT_PEER_FAILED, ABORT_NO_SPACE,

@@ -22,6 +22,11 @@ F16, BF16, U8 = 0, 1, 2
 _vp, _i, _sz, _i32p = C.c_void_p, C.c_int, C.c_size_t, C.POINTER(C.c_int32)
 
 
+class ReqInfo(C.Structure):
+    _fields_ = [("is_queuing", C.c_int32), ("is_head_of_line", C.c_int32), ("is_fake", C.c_int32),
+                ("priority", C.c_int32), ("demand", C.c_double), ("physical_usage", C.c_double)]
+
+
 class _Counters(C.Structure):
     _fields_ = [("kernel_launches", C.c_ulonglong), ("copy_launches", C.c_ulonglong),
                 ("bytes_moved", C.c_ulonglong), ("id_uploads", C.c_ulonglong)]
@@ -65,6 +70,10 @@ EXPORTS = {
     "llx_migration_blocks_migrated": (_i, [_vp]),
     "llx_migration_stages": (_i, [_vp]),
     "llx_migration_destroy": (_i, [_vp]),
+    "llx_calc_freeness": (_i, [C.POINTER(ReqInfo), _i, C.c_double, C.POINTER(C.c_double), _i, _i,
+                               C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "llx_pair_instances": (_i, [C.POINTER(C.c_double), _i, C.c_double, C.c_double, _i32p, _i32p, _i, C.POINTER(_i)]),
+    "llx_migration_order": (_i, [_i32p, _i32p, _i, _i32p]),
     "llx_append_tokens": (_i, [_vp, _i32p, _i, _i, _i, _vp, _vp]),
     "llx_decode_attention": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _i, _i, C.c_float, _vp]),
     "llx_set_option": (_i, [_i, C.c_longlong]),
@@ -331,6 +340,37 @@ class Migration:
             if self._h:
                 load().llx_migration_destroy(self._h)
                 self._h = 0
+
+
+def calc_freeness(reqs, M: float, headroom_for_priority, is_terminating: bool = False):
+    """reqs: iterable of (is_queuing, is_head_of_line, is_fake, priority, demand, physical_usage) -> (F, sum V)"""
+    reqs = list(reqs)
+    arr = (ReqInfo * max(len(reqs), 1))(*[ReqInfo(int(a), int(b), int(c), int(p), float(d), float(u))
+                                          for a, b, c, p, d, u in reqs])
+    hr = (C.c_double * len(headroom_for_priority))(*[float(x) for x in headroom_for_priority])
+    f, tot = C.c_double(), C.c_double()
+    _check(load().llx_calc_freeness(arr, len(reqs), float(M), hr, len(headroom_for_priority), int(is_terminating),
+                                    C.byref(f), C.byref(tot)))
+    return f.value, tot.value
+
+
+def pair_instances(freeness, src_below: float, dst_above: float):
+    f = np.ascontiguousarray(np.asarray(freeness, dtype=np.float64).reshape(-1))
+    s, d = np.empty(max(f.size, 1), np.int32), np.empty(max(f.size, 1), np.int32)
+    n = _i()
+    _check(load().llx_pair_instances(f.ctypes.data_as(C.POINTER(C.c_double)), f.size, src_below, dst_above,
+                                     s.ctypes.data_as(_i32p), d.ctypes.data_as(_i32p), f.size, C.byref(n)))
+    return list(zip(s[:n.value].tolist(), d[:n.value].tolist()))
+
+
+def migration_order(priority, seq_len):
+    p, pp = _ids(priority)
+    q, qp = _ids(seq_len)
+    if p.size != q.size:
+        raise LlxError(-1, "LLX_ERR_INVALID_ARG", "priority/seq_len differ in length")
+    out = np.empty(max(p.size, 1), np.int32)
+    _check(load().llx_migration_order(pp, qp, p.size, out.ctypes.data_as(_i32p)))
+    return out[:p.size].tolist()
 
 
 def append_tokens(pool: Pool, block_table, t0: int, t1: int, dev_values_ptr: int, stream=None):

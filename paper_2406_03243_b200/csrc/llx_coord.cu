@@ -241,3 +241,77 @@ llx_status llx_migration_destroy(llx_migration* g) {
 }
 
 }  // extern "C"
+
+// ---- NEXT-4: virtual usage and freeness (Algorithm 1), pairing -------------
+#include <algorithm>
+#include <limits>
+
+extern "C" {
+
+llx_status llx_calc_freeness(const llx_req_info* reqs, int n, double M, const double* headroom_for_priority,
+                             int num_priorities, int is_terminating, double* freeness, double* total_virtual_usage) {
+    if (n < 0 || num_priorities < 1 || !headroom_for_priority || !freeness || (n > 0 && !reqs))
+        return fail(LLX_ERR_INVALID_ARG, "bad arguments (n=%d, num_priorities=%d)", n, num_priorities);
+    // instance.numRequests[p]: the running requests of each priority (they share that priority's headroom)
+    std::vector<int> per_prio((size_t)num_priorities, 0);
+    int running = 0;
+    for (int i = 0; i < n; ++i) {
+        const llx_req_info& r = reqs[i];
+        if (r.priority < 0 || r.priority >= num_priorities)
+            return fail(LLX_ERR_INVALID_ARG, "reqs[%d].priority = %d not in [0,%d)", i, r.priority, num_priorities);
+        if (!r.is_queuing && !r.is_fake) {
+            ++per_prio[(size_t)r.priority];
+            ++running;
+        }
+    }
+    double total = 0.0;
+    for (int i = 0; i < n; ++i) {
+        const llx_req_info& r = reqs[i];
+        double v;
+        if (r.is_queuing)
+            v = r.is_head_of_line ? r.demand : 0.0;  // lines 2-5
+        else if (r.is_fake)
+            v = std::numeric_limits<double>::infinity();  // lines 6-7
+        else
+            v = r.physical_usage + headroom_for_priority[r.priority] / per_prio[(size_t)r.priority];  // lines 8, 10
+        total += v;
+    }
+    if (is_terminating) total += std::numeric_limits<double>::infinity();  // lines 12-13: the fake request
+    const double B = running > 0 ? (double)running : 1.0;
+    *freeness = (M - total) / B;  // line 17
+    if (total_virtual_usage) *total_virtual_usage = total;
+    return LLX_OK;
+}
+
+llx_status llx_pair_instances(const double* freeness, int n, double src_below, double dst_above, int32_t* src_out,
+                              int32_t* dst_out, int cap, int* n_pairs) {
+    if (n < 0 || !n_pairs || (n > 0 && !freeness) || cap < 0 || (cap > 0 && (!src_out || !dst_out)))
+        return fail(LLX_ERR_INVALID_ARG, "bad arguments");
+    if (src_below > dst_above) return fail(LLX_ERR_INVALID_ARG, "thresholds overlap: src_below %g > dst_above %g", src_below, dst_above);
+    std::vector<int32_t> src, dst;
+    for (int i = 0; i < n; ++i) {
+        if (freeness[i] < src_below) src.push_back(i);
+        if (freeness[i] > dst_above) dst.push_back(i);
+    }
+    std::stable_sort(src.begin(), src.end(), [&](int32_t a, int32_t b) { return freeness[a] < freeness[b]; });
+    std::stable_sort(dst.begin(), dst.end(), [&](int32_t a, int32_t b) { return freeness[a] > freeness[b]; });
+    const int pairs = (int)std::min(src.size(), dst.size());
+    *n_pairs = pairs;
+    if (pairs > cap) return fail(LLX_ERR_INVALID_ARG, "%d pairs, output holds %d", pairs, cap);
+    for (int k = 0; k < pairs; ++k) {
+        src_out[k] = src[(size_t)k];
+        dst_out[k] = dst[(size_t)k];
+    }
+    return LLX_OK;
+}
+
+llx_status llx_migration_order(const int32_t* priority, const int32_t* seq_len, int n, int32_t* order_out) {
+    if (n < 0 || (n > 0 && (!priority || !seq_len || !order_out))) return fail(LLX_ERR_INVALID_ARG, "bad arguments");
+    for (int i = 0; i < n; ++i) order_out[i] = i;
+    std::stable_sort(order_out, order_out + n, [&](int32_t a, int32_t b) {
+        return priority[a] != priority[b] ? priority[a] < priority[b] : seq_len[a] < seq_len[b];
+    });
+    return LLX_OK;
+}
+
+}  // extern "C"
