@@ -279,6 +279,11 @@ typedef enum {
     LLX_OPT_BANDWIDTH_GBPS = 10,/* bandwidth budget of device<->device copies in GB/s, read + written (0 = unlimited):
                                    one paced ring per SM instead of a few full-speed CTAs, so that a co-running
                                    decode step loses the same small share on every SM (<= 1 %) */
+    LLX_OPT_DYNAMIC_TAIL_PCT = 12, /* bulk kernel: share (%) of a long stage's chunks that is not pre-assigned to a ring but
+                                   claimed in small batches by whichever ring finishes its range first (default 6; 0 = off) */
+    LLX_OPT_DYNAMIC_TAIL_BATCH = 13, /* chunks per claim of the dynamic tail (0 = auto: 4) */
+    LLX_OPT_EXACT_RESIDENCY = 14, /* 1 (default): the bulk kernel asks for enough shared memory that no SM can hold more of its
+                                   CTAs than intended, early-launched CTAs of the next kernel included */
     LLX_OPT_VIA_HOST_MODE = 11  /* llx_migrate_via_host with a pinned-host buffer: 0 (default) copy engines through device
                                    bounce buffers, both link directions at once; 1 the kernels address the host buffer directly */
 } llx_option;

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <mutex>
+#include <unordered_map>
 #include <vector>
 
 #include "llx_attention.cuh"
@@ -63,13 +64,14 @@ int elem_bytes_of(llx_dtype d) {
 
 // ---- options / counters -------------------------------------------------------------------
 std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
-    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0};
+    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
 // ---- device properties (cached per device) ------------------------------------------------
 struct DevInfo {
     int sm_count = 0;
     int max_smem_optin = 0;
+    int smem_per_sm = 0;
     bool ready = false;
 };
 std::mutex g_dev_mu;
@@ -82,6 +84,7 @@ llx_status dev_info(int dev, DevInfo** out) {
     if (!d.ready) {
         LLX_CUDA(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
         LLX_CUDA(cudaDeviceGetAttribute(&d.max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        LLX_CUDA(cudaDeviceGetAttribute(&d.smem_per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
         LLX_CUDA(cudaFuncSetAttribute(llx_copy_bulk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
         LLX_CUDA(cudaFuncSetAttribute(llx_copy_bulk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
         d.ready = true;
@@ -134,6 +137,36 @@ llx_status ring_stage(const int32_t* a, size_t na, const int32_t* b, size_t nb, 
     s.used = true;
     *dev_out = s.dev;
     *slot_out = &s;
+    return LLX_OK;
+}
+
+// ---- claim counters of the bulk kernel's dynamic tail: one per (device, stream).  Launches of one stream are
+// ordered (with programmatic dependent launch too: the claims come after griddepcontrol.wait), and every launch
+// leaves its counter at zero again (its last claim resets it), so a stream's launches can share one counter
+// without any event between them — an event record between two kernels would cost the PDL overlap. ----------
+constexpr int kDynCounters = 4096;
+std::mutex g_dyn_mu;
+unsigned int* g_dyn_counters[64] = {};
+std::unordered_map<cudaStream_t, int> g_dyn_of_stream[64];
+
+// *counter = nullptr when the device's counters are all taken (the launch then runs without a dynamic tail)
+llx_status dyn_counter_get(int dev, cudaStream_t st, unsigned int** counter) {
+    std::lock_guard<std::mutex> lk(g_dyn_mu);
+    if (!g_dyn_counters[dev]) {
+        LLX_CUDA(cudaMalloc(&g_dyn_counters[dev], kDynCounters * sizeof(unsigned int)));
+        LLX_CUDA(cudaMemset(g_dyn_counters[dev], 0, kDynCounters * sizeof(unsigned int)));
+        LLX_CUDA(cudaDeviceSynchronize());
+    }
+    auto& m = g_dyn_of_stream[dev];
+    auto it = m.find(st);
+    if (it == m.end()) {
+        if ((int)m.size() >= kDynCounters) {
+            *counter = nullptr;
+            return LLX_OK;
+        }
+        it = m.emplace(st, (int)m.size()).first;
+    }
+    *counter = g_dyn_counters[dev] + it->second;
     return LLX_OK;
 }
 
@@ -211,16 +244,19 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     const int slices = 2 * layers;
 
     if (kern == 2) {
-        // Tuned on B200 (profiles/r01_copy_sweep.md): 2 CTAs per SM, each one ring of 4 x 8 KiB, every ring
-        // streaming a CONTIGUOUS range of chunks.  More bytes in flight than ~64 KiB per SM lowers DRAM efficiency.
-        if (nstages <= 0) nstages = budget > 0 ? 2 : 4;
-        if (chunk <= 0) chunk = budget > 0 ? 2048 : 8192;  // paced: a 4 KiB ring stays below the L1 carve-out step
+        // Tuned on B200 (profiles/r01_copy_sweep.md, r01_dynamic_tail.md): ONE CTA per SM with one ring of 3 x 32 KiB,
+        // every ring streaming a contiguous range of chunks and the last 6 % of the stage claimed dynamically
+        // (6.57 TB/s at 112 blocks, 6.66 TB/s at >= 256).  More bytes in flight per SM lowers DRAM efficiency.
+        // A short stage (the final one: 2 blocks) is latency-bound: smaller chunks over twice as many rings.
+        const bool short_stage = total_bytes < (64ll << 20);
+        if (nstages <= 0) nstages = budget > 0 ? 2 : short_stage ? 4 : 3;
+        if (chunk <= 0) chunk = budget > 0 ? 2048 : short_stage ? 8192 : 32768;  // paced: a 4 KiB ring stays below the L1 carve-out step
         if (chunk > tile_bytes) chunk = tile_bytes;
         chunk &= ~15ll;
         int rings = (int)g_opt_rings.load();
         if (rings <= 0) rings = 1;
         threads = 32 * rings;
-        smem = (((size_t)rings * nstages * 8 + 127) & ~(size_t)127) + (size_t)rings * nstages * chunk;
+        smem = (((size_t)rings * nstages * 12 + 127) & ~(size_t)127) + (size_t)rings * nstages * chunk;
         if ((long long)smem > di->max_smem_optin) return fail(LLX_ERR_INVALID_ARG, "ring of %d x %lld bytes exceeds shared memory", nstages, chunk);
     } else {
         if (budget > 0) {  // ~2 GB/s (rd+wr) per warp keeps the loads latency-bound and gentle; spread over all SMs
@@ -247,8 +283,20 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     if (kern == 2) {
         int per_sm = (int)((size_t)di->max_smem_optin / (smem + 1024));  // 1 KiB per-CTA reservation
         if (per_sm > 2) per_sm = 2;
-        if (per_sm < 1 || budget > 0) per_sm = 1;
+        if (per_sm < 1 || budget > 0 || total_bytes >= (64ll << 20)) per_sm = 1;
         grid = di->sm_count * per_sm;
+        // Exact residency: with programmatic dependent launch the NEXT kernel's CTAs are placed while this kernel
+        // still runs, wherever shared memory is free — several on one SM if they fit.  A ring's share of the stage is
+        // fixed, so an SM that ends up with more rings than its neighbours becomes the straggler (measured: 3 CTAs/SM
+        // of 25 KiB: 351 us per step without PDL, 449-509 us with it).  Asking for just over 1/(per_sm+1) of the
+        // SM's shared memory caps every SM at per_sm bulk CTAs, of this launch and of the next one together.
+        long long want = per_sm;  // CTAs per SM the launch is meant to have
+        const long long capv = g_opt_max_ctas.load();
+        if (capv > 0) want = (capv % di->sm_count == 0) ? capv / di->sm_count : 0;
+        if (g_opt_smem_pad.load() && budget <= 0 && want >= 1 && want <= 6) {
+            const size_t floor_bytes = (size_t)di->smem_per_sm / (size_t)(want + 1) - 1024 + 128;
+            if (smem < floor_bytes && floor_bytes <= (size_t)di->max_smem_optin) smem = floor_bytes;
+        }
     } else if (budget <= 0) {
         // A side in host memory is bound by the host link (~52 GB/s): one CTA per SM already saturates it
         // (measured: 52.7 GB/s with 74..296 CTAs, 51.5 with 1184) and leaves the SMs to whatever else is running.
@@ -286,6 +334,31 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     a.blocked_order = (int)g_opt_order.load();
     a.l2_hint = (int)g_opt_l2hint.load();
     a.pace_ns = (int)pace_ns;
+    a.dyn_units = 0;
+    a.dyn_batch = 1;
+    a.dyn_claims = 0;
+    a.dyn_counter = nullptr;
+    {
+        // Dynamic tail (bulk kernel, blocked order, stages long enough to have a tail worth evening out): SMs do not
+        // stream at exactly the same rate, so with fixed ranges the fastest rings idle at the end (ncu: SM active
+        // cycles avg 96.4 % vs max 98.9 % of the kernel).  The last dyn_pct % of the units are claimed in batches.
+        // Measured (B200, 7B tiles): 112 blocks 295.4 -> 291.3 us, 256 blocks 672 -> 656 us at 4-8 %; 1 % and 15 %
+        // give half of that, 100 % (no contiguous ranges at all) is 3 % slower than none.
+        const long long pct = g_opt_dyn_pct.load();
+        const long long nrings = (long long)grid * (threads / 32);
+        if (kern == 2 && a.blocked_order && pct > 0 && budget <= 0 && units >= nrings * 16) {
+            const long long batch = g_opt_dyn_batch.load() > 0 ? g_opt_dyn_batch.load() : 4;
+            long long dyn = units * pct / 100 / batch * batch;
+            if (dyn > 0) {
+                if ((rc = dyn_counter_get(device, st, &a.dyn_counter)) != LLX_OK) return rc;
+                if (a.dyn_counter) {
+                    a.dyn_units = (int)dyn;
+                    a.dyn_batch = (int)batch;
+                    a.dyn_claims = (unsigned int)(dyn / batch + nrings);
+                }
+            }
+        }
+    }
 
     static thread_local IdPack pack;  // 2 KiB; only the first n entries are meaningful
     const bool byval = n <= g_opt_byval.load();
@@ -865,6 +938,18 @@ llx_status llx_set_option(llx_option opt, long long v) {
             if (v < 0 || v > 1) break;
             g_opt_via_host = v;
             return LLX_OK;
+        case LLX_OPT_DYNAMIC_TAIL_PCT:
+            if (v < 0 || v > 100) break;
+            g_opt_dyn_pct = v;
+            return LLX_OK;
+        case LLX_OPT_DYNAMIC_TAIL_BATCH:
+            if (v < 0 || v > 4096) break;
+            g_opt_dyn_batch = v;
+            return LLX_OK;
+        case LLX_OPT_EXACT_RESIDENCY:
+            if (v < 0 || v > 1) break;
+            g_opt_smem_pad = v;
+            return LLX_OK;
     }
     return fail(LLX_ERR_INVALID_ARG, "option %d: bad value %lld", (int)opt, v);
 }
@@ -882,6 +967,9 @@ long long llx_get_option(llx_option opt) {
         case LLX_OPT_PDL: return g_opt_pdl;
         case LLX_OPT_BANDWIDTH_GBPS: return g_opt_budget;
         case LLX_OPT_VIA_HOST_MODE: return g_opt_via_host;
+        case LLX_OPT_DYNAMIC_TAIL_PCT: return g_opt_dyn_pct;
+        case LLX_OPT_DYNAMIC_TAIL_BATCH: return g_opt_dyn_batch;
+        case LLX_OPT_EXACT_RESIDENCY: return g_opt_smem_pad;
     }
     return -1;
 }

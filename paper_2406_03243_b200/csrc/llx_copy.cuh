@@ -48,6 +48,11 @@ struct CopyArgs {
     int blocked_order;  // 0: worker w takes units w, w+W, ...; 1: worker w takes a contiguous range
     int l2_hint;        // bit0: loads L2::evict_first, bit1: stores L2::evict_first (bulk kernel)
     int pace_ns;        // bulk kernel: minimum time between two chunks of one ring (0 = unthrottled)
+    // bulk kernel, blocked order: the last dyn_units units are not pre-assigned; rings that finish their
+    // contiguous range early claim them in batches of dyn_batch from *dyn_counter (evens out the tail)
+    int dyn_units, dyn_batch;
+    unsigned int dyn_claims;    // claims this launch makes in total (batches + one failed claim per ring): the last one resets the counter
+    unsigned int* dyn_counter;  // device, zero before the launch
 };
 
 __device__ __forceinline__ uint4 ld_stream16(const void* p) {
@@ -219,9 +224,10 @@ __device__ __forceinline__ void bulk_wait_read() {
 }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-// Shared memory: [rings_per_cta][nstages] mbarriers (8 B each, padded to 128 B per ring group),
-// then [rings_per_cta][nstages][chunk_bytes] data.  Ring r of the grid handles units
-// r, r+nrings, r+2*nrings, ...; lane 0 of each warp is the ring's only working thread.
+// Shared memory: [rings_per_cta][nstages] mbarriers (8 B each) and [rings_per_cta][nstages] unit numbers (4 B each),
+// padded to 128 B, then [rings_per_cta][nstages][chunk_bytes] data.  Lane 0 of each warp is the ring's only
+// working thread.  Striped order: ring r handles units r, r+nrings, ...  Blocked order: ring r streams the
+// contiguous range [r*Ts/W, (r+1)*Ts/W) of the first Ts = total - dyn_units units, then claims batches of the rest.
 template <bool BYVAL>
 __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack ids, int nstages) {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -229,8 +235,9 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
     const int rings_per_cta = blockDim.x >> 5;
     if ((threadIdx.x & 31) != 0) return;
 
-    const int bar_bytes = ((rings_per_cta * nstages * 8) + 127) & ~127;
+    const int bar_bytes = ((rings_per_cta * nstages * 12) + 127) & ~127;
     const uint32_t bar0 = smem_u32(smem) + warp * nstages * 8;
+    int* unit_of = reinterpret_cast<int*>(smem + rings_per_cta * nstages * 8) + warp * nstages;
     const uint32_t buf0 = smem_u32(smem) + bar_bytes + warp * nstages * a.chunk_bytes;
 
     for (int s = 0; s < nstages; ++s) mbar_init(bar0 + s * 8, 1);
@@ -241,25 +248,44 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
 
     const int ring = blockIdx.x * rings_per_cta + warp;
     const int nrings = gridDim.x * rings_per_cta;
-    int K, u0, ustep;  // this ring handles units u0, u0+ustep, ... (K of them)
+    // the ring's unit stream: a pre-assigned arithmetic sequence, then (blocked order only) claimed batches
+    int s_next, s_end, s_step;
+    const int static_units = a.total_units - a.dyn_units;
     if (a.blocked_order) {
-        // balanced contiguous ranges: ring r takes [r*T/W, (r+1)*T/W)
-        u0 = (int)((long long)ring * a.total_units / nrings);
-        ustep = 1;
-        K = (int)((long long)(ring + 1) * a.total_units / nrings) - u0;
-        if (K <= 0) return;
+        s_next = (int)((long long)ring * static_units / nrings);
+        s_end = (int)((long long)(ring + 1) * static_units / nrings);
+        s_step = 1;
     } else {
-        if (ring >= a.total_units) return;
-        u0 = ring;
-        ustep = nrings;
-        K = (a.total_units - ring + nrings - 1) / nrings;
+        s_next = ring;
+        s_end = a.total_units;
+        s_step = nrings;
     }
+    int d_next = 0, d_end = 0;
+    bool dyn_done = a.dyn_units == 0;
+    auto next_unit = [&]() -> int {
+        if (s_next < s_end) {
+            const int u = s_next;
+            s_next += s_step;
+            return u;
+        }
+        if (d_next < d_end) return d_next++;
+        if (dyn_done) return -1;
+        const unsigned int b = atomicAdd(a.dyn_counter, 1u);
+        if (b == a.dyn_claims - 1) *a.dyn_counter = 0;  // every ring fails exactly once: this was the launch's last claim
+        const long long lo = (long long)b * a.dyn_batch;
+        if (lo >= a.dyn_units) {
+            dyn_done = true;
+            return -1;
+        }
+        d_next = static_units + (int)lo;
+        d_end = d_next + a.dyn_batch < a.total_units ? d_next + a.dyn_batch : a.total_units;
+        return d_next++;
+    };
     const uint64_t pol = policy_evict_first();
     const bool hint_ld = a.l2_hint & 1, hint_st = a.l2_hint & 2;
     unsigned long long deadline = a.pace_ns > 0 ? global_timer_ns() : 0ull;
 
-    auto addr_of = [&](int k) -> UnitAddr {
-        int u = u0 + k * ustep;
+    auto addr_of = [&](int u) -> UnitAddr {
         int i, slice, c;
         unit_coords(a, u, i, slice, c);
         int item_s = i, item_d = i;
@@ -267,9 +293,9 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
         if (a.dst_indexed) item_d = BYVAL ? ids.dst[i] : __ldg(a.dst_ids + i);
         return unit_addr(a, slice, c, item_s, item_d);
     };
-    auto issue_load = [&](int k) {
-        const int s = k % nstages;
-        UnitAddr ua = addr_of(k);
+    auto issue_load = [&](int s, int u) {
+        unit_of[s] = u;
+        UnitAddr ua = addr_of(u);
         mbar_expect_tx(bar0 + s * 8, (uint32_t)ua.len);
         if (hint_ld)
             bulk_g2s_hint(buf0 + s * a.chunk_bytes, ua.src, (uint32_t)ua.len, bar0 + s * 8, pol);
@@ -277,12 +303,16 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
             bulk_g2s(buf0 + s * a.chunk_bytes, ua.src, (uint32_t)ua.len, bar0 + s * 8);
     };
 
-    const int pre = K < nstages ? K : nstages;
-    for (int k = 0; k < pre; ++k) issue_load(k);
-    for (int k = 0; k < K; ++k) {
+    int issued = 0;
+    for (; issued < nstages; ++issued) {
+        const int u = next_unit();
+        if (u < 0) break;
+        issue_load(issued, u);
+    }
+    for (int k = 0; k < issued; ++k) {
         const int s = k % nstages;
         mbar_wait(bar0 + s * 8, (uint32_t)((k / nstages) & 1));
-        UnitAddr ua = addr_of(k);
+        UnitAddr ua = addr_of(unit_of[s]);
         if (hint_st)
             bulk_s2g_hint(ua.dst, buf0 + s * a.chunk_bytes, (uint32_t)ua.len, pol);
         else
@@ -299,9 +329,13 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
         }
         // refill the stage whose store was committed one iteration ago: allowing the newest
         // group to stay pending keeps one store and nstages-1 loads in flight per ring
-        if (k >= 1 && k - 1 + nstages < K) {
-            bulk_wait_read<1>();
-            issue_load(k - 1 + nstages);
+        if (k >= 1 && issued == k - 1 + nstages) {
+            const int u = next_unit();
+            if (u >= 0) {
+                bulk_wait_read<1>();
+                issue_load((k - 1) % nstages, u);
+                ++issued;
+            }
         }
     }
     bulk_wait_all();

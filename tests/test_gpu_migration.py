@@ -20,7 +20,9 @@ KERNELS = [dict(copy_kernel=2), dict(copy_kernel=1), dict(copy_kernel=2, chunk_b
            dict(copy_kernel=1, chunk_bytes=2048), dict(copy_kernel=2, ids_by_value_max=0),
            dict(copy_kernel=1, ids_by_value_max=0), dict(copy_kernel=2, max_ctas=3), dict(copy_kernel=1, max_ctas=1),
            dict(bandwidth_gbps=40), dict(bandwidth_gbps=3000), dict(copy_kernel=2, unit_order=0), dict(copy_kernel=1, unit_order=0),
-           dict(copy_kernel=2, l2_hint=3, rings_per_cta=2), dict(pdl=0)]
+           dict(copy_kernel=2, l2_hint=3, rings_per_cta=2), dict(pdl=0),
+           dict(copy_kernel=2, dynamic_tail_pct=30, max_ctas=2, chunk_bytes=1024),
+           dict(copy_kernel=2, dynamic_tail_pct=100, max_ctas=3, chunk_bytes=512, ring_stages=3, rings_per_cta=2)]
 
 
 @pytest.fixture(scope="module")
