@@ -1,6 +1,8 @@
 """Sweep the copy-kernel launch options on the current GPU and print GB/s (rd+wr) per configuration.
 
     python -m paper_2406_03243_b200.tune [--blocks 128,112,14,2] [--top 25] [--quick]
+    python -m paper_2406_03243_b200.tune --mode tail     # dynamic-tail share x batch, then ring shapes under it
+    python -m paper_2406_03243_b200.tune --mode step     # the whole configs[1] step under global option sets
 
 The defaults compiled into libllx.so (llx_api.cu, launch_copy) come from this sweep on a B200; the output
 of one run is kept in profiles/r01_copy_sweep.md.  Workload: configs[1] pools (LLaMA-7B shape, 2 x 2000
@@ -16,12 +18,97 @@ import sys
 import numpy as np
 
 
+def _setup():
+    import torch
+
+    import paper_2406_03243_b200 as llx
+    import synth
+    from paper_2406_03243_b200.suite import Pools
+    llx.load()
+    g = synth.CONFIGS["llama7b"]
+    nb = g["num_blocks"]
+    p = Pools(torch, llx, g, nb, nb)
+    return torch, llx, synth, g, nb, p, torch.cuda.Stream()
+
+
+def _back_to_back(torch, st, fn, reps=7, inner=10):
+    """us per launch, `inner` launches between one pair of events (launch gaps overlapped as in a real stream)."""
+    for _ in range(3):
+        fn()
+    st.synchronize()
+    ts = []
+    for _ in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(st)
+        for _ in range(inner):
+            fn()
+        b.record(st)
+        st.synchronize()
+        ts.append(a.elapsed_time(b) / inner)
+    return statistics.median(ts) * 1e3
+
+
+def mode_tail():
+    torch, llx, synth, g, nb, p, st = _setup()
+    s_tab, d_tab = synth.block_permutation(1, nb), synth.block_permutation(2, nb)
+    for n in (112, 128, 256):
+        nbytes = 2 * n * p.src.block_bytes
+        mig = lambda: llx.migrate_stage(p.src, s_tab[:n], p.dst, d_tab[:n], stream=st)
+        print(f"\n== {n} blocks, bulk kernel, back-to-back launches; GB/s = rd+wr")
+        print("| us | GB/s | chunk | stages | CTAs | tail % | batch |\n|---|---|---|---|---|---|---|")
+        for chunk, stages, cap in ((8192, 4, 296), (32768, 3, 148), (32768, 2, 296), (8192, 3, 444)):
+            for pct, batch in [(0, 0)] + [(q, b) for q in (1, 3, 6, 10, 15, 30, 100) for b in ((4,) if q != 6 else (1, 4, 16, 32))]:
+                with llx.options(chunk_bytes=chunk, ring_stages=stages, max_ctas=cap, dynamic_tail_pct=pct, dynamic_tail_batch=batch):
+                    t = _back_to_back(torch, st, mig)
+                print(f"| {t:.1f} | {nbytes / t / 1e3:.0f} | {chunk} | {stages} | {cap} | {pct} | {batch or '-'} |")
+    return 0
+
+
+def mode_step():
+    torch, llx, synth, g, nb, p, st = _setup()
+    s_tab, d_tab = synth.block_permutation(1, nb)[:128], synth.block_permutation(2, nb)[:128]
+    tok_bytes = g["layers"] * 2 * g["kv_heads"] * g["head_dim"] * 2
+    vals = torch.zeros(16 * tok_bytes, dtype=torch.uint8, device="cuda")
+    schedule, start = (112, 14, 2), 2032
+
+    def step():
+        tokens, m = start, 0
+        for k, n in enumerate(schedule):
+            llx.migrate_stage(p.src, s_tab[m:m + n], p.dst, d_tab[m:m + n], stream=st)
+            m += n
+            if k < 2:
+                llx.append_tokens(p.src, s_tab, tokens, tokens + 8, vals.data_ptr() + (tokens - start) * tok_bytes, stream=st)
+                tokens += 8
+    nbytes = 2 * 128 * p.src.block_bytes
+    cfgs = {"8Kx4 2/SM static (round-1 default until now)": dict(chunk_bytes=8192, ring_stages=4, max_ctas=296, dynamic_tail_pct=0),
+            "auto (32Kx3 1/SM tail 6 %; short stages 8Kx4 2/SM)": dict(),
+            "8Kx4 2/SM tail 6 %": dict(chunk_bytes=8192, ring_stages=4, max_ctas=296),
+            "8Kx3 3/SM tail 6 %": dict(chunk_bytes=8192, ring_stages=3, max_ctas=444),
+            "8Kx3 3/SM static": dict(chunk_bytes=8192, ring_stages=3, max_ctas=444, dynamic_tail_pct=0),
+            "32Kx3 1/SM tail 6 %": dict(chunk_bytes=32768, ring_stages=3, max_ctas=148),
+            "32Kx2 2/SM tail 6 %": dict(chunk_bytes=32768, ring_stages=2, max_ctas=296),
+            "16Kx3 2/SM tail 6 %": dict(chunk_bytes=16384, ring_stages=3, max_ctas=296)}
+    print("configs[1] step (stages 112/14/2 + two 8-token appends), 600 steps back to back, us per step\n")
+    print("| option set (all three stages) | exact residency | PDL | us/step | GB/s |\n|---|---|---|---|---|")
+    for name, o in cfgs.items():
+        for pad, pdl in ((1, 1), (0, 1), (1, 0)):
+            with llx.options(exact_residency=pad, pdl=pdl, **o):
+                t = _back_to_back(torch, st, step, reps=3, inner=200)
+            print(f"| {name} | {pad} | {pdl} | {t:.2f} | {nbytes / t / 1e3:.0f} |")
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--mode", choices=["sweep", "tail", "step"], default="sweep")
     ap.add_argument("--blocks", default="128,112,14,2")
     ap.add_argument("--top", type=int, default=25)
     ap.add_argument("--quick", action="store_true")
     args = ap.parse_args()
+    if args.mode == "tail":
+        return mode_tail()
+    if args.mode == "step":
+        return mode_step()
     import torch
 
     import paper_2406_03243_b200 as llx
