@@ -433,8 +433,28 @@ def measure_downtime(torch, llx, w, stream, reps=100):
     dp = d_ids.ctypes.data_as(C.POINTER(C.c_int32))
     sh, dh, st = w.src.handle, w.dst.handle, stream.cuda_stream
     tok_bytes = g["layers"] * 2 * g["kv_heads"] * g["head_dim"] * 2
-    host_us, gpu_us = [], []
+    host_us, gpu_us, wait_us = [], [], []
     ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def earlier_stages():
+        tokens, mm = START_TOKENS, 0
+        for k, n in enumerate(SCHEDULE[:-1]):
+            llx.migrate_stage(w.src, w.s_tab[mm:mm + n], w.dst, w.d_tab[mm:mm + n], stream=stream)
+            mm += n
+            llx.append_tokens(w.src, w.s_tab, tokens, tokens + APPENDS[k],
+                              w.append_dev.data_ptr() + (tokens - START_TOKENS) * tok_bytes, stream=stream)
+            tokens += APPENDS[k]
+        stream.synchronize()
+
+    for rep in range(reps + 5):      # the library's own blocking call: completion flag in pinned host memory
+        earlier_stages()
+        t0 = time.perf_counter_ns()
+        rc = lib.llx_migrate_stage_wait(sh, sp, dh, dp, n_final, st)
+        t1 = time.perf_counter_ns()
+        assert rc == 0
+        if rep >= 5:
+            wait_us.append((t1 - t0) / 1e3)
+    wait_us.sort()
     for rep in range(reps + 5):
         tokens, mm = START_TOKENS, 0
         for k, n in enumerate(SCHEDULE[:-1]):
@@ -463,9 +483,12 @@ def measure_downtime(torch, llx, w, stream, reps=100):
     q = lambda v, p: v[min(len(v) - 1, int(p * len(v)))]
     return {"final_stage_blocks": n_final, "final_stage_bytes_rd_plus_wr": 2 * n_final * w.src.block_bytes,
             "host_median": q(host_us, 0.5), "host_p99": q(host_us, 0.99), "host_min": host_us[0],
+            "host_wait_call_median": q(wait_us, 0.5), "host_wait_call_p99": q(wait_us, 0.99), "host_wait_call_min": wait_us[0],
             "gpu_median": q(gpu_us, 0.5), "gpu_min": gpu_us[0], "reps": reps,
-            "definition": "host wall clock from entering llx_migrate_stage(final) to return of the stream "
-                          "synchronize; gpu_* = CUDA-event duration of the same launch repeated (L2-warm)"}
+            "definition": "host_*: host wall clock from entering llx_migrate_stage(final) to return of the stream "
+                          "synchronize; host_wait_call_*: the same interval around ONE llx_migrate_stage_wait call "
+                          "(the kernel's last CTA writes a pinned host word the caller spins on); gpu_* = CUDA-event "
+                          "duration of the same launch repeated (L2-warm)"}
 
 
 def run_suite(torch, llx, stream):

@@ -121,6 +121,15 @@ llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, i
 llx_status llx_migrate_stage(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
                              const int32_t* dst_block_ids, int n, void* cuda_stream);
 
+/* The final stage as ONE blocking call (its duration is the request's downtime): llx_migrate_stage,
+ * then the call returns only when the copy — and everything enqueued on cuda_stream before it — is complete.
+ * The kernel's last CTA writes a word in pinned host memory that the calling thread spins on, which is shorter
+ * than a stream synchronize through the driver; if that is not possible (another copy kernel selected by an
+ * option, all flag slots in use) it falls back to the stream synchronize.  Same checks and errors as
+ * llx_migrate_stage; LLX_ERR_CUDA also reports an asynchronous fault of the copy itself. */
+llx_status llx_migrate_stage_wait(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
+                                  const int32_t* dst_block_ids, int n, void* cuda_stream);
+
 /* ---- S5: many requests in ONE launch (the source migrates its chosen
  * requests one after another; batching them is this build's extension) -------------------- */
 

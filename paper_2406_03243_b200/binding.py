@@ -49,6 +49,7 @@ EXPORTS = {
     "llx_pool_fill_u16": (_i, [_vp, C.c_uint16, _vp]),
     "llx_plan_stage": (_i, [_i, _i, _i, _i, C.POINTER(_i), C.POINTER(_i)]),
     "llx_migrate_stage": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp]),
+    "llx_migrate_stage_wait": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp]),
     "llx_migrate_batch": (_i, [_vp, _vp, _i32p, _i32p, _i32p, _i, _vp]),
     "llx_staging_bytes": (_sz, [_vp, _i]),
     "llx_staging_alloc_pinned": (_i, [_sz, C.POINTER(_vp), C.POINTER(_vp)]),
@@ -210,6 +211,15 @@ def migrate_stage(src: Pool, src_block_ids, dst: Pool, dst_block_ids, stream=Non
     if s.size != d.size:
         raise LlxError(-1, "LLX_ERR_INVALID_ARG", "src/dst id lists differ in length")
     _check(load().llx_migrate_stage(src.handle, sp, dst.handle, dp, s.size, _stream(stream)))
+
+
+def migrate_stage_wait(src: Pool, src_block_ids, dst: Pool, dst_block_ids, stream=None):
+    """llx_migrate_stage + wait for its completion (the final stage: downtime ends when this returns)."""
+    s, sp = _ids(src_block_ids)
+    d, dp = _ids(dst_block_ids)
+    if s.size != d.size:
+        raise LlxError(-1, "LLX_ERR_INVALID_ARG", "src/dst id lists differ in length")
+    _check(load().llx_migrate_stage_wait(src.handle, sp, dst.handle, dp, s.size, _stream(stream)))
 
 
 def migrate_batch(src: Pool, dst: Pool, req_offsets, src_block_ids, dst_block_ids, stream=None):

@@ -170,6 +170,53 @@ llx_status dyn_counter_get(int dev, cudaStream_t st, unsigned int** counter) {
     return LLX_OK;
 }
 
+// ---- completion flags of llx_migrate_stage_wait: a word in mapped pinned host memory that the kernel's last
+// ring writes, plus the device counter that finds the last ring.  A few slots, one per concurrent waiter. ----
+struct DoneSlot {
+    volatile unsigned int* host = nullptr;  // mapped pinned word
+    unsigned int* dev_alias = nullptr;
+    unsigned int* counter = nullptr;  // device
+    unsigned int seq = 0;
+    bool busy = false;
+};
+constexpr int kDoneSlots = 16;
+std::mutex g_done_mu;
+DoneSlot g_done[64][kDoneSlots];
+
+struct DoneReq {  // set by llx_migrate_stage_wait around its launch_copy
+    DoneSlot* slot = nullptr;
+    bool armed = false;  // launch_copy attached the flag to the kernel it launched
+};
+thread_local DoneReq* tl_done = nullptr;
+
+llx_status done_slot_get(int dev, DoneSlot** out) {
+    std::lock_guard<std::mutex> lk(g_done_mu);
+    for (auto& d : g_done[dev]) {
+        if (d.busy) continue;
+        if (!d.host) {
+            void* h = nullptr;
+            LLX_CUDA(cudaHostAlloc(&h, 64, cudaHostAllocMapped | cudaHostAllocPortable));
+            void* da = nullptr;
+            LLX_CUDA(cudaHostGetDevicePointer(&da, h, 0));
+            LLX_CUDA(cudaMalloc(&d.counter, sizeof(unsigned int)));
+            LLX_CUDA(cudaMemset(d.counter, 0, sizeof(unsigned int)));
+            LLX_CUDA(cudaDeviceSynchronize());
+            d.host = (volatile unsigned int*)h;
+            *d.host = 0;
+            d.dev_alias = (unsigned int*)da;
+        }
+        d.busy = true;
+        *out = &d;
+        return LLX_OK;
+    }
+    *out = nullptr;  // all slots taken: the caller falls back to the stream synchronize
+    return LLX_OK;
+}
+void done_slot_put(DoneSlot* d) {
+    std::lock_guard<std::mutex> lk(g_done_mu);
+    d->busy = false;
+}
+
 // ---- validation ------------------------------------------------------------------------------
 llx_status check_pool(const llx_pool* p, const char* name) {
     if (!p || !p->data) return fail(LLX_ERR_INVALID_ARG, "%s pool is NULL", name);
@@ -338,6 +385,18 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     a.dyn_batch = 1;
     a.dyn_claims = 0;
     a.dyn_counter = nullptr;
+    a.done_counter = nullptr;
+    a.done_flag = nullptr;
+    a.done_value = 0;
+    a.done_rings = 0;
+    if (tl_done && tl_done->slot && kern == 2) {
+        DoneSlot* d = tl_done->slot;
+        a.done_counter = d->counter;
+        a.done_flag = d->dev_alias;
+        a.done_value = ++d->seq;
+        a.done_rings = (unsigned int)((long long)grid * (threads / 32));
+        tl_done->armed = true;
+    }
     {
         // Dynamic tail (bulk kernel, blocked order, stages long enough to have a tail worth evening out): SMs do not
         // stream at exactly the same rate, so with fixed ranges the fastest rings idle at the end (ncu: SM active
@@ -615,6 +674,45 @@ llx_status llx_migrate_stage(const llx_pool* src, const int32_t* src_ids, llx_po
     if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
     return launch_copy(pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
                        (cudaStream_t)stream);
+}
+
+llx_status llx_migrate_stage_wait(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
+                                  void* stream) {
+    if (n <= 0 || !src) return llx_migrate_stage(src, src_ids, dst, dst_ids, n, stream);  // nothing to wait for / argument error
+    DoneSlot* slot = nullptr;
+    llx_status rc = done_slot_get(src->device, &slot);
+    if (rc != LLX_OK) return rc;
+    DoneReq req;
+    req.slot = slot;
+    tl_done = &req;
+    rc = llx_migrate_stage(src, src_ids, dst, dst_ids, n, stream);
+    tl_done = nullptr;
+    if (rc != LLX_OK) {
+        if (slot) done_slot_put(slot);
+        return rc;
+    }
+    if (!req.armed) {  // no flag on this launch (another kernel was selected, or no free slot)
+        if (slot) done_slot_put(slot);
+        LLX_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+        return LLX_OK;
+    }
+    // spin on the word the kernel's last ring writes; an unset flag after 1e8 polls (seconds) means the launch
+    // failed asynchronously: let the stream synchronize report it
+    const unsigned int want = slot->seq;
+    bool seen = false;
+    for (long long i = 0; i < 100000000ll; ++i) {
+        if (*slot->host == want) {
+            seen = true;
+            break;
+        }
+#if defined(__x86_64__)
+        __builtin_ia32_pause();
+#endif
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    done_slot_put(slot);
+    if (!seen) LLX_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    return LLX_OK;
 }
 
 llx_status llx_migrate_batch(const llx_pool* src, llx_pool* dst, const int32_t* off, const int32_t* src_ids,

@@ -53,6 +53,11 @@ struct CopyArgs {
     int dyn_units, dyn_batch;
     unsigned int dyn_claims;    // claims this launch makes in total (batches + one failed claim per ring): the last one resets the counter
     unsigned int* dyn_counter;  // device, zero before the launch
+    // completion flag (llx_migrate_stage_wait): the ring that finishes last writes done_value to *done_flag
+    // (mapped pinned host memory) so that the host can spin on a word instead of going through the driver
+    unsigned int* done_counter;  // device, zero before the launch; nullptr = no flag
+    volatile unsigned int* done_flag;
+    unsigned int done_value, done_rings;
 };
 
 __device__ __forceinline__ uint4 ld_stream16(const void* p) {
@@ -338,7 +343,15 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
             }
         }
     }
-    bulk_wait_all();
+    bulk_wait_all();  // this ring's stores are complete
+    if (a.done_counter) {
+        __threadfence();
+        if (atomicAdd(a.done_counter, 1u) == a.done_rings - 1) {  // every ring has finished its stores
+            *a.done_counter = 0;
+            __threadfence_system();
+            *a.done_flag = a.done_value;
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------

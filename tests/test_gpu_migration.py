@@ -400,3 +400,28 @@ def test_migration_session_abort_releases_reservation_and_touches_nothing_else(e
     with pytest.raises(llx.LlxError) as e:
         llx.Migration(src.pool, src_mgr, dst.pool, wrong, g["block_size"], 2)
     assert e.value.name == "LLX_ERR_GEOMETRY_MISMATCH"
+
+
+@pytest.mark.parametrize("opts", [dict(), dict(copy_kernel=1), dict(copy_kernel=2, max_ctas=5), dict(bandwidth_gbps=500)])
+def test_migrate_stage_wait_returns_after_completion(env, opts):     # S4: the final stage as one blocking call
+    H, llx = env
+    g = RAGGED
+    src, dst, h_src, h_dst = make(H, g, seed=12)
+    torch.cuda.synchronize()
+    st, other = torch.cuda.Stream(), torch.cuda.Stream()
+    for rep in range(4):                                             # flag slots and sequence numbers are reused
+        s_ids = synth.block_permutation(60 + rep, g["num_blocks"])[:9]
+        d_ids = synth.block_permutation(70 + rep, g["num_blocks"])[:9]
+        with llx.options(**opts):
+            llx.migrate_stage(src.pool, s_ids[:6], dst.pool, d_ids[:6], stream=st)        # earlier stage, not synchronised
+            llx.migrate_stage_wait(src.pool, s_ids[6:], dst.pool, d_ids[6:], stream=st)
+        with torch.cuda.stream(other):                               # no synchronize of `st`: the call itself waited
+            snap = dst.view.clone()
+        other.synchronize()
+        om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+        H.assert_pool_equal(snap.cpu().numpy().view(np.uint16), h_dst)
+    llx.migrate_stage_wait(src.pool, [], dst.pool, [], stream=st)    # n == 0
+    with pytest.raises(llx.LlxError) as e:
+        llx.migrate_stage_wait(src.pool, [0, 1], dst.pool, [3, 3], stream=st)
+    assert e.value.name == "LLX_ERR_DUPLICATE_DST"
+    H.assert_pool_equal(dst.host(), h_dst)
