@@ -425,3 +425,36 @@ def test_migrate_stage_wait_returns_after_completion(env, opts):     # S4: the f
         llx.migrate_stage_wait(src.pool, [0, 1], dst.pool, [3, 3], stream=st)
     assert e.value.name == "LLX_ERR_DUPLICATE_DST"
     H.assert_pool_equal(dst.host(), h_dst)
+
+
+@pytest.mark.parametrize("opts", KERNELS)
+def test_guard_bands_around_pools_and_staging_stay_intact(env, opts):
+    """compute-sanitizer is closed on this pool of machines, so out-of-bounds writes are looked for directly:
+    pools and the staging buffer sit between 64 KiB guard bands that must keep their pattern."""
+    H, llx = env
+    g = RAGGED
+    L, nb, te = g["layers"], g["num_blocks"], H.tile_elems(g)
+    guard = 64 << 10
+    nbytes = llx.pool_bytes_for(L, g["kv_heads"], g["head_dim"], g["block_size"], llx.F16, nb)
+    n = 7
+    stg_bytes = n * 2 * L * te * 2
+    bufs = []
+    for size in (nbytes, nbytes, stg_bytes):
+        raw = torch.full((size + 2 * guard,), 0x5A, dtype=torch.uint8, device="cuda")
+        bufs.append(raw)
+    src = llx.pool_wrap(bufs[0].data_ptr() + guard, nbytes, L, g["kv_heads"], g["head_dim"], g["block_size"], llx.F16, nb)
+    dst = llx.pool_wrap(bufs[1].data_ptr() + guard, nbytes, L, g["kv_heads"], g["head_dim"], g["block_size"], llx.F16, nb)
+    bufs[0][guard:guard + nbytes] = torch.randint(0, 255, (nbytes,), dtype=torch.uint8, device="cuda")
+    ids_s = np.array([0, nb - 1, 1, nb - 2, 5, 17, 3])               # first and last blocks of every slice
+    ids_d = np.array([nb - 1, 0, nb - 2, 1, 9, 2, 30])
+    with llx.options(**opts):
+        llx.migrate_stage(src, ids_s, dst, ids_d)
+        llx.pack(src, ids_s, bufs[2].data_ptr() + guard, stg_bytes)
+        llx.unpack(bufs[2].data_ptr() + guard, stg_bytes, dst, ids_d)
+        llx.migrate_via_host(src, ids_s, dst, ids_d, bufs[2].data_ptr() + guard, stg_bytes, chunk_blocks=3)
+    torch.cuda.synchronize()
+    for raw, size in zip(bufs, (nbytes, nbytes, stg_bytes)):
+        assert bool((raw[:guard] == 0x5A).all()) and bool((raw[guard + size:] == 0x5A).all()), "guard band overwritten"
+    sv = bufs[0][guard:guard + nbytes].view(torch.int16).view(L, 2, nb, te)
+    dv = bufs[1][guard:guard + nbytes].view(torch.int16).view(L, 2, nb, te)
+    assert bool(torch.equal(dv[:, :, torch.from_numpy(ids_d).cuda()], sv[:, :, torch.from_numpy(ids_s).cuda()]))
