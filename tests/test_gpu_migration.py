@@ -458,3 +458,38 @@ def test_guard_bands_around_pools_and_staging_stay_intact(env, opts):
     sv = bufs[0][guard:guard + nbytes].view(torch.int16).view(L, 2, nb, te)
     dv = bufs[1][guard:guard + nbytes].view(torch.int16).view(L, 2, nb, te)
     assert bool(torch.equal(dv[:, :, torch.from_numpy(ids_d).cuda()], sv[:, :, torch.from_numpy(ids_s).cuda()]))
+
+
+@pytest.mark.parametrize("n", [255, 256, 257])
+def test_ids_by_value_boundary(env, n):
+    """256 pairs still travel in the kernel parameters, 257 go through the pinned id ring."""
+    H, llx = env
+    g = dict(TINY, num_blocks=300)
+    src, dst, h_src, h_dst = make(H, g, seed=3)
+    s_ids = synth.block_permutation(80, 300)[:n]
+    d_ids = synth.block_permutation(81, 300)[:n]
+    c0 = llx.counters()["id_uploads"]
+    llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids)
+    assert llx.counters()["id_uploads"] - c0 == (1 if n > 256 else 0)
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
+
+
+def test_default_launch_shape_with_dynamic_tail_on_a_mid_size_stage(env):
+    """A stage long enough (>= 64 MiB, >= 16 chunks per ring) that the DEFAULT options take the one-CTA-per-SM ring
+    with the dynamic tail; three launches back to back on one stream share the self-resetting claim counter."""
+    H, llx = env
+    g = dict(layers=4, kv_heads=8, head_dim=128, block_size=16, elem_bytes=2, num_blocks=700)      # 32 KiB tiles
+    src = H.DevPool(g)
+    src.fill_device_random(21)
+    dst = H.DevPool(g, fill=SENT)
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    perm_s, perm_d = synth.block_permutation(90, 700), synth.block_permutation(91, 700)
+    for a, b in ((0, 330), (330, 660), (660, 700)):                 # 330 blocks = 82.5 MiB: 2640 chunks of 32 KiB over 148 rings
+        llx.migrate_stage(src.pool, perm_s[a:b], dst.pool, perm_d[a:b], stream=st)
+    st.synchronize()
+    h_src = src.host()
+    h_dst = om.new_pool(g["layers"], 700, H.tile_elems(g), fill=SENT)
+    om.migrate_stage(h_src, perm_s, h_dst, perm_d)
+    H.assert_pool_equal(dst.host(), h_dst)
