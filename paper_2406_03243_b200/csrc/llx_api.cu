@@ -266,6 +266,7 @@ struct Side {
     const int32_t* ids;  // host ids or nullptr (contiguous side)
     long long slice_stride, item_stride;
     bool host_memory;  // staging in mapped host memory
+    int device = -1;   // pool side: the device its memory lives on (-1: staging)
 };
 
 llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers, long long tile_bytes, int device,
@@ -276,7 +277,9 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
 
     // kernel choice: the bulk-async ring for device<->device, the LDG/STG kernel when a side is host memory
     long long kern = g_opt_kernel.load();
-    if (kern == 0) kern = (src.host_memory || dst.host_memory) ? 1 : 2;
+    // a peer-mapped destination (another GPU) is written with plain 16-byte stores: NVLink, not HBM, is the bound
+    const bool peer = src.device >= 0 && dst.device >= 0 && src.device != dst.device;
+    if (kern == 0) kern = (src.host_memory || dst.host_memory || peer) ? 1 : 2;
     // Bandwidth budget: paced register-staged copies, no shared memory.  Measured
     // on B200: a co-resident CTA that holds > ~6 KB of shared memory shrinks the L1 of its SM and slows a
     // bandwidth-bound decode kernel by 30 %, and a few full-speed CTAs turn their SMs into stragglers.
@@ -456,7 +459,7 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
 }
 
 Side pool_side(const llx_pool* p, const int32_t* ids) {
-    return Side{p->data, ids, (long long)p->num_blocks * p->tile_bytes, p->tile_bytes, false};
+    return Side{p->data, ids, (long long)p->num_blocks * p->tile_bytes, p->tile_bytes, false, p->device};
 }
 llx_status staging_side(const void* staging, int layers, long long tile_bytes, Side* out) {
     cudaPointerAttributes at;
@@ -473,8 +476,19 @@ llx_status staging_side(const void* staging, int layers, long long tile_bytes, S
 llx_status check_pair(const llx_pool* src, const llx_pool* dst) {
     llx_status rc = check_pool(src, "src");
     if (rc != LLX_OK) return rc;
-    rc = check_pool(dst, "dst");
-    if (rc != LLX_OK) return rc;
+    // The destination may live on ANOTHER GPU (the two instances are different
+    // machines): the kernel runs on the source's device and stores straight into the peer-mapped pool over NVLink.
+    if (dst && dst->data && dst->device != src->device) {
+        int can = 0;
+        LLX_CUDA(cudaDeviceCanAccessPeer(&can, src->device, dst->device));
+        if (!can) return fail(LLX_ERR_INVALID_ARG, "device %d cannot access the dst pool on device %d", src->device, dst->device);
+        cudaError_t e = cudaDeviceEnablePeerAccess(dst->device, 0);
+        if (e == cudaErrorPeerAccessAlreadyEnabled) cudaGetLastError();
+        else if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceEnablePeerAccess");
+    } else {
+        rc = check_pool(dst, "dst");
+        if (rc != LLX_OK) return rc;
+    }
     if (src == dst) return fail(LLX_ERR_ALIAS, "src and dst are the same pool");
     const unsigned char *a0 = src->data, *a1 = a0 + pool_bytes(src), *b0 = dst->data, *b1 = b0 + pool_bytes(dst);
     if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "src and dst pools overlap in memory");
