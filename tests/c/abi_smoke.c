@@ -1,0 +1,65 @@
+/* Plain C99 client of the llx C ABI: proves the header is C (not C++) and that the host-only entry points
+ * link and behave without a device.  Built and run by tests/test_abi.py. */
+#include <stdio.h>
+#include <string.h>
+
+#include "llx.h"
+
+#define CHECK(cond)                                                   \
+    do {                                                              \
+        if (!(cond)) {                                                \
+            printf("FAILED line %d: %s (%s)\n", __LINE__, #cond, llx_last_error()); \
+            return 1;                                                 \
+        }                                                             \
+    } while (0)
+
+int main(void) {
+    int n = 0, fin = 0, i;
+    llx_blockmgr *a = NULL, *b = NULL;
+    llx_migration* mig = NULL;
+    int32_t table[8], ids[8], dst_table[8];
+    double f = 0.0, total = 0.0, headroom[2] = {0.0, 12016.0};
+    llx_req_info reqs[2];
+
+    CHECK(strstr(llx_version(), "sm_100a") != NULL);
+    CHECK(llx_pool_bytes_for(32, 32, 128, 16, LLX_F16, 1) == 2u * 32u * 131072u); /* 128 KB per block */
+    CHECK(llx_plan_stage(2032, 0, 16, 2, &n, &fin) == LLX_OK && n == 127 && fin == 0);
+    CHECK(llx_plan_stage(2048, 126, 16, 2, &n, &fin) == LLX_OK && n == 2 && fin == 1);
+    CHECK(llx_plan_stage(16, 2, 16, 2, &n, &fin) == LLX_ERR_INVALID_ARG);
+
+    /* the handshake without pools: coordination only */
+    CHECK(llx_blockmgr_create(16, &a) == LLX_OK && llx_blockmgr_create(6, &b) == LLX_OK);
+    CHECK(llx_blockmgr_alloc(a, 8, table) == LLX_OK && table[0] == 0 && table[7] == 7);
+    CHECK(llx_migration_begin(NULL, a, NULL, b, 4, 1, &mig) == LLX_OK);
+    CHECK(llx_migration_stage(mig, table, 8, 18, LLX_REQ_RUNNING, NULL, &n, &fin, ids) == LLX_OK && n == 4 && !fin);
+    CHECK(llx_migration_state(mig) == LLX_MIG_COPYING && llx_blockmgr_num_free(b) == 2);
+    CHECK(llx_migration_stage(mig, table, 8, 19, LLX_REQ_RUNNING, NULL, &n, &fin, ids) == LLX_OK && n == 1 && fin);
+    CHECK(llx_migration_commit(mig, table, 5, LLX_REQ_RUNNING, dst_table, 8, &n) == LLX_OK && n == 5);
+    for (i = 0; i < 5; ++i) CHECK(dst_table[i] == i);
+    CHECK(llx_migration_state(mig) == LLX_MIG_COMMITTED && llx_blockmgr_num_free(a) == 13 && llx_blockmgr_num_free(b) == 1);
+    CHECK(llx_migration_destroy(mig) == LLX_OK);
+    /* destination out of space: abort, nothing reserved */
+    CHECK(llx_migration_begin(NULL, a, NULL, b, 4, 1, &mig) == LLX_OK);
+    CHECK(llx_migration_stage(mig, table + 5, 3, 12, LLX_REQ_RUNNING, NULL, &n, &fin, ids) == LLX_OK && n == 0);
+    CHECK(llx_migration_state(mig) == LLX_MIG_ABORTED && llx_migration_abort_reason(mig) == LLX_ABORT_NO_SPACE);
+    CHECK(llx_blockmgr_num_free(b) == 1);
+    llx_migration_destroy(mig);
+    llx_blockmgr_destroy(a);
+    llx_blockmgr_destroy(b);
+
+    /* Algorithm 1 with the paper's numbers: capacity 13,616 tokens, target load 1,600 tokens for high priority */
+    memset(reqs, 0, sizeof reqs);
+    reqs[0].priority = 1;
+    reqs[0].physical_usage = 1000.0;
+    reqs[1].physical_usage = 601.0;
+    CHECK(llx_calc_freeness(reqs, 2, 13616.0, headroom, 2, 0, &f, &total) == LLX_OK);
+    CHECK(total == 1601.0 + 12016.0 && f < 0.0); /* real load 1601 > 1600: virtually overloaded */
+    reqs[1].physical_usage = 600.0;
+    CHECK(llx_calc_freeness(reqs, 2, 13616.0, headroom, 2, 0, &f, &total) == LLX_OK && f == 0.0);
+
+    /* no device here or bad arguments: data calls fail loudly, never compute on the CPU */
+    CHECK(llx_migrate_stage(NULL, NULL, NULL, NULL, 1, NULL) == LLX_ERR_INVALID_ARG);
+    CHECK(strcmp(llx_status_str(LLX_ERR_NO_SPACE), "LLX_ERR_NO_SPACE") == 0);
+    printf("abi_smoke ok\n");
+    return 0;
+}

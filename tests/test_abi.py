@@ -119,3 +119,23 @@ def test_plan_stage_matches_oracle_on_every_state(llx):
     for bad in [(16, 2, 16, 2), (-1, 0, 16, 2), (16, 0, 0, 2), (16, 0, 16, 0)]:
         with pytest.raises(llx.LlxError):
             llx.plan_stage(*bad)
+
+
+def test_header_is_plain_c99_and_a_c_client_links_and_runs(llx, tmp_path):
+    """The boundary is a C ABI: the header compiles as C99 with -pedantic, and a C program (tests/c/abi_smoke.c)
+    drives the host-only entry points — planner, block manager, handshake, Algorithm 1 — through libllx.so."""
+    import shutil
+    gcc = shutil.which("gcc")
+    if not gcc:
+        pytest.skip("gcc unavailable")
+    r = subprocess.run([gcc, "-fsyntax-only", "-x", "c", "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", HEADER],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    libdir = os.path.join(ROOT, "paper_2406_03243_b200")
+    exe = str(tmp_path / "abi_smoke")
+    r = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"),
+                        os.path.join(ROOT, "tests", "c", "abi_smoke.c"), "-o", exe, "-L", libdir, "-lllx",
+                        "-Wl,-rpath," + libdir], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    r = subprocess.run([exe], capture_output=True, text=True)
+    assert r.returncode == 0 and "abi_smoke ok" in r.stdout, r.stdout + r.stderr
