@@ -148,7 +148,11 @@ size_t     llx_staging_bytes(const llx_pool* pool, int n);
  * *host_ptr is the CPU address, *dev_alias the address to pass as `staging` (equal under UVA). */
 llx_status llx_staging_alloc_pinned(size_t bytes, void** host_ptr, void** dev_alias);
 llx_status llx_staging_free_pinned(void* host_ptr);
-/* staging[i][l][kv][:] = src[l][kv][src_block_ids[i]][:] */
+/* staging[i][l][kv][:] = src[l][kv][src_block_ids[i]][:]
+ * With a pinned-host buffer the tiles are gathered into a library-owned device bounce buffer in ~64 MiB chunks and
+ * each chunk crosses the host link on the copy engine (all on cuda_stream; first use allocates the bounce buffers and
+ * synchronises the device).  LLX_OPT_VIA_HOST_MODE=1 or an explicit LLX_OPT_COPY_KERNEL makes the kernel write the
+ * pinned buffer directly instead (zero-copy). */
 llx_status llx_pack(const llx_pool* src, const int32_t* src_block_ids, int n, void* staging, size_t staging_bytes,
                     void* cuda_stream);
 /* dst[l][kv][dst_block_ids[i]][:] = staging[i][l][kv][:]   (dst ids distinct) */
@@ -293,8 +297,8 @@ typedef enum {
     LLX_OPT_DYNAMIC_TAIL_BATCH = 13, /* chunks per claim of the dynamic tail (0 = auto: 4) */
     LLX_OPT_EXACT_RESIDENCY = 14, /* 1 (default): the bulk kernel asks for enough shared memory that no SM can hold more of its
                                    CTAs than intended, early-launched CTAs of the next kernel included */
-    LLX_OPT_VIA_HOST_MODE = 11  /* llx_migrate_via_host with a pinned-host buffer: 0 (default) copy engines through device
-                                   bounce buffers, both link directions at once; 1 the kernels address the host buffer directly */
+    LLX_OPT_VIA_HOST_MODE = 11  /* llx_pack / llx_unpack / llx_migrate_via_host with a pinned-host buffer: 0 (default) copy engines
+                                   through device bounce buffers; 1 the kernels address the host buffer directly (zero-copy) */
 } llx_option;
 /* Process-wide; takes effect for later calls.  Returns LLX_ERR_INVALID_ARG for a bad value. */
 llx_status llx_set_option(llx_option opt, long long value);

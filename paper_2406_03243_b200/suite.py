@@ -177,6 +177,13 @@ def staging_host(torch, llx, p: Pools, stream, nb):
     res["llx_unpack_from_pinned_host_GBps"] = nbytes / t["median_ms"] / 1e6
     res["pack_frac_of_link_peak"] = res["llx_pack_to_pinned_host_GBps"] / res["link_peak_d2h_GBps"]
     res["unpack_frac_of_link_peak"] = res["llx_unpack_from_pinned_host_GBps"] / res["link_peak_h2d_GBps"]
+    with llx.options(via_host_mode=1):       # the kernels address the pinned buffer themselves
+        t = _time_stream(torch, stream, lambda: llx.pack(p.src, s_tab, pin.dev_alias, nbytes, stream=stream), reps=5, warm=1)
+        res["llx_pack_zero_copy_GBps"] = nbytes / t["median_ms"] / 1e6
+        t = _time_stream(torch, stream, lambda: llx.unpack(pin.dev_alias, nbytes, p.dst, d_tab, stream=stream), reps=5, warm=1)
+        res["llx_unpack_zero_copy_GBps"] = nbytes / t["median_ms"] / 1e6
+    t = _time_stream(torch, stream, lambda: llx.migrate_via_host(p.src, s_tab, p.dst, d_tab, pin.dev_alias, nbytes, stream=stream), reps=5, warm=1)
+    res["llx_migrate_via_host_roundtrip_ms"] = t["median_ms"]
     # alternative: pack into a DEVICE buffer, then one copy-engine transfer (and back)
     stg = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     hbuf = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
