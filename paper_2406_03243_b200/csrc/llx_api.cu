@@ -110,7 +110,8 @@ int g_ring_next = 0;
 // copy; returns the device address.  The caller records the slot's event after its launch.
 llx_status ring_stage(const int32_t* a, size_t na, const int32_t* b, size_t nb, cudaStream_t st, int32_t** dev_out,
                       IdSlot** slot_out) {
-    std::lock_guard<std::mutex> lk(g_ring_mu);
+    // the caller holds g_ring_mu from here until it has recorded the slot's event behind its kernel launch:
+    // another thread must not be handed this slot before that event exists
     IdSlot& s = g_ring[g_ring_next];
     g_ring_next = (g_ring_next + 1) % kIdSlots;
     if (s.used) LLX_CUDA(cudaEventSynchronize(s.ev));
@@ -424,12 +425,14 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
 
     static thread_local IdPack pack;  // 2 KiB; only the first n entries are meaningful
     const bool byval = n <= g_opt_byval.load();
+    std::unique_lock<std::mutex> ring_lk(g_ring_mu, std::defer_lock);
     IdSlot* slot = nullptr;
     if (byval) {
         if (src.ids) memcpy(pack.src, src.ids, n * sizeof(int32_t));
         if (dst.ids) memcpy(pack.dst, dst.ids, n * sizeof(int32_t));
     } else {
         int32_t* dev_ids = nullptr;
+        ring_lk.lock();
         rc = ring_stage(src.ids, src.ids ? n : 0, dst.ids, dst.ids ? n : 0, st, &dev_ids, &slot);
         if (rc != LLX_OK) return rc;
         if (src.ids) a.src_ids = dev_ids;
@@ -959,6 +962,7 @@ llx_status llx_append_tokens(llx_pool* p, const int32_t* table, int table_len, i
     static thread_local IdPack pack;
     cudaStream_t st = (cudaStream_t)stream;
     IdSlot* slot = nullptr;
+    std::unique_lock<std::mutex> ring_lk(g_ring_mu, std::defer_lock);
     const int grid = ntok * a.slices;
     cudaError_t e;
     if (ntok <= kIdsByValueCap) {
@@ -966,6 +970,7 @@ llx_status llx_append_tokens(llx_pool* p, const int32_t* table, int table_len, i
         e = launch_k(llx_append_kernel<true>, grid, 128, 0, st, a, pack);
     } else {
         int32_t* dev_ids = nullptr;
+        ring_lk.lock();
         if ((rc = ring_stage(tb.data(), ntok, nullptr, 0, st, &dev_ids, &slot)) != LLX_OK) return rc;
         a.tok_block = dev_ids;
         e = launch_k(llx_append_kernel<false>, grid, 128, 0, st, a, pack);

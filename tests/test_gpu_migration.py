@@ -510,3 +510,47 @@ def test_destination_pool_on_a_peer_gpu(env):                       # NEXT-2; ne
     om.migrate_stage(h_src, s_ids, h_dst, d_ids)
     with torch.cuda.device(1):
         H.assert_pool_equal(dst.host(), h_dst)
+
+
+def test_two_host_threads_on_two_streams(env):
+    """llx.h: "calls on distinct streams from distinct threads are safe".  Two threads migrate different requests
+    between the same pools at the same time: long id lists (pinned id ring), pinned-host pack (shared bounce
+    buffers) and the blocking final-stage call (flag slots)."""
+    import threading
+    H, llx = env
+    g = dict(TINY, num_blocks=1400)
+    src, dst, h_src, h_dst = make(H, g, seed=6)
+    torch.cuda.synchronize()
+    perm_s, perm_d = synth.block_permutation(7, 1400), synth.block_permutation(8, 1400)
+    errors, packs = [], {}
+
+    def worker(tid):
+        try:
+            torch.cuda.set_device(0)
+            st = torch.cuda.Stream()
+            lo = tid * 700
+            pin = llx.PinnedStaging(llx.staging_bytes(src.pool, 40))
+            for it in range(12):
+                a = lo + (it % 2) * 300
+                llx.migrate_stage(src.pool, perm_s[a:a + 300], dst.pool, perm_d[a:a + 300], stream=st)      # 300 > 256: id ring
+                llx.pack(src.pool, perm_s[lo + 600:lo + 640], pin.dev_alias, pin.nbytes, stream=st)
+                llx.migrate_stage_wait(src.pool, perm_s[lo + 640:lo + 700], dst.pool, perm_d[lo + 640:lo + 700], stream=st)
+            st.synchronize()
+            packs[tid] = pin.as_numpy().copy()
+            pin.free()
+        except Exception as e:  # noqa: BLE001
+            errors.append(repr(e))
+
+    ts = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    assert not errors, errors
+    for tid in range(2):
+        lo = tid * 700
+        om.migrate_stage(h_src, perm_s[lo:lo + 600], h_dst, perm_d[lo:lo + 600])
+        om.migrate_stage(h_src, perm_s[lo + 640:lo + 700], h_dst, perm_d[lo + 640:lo + 700])
+        want = om.pack(h_src, perm_s[lo + 600:lo + 640])
+        assert np.array_equal(packs[tid].reshape(want.shape), want)
+    H.assert_pool_equal(dst.host(), h_dst)
