@@ -320,7 +320,8 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
             if (wpc < 1) wpc = 1;
             if (wpc > 8) wpc = 8;
             threads = (int)wpc * 32;
-            chunk = (long long)threads * 16 * 4;
+            if (g_opt_rings.load() > 0) threads = (int)g_opt_rings.load() * 32;  // experiments: warps per paced CTA
+            if (chunk <= 0) chunk = (long long)threads * 16 * 4;
         } else if (chunk <= 0) {
             chunk = 256 * 16 * 4;
         }
