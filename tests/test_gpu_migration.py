@@ -554,3 +554,35 @@ def test_two_host_threads_on_two_streams(env):
         want = om.pack(h_src, perm_s[lo + 600:lo + 640])
         assert np.array_equal(packs[tid].reshape(want.shape), want)
     H.assert_pool_equal(dst.host(), h_dst)
+
+
+@pytest.mark.parametrize("dtype_name,elem", [("U8", 1), ("BF16", 2)])
+def test_other_element_types_are_bit_copied(env, dtype_name, elem):
+    """Migration is dtype-agnostic: only the element size enters (tile_bytes).  One-byte elements halve the tile."""
+    H, llx = env
+    g = dict(layers=3, kv_heads=5, head_dim=48, block_size=16, num_blocks=50)
+    dt = getattr(llx, dtype_name)
+    te_bytes = g["block_size"] * g["kv_heads"] * g["head_dim"] * elem              # 3840 or 7680 bytes
+    nbytes = llx.pool_bytes_for(g["layers"], g["kv_heads"], g["head_dim"], g["block_size"], dt, 50)
+    assert nbytes == 50 * 2 * g["layers"] * te_bytes
+    rs = torch.randint(0, 256, (nbytes,), dtype=torch.uint8, device="cuda")
+    rd = torch.full((nbytes,), 0xAD, dtype=torch.uint8, device="cuda")
+    src = llx.pool_wrap(rs.data_ptr(), nbytes, g["layers"], g["kv_heads"], g["head_dim"], g["block_size"], dt, 50)
+    dst = llx.pool_wrap(rd.data_ptr(), nbytes, g["layers"], g["kv_heads"], g["head_dim"], g["block_size"], dt, 50)
+    assert src.tile_bytes == te_bytes
+    s_ids, d_ids = synth.block_permutation(1, 50)[:9], synth.block_permutation(2, 50)[:9]
+    llx.migrate_stage(src, s_ids, dst, d_ids)
+    torch.cuda.synchronize()
+    # oracle on 16-bit words: a one-byte pool is viewed as half as many uint16 per tile (a bit copy either way)
+    h_src = rs.cpu().numpy().view(np.uint16).reshape(g["layers"], 2, 50, te_bytes // 2)
+    h_dst = np.full_like(h_src, 0xADAD)
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    got = rd.cpu().numpy().view(np.uint16).reshape(h_dst.shape)
+    H.assert_pool_equal(got, h_dst)
+    other_dt = llx.F16 if elem == 1 else llx.U8                      # same shape, other element size
+    extra = torch.empty(llx.pool_bytes_for(g["layers"], g["kv_heads"], g["head_dim"], g["block_size"], other_dt, 50),
+                        dtype=torch.uint8, device="cuda")
+    other = llx.pool_wrap(extra.data_ptr(), extra.numel(), g["layers"], g["kv_heads"], g["head_dim"], g["block_size"], other_dt, 50)
+    with pytest.raises(llx.LlxError) as e:
+        llx.migrate_stage(src, [0], other, [1])
+    assert e.value.name == "LLX_ERR_GEOMETRY_MISMATCH"
