@@ -98,9 +98,26 @@ def mode_step():
     return 0
 
 
+def mode_refcopy():
+    """torch's contiguous copy_ of stage 0's byte count next to llx_migrate_stage of 112 blocks (for an ncu comparison)."""
+    torch, llx, synth, g, nb, p, st = _setup()
+    s_tab, d_tab = synth.block_permutation(1, nb)[:112], synth.block_permutation(2, nb)[:112]
+    a = torch.empty(112 * p.src.block_bytes, dtype=torch.uint8, device="cuda")
+    b = torch.empty_like(a)
+    with torch.cuda.stream(st):
+        for _ in range(5):
+            b.copy_(a)
+            llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=st)
+        t1 = _back_to_back(torch, st, lambda: b.copy_(a))
+    t2 = _back_to_back(torch, st, lambda: llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=st))
+    nbytes = 2 * a.numel()
+    print(f"torch copy_ {t1:.1f} us {nbytes / t1 / 1e3:.0f} GB/s | llx_migrate_stage {t2:.1f} us {nbytes / t2 / 1e3:.0f} GB/s")
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--mode", choices=["sweep", "tail", "step"], default="sweep")
+    ap.add_argument("--mode", choices=["sweep", "tail", "step", "refcopy"], default="sweep")
     ap.add_argument("--blocks", default="128,112,14,2")
     ap.add_argument("--top", type=int, default=25)
     ap.add_argument("--quick", action="store_true")
@@ -109,6 +126,8 @@ def main():
         return mode_tail()
     if args.mode == "step":
         return mode_step()
+    if args.mode == "refcopy":
+        return mode_refcopy()
     import torch
 
     import paper_2406_03243_b200 as llx
