@@ -160,3 +160,42 @@ def test_llama30b_batch_of_64_requests(env):
         om.migrate_batch(h_src, h_dst, off, s_ids, d_ids)
         H.assert_pool_equal(dst.host_layer(l), h_dst)
     check_untouched_and_mapping_on_device(src, dst, s_ids, d_ids, range(0, g["layers"], 6))
+
+
+def test_llama7b_2048_tokens_through_the_pinned_host_buffer(env):
+    """bench.py's e2e leg: llx_migrate_via_host of the 128-block request with the library's own chunk schedule
+    (64 MiB chunks), plus llx_pack / llx_unpack through the same 1 GiB pinned buffer."""
+    H, llx = env
+    g = synth.CONFIGS["llama7b"]
+    if free_gib() < 34:
+        pytest.skip("needs two 15.6 GiB pools")
+    L, te = g["layers"], H.tile_elems(g)
+    sample_layers = [0, 19, 31]
+    src, dst = H.DevPool(g), H.DevPool(g, fill=SENT)
+    src.fill_device_random(4321)
+    src.fill_from_synth(0, 0, layers=sample_layers)
+    s_tab = synth.block_permutation(1, g["num_blocks"])[:128]
+    d_tab = synth.block_permutation(2, g["num_blocks"])[:128]
+    nbytes = llx.staging_bytes(src.pool, 128)
+    pin = llx.PinnedStaging(nbytes)
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    llx.migrate_via_host(src.pool, s_tab, dst.pool, d_tab, pin.dev_alias, nbytes, stream=st)
+    st.synchronize()
+    buf = pin.as_numpy().reshape(128, L, 2, te)
+    for l in sample_layers:
+        h_src = H.host_pool_from_synth(g, 0, 0, layers=[l])
+        h_dst = om.new_pool(1, g["num_blocks"], te, fill=SENT)
+        want = om.migrate_via_buffer(h_src, s_tab, h_dst, d_tab)
+        H.assert_pool_equal(dst.host_layer(l), h_dst)
+        assert np.array_equal(buf[:, l], want[:, 0])                 # the pinned buffer holds the fused blocks (A6)
+    check_untouched_and_mapping_on_device(src, dst, s_tab, d_tab, range(L))
+    # the two halves on their own: pack into the buffer, unpack into other destination blocks
+    d2 = synth.block_permutation(9, g["num_blocks"])
+    d2 = d2[~np.isin(d2, d_tab)][:128]
+    pin.as_numpy()[:] = 0
+    llx.pack(src.pool, s_tab, pin.dev_alias, nbytes, stream=st)
+    llx.unpack(pin.dev_alias, nbytes, dst.pool, d2, stream=st)
+    st.synchronize()
+    check_untouched_and_mapping_on_device(src, dst, np.concatenate([s_tab, s_tab]), np.concatenate([d_tab, d2]), range(0, L, 5))
+    pin.free()
