@@ -290,7 +290,7 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     const long long total_bytes = n * 2 * layers * tile_bytes;
     long long chunk = g_opt_chunk.load();
     int nstages = (int)g_opt_stages.load();
-    int threads = 256, grid = 0;
+    int threads = 256, grid = 0, long_per_sm = 1;
     size_t smem = 0;
     const int slices = 2 * layers;
 
@@ -300,10 +300,14 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         // (6.57 TB/s at 112 blocks, 6.66 TB/s at >= 256).  More bytes in flight per SM lowers DRAM efficiency.
         // A short stage (the final one: 2 blocks) is latency-bound: smaller chunks over twice as many rings.
         const bool short_stage = total_bytes < (64ll << 20);
-        if (nstages <= 0) nstages = budget > 0 ? 2 : short_stage ? 4 : 3;
         if (chunk <= 0) chunk = budget > 0 ? 2048 : short_stage ? 8192 : 32768;  // paced: a 4 KiB ring stays below the L1 carve-out step
         if (chunk > tile_bytes) chunk = tile_bytes;
         chunk &= ~15ll;
+        // Small tiles cap the chunk, and one thread cannot issue small bulk copies fast enough to keep its SM's share
+        // of HBM busy (measured, long stages: 8 KiB tiles 3.5 TB/s with one ring per SM, 6.0 TB/s with two; 4 KiB
+        // tiles 2.0 -> 6.0 TB/s with four): more CTAs per SM, ~64-96 KiB in flight per SM in every case.
+        long_per_sm = chunk >= 16384 ? 1 : chunk >= 8192 ? 2 : 4;
+        if (nstages <= 0) nstages = budget > 0 ? 2 : short_stage ? 4 : chunk >= 32768 ? 3 : chunk >= 16384 ? 6 : 4;
         int rings = (int)g_opt_rings.load();
         if (rings <= 0) rings = 1;
         threads = 32 * rings;
@@ -335,7 +339,8 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     if (kern == 2) {
         int per_sm = (int)((size_t)di->max_smem_optin / (smem + 1024));  // 1 KiB per-CTA reservation
         if (per_sm > 2) per_sm = 2;
-        if (per_sm < 1 || budget > 0 || total_bytes >= (64ll << 20)) per_sm = 1;
+        if (per_sm < 1 || budget > 0) per_sm = 1;
+        if (budget <= 0 && total_bytes >= (64ll << 20)) per_sm = long_per_sm;
         grid = di->sm_count * per_sm;
         // Exact residency: with programmatic dependent launch the NEXT kernel's CTAs are placed while this kernel
         // still runs, wherever shared memory is free — several on one SM if they fit.  A ring's share of the stage is
