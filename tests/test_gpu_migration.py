@@ -586,3 +586,25 @@ def test_other_element_types_are_bit_copied(env, dtype_name, elem):
     with pytest.raises(llx.LlxError) as e:
         llx.migrate_stage(src, [0], other, [1])
     assert e.value.name == "LLX_ERR_GEOMETRY_MISMATCH"
+
+
+@pytest.mark.parametrize("heads,blocks", [(2, 1500), (4, 800), (8, 420)])     # 4 KiB, 8 KiB, 16 KiB tiles
+def test_long_stage_of_small_tiles_uses_several_ctas_per_sm(env, heads, blocks):
+    """>= 64 MiB of small tiles: the default launch shape takes 4 / 2 / 1 CTAs per SM (chunk = tile) with the dynamic tail."""
+    H, llx = env
+    g = dict(layers=8, kv_heads=heads, head_dim=64, block_size=16, elem_bytes=2, num_blocks=blocks)
+    src = H.DevPool(g)
+    src.fill_device_random(31 + heads)
+    dst = H.DevPool(g, fill=SENT)
+    n = blocks - 100
+    assert 2 * g["layers"] * src.pool.tile_bytes * n >= 64 << 20
+    s_ids, d_ids = synth.block_permutation(3, blocks)[:n], synth.block_permutation(4, blocks)[:n]
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, stream=st)
+    llx.migrate_stage(src.pool, s_ids[:50], dst.pool, d_ids[:50], stream=st)       # a short stage right behind it
+    st.synchronize()
+    h_src = src.host()
+    h_dst = om.new_pool(g["layers"], blocks, H.tile_elems(g), fill=SENT)
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
