@@ -425,6 +425,118 @@ def auto_budget(torch, llx, stream_unused=None, target_pct=1.0, rounds=12):
     return res
 
 
+# ---- the paper's Fig. 10 situation on one B200: a request migrates WHILE its batch keeps decoding -------------
+def live_migration(torch, llx, stream_unused=None, budgets=(0, 100, 25), start_tokens=2040):
+    """One request of a 32-sequence decode batch is migrated live (§6.2): the decode loop keeps
+    appending one token per step to its last source block while the session (llx_migration_*: planner, PRE-ALLOC,
+    copy) moves the completed blocks; when the planner names the final stage the request is drained, the last blocks
+    are copied (downtime) and the request resumes on the destination.  Reported per bandwidth budget: stages and
+    their sizes, copy time, downtime, decode-step time during the migration vs before."""
+    g = dict(synth.CONFIGS["llama7b"])
+    L, H, D, S = g["layers"], g["kv_heads"], g["head_dim"], g["block_size"]
+    B, MB = 32, 256
+    ctx0 = synth.context_lengths(4, B, 128, 4096).copy()
+    r = 0
+    ctx0[r] = start_tokens                                    # the migrating request
+    nb_src, nb_dst = B * 256 + 256, g["num_blocks"]
+    block_bytes = 2 * L * S * H * D * 2
+    if (nb_src + nb_dst) * block_bytes > _free(torch) - (4 << 30):
+        return {"skipped": "not enough device memory"}
+    p = Pools(torch, llx, g, nb_src, nb_dst)
+    scale = 1.0 / float(np.sqrt(D))
+    lo, hi = torch.cuda.Stream.priority_range()
+    s_dec, s_mig = torch.cuda.Stream(priority=hi), torch.cuda.Stream(priority=lo)
+    q = torch.from_numpy(synth.queries_f16(5, B, H, D).view(np.int16)).cuda()
+    o = torch.zeros_like(q)
+    tok_bytes = L * 2 * H * D * 2
+    new_vals = torch.randint(-0x3C00, 0x3C00, (64, L, 2, H * D), dtype=torch.int16, device="cuda")   # K/V of the tokens decoded meanwhile
+    out = {"batch": B, "request_start_tokens": start_tokens, "runs": []}
+
+    for budget in budgets:
+        src_mgr, dst_mgr = llx.BlockManager(nb_src), llx.BlockManager(nb_dst)
+        dst_mgr.alloc(500)                                    # the destination serves other requests already
+        need = [-(-int(c) // S) for c in ctx0]
+        bt = np.zeros((B, MB), dtype=np.int32)
+        tables = []
+        for b in range(B):
+            t = src_mgr.alloc(need[b] + (8 if b == r else 0))   # room for the tokens decoded during the migration
+            tables.append(t)
+            bt[b, :len(t)] = t
+        d_bt = torch.from_numpy(bt).cuda()
+        ctx = ctx0.copy()
+        d_ctx = torch.from_numpy(ctx).cuda()
+        table_r = tables[r]
+        tokens = int(ctx[r])
+
+        def decode_step(pool, with_append=True):
+            nonlocal tokens
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(s_dec)
+            if with_append:                                   # the step's new token of the migrating request (S8)
+                llx.append_tokens(pool, table_r, tokens, tokens + 1,
+                                  new_vals.data_ptr() + (tokens - start_tokens) * tok_bytes, stream=s_dec)
+                tokens += 1
+                with torch.cuda.stream(s_dec):
+                    d_ctx[r] = tokens
+            for l in range(L):
+                llx.decode_attention(pool, l, q.data_ptr(), o.data_ptr(), d_bt.data_ptr(), d_ctx.data_ptr(), B, MB, scale,
+                                     stream=s_dec)
+            b_.record(s_dec)
+            s_dec.synchronize()                               # the engine samples the token: one host sync per step
+            return a.elapsed_time(b_)
+
+        for _ in range(3):
+            decode_step(p.src)
+        before = statistics.median([decode_step(p.src) for _ in range(8)])     # same step (append + 32 layers), no migration
+        tokens_at_start = tokens
+        mig = llx.Migration(p.src, src_mgr, p.dst, dst_mgr, S, 2)
+        stages, during, t_start = [], [], time.perf_counter()
+        with llx.options(bandwidth_gbps=budget):
+            while True:
+                n, fin, _ = mig.stage(table_r, tokens, stream=s_mig)
+                ev = torch.cuda.Event()
+                ev.record(s_mig)
+                stages.append(n)
+                assert not fin and mig.state == llx.MIG_COPYING
+                while not ev.query():                         # decoding continues while the stage copies
+                    during.append(decode_step(p.src))
+                n_next, fin_next = llx.plan_stage(tokens, mig.blocks_migrated, S, 2)
+                if fin_next:
+                    break
+        copy_ms = (time.perf_counter() - t_start) * 1e3
+        # final stage: the request is drained (no more decode steps for it), the last blocks move, it resumes on dst
+        llx.set_option(llx.OPT_BANDWIDTH_GBPS, 0)             # the final stage always runs at full speed
+        t0 = time.perf_counter_ns()
+        n, fin, _ = mig.stage(table_r, tokens, stream=s_mig)  # handshake round (check, plan, PRE-ALLOC) + copy
+        s_mig.synchronize()
+        t1 = time.perf_counter_ns()
+        dst_table = mig.commit(table_r[:-(-tokens // S)])
+        downtime_us, commit_us = (t1 - t0) / 1e3, (time.perf_counter_ns() - t1) / 1e3
+        assert fin and mig.state == llx.MIG_COMMITTED
+        stages.append(n)
+        # resume on the destination: attention of the request over (dst pool, dst table) == over (src pool, src table)
+        bt1 = np.zeros((1, MB), dtype=np.int32)
+        bt1[0, :len(dst_table)] = dst_table
+        d_bt1, d_ctx1 = torch.from_numpy(bt1).cuda(), torch.tensor([tokens], dtype=torch.int32, device="cuda")
+        o_src, o_dst = torch.zeros_like(q[:1]), torch.zeros_like(q[:1])
+        llx.decode_attention(p.src, L - 1, q.data_ptr(), o_src.data_ptr(), d_bt.data_ptr(), d_ctx1.data_ptr(), 1, MB, scale, stream=s_dec)
+        llx.decode_attention(p.dst, L - 1, q.data_ptr(), o_dst.data_ptr(), d_bt1.data_ptr(), d_ctx1.data_ptr(), 1, MB, scale, stream=s_dec)
+        s_dec.synchronize()
+        out["runs"].append({
+            "bandwidth_budget_GBps": budget, "stages_blocks": stages, "num_stages": len(stages),
+            "tokens_at_start": tokens_at_start, "tokens_at_commit": tokens, "decode_steps_during_migration": len(during),
+            "copy_phase_ms": copy_ms, "downtime_us_final_stage": downtime_us, "commit_us": commit_us,
+            "decode_step_ms_before": before, "decode_step_ms_during": statistics.median(during) if during else None,
+            "decode_slowdown_pct": 100.0 * (statistics.median(during) / before - 1.0) if during else None,
+            "resume_on_destination_bit_identical": bool(torch.equal(o_src, o_dst)),
+            "src_free_blocks_after": src_mgr.num_free, "dst_free_blocks_after": dst_mgr.num_free})
+        del mig
+    out["paper"] = "Llumnix Fig. 10: downtime 20-30 ms, always 2 stages, <= 1 % decode slowdown (A10, 64 Gb/s, PAPER.md:287-289)"
+    del p
+    _free(torch)
+    return out
+
+
 def run(torch, llx, stream):
     res = {}
     g = synth.CONFIGS["llama7b"]
@@ -437,12 +549,13 @@ def run(torch, llx, stream):
     _free(torch)
     res["interference_decode_batch32"] = interference(torch, llx, stream)
     res["auto_budget_1pct"] = auto_budget(torch, llx, stream, target_pct=1.0)
+    res["live_migration_during_decode"] = live_migration(torch, llx, stream)
     res["batch_llama30b_64req"] = batch_30b(torch, llx, stream)
     return res
 
 
 def main():
-    """python -m paper_2406_03243_b200.suite [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | batch)"""
+    """python -m paper_2406_03243_b200.suite [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch)"""
     import argparse
     import json
 
@@ -463,6 +576,8 @@ def main():
         res = interference(torch, llx, stream)
     elif args.only == "autobudget":
         res = auto_budget(torch, llx, stream)
+    elif args.only == "live":
+        res = live_migration(torch, llx, stream)
     elif args.only == "batch":
         res = batch_30b(torch, llx, stream)
     else:
