@@ -117,7 +117,12 @@ llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, i
  * Whole tiles, including unused token slots of a partly filled last block.  One kernel
  * launch on `cuda_stream`.  Checked: same geometry (num_blocks may differ), ids in range,
  * no duplicate destination id (duplicate source ids are legal: prefix-shared blocks),
- * src and dst distinct and non-overlapping.  src is never written. */
+ * src and dst distinct and non-overlapping.  src is never written.
+ * The call runs on the SOURCE pool's device (which must be current; cuda_stream belongs to it).  dst may live on
+ * another GPU with peer access: the kernel then stores straight into the peer-mapped pool (the two
+ * instances are different machines); LLX_ERR_INVALID_ARG if the devices cannot access each other.
+ * Long stages claim their last chunks from a small per-stream counter array the library allocates on first use
+ * (that one call synchronises the device). */
 llx_status llx_migrate_stage(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
                              const int32_t* dst_block_ids, int n, void* cuda_stream);
 
