@@ -608,3 +608,40 @@ def test_long_stage_of_small_tiles_uses_several_ctas_per_sm(env, heads, blocks):
     h_dst = om.new_pool(g["layers"], blocks, H.tile_elems(g), fill=SENT)
     om.migrate_stage(h_src, s_ids, h_dst, d_ids)
     H.assert_pool_equal(dst.host(), h_dst)
+
+
+def test_stages_are_stream_capturable_into_a_cuda_graph(env):
+    """Stages of <= 256 pairs carry their ids in the kernel parameters and touch no host state at launch, so a whole
+    staged migration (copies + appends) can be captured once and replayed (first-use allocations happen in a warm-up)."""
+    H, llx = env
+    g = TINY
+    S, te_tok = g["block_size"], g["kv_heads"] * g["head_dim"]
+    src, dst, h_src, h_dst = make(H, g)
+    s_tab = synth.block_permutation(1, g["num_blocks"])[:7]
+    d_tab = synth.block_permutation(2, g["num_blocks"])[:7]
+    values = lambda t, l, kv: synth.append_values_f16(3, t, l, kv, te_tok)
+    vals = np.stack([np.stack([np.stack([values(t, l, kv) for kv in range(2)]) for l in range(g["layers"])]) for t in range(97, 100)])
+    dev_vals = torch.from_numpy(vals.view(np.int16)).cuda()
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+
+    def staged():
+        llx.migrate_stage(src.pool, s_tab[:5], dst.pool, d_tab[:5], stream=st)
+        llx.append_tokens(src.pool, s_tab, 97, 100, dev_vals.data_ptr(), stream=st)
+        llx.migrate_stage(src.pool, s_tab[5:], dst.pool, d_tab[5:], stream=st)
+
+    staged()                                                         # warm-up outside the capture
+    st.synchronize()
+    dst.view.fill_(int(np.array(SENT, np.uint16).view(np.int16)))
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=st):
+        staged()
+    torch.cuda.synchronize()
+    assert bool((dst.view == int(np.array(SENT, np.uint16).view(np.int16))).all())      # capturing ran nothing
+    graph.replay()
+    graph.replay()
+    torch.cuda.synchronize()
+    om.staged_migration(h_src, s_tab, h_dst, d_tab, (5, 2), (3,), S, 97, values)
+    H.assert_pool_equal(dst.host(), h_dst)
+    H.assert_pool_equal(src.host(), h_src)
