@@ -57,6 +57,28 @@ int main(void) {
     reqs[1].physical_usage = 600.0;
     CHECK(llx_calc_freeness(reqs, 2, 13616.0, headroom, 2, 0, &f, &total) == LLX_OK && f == 0.0);
 
+    /* block manager error paths leave the manager unchanged; pairing and ordering */
+    {
+        llx_blockmgr* m = NULL;
+        int32_t got[4], bad_twice[2] = {1, 1}, bad_range[1] = {9}, order[5], srcs[4], dsts[4];
+        int32_t prio[5] = {1, 0, 0, 1, 0}, len[5] = {5, 9, 3, 2, 3};
+        double fr[6] = {5.0, 80.0, -3.0, 70.0, 20.0, 61.0};
+        int pairs = 0;
+        CHECK(llx_blockmgr_create(4, &m) == LLX_OK && llx_blockmgr_alloc(m, 3, got) == LLX_OK);
+        CHECK(llx_blockmgr_alloc(m, 2, got) == LLX_ERR_NO_SPACE && llx_blockmgr_num_free(m) == 1);
+        CHECK(llx_blockmgr_release(m, bad_twice, 2) == LLX_ERR_INVALID_ARG && llx_blockmgr_num_free(m) == 1);
+        CHECK(llx_blockmgr_release(m, bad_range, 1) == LLX_ERR_BLOCK_OUT_OF_RANGE);
+        CHECK(llx_blockmgr_release(m, got, 0) == LLX_OK && llx_blockmgr_destroy(m) == LLX_OK);
+        CHECK(llx_pair_instances(fr, 6, 10.0, 60.0, srcs, dsts, 4, &pairs) == LLX_OK && pairs == 2);
+        CHECK(srcs[0] == 2 && dsts[0] == 1 && srcs[1] == 0 && dsts[1] == 3);
+        CHECK(llx_pair_instances(fr, 6, 10.0, 60.0, srcs, dsts, 1, &pairs) == LLX_ERR_INVALID_ARG && pairs == 2);
+        CHECK(llx_migration_order(prio, len, 5, order) == LLX_OK);
+        CHECK(order[0] == 2 && order[1] == 4 && order[2] == 1 && order[3] == 3 && order[4] == 0);
+        CHECK(llx_set_option(LLX_OPT_CHUNK_BYTES, 100) == LLX_ERR_INVALID_ARG);
+        CHECK(llx_set_option(LLX_OPT_DYNAMIC_TAIL_PCT, 8) == LLX_OK && llx_get_option(LLX_OPT_DYNAMIC_TAIL_PCT) == 8);
+        CHECK(llx_set_option(LLX_OPT_DYNAMIC_TAIL_PCT, 6) == LLX_OK);
+    }
+
     /* no device here or bad arguments: data calls fail loudly, never compute on the CPU */
     CHECK(llx_migrate_stage(NULL, NULL, NULL, NULL, 1, NULL) == LLX_ERR_INVALID_ARG);
     CHECK(strcmp(llx_status_str(LLX_ERR_NO_SPACE), "LLX_ERR_NO_SPACE") == 0);

@@ -139,3 +139,34 @@ def test_header_is_plain_c99_and_a_c_client_links_and_runs(llx, tmp_path):
     assert r.returncode == 0, r.stderr
     r = subprocess.run([exe], capture_output=True, text=True)
     assert r.returncode == 0 and "abi_smoke ok" in r.stdout, r.stdout + r.stderr
+
+
+def test_host_side_under_asan_and_ubsan(tmp_path):
+    """The host side of the library (validation, planner, block manager, handshake, Algorithm 1) built with
+    -fsanitize=address,undefined and driven by the C client: no report, exit 0.  (The device side cannot be run under
+    compute-sanitizer on this pool of machines.)"""
+    import shutil
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    gcc = shutil.which("gcc")
+    if not gcc or not os.path.exists(nvcc):
+        pytest.skip("toolchain unavailable")
+    probe = subprocess.run([gcc, "-fsanitize=address,undefined", "-x", "c", "-", "-o", str(tmp_path / "probe")],
+                           input="int main(void){return 0;}", capture_output=True, text=True)
+    if probe.returncode != 0:
+        pytest.skip("libasan/libubsan unavailable")
+    csrc = os.path.join(ROOT, "paper_2406_03243_b200", "csrc")
+    lib = str(tmp_path / "libllx.so")
+    r = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O1", "-g", "-std=c++17", "-shared", "-Xcompiler",
+                        "-fPIC,-fsanitize=address,-fsanitize=undefined,-fno-omit-frame-pointer", "-diag-suppress", "550",
+                        "-o", lib, os.path.join(csrc, "llx_api.cu"), os.path.join(csrc, "llx_coord.cu"), "-lasan", "-lubsan"],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr[-2000:]
+    exe = str(tmp_path / "abi_smoke_asan")
+    r = subprocess.run([gcc, "-std=c99", "-g", "-fsanitize=address,undefined", "-I", os.path.join(ROOT, "include"),
+                        os.path.join(ROOT, "tests", "c", "abi_smoke.c"), "-o", exe, "-L", str(tmp_path), "-lllx",
+                        "-Wl,-rpath," + str(tmp_path)], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    env = dict(os.environ, ASAN_OPTIONS="detect_leaks=0:protect_shadow_gap=0:halt_on_error=1", UBSAN_OPTIONS="halt_on_error=1")
+    r = subprocess.run([exe], capture_output=True, text=True, env=env)
+    assert r.returncode == 0 and "abi_smoke ok" in r.stdout and "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr, \
+        r.stdout + r.stderr[-3000:]
