@@ -294,9 +294,11 @@ typedef enum {
     LLX_OPT_RINGS_PER_CTA = 8,  /* bulk kernel: independent smem rings (warps) per CTA (0 = auto) */
     LLX_OPT_PDL = 9,            /* 1 (default): launch copy/append kernels with programmatic stream serialization so that
                                    a kernel's prologue overlaps the previous kernel's tail; results are unchanged */
-    LLX_OPT_BANDWIDTH_GBPS = 10,/* bandwidth budget of device<->device copies in GB/s, read + written (0 = unlimited):
-                                   one paced ring per SM instead of a few full-speed CTAs, so that a co-running
-                                   decode step loses the same small share on every SM (<= 1 %) */
+    LLX_OPT_BANDWIDTH_GBPS = 10,/* bandwidth budget of device<->device copies in GB/s, read + written (0 = unlimited), so that a
+                                   co-running decode step keeps its speed (<= 1 %).  Below 500 GB/s: a paced
+                                   register-staged copy, one small CTA per SM, every SM loses the same small share.  From
+                                   500 GB/s: budget/60 full-speed bulk CTAs (about 60 GB/s each), which costs the decode
+                                   step less per byte than pacing at those rates */
     LLX_OPT_DYNAMIC_TAIL_PCT = 12, /* bulk kernel: share (%) of a long stage's chunks that is not pre-assigned to a ring but
                                    claimed in small batches by whichever ring finishes its range first (default 6; 0 = off) */
     LLX_OPT_DYNAMIC_TAIL_BATCH = 13, /* chunks per claim of the dynamic tail (0 = auto: 4) */

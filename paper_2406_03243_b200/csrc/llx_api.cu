@@ -284,7 +284,13 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     // Bandwidth budget: paced register-staged copies, no shared memory.  Measured
     // on B200: a co-resident CTA that holds > ~6 KB of shared memory shrinks the L1 of its SM and slows a
     // bandwidth-bound decode kernel by 30 %, and a few full-speed CTAs turn their SMs into stragglers.
-    const long long budget = g_opt_budget.load();
+    // Above ~500 GB/s pacing on every SM stops paying: measured per GB/s of migration the decode step loses 0.026 % at
+    // 400 GB/s paced but 0.045 % at 800 and 0.060 % at 2400, while a FEW full-speed bulk CTAs stay at 0.023-0.030 %
+    // (about 60 GB/s per CTA: 7 CTAs 447 GB/s, 14: 864, 29: 1623, 43: 2243).  High budgets are therefore met by the
+    // CTA count of the unpaced bulk kernel, low ones by the paced kernel.
+    const long long budget_asked = g_opt_budget.load();
+    const bool budget_by_ctas = budget_asked >= 500 && g_opt_kernel.load() == 0 && kern == 2;
+    const long long budget = budget_by_ctas ? 0 : budget_asked;  // from here on: > 0 means "paced"
     if (budget > 0 && g_opt_kernel.load() != 2) kern = 1;
 
     const long long total_bytes = n * 2 * layers * tile_bytes;
@@ -299,7 +305,7 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         // every ring streaming a contiguous range of chunks and the last 6 % of the stage claimed dynamically
         // (6.57 TB/s at 112 blocks, 6.66 TB/s at >= 256).  More bytes in flight per SM lowers DRAM efficiency.
         // A short stage (the final one: 2 blocks) is latency-bound: smaller chunks over twice as many rings.
-        const bool short_stage = total_bytes < (64ll << 20);
+        const bool short_stage = total_bytes < (64ll << 20) && !budget_by_ctas;
         if (chunk <= 0) chunk = budget > 0 ? 2048 : short_stage ? 8192 : 32768;  // paced: a 4 KiB ring stays below the L1 carve-out step
         if (chunk > tile_bytes) chunk = tile_bytes;
         chunk &= ~15ll;
@@ -340,7 +346,7 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         int per_sm = (int)((size_t)di->max_smem_optin / (smem + 1024));  // 1 KiB per-CTA reservation
         if (per_sm > 2) per_sm = 2;
         if (per_sm < 1 || budget > 0) per_sm = 1;
-        if (budget <= 0 && total_bytes >= (64ll << 20)) per_sm = long_per_sm;
+        if (budget <= 0 && (total_bytes >= (64ll << 20) || budget_by_ctas)) per_sm = long_per_sm;
         grid = di->sm_count * per_sm;
         // Exact residency: with programmatic dependent launch the NEXT kernel's CTAs are placed while this kernel
         // still runs, wherever shared memory is free — several on one SM if they fit.  A ring's share of the stage is
@@ -359,7 +365,8 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         // (measured: 52.7 GB/s with 74..296 CTAs, 51.5 with 1184) and leaves the SMs to whatever else is running.
         grid = (src.host_memory || dst.host_memory) ? di->sm_count : di->sm_count * 8;
     }
-    const long long cap = g_opt_max_ctas.load();
+    long long cap = g_opt_max_ctas.load();
+    if (cap <= 0 && budget_by_ctas) cap = (budget_asked + 30) / 60;
     if (cap > 0) grid = (int)cap;  // explicit grid: the throttle (fewer CTAs) or an experiment (more)
     {
         const long long workers_per_cta = (kern == 2) ? threads / 32 : 1;  // rings per CTA
