@@ -539,6 +539,8 @@ def live_migration(torch, llx, stream_unused=None, budgets=(0, 100, 25), start_t
             "resume_on_destination_bit_identical": bool(torch.equal(o_src, o_dst)),
             "src_free_blocks_after": src_mgr.num_free, "dst_free_blocks_after": dst_mgr.num_free})
         del mig
+    out["note"] = ("decode_slowdown_pct here is UNPAIRED (median step during the migration vs 8 steps before it, one host sync per "
+                   "step) and good to about +-2 %; the paired figures are in interference_decode_batch32 / auto_budget_1pct")
     out["paper"] = "Llumnix Fig. 10: downtime 20-30 ms, always 2 stages, <= 1 % decode slowdown (A10, 64 Gb/s, PAPER.md:287-289)"
     del p
     _free(torch)
