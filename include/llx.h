@@ -40,6 +40,19 @@
  *   - The library never allocates or frees BLOCKS: reservation is the caller's job
  *     (the paper's PRE-ALLOC).  An aborted migration needs no byte rollback.
  *   - There is no CPU fallback: without a CUDA device every data call returns LLX_ERR_CUDA.
+ *   - Threads.  Data calls may be issued from several host threads at once, on distinct streams, between the same
+ *     or different pools; work of one stream runs in the order enqueued.  Launch policy is PER CALL
+ *     (llx_launch_opts, the *_ex entry points): one thread's bandwidth budget never touches another thread's final
+ *     stage.  llx_set_option only changes the process defaults that a call inherits for fields it leaves at
+ *     LLX_OPT_DEFAULT.  llx_decode_attention calls on one pool must be ordered on one stream (they share the pool's
+ *     workspace); llx_blockmgr / llx_migration objects are not thread-safe per object.
+ *   - CUDA graphs.  llx_migrate_stage(_ex), llx_migrate_batch(_ex), llx_pack / llx_unpack with a DEVICE buffer (id lists of
+ *     <= 256 pairs: the ids then travel in the kernel parameters), llx_append_tokens (<= 256 tokens) and
+ *     llx_decode_attention (workspace already large enough) may be stream-captured and replayed on any stream.
+ *     Calls that would have to allocate, synchronise or stage ids through pinned memory while `cuda_stream` is
+ *     capturing return LLX_ERR_STATE and enqueue nothing (longer id lists, pinned-host staging,
+ *     llx_migrate_via_host, llx_migrate_stage_wait, a first-use allocation).  Captured long stages run without the
+ *     dynamic tail (its claim counter belongs to a stream, a graph may replay anywhere).
  */
 #ifndef LLX_H_
 #define LLX_H_
@@ -111,6 +124,40 @@ llx_status llx_pool_fill_u16(llx_pool* pool, uint16_t pattern, void* cuda_stream
 llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, int last_stage_max_blocks, int* n,
                           int* is_final);
 
+/* ---- launch policy of ONE call -------------------------------------------------------------------------------
+ *
+ * The paper's own scenario needs two policies at once: non-final stages must not slow the co-running requests
+ * (<= 1 %) while the final stage must be as short as possible because its duration IS the downtime
+ * (PAPER.md:134), and a source migrates several requests continuously.  Policy is therefore an
+ * argument of the call, not process state.  Every field: LLX_OPT_DEFAULT (-1) = inherit the process default
+ * (llx_set_option; shipped defaults are "auto"), otherwise the meaning and range of the llx_option of the same name. */
+#define LLX_OPT_DEFAULT (-1)
+typedef enum {
+    LLX_ROUTE_AUTO = 0, /* peer route exactly when the pools live on different GPUs */
+    LLX_ROUTE_PEER = 1  /* take the cross-GPU route (kernel choice, launch shape, addressing of SURVEY NEXT-2) although both
+                           pools are on one device: how a single-GPU box executes that branch.  Results are unchanged. */
+} llx_route;
+typedef struct llx_launch_opts {
+    uint32_t struct_size;      /* sizeof(llx_launch_opts) as the caller compiled it; set by llx_launch_opts_init */
+    int32_t bandwidth_gbps;    /* LLX_OPT_BANDWIDTH_GBPS: budget of THIS call in GB/s read+written, 0 = unlimited */
+    int32_t max_ctas;          /* LLX_OPT_MAX_CTAS */
+    int32_t copy_kernel;       /* LLX_OPT_COPY_KERNEL */
+    int32_t chunk_bytes;       /* LLX_OPT_CHUNK_BYTES */
+    int32_t ring_stages;       /* LLX_OPT_RING_STAGES */
+    int32_t rings_per_cta;     /* LLX_OPT_RINGS_PER_CTA */
+    int32_t ids_by_value_max;  /* LLX_OPT_IDS_BY_VALUE_MAX */
+    int32_t unit_order;        /* LLX_OPT_UNIT_ORDER */
+    int32_t l2_hint;           /* LLX_OPT_L2_HINT */
+    int32_t pdl;               /* LLX_OPT_PDL */
+    int32_t dynamic_tail_pct;  /* LLX_OPT_DYNAMIC_TAIL_PCT */
+    int32_t dynamic_tail_batch;/* LLX_OPT_DYNAMIC_TAIL_BATCH */
+    int32_t exact_residency;   /* LLX_OPT_EXACT_RESIDENCY */
+    int32_t via_host_mode;     /* LLX_OPT_VIA_HOST_MODE */
+    int32_t route;             /* llx_route; LLX_OPT_DEFAULT = LLX_ROUTE_AUTO */
+} llx_launch_opts;
+/* Sets struct_size and every field to LLX_OPT_DEFAULT. */
+void llx_launch_opts_init(llx_launch_opts* opts);
+
 /* ---- S3/S4: one migration stage (reserved dst blocks PAPER.md:142) -------- */
 
 /* for i<n, l<layers, kv<2:  dst[l][kv][dst_block_ids[i]][:] = src[l][kv][src_block_ids[i]][:]
@@ -125,15 +172,24 @@ llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, i
  * (that one call synchronises the device). */
 llx_status llx_migrate_stage(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
                              const int32_t* dst_block_ids, int n, void* cuda_stream);
+/* The same with this call's own launch policy (opts == NULL: process defaults, i.e. llx_migrate_stage).
+ * LLX_ERR_INVALID_ARG for a field out of its option's range or a struct_size this library does not know. */
+llx_status llx_migrate_stage_ex(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
+                                const int32_t* dst_block_ids, int n, void* cuda_stream, const llx_launch_opts* opts);
 
 /* The final stage as ONE blocking call (its duration is the request's downtime): llx_migrate_stage,
  * then the call returns only when the copy — and everything enqueued on cuda_stream before it — is complete.
- * The kernel's last CTA writes a word in pinned host memory that the calling thread spins on, which is shorter
- * than a stream synchronize through the driver; if that is not possible (another copy kernel selected by an
- * option, all flag slots in use) it falls back to the stream synchronize.  Same checks and errors as
- * llx_migrate_stage; LLX_ERR_CUDA also reports an asynchronous fault of the copy itself. */
+ * The kernel's last CTA writes a word in pinned host memory that the calling thread spins on (measured on B200: no
+ * shorter than a stream synchronize through the driver, 18.2 vs 17.4 us median — the driver's completion path is a spin
+ * too; this is the convenient form, not an optimisation); if that is not possible (another copy kernel selected, all
+ * flag slots in use) it falls back to the stream synchronize.  Always runs UNTHROTTLED: a bandwidth budget or CTA cap,
+ * from the process defaults or from `opts`, is ignored — the downtime is not where bandwidth is saved.
+ * Same checks and errors as llx_migrate_stage; LLX_ERR_CUDA also reports an asynchronous fault of the copy itself;
+ * LLX_ERR_STATE while cuda_stream is being captured. */
 llx_status llx_migrate_stage_wait(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
                                   const int32_t* dst_block_ids, int n, void* cuda_stream);
+llx_status llx_migrate_stage_wait_ex(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
+                                     const int32_t* dst_block_ids, int n, void* cuda_stream, const llx_launch_opts* opts);
 
 /* ---- S5: many requests in ONE launch (the source migrates its chosen
  * requests one after another; batching them is this build's extension) -------------------- */
@@ -143,6 +199,9 @@ llx_status llx_migrate_stage_wait(const llx_pool* src, const int32_t* src_block_
  * llx_migrate_stage calls.  Destination ids must be distinct across the whole batch. */
 llx_status llx_migrate_batch(const llx_pool* src, llx_pool* dst, const int32_t* req_offsets,
                              const int32_t* src_block_ids, const int32_t* dst_block_ids, int R, void* cuda_stream);
+llx_status llx_migrate_batch_ex(const llx_pool* src, llx_pool* dst, const int32_t* req_offsets,
+                                const int32_t* src_block_ids, const int32_t* dst_block_ids, int R, void* cuda_stream,
+                                const llx_launch_opts* opts);
 
 /* ---- S6: block fusion — gather into / scatter from ONE contiguous buffer -- */
 
@@ -163,6 +222,10 @@ llx_status llx_pack(const llx_pool* src, const int32_t* src_block_ids, int n, vo
 /* dst[l][kv][dst_block_ids[i]][:] = staging[i][l][kv][:]   (dst ids distinct) */
 llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, const int32_t* dst_block_ids, int n,
                       void* cuda_stream);
+llx_status llx_pack_ex(const llx_pool* src, const int32_t* src_block_ids, int n, void* staging, size_t staging_bytes,
+                       void* cuda_stream, const llx_launch_opts* opts);
+llx_status llx_unpack_ex(const void* staging, size_t staging_bytes, llx_pool* dst, const int32_t* dst_block_ids, int n,
+                         void* cuda_stream, const llx_launch_opts* opts);
 
 /* The paper's whole transfer route in one call: gather into the contiguous buffer, then scatter
  * from it into the destination's reserved blocks.  Result: dst as after llx_migrate_stage, staging as after llx_pack.
@@ -176,6 +239,9 @@ llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, 
 llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
                                 const int32_t* dst_block_ids, int n, void* staging, size_t staging_bytes,
                                 int chunk_blocks, void* cuda_stream);
+llx_status llx_migrate_via_host_ex(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
+                                   const int32_t* dst_block_ids, int n, void* staging, size_t staging_bytes,
+                                   int chunk_blocks, void* cuda_stream, const llx_launch_opts* opts);
 
 /* ---- NEXT-3: block manager + migration handshake (Fig. 7) -- host logic only ------------------
  *
@@ -229,6 +295,10 @@ llx_status llx_migration_commit(llx_migration* mig, const int32_t* src_block_tab
                                 int32_t* dst_table_out, int cap, int* n_out);
 /* Either side may abort before the commit ("if the other side fails"). */
 llx_status llx_migration_abort(llx_migration* mig, llx_abort_reason reason);
+/* Launch policy of the session's NON-FINAL stages (the struct is copied; NULL = back to the process defaults), e.g. a
+ * bandwidth budget that keeps the co-running decode steps within 1 %.  The FINAL stage ignores
+ * bandwidth_gbps and max_ctas and always runs at full speed: its duration is the request's downtime. */
+llx_status llx_migration_set_stage_opts(llx_migration* mig, const llx_launch_opts* opts);
 llx_mig_state    llx_migration_state(const llx_migration* mig);
 llx_abort_reason llx_migration_abort_reason(const llx_migration* mig);
 int              llx_migration_blocks_migrated(const llx_migration* mig);
@@ -259,6 +329,30 @@ llx_status llx_pair_instances(const double* freeness, int n, double src_below, d
 /* The order in which a source offers its requests: lower priority first, then shorter sequence, then lower index. */
 llx_status llx_migration_order(const int32_t* priority, const int32_t* seq_len, int n, int32_t* order_out);
 
+/* One migration round of ONE (source, destination) pair as ONE batch: the step between the policy and the hot path
+ * ("The llumlet of each source instance then starts to migrate requests to the destination continuously,
+ * until it is no longer set in the source state.  The llumlet prefers the requests with lower priorities and shorter
+ * sequence lengths").  Reading A31:
+ *   1. candidates = the source's RUNNING requests (not queuing, not fake) in llx_migration_order(priority, seq_len);
+ *   2. while the source's freeness — llx_calc_freeness over the requests it still has — is below src_below (it is still
+ *      "in the source state") and a candidate is left: PRE-ALLOC all blocks of the next candidate on dst_mgr, all or
+ *      nothing; the first request the destination cannot hold while keeping dst_reserve_blocks free
+ *      ends the round; otherwise the request joins the batch and leaves the source's request set.
+ * reqs / seq_len: HOST arrays of n entries.  Request r's block table on the source is
+ * src_block_tables[table_offsets[r] .. table_offsets[r+1]) (HOST int32; n+1 offsets; empty for queuing requests).
+ * Outputs (HOST): chosen_out int32[n] = the requests taken, in the order taken; *n_chosen; and exactly the arguments of
+ * llx_migrate_batch: req_offsets_out int32[n+1] (the first *n_chosen+1 entries are written), src_ids_out / dst_ids_out
+ * int32[cap_pairs], *n_pairs.  The destination ids are RESERVED in dst_mgr when the call returns LLX_OK; after the batch
+ * has completed the caller releases src_ids_out on the source's manager (the commit of PAPER.md:142) — or releases
+ * dst_ids_out on dst_mgr to abort.  LLX_ERR_INVALID_ARG (cap_pairs too small, bad offsets, ...) reserves nothing.
+ * Host arithmetic only; nothing is launched. */
+llx_status llx_plan_migration_batch(const llx_req_info* reqs, const int32_t* seq_len, int n, double M,
+                                    const double* headroom_for_priority, int num_priorities, int is_terminating,
+                                    double src_below, const int32_t* table_offsets, const int32_t* src_block_tables,
+                                    llx_blockmgr* dst_mgr, int dst_reserve_blocks, int32_t* chosen_out, int* n_chosen,
+                                    int32_t* req_offsets_out, int32_t* src_ids_out, int32_t* dst_ids_out, int cap_pairs,
+                                    int* n_pairs);
+
 /* ---- S8: append-only growth while decoding continues --------------- */
 
 /* Writes the K and V vectors of tokens t0..t1-1 of one request into their slots: token t
@@ -274,8 +368,10 @@ llx_status llx_append_tokens(llx_pool* pool, const int32_t* block_table, int tab
  *   o[b][h] = sum_t softmax_t(scale * q[b][h].k_t[h]) v_t[h],  t < dev_ctx_lens[b],
  * K/V of token t read from block dev_block_tables[b*max_blocks + t/block_size], slot t%block_size.
  * dev_q, dev_out: DEVICE fp16 [B, kv_heads, head_dim].  Requires LLX_F16, head_dim 64 or 128.
- * ctx_len 0 gives zeros.  Uses a per-pool workspace that grows on demand (first call and
- * growth synchronise the device); calls on one pool must be ordered on one stream. */
+ * ctx_len 0 gives zeros.  Precondition: dev_ctx_lens[b] <= max_blocks*block_size and every table entry a sequence
+ * uses is a valid block id; the lengths live on the device, so they are not checked on the host — a longer ctx_len is
+ * CLAMPED to max_blocks*block_size in the kernels (never an out-of-row table read).  Uses a per-pool workspace that grows
+ * on demand (first call and growth synchronise the device); calls on one pool must be ordered on one stream. */
 llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* dev_q, void* dev_out,
                                 const int32_t* dev_block_tables, const int32_t* dev_ctx_lens, int B, int max_blocks,
                                 float scale, void* cuda_stream);
@@ -307,7 +403,8 @@ typedef enum {
     LLX_OPT_VIA_HOST_MODE = 11  /* llx_pack / llx_unpack / llx_migrate_via_host with a pinned-host buffer: 0 (default) copy engines
                                    through device bounce buffers; 1 the kernels address the host buffer directly (zero-copy) */
 } llx_option;
-/* Process-wide; takes effect for later calls.  Returns LLX_ERR_INVALID_ARG for a bad value. */
+/* Process-wide DEFAULTS: what a later call uses for every policy field it does not set itself (llx_launch_opts).
+ * For experiments and process-wide tuning; per-request policy belongs in the call.  LLX_ERR_INVALID_ARG for a bad value. */
 llx_status llx_set_option(llx_option opt, long long value);
 long long  llx_get_option(llx_option opt);
 

@@ -38,6 +38,13 @@ Readings (A27-A30):
        (PAPER.md:225); ties broken by the lower instance index.  Requests to migrate: lower priority
        first, then shorter sequence, then lower index ("prefers the requests with lower
        priorities and shorter sequence lengths").
+  A31  one migration round of one (source, destination) pair, taken as ONE batch ("The llumlet of each
+       source instance then starts to migrate requests to the destination continuously, until it is no longer set in
+       the source state"): the source offers its RUNNING requests in `migration_order`; before each request it
+       recomputes its own freeness over the requests it still has and stops once F >= src_below (it would no longer be
+       chosen as a source); the request's blocks are pre-allocated on the destination all-or-nothing (PAPER.md:142);
+       the first request the destination cannot hold ends the round.  The paper re-evaluates the thresholds "in the
+       next round"; evaluating them after every request is the same rule at the finest round length.
 """
 from __future__ import annotations
 
@@ -105,3 +112,32 @@ def pair_instances(freeness, src_below: float, dst_above: float):
 def migration_order(priority, seq_len):
     """request indices in the order the source llumlet offers them for migration."""
     return sorted(range(len(priority)), key=lambda i: (priority[i], seq_len[i], i))
+
+
+def plan_migration_batch(instance: Instance, seq_len, block_tables, src_below: float, dst_mgr, dst_reserve_blocks: int = 0):
+    """One migration round of one (source, destination) pair (reading A31).  `block_tables[r]` is request r's block
+    table on the source (empty for queuing requests); `dst_mgr` is the destination's oracle.handshake.BlockManager.
+    Returns (chosen request indices in the order taken, req_offsets, src_ids, dst_ids) — the arguments of
+    oracle.kv_migration.migrate_batch.  The destination blocks are reserved in `dst_mgr`."""
+    requests = list(instance.requests)
+    remaining = list(range(len(requests)))                      # the requests the source still has
+    order = migration_order([r.priority for r in requests], seq_len)
+    chosen, req_offsets, src_ids, dst_ids = [], [0], [], []
+    for r in order:
+        if requests[r].is_queuing or requests[r].is_fake:
+            continue                                            # no KV cache on this instance: nothing to migrate
+        still_here = Instance(instance.M, [requests[i] for i in remaining], instance.headroom_for_priority,
+                              instance.is_terminating)
+        F, _ = calc_freeness(still_here)
+        if not F < src_below:
+            break                                               # "no longer set in the source state"
+        table = [int(b) for b in block_tables[r]]
+        if len(table) > dst_mgr.num_free() - dst_reserve_blocks:
+            break                                               # PRE-ALLOC would fail: abort, the round ends (PAPER.md:142)
+        ids = dst_mgr.allocate(len(table))                      # PRE-ALLOC, all or nothing
+        chosen.append(r)
+        src_ids += table
+        dst_ids += ids
+        req_offsets.append(len(src_ids))
+        remaining.remove(r)
+    return chosen, req_offsets, src_ids, dst_ids

@@ -28,6 +28,36 @@ class ReqInfo(C.Structure):
                 ("priority", C.c_int32), ("demand", C.c_double), ("physical_usage", C.c_double)]
 
 
+OPT_DEFAULT = -1
+ROUTE_AUTO, ROUTE_PEER = 0, 1
+
+
+class LaunchOpts(C.Structure):
+    """llx_launch_opts: the launch policy of ONE call.  LaunchOpts(bandwidth_gbps=25) leaves every other field at
+    LLX_OPT_DEFAULT (inherit the process default)."""
+    _fields_ = [("struct_size", C.c_uint32)] + [(k, C.c_int32) for k in (
+        "bandwidth_gbps", "max_ctas", "copy_kernel", "chunk_bytes", "ring_stages", "rings_per_cta", "ids_by_value_max",
+        "unit_order", "l2_hint", "pdl", "dynamic_tail_pct", "dynamic_tail_batch", "exact_residency", "via_host_mode",
+        "route")]
+
+    def __init__(self, **kw):
+        super().__init__()
+        load().llx_launch_opts_init(C.byref(self))
+        for k, v in kw.items():
+            if k not in dict(self._fields_) or k == "struct_size":
+                raise TypeError(f"llx_launch_opts has no field {k!r}")
+            setattr(self, k, int(v))
+
+
+def _opts(o):
+    """None | dict | LaunchOpts -> pointer argument of the *_ex entry points."""
+    if o is None:
+        return None
+    if isinstance(o, dict):
+        o = LaunchOpts(**o)
+    return C.byref(o)
+
+
 class _Counters(C.Structure):
     _fields_ = [("kernel_launches", C.c_ulonglong), ("copy_launches", C.c_ulonglong),
                 ("bytes_moved", C.c_ulonglong), ("id_uploads", C.c_ulonglong)]
@@ -48,15 +78,22 @@ EXPORTS = {
     "llx_pool_download": (_i, [_vp, _i, _i, _i, _i, _vp, _vp]),
     "llx_pool_fill_u16": (_i, [_vp, C.c_uint16, _vp]),
     "llx_plan_stage": (_i, [_i, _i, _i, _i, C.POINTER(_i), C.POINTER(_i)]),
+    "llx_launch_opts_init": (None, [C.POINTER(LaunchOpts)]),
     "llx_migrate_stage": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp]),
+    "llx_migrate_stage_ex": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp, C.POINTER(LaunchOpts)]),
     "llx_migrate_stage_wait": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp]),
+    "llx_migrate_stage_wait_ex": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp, C.POINTER(LaunchOpts)]),
     "llx_migrate_batch": (_i, [_vp, _vp, _i32p, _i32p, _i32p, _i, _vp]),
+    "llx_migrate_batch_ex": (_i, [_vp, _vp, _i32p, _i32p, _i32p, _i, _vp, C.POINTER(LaunchOpts)]),
     "llx_staging_bytes": (_sz, [_vp, _i]),
     "llx_staging_alloc_pinned": (_i, [_sz, C.POINTER(_vp), C.POINTER(_vp)]),
     "llx_staging_free_pinned": (_i, [_vp]),
     "llx_pack": (_i, [_vp, _i32p, _i, _vp, _sz, _vp]),
+    "llx_pack_ex": (_i, [_vp, _i32p, _i, _vp, _sz, _vp, C.POINTER(LaunchOpts)]),
     "llx_unpack": (_i, [_vp, _sz, _vp, _i32p, _i, _vp]),
+    "llx_unpack_ex": (_i, [_vp, _sz, _vp, _i32p, _i, _vp, C.POINTER(LaunchOpts)]),
     "llx_migrate_via_host": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp, _sz, _i, _vp]),
+    "llx_migrate_via_host_ex": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp, _sz, _i, _vp, C.POINTER(LaunchOpts)]),
     "llx_blockmgr_create": (_i, [_i, C.POINTER(_vp)]),
     "llx_blockmgr_destroy": (_i, [_vp]),
     "llx_blockmgr_num_free": (_i, [_vp]),
@@ -67,6 +104,7 @@ EXPORTS = {
     "llx_migration_stage": (_i, [_vp, _i32p, _i, _i, _i, _vp, C.POINTER(_i), C.POINTER(_i), _i32p]),
     "llx_migration_commit": (_i, [_vp, _i32p, _i, _i, _i32p, _i, C.POINTER(_i)]),
     "llx_migration_abort": (_i, [_vp, _i]),
+    "llx_migration_set_stage_opts": (_i, [_vp, C.POINTER(LaunchOpts)]),
     "llx_migration_state": (_i, [_vp]),
     "llx_migration_abort_reason": (_i, [_vp]),
     "llx_migration_blocks_migrated": (_i, [_vp]),
@@ -76,6 +114,8 @@ EXPORTS = {
                                C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "llx_pair_instances": (_i, [C.POINTER(C.c_double), _i, C.c_double, C.c_double, _i32p, _i32p, _i, C.POINTER(_i)]),
     "llx_migration_order": (_i, [_i32p, _i32p, _i, _i32p]),
+    "llx_plan_migration_batch": (_i, [C.POINTER(ReqInfo), _i32p, _i, C.c_double, C.POINTER(C.c_double), _i, _i, C.c_double,
+                                      _i32p, _i32p, _vp, _i, _i32p, C.POINTER(_i), _i32p, _i32p, _i32p, _i, C.POINTER(_i)]),
     "llx_append_tokens": (_i, [_vp, _i32p, _i, _i, _i, _vp, _vp]),
     "llx_decode_attention": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _i, _i, C.c_float, _vp]),
     "llx_set_option": (_i, [_i, C.c_longlong]),
@@ -205,30 +245,40 @@ def plan_stage(num_tokens: int, blocks_migrated: int, block_size: int, last_stag
     return n.value, bool(f.value)
 
 
-def migrate_stage(src: Pool, src_block_ids, dst: Pool, dst_block_ids, stream=None):
+def migrate_stage(src: Pool, src_block_ids, dst: Pool, dst_block_ids, stream=None, opts=None):
+    """opts: None (llx_migrate_stage), or a dict / LaunchOpts = this call's own launch policy (llx_migrate_stage_ex)."""
     s, sp = _ids(src_block_ids)
     d, dp = _ids(dst_block_ids)
     if s.size != d.size:
         raise LlxError(-1, "LLX_ERR_INVALID_ARG", "src/dst id lists differ in length")
-    _check(load().llx_migrate_stage(src.handle, sp, dst.handle, dp, s.size, _stream(stream)))
+    if opts is None:
+        _check(load().llx_migrate_stage(src.handle, sp, dst.handle, dp, s.size, _stream(stream)))
+    else:
+        _check(load().llx_migrate_stage_ex(src.handle, sp, dst.handle, dp, s.size, _stream(stream), _opts(opts)))
 
 
-def migrate_stage_wait(src: Pool, src_block_ids, dst: Pool, dst_block_ids, stream=None):
+def migrate_stage_wait(src: Pool, src_block_ids, dst: Pool, dst_block_ids, stream=None, opts=None):
     """llx_migrate_stage + wait for its completion (the final stage: downtime ends when this returns)."""
     s, sp = _ids(src_block_ids)
     d, dp = _ids(dst_block_ids)
     if s.size != d.size:
         raise LlxError(-1, "LLX_ERR_INVALID_ARG", "src/dst id lists differ in length")
-    _check(load().llx_migrate_stage_wait(src.handle, sp, dst.handle, dp, s.size, _stream(stream)))
+    if opts is None:
+        _check(load().llx_migrate_stage_wait(src.handle, sp, dst.handle, dp, s.size, _stream(stream)))
+    else:
+        _check(load().llx_migrate_stage_wait_ex(src.handle, sp, dst.handle, dp, s.size, _stream(stream), _opts(opts)))
 
 
-def migrate_batch(src: Pool, dst: Pool, req_offsets, src_block_ids, dst_block_ids, stream=None):
+def migrate_batch(src: Pool, dst: Pool, req_offsets, src_block_ids, dst_block_ids, stream=None, opts=None):
     o, op = _ids(req_offsets)
     s, sp = _ids(src_block_ids)
     d, dp = _ids(dst_block_ids)
     if o.size < 1 or s.size != d.size or int(o[-1]) != s.size:
         raise LlxError(-1, "LLX_ERR_INVALID_ARG", "req_offsets[-1] must equal the number of id pairs")
-    _check(load().llx_migrate_batch(src.handle, dst.handle, op, sp, dp, o.size - 1, _stream(stream)))
+    if opts is None:
+        _check(load().llx_migrate_batch(src.handle, dst.handle, op, sp, dp, o.size - 1, _stream(stream)))
+    else:
+        _check(load().llx_migrate_batch_ex(src.handle, dst.handle, op, sp, dp, o.size - 1, _stream(stream), _opts(opts)))
 
 
 def staging_bytes(pool: Pool, n: int) -> int:
@@ -257,24 +307,34 @@ class PinnedStaging:
             self.free()
 
 
-def pack(src: Pool, src_block_ids, staging_ptr: int, staging_nbytes: int, stream=None):
+def pack(src: Pool, src_block_ids, staging_ptr: int, staging_nbytes: int, stream=None, opts=None):
     s, sp = _ids(src_block_ids)
-    _check(load().llx_pack(src.handle, sp, s.size, staging_ptr, staging_nbytes, _stream(stream)))
+    if opts is None:
+        _check(load().llx_pack(src.handle, sp, s.size, staging_ptr, staging_nbytes, _stream(stream)))
+    else:
+        _check(load().llx_pack_ex(src.handle, sp, s.size, staging_ptr, staging_nbytes, _stream(stream), _opts(opts)))
 
 
-def unpack(staging_ptr: int, staging_nbytes: int, dst: Pool, dst_block_ids, stream=None):
+def unpack(staging_ptr: int, staging_nbytes: int, dst: Pool, dst_block_ids, stream=None, opts=None):
     d, dp = _ids(dst_block_ids)
-    _check(load().llx_unpack(staging_ptr, staging_nbytes, dst.handle, dp, d.size, _stream(stream)))
+    if opts is None:
+        _check(load().llx_unpack(staging_ptr, staging_nbytes, dst.handle, dp, d.size, _stream(stream)))
+    else:
+        _check(load().llx_unpack_ex(staging_ptr, staging_nbytes, dst.handle, dp, d.size, _stream(stream), _opts(opts)))
 
 
 def migrate_via_host(src: Pool, src_block_ids, dst: Pool, dst_block_ids, staging_ptr: int, staging_nbytes: int,
-                     chunk_blocks: int = 0, stream=None):
+                     chunk_blocks: int = 0, stream=None, opts=None):
     s, sp = _ids(src_block_ids)
     d, dp = _ids(dst_block_ids)
     if s.size != d.size:
         raise LlxError(-1, "LLX_ERR_INVALID_ARG", "src/dst id lists differ in length")
-    _check(load().llx_migrate_via_host(src.handle, sp, dst.handle, dp, s.size, staging_ptr, staging_nbytes,
-                                       chunk_blocks, _stream(stream)))
+    if opts is None:
+        _check(load().llx_migrate_via_host(src.handle, sp, dst.handle, dp, s.size, staging_ptr, staging_nbytes,
+                                           chunk_blocks, _stream(stream)))
+    else:
+        _check(load().llx_migrate_via_host_ex(src.handle, sp, dst.handle, dp, s.size, staging_ptr, staging_nbytes,
+                                              chunk_blocks, _stream(stream), _opts(opts)))
 
 
 REQ_RUNNING, REQ_FINISHED, REQ_PREEMPTED, REQ_PEER_FAILED = range(4)
@@ -346,6 +406,10 @@ class Migration:
     def abort(self, reason: int = ABORT_PEER_FAILED):
         _check(load().llx_migration_abort(self._h, reason))
 
+    def set_stage_opts(self, opts):
+        """Launch policy of the non-final stages (dict / LaunchOpts / None); the final stage always runs unthrottled."""
+        _check(load().llx_migration_set_stage_opts(self._h, _opts(opts)))
+
     def __del__(self):
         with contextlib.suppress(Exception):
             if self._h:
@@ -384,6 +448,35 @@ def migration_order(priority, seq_len):
     return out[:p.size].tolist()
 
 
+def plan_migration_batch(reqs, seq_len, M: float, headroom_for_priority, src_below: float, block_tables,
+                         dst_mgr: BlockManager, dst_reserve_blocks: int = 0, is_terminating: bool = False):
+    """llx_plan_migration_batch.  reqs as in calc_freeness; block_tables: one id list per request (empty for queuing
+    requests).  -> (chosen, req_offsets, src_ids, dst_ids): the last three are the arguments of migrate_batch."""
+    reqs = list(reqs)
+    n = len(reqs)
+    arr = (ReqInfo * max(n, 1))(*[ReqInfo(int(a), int(b), int(c), int(p), float(d), float(u)) for a, b, c, p, d, u in reqs])
+    hr = (C.c_double * len(headroom_for_priority))(*[float(x) for x in headroom_for_priority])
+    sl, slp = _ids(seq_len)
+    if sl.size != n or len(block_tables) != n:
+        raise LlxError(-1, "LLX_ERR_INVALID_ARG", "reqs / seq_len / block_tables differ in length")
+    off = np.zeros(n + 1, dtype=np.int32)
+    for r, t in enumerate(block_tables):
+        off[r + 1] = off[r] + len(t)
+    flat, flatp = _ids(np.concatenate([np.asarray(t, dtype=np.int32).reshape(-1) for t in block_tables])
+                       if n else np.zeros(0, np.int32))
+    cap = int(off[-1])
+    chosen, ro = np.empty(max(n, 1), np.int32), np.empty(n + 1, np.int32)
+    s_out, d_out = np.empty(max(cap, 1), np.int32), np.empty(max(cap, 1), np.int32)
+    nc, npairs = _i(), _i()
+    _check(load().llx_plan_migration_batch(arr, slp, n, float(M), hr, len(headroom_for_priority), int(is_terminating),
+                                           float(src_below), off.ctypes.data_as(_i32p), flatp, dst_mgr.handle,
+                                           int(dst_reserve_blocks), chosen.ctypes.data_as(_i32p), C.byref(nc),
+                                           ro.ctypes.data_as(_i32p), s_out.ctypes.data_as(_i32p), d_out.ctypes.data_as(_i32p),
+                                           cap, C.byref(npairs)))
+    k, m = nc.value, npairs.value
+    return chosen[:k].tolist(), ro[:k + 1].copy(), s_out[:m].copy(), d_out[:m].copy()
+
+
 def append_tokens(pool: Pool, block_table, t0: int, t1: int, dev_values_ptr: int, stream=None):
     t, tp = _ids(block_table)
     _check(load().llx_append_tokens(pool.handle, tp, t.size, t0, t1, dev_values_ptr, _stream(stream)))
@@ -405,7 +498,8 @@ def get_option(opt: int) -> int:
 
 @contextlib.contextmanager
 def options(**kw):
-    """Temporarily set options by lower-case name, e.g. options(copy_kernel=1, max_ctas=16)."""
+    """Temporarily set PROCESS-WIDE default options by lower-case name, e.g. options(copy_kernel=1, max_ctas=16).
+    For experiments; the policy of one call belongs in its `opts=` argument (llx_launch_opts)."""
     names = dict(copy_kernel=OPT_COPY_KERNEL, max_ctas=OPT_MAX_CTAS, chunk_bytes=OPT_CHUNK_BYTES,
                  ring_stages=OPT_RING_STAGES, ids_by_value_max=OPT_IDS_BY_VALUE_MAX,
                  attn_split_tokens=OPT_ATTN_SPLIT_TOKENS, unit_order=OPT_UNIT_ORDER, l2_hint=OPT_L2_HINT,

@@ -5,6 +5,8 @@
 
 #include <atomic>
 #include <cstdarg>
+#include <cstddef>
+#include <new>
 #include <cstdio>
 #include <cstring>
 #include <mutex>
@@ -67,6 +69,102 @@ std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt
     g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
+// Range of every option: shared by llx_set_option (process defaults) and by the per-call llx_launch_opts.
+bool opt_valid(int opt, long long v) {
+    switch (opt) {
+        case LLX_OPT_COPY_KERNEL: return v >= 0 && v <= 2;
+        case LLX_OPT_MAX_CTAS: return v >= 0 && v <= (1 << 20);
+        case LLX_OPT_CHUNK_BYTES: return v >= 0 && (v % 16) == 0 && v <= (200 << 10);
+        case LLX_OPT_RING_STAGES: return v >= 0 && v != 1 && v <= 14;
+        case LLX_OPT_IDS_BY_VALUE_MAX: return v >= 0 && v <= kIdsByValueCap;
+        case LLX_OPT_ATTN_SPLIT_TOKENS: return v >= 0 && (v % 8) == 0;
+        case LLX_OPT_UNIT_ORDER: return v >= 0 && v <= 1;
+        case LLX_OPT_L2_HINT: return v >= 0 && v <= 3;
+        case LLX_OPT_RINGS_PER_CTA: return v >= 0 && v <= 8;
+        case LLX_OPT_PDL: return v >= 0 && v <= 1;
+        case LLX_OPT_BANDWIDTH_GBPS: return v >= 0 && v <= 100000;
+        case LLX_OPT_VIA_HOST_MODE: return v >= 0 && v <= 1;
+        case LLX_OPT_DYNAMIC_TAIL_PCT: return v >= 0 && v <= 100;
+        case LLX_OPT_DYNAMIC_TAIL_BATCH: return v >= 0 && v <= 4096;
+        case LLX_OPT_EXACT_RESIDENCY: return v >= 0 && v <= 1;
+    }
+    return false;
+}
+
+// The launch policy of ONE call: the process defaults overridden by whatever the call's llx_launch_opts sets.
+// Resolved once at the entry point and passed down by value, so concurrent callers never see each other's policy.
+struct Policy {
+    long long kernel, max_ctas, chunk, stages, byval, order, l2hint, rings, pdl, budget, via_host, dyn_pct, dyn_batch, smem_pad;
+    int route;
+    bool kernel_explicit;  // the copy kernel was chosen by the caller (option or opts), not by "auto"
+};
+
+llx_status resolve_policy(const llx_launch_opts* o, Policy* p) {
+    p->kernel = g_opt_kernel.load();
+    p->max_ctas = g_opt_max_ctas.load();
+    p->chunk = g_opt_chunk.load();
+    p->stages = g_opt_stages.load();
+    p->byval = g_opt_byval.load();
+    p->order = g_opt_order.load();
+    p->l2hint = g_opt_l2hint.load();
+    p->rings = g_opt_rings.load();
+    p->pdl = g_opt_pdl.load();
+    p->budget = g_opt_budget.load();
+    p->via_host = g_opt_via_host.load();
+    p->dyn_pct = g_opt_dyn_pct.load();
+    p->dyn_batch = g_opt_dyn_batch.load();
+    p->smem_pad = g_opt_smem_pad.load();
+    p->route = LLX_ROUTE_AUTO;
+    if (o) {
+        // a caller compiled against an older, shorter struct is served: fields beyond its struct_size keep the defaults
+        if (o->struct_size < 2 * sizeof(int32_t) || o->struct_size > sizeof(llx_launch_opts) || (o->struct_size % sizeof(int32_t)) != 0)
+            return fail(LLX_ERR_INVALID_ARG, "llx_launch_opts.struct_size = %u (this library: %zu); use llx_launch_opts_init", o->struct_size, sizeof(llx_launch_opts));
+#define LLX_FIELD(field, opt, dst)                                                                            \
+    if (offsetof(llx_launch_opts, field) + sizeof(int32_t) <= o->struct_size && o->field != LLX_OPT_DEFAULT) { \
+        if (!opt_valid(opt, o->field)) return fail(LLX_ERR_INVALID_ARG, "llx_launch_opts." #field " = %d: bad value", (int)o->field); \
+        p->dst = o->field;                                                                                    \
+    }
+        LLX_FIELD(bandwidth_gbps, LLX_OPT_BANDWIDTH_GBPS, budget)
+        LLX_FIELD(max_ctas, LLX_OPT_MAX_CTAS, max_ctas)
+        LLX_FIELD(copy_kernel, LLX_OPT_COPY_KERNEL, kernel)
+        LLX_FIELD(chunk_bytes, LLX_OPT_CHUNK_BYTES, chunk)
+        LLX_FIELD(ring_stages, LLX_OPT_RING_STAGES, stages)
+        LLX_FIELD(rings_per_cta, LLX_OPT_RINGS_PER_CTA, rings)
+        LLX_FIELD(ids_by_value_max, LLX_OPT_IDS_BY_VALUE_MAX, byval)
+        LLX_FIELD(unit_order, LLX_OPT_UNIT_ORDER, order)
+        LLX_FIELD(l2_hint, LLX_OPT_L2_HINT, l2hint)
+        LLX_FIELD(pdl, LLX_OPT_PDL, pdl)
+        LLX_FIELD(dynamic_tail_pct, LLX_OPT_DYNAMIC_TAIL_PCT, dyn_pct)
+        LLX_FIELD(dynamic_tail_batch, LLX_OPT_DYNAMIC_TAIL_BATCH, dyn_batch)
+        LLX_FIELD(exact_residency, LLX_OPT_EXACT_RESIDENCY, smem_pad)
+        LLX_FIELD(via_host_mode, LLX_OPT_VIA_HOST_MODE, via_host)
+#undef LLX_FIELD
+        if (offsetof(llx_launch_opts, route) + sizeof(int32_t) <= o->struct_size && o->route != LLX_OPT_DEFAULT) {
+            if (o->route != LLX_ROUTE_AUTO && o->route != LLX_ROUTE_PEER) return fail(LLX_ERR_INVALID_ARG, "llx_launch_opts.route = %d", (int)o->route);
+            p->route = o->route;
+        }
+    }
+    p->kernel_explicit = p->kernel != 0;
+    return LLX_OK;
+}
+
+// Is work enqueued on `st` being captured into a CUDA graph?  Calls that must allocate, synchronise or stage ids through
+// pinned memory refuse (LLX_ERR_STATE) instead of invalidating the capture.
+llx_status stream_capturing(cudaStream_t st, bool* capturing) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    cudaError_t e = cudaStreamIsCapturing(st, &cs);
+    if (e != cudaSuccess) return fail(LLX_ERR_CUDA, "cudaStreamIsCapturing: %s", cudaGetErrorString(e));
+    *capturing = cs != cudaStreamCaptureStatusNone;
+    return LLX_OK;
+}
+llx_status refuse_if_capturing(cudaStream_t st, const char* what) {
+    bool cap = false;
+    llx_status rc = stream_capturing(st, &cap);
+    if (rc != LLX_OK) return rc;
+    if (cap) return fail(LLX_ERR_STATE, "%s cannot be captured into a CUDA graph (it allocates, synchronises or stages through pinned memory)", what);
+    return LLX_OK;
+}
+
 // ---- device properties (cached per device) ------------------------------------------------
 struct DevInfo {
     int sm_count = 0;
@@ -77,11 +175,13 @@ struct DevInfo {
 std::mutex g_dev_mu;
 DevInfo g_dev[64];
 
-llx_status dev_info(int dev, DevInfo** out) {
+// `dev` must be the CURRENT device (cudaFuncSetAttribute acts on it): every caller passes the device its kernel runs on.
+llx_status dev_info(int dev, DevInfo** out, bool capturing = false) {
     if (dev < 0 || dev >= 64) return fail(LLX_ERR_INVALID_ARG, "device %d unsupported", dev);
     std::lock_guard<std::mutex> lk(g_dev_mu);
     DevInfo& d = g_dev[dev];
     if (!d.ready) {
+        if (capturing) return fail(LLX_ERR_STATE, "first llx call on device %d inside a stream capture: warm up outside the capture", dev);
         LLX_CUDA(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
         LLX_CUDA(cudaDeviceGetAttribute(&d.max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
         LLX_CUDA(cudaDeviceGetAttribute(&d.smem_per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
@@ -102,18 +202,21 @@ struct IdSlot {
     bool used = false;
 };
 constexpr int kIdSlots = 8;
-std::mutex g_ring_mu;
-IdSlot g_ring[kIdSlots];
-int g_ring_next = 0;
+struct IdRing {  // one per device: a slot's device buffer and event belong to the device whose kernels read it
+    std::mutex mu;
+    IdSlot slots[kIdSlots];
+    int next = 0;
+};
+IdRing g_ring[64];
 
 // Copies `count` ids made of up to two host arrays (a then b) into a slot and enqueues the H2D
 // copy; returns the device address.  The caller records the slot's event after its launch.
-llx_status ring_stage(const int32_t* a, size_t na, const int32_t* b, size_t nb, cudaStream_t st, int32_t** dev_out,
+llx_status ring_stage(IdRing& ring, const int32_t* a, size_t na, const int32_t* b, size_t nb, cudaStream_t st, int32_t** dev_out,
                       IdSlot** slot_out) {
-    // the caller holds g_ring_mu from here until it has recorded the slot's event behind its kernel launch:
+    // the caller holds ring.mu from here until it has recorded the slot's event behind its kernel launch:
     // another thread must not be handed this slot before that event exists
-    IdSlot& s = g_ring[g_ring_next];
-    g_ring_next = (g_ring_next + 1) % kIdSlots;
+    IdSlot& s = ring.slots[ring.next];
+    ring.next = (ring.next + 1) % kIdSlots;
     if (s.used) LLX_CUDA(cudaEventSynchronize(s.ev));
     const size_t need = na + nb;
     if (need > s.cap) {
@@ -139,6 +242,17 @@ llx_status ring_stage(const int32_t* a, size_t na, const int32_t* b, size_t nb, 
     *dev_out = s.dev;
     *slot_out = &s;
     return LLX_OK;
+}
+
+// Records the slot's event behind the launch that reads it.  If the record fails the slot would be reused while its
+// copy or kernel is still pending, so the stream is drained instead and the error reported.
+llx_status ring_close(IdSlot* slot, cudaStream_t st) {
+    if (!slot) return LLX_OK;
+    cudaError_t e = cudaEventRecord(slot->ev, st);
+    if (e == cudaSuccess) return LLX_OK;
+    cudaStreamSynchronize(st);
+    slot->used = false;
+    return cuda_fail(e, "cudaEventRecord (id ring)");
 }
 
 // ---- claim counters of the bulk kernel's dynamic tail: one per (device, stream).  Launches of one stream are
@@ -247,7 +361,7 @@ size_t pool_bytes(const llx_pool* p) { return (size_t)p->num_blocks * 2 * p->lay
 // resident and run its prologue while the previous one drains; the kernels order their memory
 // accesses themselves with griddepcontrol.wait, so stream semantics are unchanged. ----------------
 template <typename... KArgs, typename... Args>
-cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+cudaError_t launch_k(bool pdl, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
     cfg.blockDim = block;
@@ -257,7 +371,7 @@ cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sme
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = g_opt_pdl.load() ? 1 : 0;
+    cfg.numAttrs = pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
@@ -270,16 +384,20 @@ struct Side {
     int device = -1;   // pool side: the device its memory lives on (-1: staging)
 };
 
-llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers, long long tile_bytes, int device,
-                       cudaStream_t st) {
-    DevInfo* di = nullptr;
-    llx_status rc = dev_info(device, &di);
+// `device` = the device the kernel runs on = the current device (the source pool's for a migration).
+llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long long n, int layers, long long tile_bytes,
+                       int device, cudaStream_t st) {
+    bool capturing = false;
+    llx_status rc = stream_capturing(st, &capturing);
     if (rc != LLX_OK) return rc;
+    DevInfo* di = nullptr;
+    if ((rc = dev_info(device, &di, capturing)) != LLX_OK) return rc;
 
     // kernel choice: the bulk-async ring for device<->device, the LDG/STG kernel when a side is host memory
-    long long kern = g_opt_kernel.load();
-    // a peer-mapped destination (another GPU) is written with plain 16-byte stores: NVLink, not HBM, is the bound
-    const bool peer = src.device >= 0 && dst.device >= 0 && src.device != dst.device;
+    long long kern = pol.kernel;
+    // a peer-mapped destination (another GPU) is written with plain 16-byte stores: NVLink, not HBM, is the bound.
+    // LLX_ROUTE_PEER takes the same route with both pools on one device (how a single-GPU box executes this branch).
+    const bool peer = pol.route == LLX_ROUTE_PEER || (src.device >= 0 && dst.device >= 0 && src.device != dst.device);
     if (kern == 0) kern = (src.host_memory || dst.host_memory || peer) ? 1 : 2;
     // Bandwidth budget: paced register-staged copies, no shared memory.  Measured
     // on B200: a co-resident CTA that holds > ~6 KB of shared memory shrinks the L1 of its SM and slows a
@@ -288,14 +406,14 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     // 400 GB/s paced but 0.045 % at 800 and 0.060 % at 2400, while a FEW full-speed bulk CTAs stay at 0.023-0.030 %
     // (about 60 GB/s per CTA: 7 CTAs 447 GB/s, 14: 864, 29: 1623, 43: 2243).  High budgets are therefore met by the
     // CTA count of the unpaced bulk kernel, low ones by the paced kernel.
-    const long long budget_asked = g_opt_budget.load();
-    const bool budget_by_ctas = budget_asked >= 500 && g_opt_kernel.load() == 0 && kern == 2;
+    const long long budget_asked = pol.budget;
+    const bool budget_by_ctas = budget_asked >= 500 && pol.kernel == 0 && kern == 2;
     const long long budget = budget_by_ctas ? 0 : budget_asked;  // from here on: > 0 means "paced"
-    if (budget > 0 && g_opt_kernel.load() != 2) kern = 1;
+    if (budget > 0 && pol.kernel != 2) kern = 1;
 
     const long long total_bytes = n * 2 * layers * tile_bytes;
-    long long chunk = g_opt_chunk.load();
-    int nstages = (int)g_opt_stages.load();
+    long long chunk = pol.chunk;
+    int nstages = (int)pol.stages;
     int threads = 256, grid = 0, long_per_sm = 1;
     size_t smem = 0;
     const int slices = 2 * layers;
@@ -314,7 +432,7 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         // tiles 2.0 -> 6.0 TB/s with four): more CTAs per SM, ~64-96 KiB in flight per SM in every case.
         long_per_sm = chunk >= 16384 ? 1 : chunk >= 8192 ? 2 : 4;
         if (nstages <= 0) nstages = budget > 0 ? 2 : short_stage ? 4 : chunk >= 32768 ? 3 : chunk >= 16384 ? 6 : 4;
-        int rings = (int)g_opt_rings.load();
+        int rings = (int)pol.rings;
         if (rings <= 0) rings = 1;
         threads = 32 * rings;
         smem = (((size_t)rings * nstages * 12 + 127) & ~(size_t)127) + (size_t)rings * nstages * chunk;
@@ -330,7 +448,7 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
             if (wpc < 1) wpc = 1;
             if (wpc > 8) wpc = 8;
             threads = (int)wpc * 32;
-            if (g_opt_rings.load() > 0) threads = (int)g_opt_rings.load() * 32;  // experiments: warps per paced CTA
+            if (pol.rings > 0) threads = (int)pol.rings * 32;  // experiments: warps per paced CTA
             if (chunk <= 0) chunk = (long long)threads * 16 * 4;
         } else if (chunk <= 0) {
             chunk = 256 * 16 * 4;
@@ -354,9 +472,9 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         // of 25 KiB: 351 us per step without PDL, 449-509 us with it).  Asking for just over 1/(per_sm+1) of the
         // SM's shared memory caps every SM at per_sm bulk CTAs, of this launch and of the next one together.
         long long want = per_sm;  // CTAs per SM the launch is meant to have
-        const long long capv = g_opt_max_ctas.load();
+        const long long capv = pol.max_ctas;
         if (capv > 0) want = (capv % di->sm_count == 0) ? capv / di->sm_count : 0;
-        if (g_opt_smem_pad.load() && budget <= 0 && want >= 1 && want <= 6) {
+        if (pol.smem_pad && budget <= 0 && want >= 1 && want <= 6) {
             const size_t floor_bytes = (size_t)di->smem_per_sm / (size_t)(want + 1) - 1024 + 128;
             if (smem < floor_bytes && floor_bytes <= (size_t)di->max_smem_optin) smem = floor_bytes;
         }
@@ -365,7 +483,7 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         // (measured: 52.7 GB/s with 74..296 CTAs, 51.5 with 1184) and leaves the SMs to whatever else is running.
         grid = (src.host_memory || dst.host_memory) ? di->sm_count : di->sm_count * 8;
     }
-    long long cap = g_opt_max_ctas.load();
+    long long cap = pol.max_ctas;
     if (cap <= 0 && budget_by_ctas) cap = (budget_asked + 30) / 60;
     if (cap > 0) grid = (int)cap;  // explicit grid: the throttle (fewer CTAs) or an experiment (more)
     {
@@ -395,8 +513,8 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     a.chunks_per_tile = (int)cpt;
     a.slices = slices;
     a.total_units = (int)units;
-    a.blocked_order = (int)g_opt_order.load();
-    a.l2_hint = (int)g_opt_l2hint.load();
+    a.blocked_order = (int)pol.order;
+    a.l2_hint = (int)pol.l2hint;
     a.pace_ns = (int)pace_ns;
     a.dyn_units = 0;
     a.dyn_batch = 1;
@@ -420,10 +538,13 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
         // cycles avg 96.4 % vs max 98.9 % of the kernel).  The last dyn_pct % of the units are claimed in batches.
         // Measured (B200, 7B tiles): 112 blocks 295.4 -> 291.3 us, 256 blocks 672 -> 656 us at 4-8 %; 1 % and 15 %
         // give half of that, 100 % (no contiguous ranges at all) is 3 % slower than none.
-        const long long pct = g_opt_dyn_pct.load();
+        // Not under stream capture: the claim counter belongs to the LAUNCHING stream, and a captured launch may be
+        // replayed on any stream, concurrently with direct launches of the capture stream that share the counter
+        // (a ring that reads an inflated claim index would stop early and chunks would never be copied).
+        const long long pct = pol.dyn_pct;
         const long long nrings = (long long)grid * (threads / 32);
-        if (kern == 2 && a.blocked_order && pct > 0 && budget <= 0 && units >= nrings * 16) {
-            const long long batch = g_opt_dyn_batch.load() > 0 ? g_opt_dyn_batch.load() : 4;
+        if (kern == 2 && a.blocked_order && pct > 0 && budget <= 0 && units >= nrings * 16 && !capturing) {
+            const long long batch = pol.dyn_batch > 0 ? pol.dyn_batch : 4;
             long long dyn = units * pct / 100 / batch * batch;
             if (dyn > 0) {
                 if ((rc = dyn_counter_get(device, st, &a.dyn_counter)) != LLX_OK) return rc;
@@ -437,16 +558,20 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     }
 
     static thread_local IdPack pack;  // 2 KiB; only the first n entries are meaningful
-    const bool byval = n <= g_opt_byval.load();
-    std::unique_lock<std::mutex> ring_lk(g_ring_mu, std::defer_lock);
+    const bool byval = n <= pol.byval || (!src.ids && !dst.ids);
+    IdRing& ring = g_ring[device];
+    std::unique_lock<std::mutex> ring_lk(ring.mu, std::defer_lock);
     IdSlot* slot = nullptr;
     if (byval) {
         if (src.ids) memcpy(pack.src, src.ids, n * sizeof(int32_t));
         if (dst.ids) memcpy(pack.dst, dst.ids, n * sizeof(int32_t));
     } else {
+        if (capturing)
+            return fail(LLX_ERR_STATE, "a stage of %lld pairs cannot be captured into a CUDA graph: id lists longer than %lld go through a pinned ring "
+                        "(host copy + event wait at launch); split the stage into calls of <= %d pairs", n, pol.byval, kIdsByValueCap);
         int32_t* dev_ids = nullptr;
         ring_lk.lock();
-        rc = ring_stage(src.ids, src.ids ? n : 0, dst.ids, dst.ids ? n : 0, st, &dev_ids, &slot);
+        rc = ring_stage(ring, src.ids, src.ids ? n : 0, dst.ids, dst.ids ? n : 0, st, &dev_ids, &slot);
         if (rc != LLX_OK) return rc;
         if (src.ids) a.src_ids = dev_ids;
         if (dst.ids) a.dst_ids = dev_ids + (src.ids ? n : 0);
@@ -454,20 +579,22 @@ llx_status launch_copy(const Side& src, const Side& dst, long long n, int layers
     }
 
     cudaError_t e;
+    const bool pdl = pol.pdl != 0;
     if (kern == 2) {
         if (byval)
-            e = launch_k(llx_copy_bulk<true>, grid, threads, smem, st, a, pack, nstages);
+            e = launch_k(pdl, llx_copy_bulk<true>, grid, threads, smem, st, a, pack, nstages);
         else
-            e = launch_k(llx_copy_bulk<false>, grid, threads, smem, st, a, pack, nstages);
+            e = launch_k(pdl, llx_copy_bulk<false>, grid, threads, smem, st, a, pack, nstages);
     } else {
         if (byval)
-            e = launch_k(llx_copy_vec16<true, 4>, grid, threads, 0, st, a, pack);
+            e = launch_k(pdl, llx_copy_vec16<true, 4>, grid, threads, 0, st, a, pack);
         else
-            e = launch_k(llx_copy_vec16<false, 4>, grid, threads, 0, st, a, pack);
+            e = launch_k(pdl, llx_copy_vec16<false, 4>, grid, threads, 0, st, a, pack);
     }
     if (e == cudaSuccess) e = cudaGetLastError();
-    if (slot) cudaEventRecord(slot->ev, st);
+    const llx_status rc_ring = ring_close(slot, st);
     if (e != cudaSuccess) return cuda_fail(e, "copy kernel launch");
+    if (rc_ring != LLX_OK) return rc_ring;
     g_launches++;
     g_copy_launches++;
     g_bytes += (unsigned long long)total_bytes;
@@ -566,7 +693,9 @@ llx_status pipe_get(int dev, size_t bounce_bytes, Pipe** out) {
 // 55.6 host->device on this B200) faster than kernels addressing the pinned buffer directly (52.7 / 51.4 GB/s),
 // so the tiles are gathered into (scattered from) a device bounce buffer chunk by chunk and the chunk is moved
 // with cudaMemcpyAsync, all on the caller's stream (a 64 MiB chunk: 10 us of kernel per 1.1 ms of link).
-llx_status staged_through_bounce(bool to_host, const llx_pool* pool, const int32_t* ids, int n, const Side& stg, cudaStream_t st) {
+llx_status staged_through_bounce(const Policy& pol, bool to_host, const llx_pool* pool, const int32_t* ids, int n, const Side& stg, cudaStream_t st) {
+    llx_status rc = refuse_if_capturing(st, "llx_pack / llx_unpack through a pinned-host buffer");
+    if (rc != LLX_OK) return rc;
     const long long block_bytes = 2ll * pool->layers * pool->tile_bytes;
     int chunk_blocks = (int)((64ll << 20) / block_bytes);
     if (chunk_blocks < 1) chunk_blocks = 1;
@@ -574,25 +703,27 @@ llx_status staged_through_bounce(bool to_host, const llx_pool* pool, const int32
     if (chunk_blocks > kIdsByValueCap) chunk_blocks = kIdsByValueCap;
     std::lock_guard<std::mutex> lk(g_pipe_mu);
     Pipe* pipe = nullptr;
-    llx_status rc = pipe_get(pool->device, (size_t)chunk_blocks * block_bytes, &pipe);
-    if (rc != LLX_OK) return rc;
+    if ((rc = pipe_get(pool->device, (size_t)chunk_blocks * block_bytes, &pipe)) != LLX_OK) return rc;
     if (pipe->idle_valid) LLX_CUDA(cudaStreamWaitEvent(st, pipe->idle, 0));
     unsigned char* bounce = pipe->bounce[to_host ? 0 : 2];
     const Side dev_side = Side{bounce, nullptr, stg.slice_stride, stg.item_stride, false};
-    for (int k = 0; k < n; k += chunk_blocks) {
+    cudaError_t ce = cudaSuccess;
+    for (int k = 0; k < n && rc == LLX_OK && ce == cudaSuccess; k += chunk_blocks) {
         const int m = (n - k < chunk_blocks) ? n - k : chunk_blocks;
         unsigned char* host = const_cast<unsigned char*>(stg.base) + (long long)k * block_bytes;
         const size_t bytes = (size_t)m * block_bytes;
         if (to_host) {
-            if ((rc = launch_copy(pool_side(pool, ids + k), dev_side, m, pool->layers, pool->tile_bytes, pool->device, st)) != LLX_OK) return rc;
-            LLX_CUDA(cudaMemcpyAsync(host, bounce, bytes, cudaMemcpyDefault, st));
+            rc = launch_copy(pol, pool_side(pool, ids + k), dev_side, m, pool->layers, pool->tile_bytes, pool->device, st);
+            if (rc == LLX_OK) ce = cudaMemcpyAsync(host, bounce, bytes, cudaMemcpyDefault, st);
         } else {
-            LLX_CUDA(cudaMemcpyAsync(bounce, host, bytes, cudaMemcpyDefault, st));
-            if ((rc = launch_copy(dev_side, pool_side(pool, ids + k), m, pool->layers, pool->tile_bytes, pool->device, st)) != LLX_OK) return rc;
+            ce = cudaMemcpyAsync(bounce, host, bytes, cudaMemcpyDefault, st);
+            if (ce == cudaSuccess) rc = launch_copy(pol, dev_side, pool_side(pool, ids + k), m, pool->layers, pool->tile_bytes, pool->device, st);
         }
     }
-    LLX_CUDA(cudaEventRecord(pipe->idle, st));
-    pipe->idle_valid = true;
+    // also on an error path: whatever was enqueued still uses the bounce buffers, the next call must wait for it
+    if (cudaEventRecord(pipe->idle, st) == cudaSuccess) pipe->idle_valid = true;
+    if (rc != LLX_OK) return rc;
+    if (ce != cudaSuccess) return cuda_fail(ce, "cudaMemcpyAsync (bounce buffer)");
     return LLX_OK;
 }
 
@@ -703,9 +834,13 @@ llx_status llx_pool_download(const llx_pool* p, int layer, int kv, int first, in
 llx_status llx_pool_fill_u16(llx_pool* p, uint16_t pattern, void* stream) {
     llx_status rc = check_pool(p, "pool");
     if (rc != LLX_OK) return rc;
+    bool capturing = false;
+    if ((rc = stream_capturing((cudaStream_t)stream, &capturing)) != LLX_OK) return rc;
+    DevInfo* di = nullptr;
+    if ((rc = dev_info(p->device, &di, capturing)) != LLX_OK) return rc;
     const long long nvec = (long long)(pool_bytes(p) / 16);
     const uint32_t w = (uint32_t)pattern | ((uint32_t)pattern << 16);
-    llx_fill_u16_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((uint4*)p->data, nvec, w);
+    llx_fill_u16_kernel<<<di->sm_count * 8, 256, 0, (cudaStream_t)stream>>>((uint4*)p->data, nvec, w);
     LLX_CUDA(cudaGetLastError());
     g_launches++;
     return LLX_OK;
@@ -730,8 +865,14 @@ llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, i
     return LLX_OK;
 }
 
-llx_status llx_migrate_stage(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
-                             void* stream) {
+void llx_launch_opts_init(llx_launch_opts* o) {
+    if (!o) return;
+    memset(o, 0xFF, sizeof *o);  // every int32 field = -1 = LLX_OPT_DEFAULT
+    o->struct_size = (uint32_t)sizeof *o;
+}
+
+static llx_status migrate_stage_checked(const Policy& pol, const llx_pool* src, const int32_t* src_ids, llx_pool* dst,
+                                        const int32_t* dst_ids, int n, void* stream) {
     llx_status rc = check_pair(src, dst);
     if (rc != LLX_OK) return rc;
     if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
@@ -740,20 +881,40 @@ llx_status llx_migrate_stage(const llx_pool* src, const int32_t* src_ids, llx_po
     if ((rc = check_range(src_ids, n, src->num_blocks, "src")) != LLX_OK) return rc;
     if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
     if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
-    return launch_copy(pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
+    return launch_copy(pol, pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
                        (cudaStream_t)stream);
 }
 
-llx_status llx_migrate_stage_wait(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
-                                  void* stream) {
-    if (n <= 0 || !src) return llx_migrate_stage(src, src_ids, dst, dst_ids, n, stream);  // nothing to wait for / argument error
-    DoneSlot* slot = nullptr;
-    llx_status rc = done_slot_get(src->device, &slot);
+llx_status llx_migrate_stage_ex(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
+                                void* stream, const llx_launch_opts* opts) {
+    LLX_TRY
+    Policy pol;
+    llx_status rc = resolve_policy(opts, &pol);
     if (rc != LLX_OK) return rc;
+    return migrate_stage_checked(pol, src, src_ids, dst, dst_ids, n, stream);
+    LLX_CATCH
+}
+llx_status llx_migrate_stage(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
+                             void* stream) {
+    return llx_migrate_stage_ex(src, src_ids, dst, dst_ids, n, stream, nullptr);
+}
+
+llx_status llx_migrate_stage_wait_ex(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
+                                     void* stream, const llx_launch_opts* opts) {
+    LLX_TRY
+    Policy pol;
+    llx_status rc = resolve_policy(opts, &pol);
+    if (rc != LLX_OK) return rc;
+    pol.budget = 0;  // the final stage is the downtime: never throttled, whatever the defaults say
+    pol.max_ctas = 0;
+    if (n <= 0 || !src) return migrate_stage_checked(pol, src, src_ids, dst, dst_ids, n, stream);  // nothing to wait for / argument error
+    if ((rc = refuse_if_capturing((cudaStream_t)stream, "llx_migrate_stage_wait (a blocking call)")) != LLX_OK) return rc;
+    DoneSlot* slot = nullptr;
+    if ((rc = done_slot_get(src->device, &slot)) != LLX_OK) return rc;
     DoneReq req;
     req.slot = slot;
     tl_done = &req;
-    rc = llx_migrate_stage(src, src_ids, dst, dst_ids, n, stream);
+    rc = migrate_stage_checked(pol, src, src_ids, dst, dst_ids, n, stream);
     tl_done = nullptr;
     if (rc != LLX_OK) {
         if (slot) done_slot_put(slot);
@@ -764,29 +925,51 @@ llx_status llx_migrate_stage_wait(const llx_pool* src, const int32_t* src_ids, l
         LLX_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
         return LLX_OK;
     }
-    // spin on the word the kernel's last ring writes; an unset flag after 1e8 polls (seconds) means the launch
-    // failed asynchronously: let the stream synchronize report it
+    // Spin on the word the kernel's last ring writes.  Every ~1e5 polls the stream is queried: an error there is an
+    // asynchronous fault of the copy (the flag will never come); a stream that reports completion has written it.
     const unsigned int want = slot->seq;
     bool seen = false;
-    for (long long i = 0; i < 100000000ll; ++i) {
+    cudaError_t qe = cudaErrorNotReady;
+    for (long long i = 0; !seen; ++i) {
         if (*slot->host == want) {
             seen = true;
             break;
+        }
+        if ((i % 100000) == 99999) {
+            qe = cudaStreamQuery((cudaStream_t)stream);
+            if (qe != cudaErrorNotReady) break;
         }
 #if defined(__x86_64__)
         __builtin_ia32_pause();
 #endif
     }
     std::atomic_thread_fence(std::memory_order_acquire);
+    if (!seen) {
+        // The slot goes back only once the kernel that holds its counter is off the device: released earlier, another
+        // waiter's kernel would share the counter and a flag could be written before that copy has landed.
+        cudaError_t se = cudaStreamSynchronize((cudaStream_t)stream);
+        done_slot_put(slot);
+        if (qe != cudaSuccess && qe != cudaErrorNotReady) return cuda_fail(qe, "final-stage copy (asynchronous fault)");
+        if (se != cudaSuccess) return cuda_fail(se, "cudaStreamSynchronize");
+        return LLX_OK;
+    }
     done_slot_put(slot);
-    if (!seen) LLX_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    LLX_CUDA(cudaGetLastError());  // a sticky asynchronous fault of this or an earlier launch
     return LLX_OK;
+    LLX_CATCH
+}
+llx_status llx_migrate_stage_wait(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
+                                  void* stream) {
+    return llx_migrate_stage_wait_ex(src, src_ids, dst, dst_ids, n, stream, nullptr);
 }
 
-llx_status llx_migrate_batch(const llx_pool* src, llx_pool* dst, const int32_t* off, const int32_t* src_ids,
-                             const int32_t* dst_ids, int R, void* stream) {
-    llx_status rc = check_pair(src, dst);
+llx_status llx_migrate_batch_ex(const llx_pool* src, llx_pool* dst, const int32_t* off, const int32_t* src_ids,
+                                const int32_t* dst_ids, int R, void* stream, const llx_launch_opts* opts) {
+    LLX_TRY
+    Policy pol;
+    llx_status rc = resolve_policy(opts, &pol);
     if (rc != LLX_OK) return rc;
+    if ((rc = check_pair(src, dst)) != LLX_OK) return rc;
     if (R < 0) return fail(LLX_ERR_INVALID_ARG, "R = %d", R);
     if (R == 0) return LLX_OK;
     if (!off) return fail(LLX_ERR_INVALID_ARG, "req_offsets is NULL");
@@ -800,8 +983,13 @@ llx_status llx_migrate_batch(const llx_pool* src, llx_pool* dst, const int32_t* 
     if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
     if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
     // every (block, layer, K|V) tile is independent, so the requests are flattened into one grid
-    return launch_copy(pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
+    return launch_copy(pol, pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
                        (cudaStream_t)stream);
+    LLX_CATCH
+}
+llx_status llx_migrate_batch(const llx_pool* src, llx_pool* dst, const int32_t* off, const int32_t* src_ids,
+                             const int32_t* dst_ids, int R, void* stream) {
+    return llx_migrate_batch_ex(src, dst, off, src_ids, dst_ids, R, stream, nullptr);
 }
 
 size_t llx_staging_bytes(const llx_pool* p, int n) { return (p && n > 0) ? (size_t)n * llx_pool_block_bytes(p) : 0; }
@@ -831,9 +1019,13 @@ llx_status llx_staging_free_pinned(void* host_ptr) {
     return LLX_OK;
 }
 
-llx_status llx_pack(const llx_pool* src, const int32_t* src_ids, int n, void* staging, size_t staging_bytes, void* stream) {
-    llx_status rc = check_pool(src, "src");
+llx_status llx_pack_ex(const llx_pool* src, const int32_t* src_ids, int n, void* staging, size_t staging_bytes, void* stream,
+                       const llx_launch_opts* opts) {
+    LLX_TRY
+    Policy pol;
+    llx_status rc = resolve_policy(opts, &pol);
     if (rc != LLX_OK) return rc;
+    if ((rc = check_pool(src, "src")) != LLX_OK) return rc;
     if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
     if (n == 0) return LLX_OK;
     if (!src_ids || !staging) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
@@ -844,14 +1036,22 @@ llx_status llx_pack(const llx_pool* src, const int32_t* src_ids, int n, void* st
     if ((rc = staging_side(staging, src->layers, src->tile_bytes, &stg)) != LLX_OK) return rc;
     const unsigned char *a0 = src->data, *a1 = a0 + pool_bytes(src), *b0 = stg.base, *b1 = b0 + llx_staging_bytes(src, n);
     if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "staging buffer overlaps the pool");
-    if (stg.host_memory && g_opt_via_host.load() == 0 && g_opt_kernel.load() == 0)
-        return staged_through_bounce(true, src, src_ids, n, stg, (cudaStream_t)stream);
-    return launch_copy(pool_side(src, src_ids), stg, n, src->layers, src->tile_bytes, src->device, (cudaStream_t)stream);
+    if (stg.host_memory && pol.via_host == 0 && pol.kernel == 0)
+        return staged_through_bounce(pol, true, src, src_ids, n, stg, (cudaStream_t)stream);
+    return launch_copy(pol, pool_side(src, src_ids), stg, n, src->layers, src->tile_bytes, src->device, (cudaStream_t)stream);
+    LLX_CATCH
+}
+llx_status llx_pack(const llx_pool* src, const int32_t* src_ids, int n, void* staging, size_t staging_bytes, void* stream) {
+    return llx_pack_ex(src, src_ids, n, staging, staging_bytes, stream, nullptr);
 }
 
-llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, const int32_t* dst_ids, int n, void* stream) {
-    llx_status rc = check_pool(dst, "dst");
+llx_status llx_unpack_ex(const void* staging, size_t staging_bytes, llx_pool* dst, const int32_t* dst_ids, int n, void* stream,
+                         const llx_launch_opts* opts) {
+    LLX_TRY
+    Policy pol;
+    llx_status rc = resolve_policy(opts, &pol);
     if (rc != LLX_OK) return rc;
+    if ((rc = check_pool(dst, "dst")) != LLX_OK) return rc;
     if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
     if (n == 0) return LLX_OK;
     if (!dst_ids || !staging) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
@@ -863,15 +1063,23 @@ llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, 
     if ((rc = staging_side(staging, dst->layers, dst->tile_bytes, &stg)) != LLX_OK) return rc;
     const unsigned char *a0 = dst->data, *a1 = a0 + pool_bytes(dst), *b0 = stg.base, *b1 = b0 + llx_staging_bytes(dst, n);
     if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "staging buffer overlaps the pool");
-    if (stg.host_memory && g_opt_via_host.load() == 0 && g_opt_kernel.load() == 0)
-        return staged_through_bounce(false, dst, dst_ids, n, stg, (cudaStream_t)stream);
-    return launch_copy(stg, pool_side(dst, dst_ids), n, dst->layers, dst->tile_bytes, dst->device, (cudaStream_t)stream);
+    if (stg.host_memory && pol.via_host == 0 && pol.kernel == 0)
+        return staged_through_bounce(pol, false, dst, dst_ids, n, stg, (cudaStream_t)stream);
+    return launch_copy(pol, stg, pool_side(dst, dst_ids), n, dst->layers, dst->tile_bytes, dst->device, (cudaStream_t)stream);
+    LLX_CATCH
+}
+llx_status llx_unpack(const void* staging, size_t staging_bytes, llx_pool* dst, const int32_t* dst_ids, int n, void* stream) {
+    return llx_unpack_ex(staging, staging_bytes, dst, dst_ids, n, stream, nullptr);
 }
 
-llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
-                                void* staging, size_t staging_bytes, int chunk_blocks, void* stream) {
-    llx_status rc = check_pair(src, dst);
+llx_status llx_migrate_via_host_ex(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
+                                   void* staging, size_t staging_bytes, int chunk_blocks, void* stream,
+                                   const llx_launch_opts* opts) {
+    LLX_TRY
+    Policy pol;
+    llx_status rc = resolve_policy(opts, &pol);
     if (rc != LLX_OK) return rc;
+    if ((rc = check_pair(src, dst)) != LLX_OK) return rc;
     if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
     if (n == 0) return LLX_OK;
     if (!src_ids || !dst_ids || !staging) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
@@ -887,6 +1095,8 @@ llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_ids, llx
         const unsigned char *a0 = p->data, *a1 = a0 + pool_bytes(p);
         if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "staging buffer overlaps a pool");
     }
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = refuse_if_capturing(st, "llx_migrate_via_host (internal streams, bounce buffers)")) != LLX_OK) return rc;
     const long long block_bytes = 2ll * src->layers * src->tile_bytes;
     // Route.  Pinned-host buffer: gather into a device bounce buffer with the copy kernel, move the chunk over
     // the host link with the copy engines (D2H on one internal stream, H2D on another: the link is full duplex,
@@ -894,7 +1104,7 @@ llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_ids, llx
     // B200: kernels that address the pinned buffer directly reach 52 GB/s per direction but share ~60 GB/s when
     // both directions run at once, so the zero-copy form (LLX_OPT_VIA_HOST_MODE=1) is kept for comparison only.
     // Device buffer: nothing crosses the link; the two kernels of a chunk simply run on two streams.
-    const bool bounce = stg.host_memory && g_opt_via_host.load() == 0;
+    const bool bounce = stg.host_memory && pol.via_host == 0;
     if (chunk_blocks <= 0) {  // ~64 MiB per chunk (measured best on B200: 24.6 ms per GiB each way; 32 MiB 24.9, 128 MiB 25.5)
         chunk_blocks = (int)((64ll << 20) / block_bytes);
         if (chunk_blocks < 1) chunk_blocks = 1;
@@ -905,50 +1115,70 @@ llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_ids, llx
     std::lock_guard<std::mutex> lk(g_pipe_mu);  // the internal streams, events and bounce buffers are shared per device
     Pipe* pipe = nullptr;
     if ((rc = pipe_get(src->device, bounce ? (size_t)chunk_blocks * block_bytes : 0, &pipe)) != LLX_OK) return rc;
-    cudaStream_t st = (cudaStream_t)stream;
     if (pipe->idle_valid) LLX_CUDA(cudaStreamWaitEvent(st, pipe->idle, 0));
+    // Every kernel of this call runs on the source's device (the current one); a destination on a peer GPU is written
+    // through its peer mapping.  From here on an error does not return at once: whatever was enqueued on the internal
+    // streams is joined into the caller's stream and `idle` is recorded first (the next call reuses the bounce buffers).
+    cudaError_t ce = cudaSuccess;
+#define LLX_STEP(call) \
+    if (rc == LLX_OK && ce == cudaSuccess) ce = (call)
+#define LLX_COPY(...) \
+    if (rc == LLX_OK && ce == cudaSuccess) rc = launch_copy(__VA_ARGS__)
     cudaEvent_t d2h_done[2] = {nullptr, nullptr};
     int idx = 0;
-    for (int k = 0; k < n; k += chunk_blocks, ++idx) {
+    for (int k = 0; k < n && rc == LLX_OK && ce == cudaSuccess; k += chunk_blocks, ++idx) {
         const int m = (n - k < chunk_blocks) ? n - k : chunk_blocks;
         const long long off = (long long)k * block_bytes;
         Side part = stg;  // chunk k's slice of the caller's buffer
         part.base = stg.base + off;
         if (!bounce) {
-            if ((rc = launch_copy(pool_side(src, src_ids + k), part, m, src->layers, src->tile_bytes, src->device, st)) != LLX_OK) return rc;
+            LLX_COPY(pol, pool_side(src, src_ids + k), part, m, src->layers, src->tile_bytes, src->device, st);
             cudaEvent_t ev = pipe->take();
-            LLX_CUDA(cudaEventRecord(ev, st));
-            LLX_CUDA(cudaStreamWaitEvent(pipe->h2d, ev, 0));
-            if ((rc = launch_copy(part, pool_side(dst, dst_ids + k), m, dst->layers, dst->tile_bytes, dst->device, pipe->h2d)) != LLX_OK) return rc;
+            LLX_STEP(cudaEventRecord(ev, st));
+            LLX_STEP(cudaStreamWaitEvent(pipe->h2d, ev, 0));
+            LLX_COPY(pol, part, pool_side(dst, dst_ids + k), m, dst->layers, dst->tile_bytes, src->device, pipe->h2d);
             continue;
         }
         const int slot = idx & 1;
         Side ga = Side{pipe->bounce[slot], nullptr, stg.slice_stride, stg.item_stride, false};
         Side sc = Side{pipe->bounce[2 + slot], nullptr, stg.slice_stride, stg.item_stride, false};
         const size_t bytes = (size_t)m * block_bytes;
-        if (d2h_done[slot]) LLX_CUDA(cudaStreamWaitEvent(st, d2h_done[slot], 0));  // bounce buffer free again
-        if ((rc = launch_copy(pool_side(src, src_ids + k), ga, m, src->layers, src->tile_bytes, src->device, st)) != LLX_OK) return rc;
+        if (d2h_done[slot]) {  // bounce buffer free again
+            LLX_STEP(cudaStreamWaitEvent(st, d2h_done[slot], 0));
+        }
+        LLX_COPY(pol, pool_side(src, src_ids + k), ga, m, src->layers, src->tile_bytes, src->device, st);
         cudaEvent_t packed = pipe->take();
-        LLX_CUDA(cudaEventRecord(packed, st));
-        LLX_CUDA(cudaStreamWaitEvent(pipe->d2h, packed, 0));
-        LLX_CUDA(cudaMemcpyAsync(const_cast<unsigned char*>(part.base), ga.base, bytes, cudaMemcpyDefault, pipe->d2h));
+        LLX_STEP(cudaEventRecord(packed, st));
+        LLX_STEP(cudaStreamWaitEvent(pipe->d2h, packed, 0));
+        LLX_STEP(cudaMemcpyAsync(const_cast<unsigned char*>(part.base), ga.base, bytes, cudaMemcpyDefault, pipe->d2h));
         cudaEvent_t landed = pipe->take();
-        LLX_CUDA(cudaEventRecord(landed, pipe->d2h));
+        LLX_STEP(cudaEventRecord(landed, pipe->d2h));
         d2h_done[slot] = landed;
-        LLX_CUDA(cudaStreamWaitEvent(pipe->h2d, landed, 0));
-        LLX_CUDA(cudaMemcpyAsync(const_cast<unsigned char*>(sc.base), part.base, bytes, cudaMemcpyDefault, pipe->h2d));
-        if ((rc = launch_copy(sc, pool_side(dst, dst_ids + k), m, dst->layers, dst->tile_bytes, dst->device, pipe->h2d)) != LLX_OK) return rc;
+        LLX_STEP(cudaStreamWaitEvent(pipe->h2d, landed, 0));
+        LLX_STEP(cudaMemcpyAsync(const_cast<unsigned char*>(sc.base), part.base, bytes, cudaMemcpyDefault, pipe->h2d));
+        LLX_COPY(pol, sc, pool_side(dst, dst_ids + k), m, dst->layers, dst->tile_bytes, src->device, pipe->h2d);
     }
-    cudaEvent_t done = pipe->take();
-    LLX_CUDA(cudaEventRecord(done, pipe->h2d));
-    LLX_CUDA(cudaStreamWaitEvent(st, done, 0));  // join: later work on the caller's stream sees the whole migration
-    LLX_CUDA(cudaEventRecord(pipe->idle, st));
-    pipe->idle_valid = true;
+#undef LLX_STEP
+#undef LLX_COPY
+    // join (also after an error): later work on the caller's stream sees everything this call enqueued
+    for (cudaStream_t side : {pipe->d2h, pipe->h2d}) {
+        cudaEvent_t done = pipe->take();
+        if (cudaEventRecord(done, side) == cudaSuccess) cudaStreamWaitEvent(st, done, 0);
+    }
+    if (cudaEventRecord(pipe->idle, st) == cudaSuccess) pipe->idle_valid = true;
+    if (rc != LLX_OK) return rc;
+    if (ce != cudaSuccess) return cuda_fail(ce, "llx_migrate_via_host (stream plumbing)");
     return LLX_OK;
+    LLX_CATCH
+}
+llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, int n,
+                                void* staging, size_t staging_bytes, int chunk_blocks, void* stream) {
+    return llx_migrate_via_host_ex(src, src_ids, dst, dst_ids, n, staging, staging_bytes, chunk_blocks, stream, nullptr);
 }
 
 llx_status llx_append_tokens(llx_pool* p, const int32_t* table, int table_len, int t0, int t1, const void* dev_values,
                              void* stream) {
+    LLX_TRY
     llx_status rc = check_pool(p, "pool");
     if (rc != LLX_OK) return rc;
     if (t0 < 0 || t1 < t0) return fail(LLX_ERR_INVALID_ARG, "bad token range [%d,%d)", t0, t1);
@@ -975,24 +1205,29 @@ llx_status llx_append_tokens(llx_pool* p, const int32_t* table, int table_len, i
     static thread_local IdPack pack;
     cudaStream_t st = (cudaStream_t)stream;
     IdSlot* slot = nullptr;
-    std::unique_lock<std::mutex> ring_lk(g_ring_mu, std::defer_lock);
+    IdRing& ring = g_ring[p->device];
+    std::unique_lock<std::mutex> ring_lk(ring.mu, std::defer_lock);
     const int grid = ntok * a.slices;
+    const bool pdl = g_opt_pdl.load() != 0;
     cudaError_t e;
     if (ntok <= kIdsByValueCap) {
         memcpy(pack.src, tb.data(), ntok * sizeof(int32_t));
-        e = launch_k(llx_append_kernel<true>, grid, 128, 0, st, a, pack);
+        e = launch_k(pdl, llx_append_kernel<true>, grid, 128, 0, st, a, pack);
     } else {
+        if ((rc = refuse_if_capturing(st, "llx_append_tokens of more than 256 tokens (ids go through a pinned ring)")) != LLX_OK) return rc;
         int32_t* dev_ids = nullptr;
         ring_lk.lock();
-        if ((rc = ring_stage(tb.data(), ntok, nullptr, 0, st, &dev_ids, &slot)) != LLX_OK) return rc;
+        if ((rc = ring_stage(ring, tb.data(), ntok, nullptr, 0, st, &dev_ids, &slot)) != LLX_OK) return rc;
         a.tok_block = dev_ids;
-        e = launch_k(llx_append_kernel<false>, grid, 128, 0, st, a, pack);
+        e = launch_k(pdl, llx_append_kernel<false>, grid, 128, 0, st, a, pack);
     }
     if (e == cudaSuccess) e = cudaGetLastError();
-    if (slot) cudaEventRecord(slot->ev, st);
+    const llx_status rc_ring = ring_close(slot, st);
     if (e != cudaSuccess) return cuda_fail(e, "append kernel launch");
+    if (rc_ring != LLX_OK) return rc_ring;
     g_launches++;
     return LLX_OK;
+    LLX_CATCH
 }
 
 llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* q, void* out, const int32_t* block_tables,
@@ -1018,6 +1253,7 @@ llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* q, 
     if (max_splits > 65535 || B > 65535) return fail(LLX_ERR_INVALID_ARG, "grid too large");
     const size_t need = (size_t)B * H * max_splits * (D + 4) * sizeof(float);
     if (need > p->attn_ws_bytes) {
+        if ((rc = refuse_if_capturing(st, "llx_decode_attention that has to grow its workspace (run the shape once outside the capture)")) != LLX_OK) return rc;
         if (p->attn_ws) {
             LLX_CUDA(cudaDeviceSynchronize());
             cudaFree(p->attn_ws);
@@ -1050,12 +1286,13 @@ llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* q, 
     const int head_groups = (H + kAttnWarps * hpw - 1) / (kAttnWarps * hpw);
     dim3 grid1(max_splits, head_groups, B), grid2(H, B);
     cudaError_t e;
+    const bool pdl = g_opt_pdl.load() != 0;
     if (D == 128) {
-        e = launch_k(llx_attn_partial<128>, grid1, kAttnWarps * 32, 0, st, a);
-        if (e == cudaSuccess) e = launch_k(llx_attn_merge<128>, grid2, 128, 0, st, a);
+        e = launch_k(pdl, llx_attn_partial<128>, grid1, kAttnWarps * 32, 0, st, a);
+        if (e == cudaSuccess) e = launch_k(pdl, llx_attn_merge<128>, grid2, 128, 0, st, a);
     } else {
-        e = launch_k(llx_attn_partial<64>, grid1, kAttnWarps * 32, 0, st, a);
-        if (e == cudaSuccess) e = launch_k(llx_attn_merge<64>, grid2, 64, 0, st, a);
+        e = launch_k(pdl, llx_attn_partial<64>, grid1, kAttnWarps * 32, 0, st, a);
+        if (e == cudaSuccess) e = launch_k(pdl, llx_attn_merge<64>, grid2, 64, 0, st, a);
     }
     if (e != cudaSuccess) return cuda_fail(e, "attention kernel launch");
     LLX_CUDA(cudaGetLastError());
@@ -1064,69 +1301,25 @@ llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* q, 
 }
 
 llx_status llx_set_option(llx_option opt, long long v) {
+    if (!opt_valid((int)opt, v)) return fail(LLX_ERR_INVALID_ARG, "option %d: bad value %lld", (int)opt, v);
     switch (opt) {
-        case LLX_OPT_COPY_KERNEL:
-            if (v < 0 || v > 2) break;
-            g_opt_kernel = v;
-            return LLX_OK;
-        case LLX_OPT_MAX_CTAS:
-            if (v < 0) break;
-            g_opt_max_ctas = v;
-            return LLX_OK;
-        case LLX_OPT_CHUNK_BYTES:
-            if (v < 0 || (v % 16) != 0 || v > (200 << 10)) break;
-            g_opt_chunk = v;
-            return LLX_OK;
-        case LLX_OPT_RING_STAGES:
-            if (v < 0 || v == 1 || v > 14) break;
-            g_opt_stages = v;
-            return LLX_OK;
-        case LLX_OPT_IDS_BY_VALUE_MAX:
-            if (v < 0 || v > kIdsByValueCap) break;
-            g_opt_byval = v;
-            return LLX_OK;
-        case LLX_OPT_ATTN_SPLIT_TOKENS:
-            if (v < 0 || (v % 8) != 0) break;
-            g_opt_attn_split = v;
-            return LLX_OK;
-        case LLX_OPT_UNIT_ORDER:
-            if (v < 0 || v > 1) break;
-            g_opt_order = v;
-            return LLX_OK;
-        case LLX_OPT_L2_HINT:
-            if (v < 0 || v > 3) break;
-            g_opt_l2hint = v;
-            return LLX_OK;
-        case LLX_OPT_RINGS_PER_CTA:
-            if (v < 0 || v > 8) break;
-            g_opt_rings = v;
-            return LLX_OK;
-        case LLX_OPT_PDL:
-            if (v < 0 || v > 1) break;
-            g_opt_pdl = v;
-            return LLX_OK;
-        case LLX_OPT_BANDWIDTH_GBPS:
-            if (v < 0 || v > 100000) break;
-            g_opt_budget = v;
-            return LLX_OK;
-        case LLX_OPT_VIA_HOST_MODE:
-            if (v < 0 || v > 1) break;
-            g_opt_via_host = v;
-            return LLX_OK;
-        case LLX_OPT_DYNAMIC_TAIL_PCT:
-            if (v < 0 || v > 100) break;
-            g_opt_dyn_pct = v;
-            return LLX_OK;
-        case LLX_OPT_DYNAMIC_TAIL_BATCH:
-            if (v < 0 || v > 4096) break;
-            g_opt_dyn_batch = v;
-            return LLX_OK;
-        case LLX_OPT_EXACT_RESIDENCY:
-            if (v < 0 || v > 1) break;
-            g_opt_smem_pad = v;
-            return LLX_OK;
+        case LLX_OPT_COPY_KERNEL: g_opt_kernel = v; break;
+        case LLX_OPT_MAX_CTAS: g_opt_max_ctas = v; break;
+        case LLX_OPT_CHUNK_BYTES: g_opt_chunk = v; break;
+        case LLX_OPT_RING_STAGES: g_opt_stages = v; break;
+        case LLX_OPT_IDS_BY_VALUE_MAX: g_opt_byval = v; break;
+        case LLX_OPT_ATTN_SPLIT_TOKENS: g_opt_attn_split = v; break;
+        case LLX_OPT_UNIT_ORDER: g_opt_order = v; break;
+        case LLX_OPT_L2_HINT: g_opt_l2hint = v; break;
+        case LLX_OPT_RINGS_PER_CTA: g_opt_rings = v; break;
+        case LLX_OPT_PDL: g_opt_pdl = v; break;
+        case LLX_OPT_BANDWIDTH_GBPS: g_opt_budget = v; break;
+        case LLX_OPT_VIA_HOST_MODE: g_opt_via_host = v; break;
+        case LLX_OPT_DYNAMIC_TAIL_PCT: g_opt_dyn_pct = v; break;
+        case LLX_OPT_DYNAMIC_TAIL_BATCH: g_opt_dyn_batch = v; break;
+        case LLX_OPT_EXACT_RESIDENCY: g_opt_smem_pad = v; break;
     }
-    return fail(LLX_ERR_INVALID_ARG, "option %d: bad value %lld", (int)opt, v);
+    return LLX_OK;
 }
 long long llx_get_option(llx_option opt) {
     switch (opt) {
@@ -1180,6 +1373,6 @@ const char* llx_status_str(llx_status s) {
     return "LLX_ERR_UNKNOWN";
 }
 const char* llx_last_error(void) { return g_err; }
-const char* llx_version(void) { return "llx 0.1 (sm_100a)"; }
+const char* llx_version(void) { return "llx 0.2 (sm_100a)"; }
 
 }  // extern "C"

@@ -77,7 +77,7 @@ __global__ void __maxnreg__(112) llx_attn_partial(const AttnArgs a) {
     griddep_wait();
     const int b = blockIdx.z;
     const int split = blockIdx.x;
-    const int ctx = a.ctx_lens[b];
+    const int ctx = min(a.ctx_lens[b], a.max_blocks * a.S);  // llx.h: a longer ctx_len is clamped, never followed past the table row
     const int t0 = split * a.split_tokens;
     if (t0 >= ctx) return;
     const int t1 = min(ctx, t0 + a.split_tokens);
@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(D) llx_attn_merge(const AttnArgs a) {
     griddep_launch();
     griddep_wait();
     const int h = blockIdx.x, b = blockIdx.y, d = threadIdx.x;
-    const int ctx = a.ctx_lens[b];
+    const int ctx = min(a.ctx_lens[b], a.max_blocks * a.S);  // llx.h: a longer ctx_len is clamped, never followed past the table row
     const int ns = (ctx + a.split_tokens - 1) / a.split_tokens;
     const float* p = a.part + ((long long)b * a.H + h) * a.max_splits * (D + 4);
     float M = -INFINITY;

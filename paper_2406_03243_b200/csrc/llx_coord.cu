@@ -31,6 +31,8 @@ struct llx_migration {
     llx_abort_reason reason = LLX_ABORT_NONE;
     int blocks_migrated = 0, stages = 0;
     std::vector<int32_t> dst_table;  // blocks reserved on the destination so far, in logical order
+    bool has_opts = false;           // launch policy of the non-final stages (llx_migration_set_stage_opts)
+    llx_launch_opts stage_opts;
 };
 
 extern "C" {
@@ -41,10 +43,15 @@ llx_status llx_blockmgr_create(int num_blocks, llx_blockmgr** out) {
     if (num_blocks <= 0) return fail(LLX_ERR_INVALID_ARG, "num_blocks = %d", num_blocks);
     llx_blockmgr* m = new (std::nothrow) llx_blockmgr();
     if (!m) return fail(LLX_ERR_OOM, "host allocation failed");
-    m->num_blocks = num_blocks;
-    m->free_stack.resize((size_t)num_blocks);
-    for (int i = 0; i < num_blocks; ++i) m->free_stack[(size_t)i] = num_blocks - 1 - i;  // pops give 0, 1, 2, ...
-    m->is_free.assign((size_t)num_blocks, 1);
+    try {
+        m->num_blocks = num_blocks;
+        m->free_stack.resize((size_t)num_blocks);
+        for (int i = 0; i < num_blocks; ++i) m->free_stack[(size_t)i] = num_blocks - 1 - i;  // pops give 0, 1, 2, ...
+        m->is_free.assign((size_t)num_blocks, 1);
+    } catch (...) {
+        delete m;
+        return fail(LLX_ERR_OOM, "host allocation failed");
+    }
     *out = m;
     return LLX_OK;
 }
@@ -83,6 +90,11 @@ llx_status llx_blockmgr_release(llx_blockmgr* m, const int32_t* ids, int n) {
         if (ids[i] < 0 || ids[i] >= m->num_blocks)
             return fail(LLX_ERR_BLOCK_OUT_OF_RANGE, "ids[%d] = %d not in [0,%d)", i, ids[i], m->num_blocks);
         if (m->is_free[(size_t)ids[i]]) return fail(LLX_ERR_INVALID_ARG, "block %d is already free", ids[i]);
+    }
+    try {
+        m->free_stack.reserve(m->free_stack.size() + (size_t)n);  // the pushes below cannot throw after this
+    } catch (...) {
+        return fail(LLX_ERR_OOM, "host allocation failed");
     }
     for (int i = 0; i < n; ++i) {  // a duplicate inside the list shows up as "already free" on its second visit
         if (m->is_free[(size_t)ids[i]]) {
@@ -152,6 +164,7 @@ llx_status llx_migration_begin(const llx_pool* src, llx_blockmgr* src_mgr, llx_p
 
 llx_status llx_migration_stage(llx_migration* g, const int32_t* table, int table_len, int num_tokens, llx_req_status status,
                                void* stream, int* n_out, int* is_final_out, int32_t* dst_ids_out) {
+    LLX_TRY
     if (!g || !n_out || !is_final_out) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
     *n_out = 0;
     *is_final_out = 0;
@@ -169,8 +182,24 @@ llx_status llx_migration_stage(llx_migration* g, const int32_t* table, int table
     const int m = g->blocks_migrated;
     if (n > 0 && (!table || table_len < m + n))
         return fail(LLX_ERR_INVALID_ARG, "source block table of %d entries, stage needs [%d,%d)", table_len, m, m + n);
+    // The commit hands src_block_table[0 .. blocks migrated) back to the source's manager, which has no reference
+    // counts: a table that names a block twice (llx_migrate_stage itself allows that for prefix-shared blocks) could
+    // be copied but never committed.  Refused here, before anything is reserved or copied.
+    if (n > 0) {
+        std::vector<unsigned char> seen((size_t)g->src_mgr->num_blocks, 0);
+        for (int i = 0; i < m + n; ++i) {
+            const int32_t b = table[i];
+            if (b < 0 || b >= g->src_mgr->num_blocks)
+                return fail(LLX_ERR_BLOCK_OUT_OF_RANGE, "src_block_table[%d] = %d not in [0,%d)", i, b, g->src_mgr->num_blocks);
+            if (seen[(size_t)b])
+                return fail(LLX_ERR_INVALID_ARG, "src_block_table names block %d twice (second at %d): a session cannot migrate prefix-shared "
+                            "blocks, the block manager keeps no reference counts", b, i);
+            seen[(size_t)b] = 1;
+        }
+    }
     // (3) PRE-ALLOC on the destination: all or nothing
     std::vector<int32_t> ids((size_t)n);
+    g->dst_table.reserve(g->dst_table.size() + (size_t)n);  // nothing below can throw once the blocks are reserved
     rc = llx_blockmgr_alloc(g->dst_mgr, n, ids.data());
     if (rc == LLX_ERR_NO_SPACE) {
         do_abort(g, LLX_ABORT_NO_SPACE);
@@ -179,7 +208,11 @@ llx_status llx_migration_stage(llx_migration* g, const int32_t* table, int table
     if (rc != LLX_OK) return rc;
     // (4) the stage's copy
     if (g->src && n > 0) {
-        rc = llx_migrate_stage(g->src, table + m, g->dst, ids.data(), n, stream);
+        // the final stage is the downtime: never throttled; earlier stages follow the session's policy
+        llx_launch_opts o;
+        if (g->has_opts) o = g->stage_opts; else llx_launch_opts_init(&o);
+        if (fin) o.bandwidth_gbps = 0, o.max_ctas = 0;
+        rc = llx_migrate_stage_ex(g->src, table + m, g->dst, ids.data(), n, stream, (g->has_opts || fin) ? &o : nullptr);
         if (rc != LLX_OK) {  // nothing was launched: give the reservation back, the session stays where it was
             llx_blockmgr_release(g->dst_mgr, ids.data(), n);
             return rc;
@@ -193,6 +226,20 @@ llx_status llx_migration_stage(llx_migration* g, const int32_t* table, int table
         for (int i = 0; i < n; ++i) dst_ids_out[i] = ids[(size_t)i];
     *n_out = n;
     *is_final_out = fin;
+    return LLX_OK;
+    LLX_CATCH
+}
+
+llx_status llx_migration_set_stage_opts(llx_migration* g, const llx_launch_opts* opts) {
+    if (!g) return fail(LLX_ERR_INVALID_ARG, "migration is NULL");
+    if (!opts) {
+        g->has_opts = false;
+        return LLX_OK;
+    }
+    if (opts->struct_size != sizeof(llx_launch_opts))
+        return fail(LLX_ERR_INVALID_ARG, "llx_launch_opts.struct_size = %u (this library: %zu); use llx_launch_opts_init", opts->struct_size, sizeof(llx_launch_opts));
+    g->stage_opts = *opts;
+    g->has_opts = true;
     return LLX_OK;
 }
 
@@ -250,6 +297,7 @@ extern "C" {
 
 llx_status llx_calc_freeness(const llx_req_info* reqs, int n, double M, const double* headroom_for_priority,
                              int num_priorities, int is_terminating, double* freeness, double* total_virtual_usage) {
+    LLX_TRY
     if (n < 0 || num_priorities < 1 || !headroom_for_priority || !freeness || (n > 0 && !reqs))
         return fail(LLX_ERR_INVALID_ARG, "bad arguments (n=%d, num_priorities=%d)", n, num_priorities);
     // instance.numRequests[p]: the running requests of each priority (they share that priority's headroom)
@@ -281,6 +329,7 @@ llx_status llx_calc_freeness(const llx_req_info* reqs, int n, double M, const do
     *freeness = (M - total) / B;  // line 17
     if (total_virtual_usage) *total_virtual_usage = total;
     return LLX_OK;
+    LLX_CATCH
 }
 
 llx_status llx_pair_instances(const double* freeness, int n, double src_below, double dst_above, int32_t* src_out,
@@ -288,6 +337,7 @@ llx_status llx_pair_instances(const double* freeness, int n, double src_below, d
     if (n < 0 || !n_pairs || (n > 0 && !freeness) || cap < 0 || (cap > 0 && (!src_out || !dst_out)))
         return fail(LLX_ERR_INVALID_ARG, "bad arguments");
     if (src_below > dst_above) return fail(LLX_ERR_INVALID_ARG, "thresholds overlap: src_below %g > dst_above %g", src_below, dst_above);
+    LLX_TRY
     std::vector<int32_t> src, dst;
     for (int i = 0; i < n; ++i) {
         if (freeness[i] < src_below) src.push_back(i);
@@ -303,6 +353,7 @@ llx_status llx_pair_instances(const double* freeness, int n, double src_below, d
         dst_out[k] = dst[(size_t)k];
     }
     return LLX_OK;
+    LLX_CATCH
 }
 
 llx_status llx_migration_order(const int32_t* priority, const int32_t* seq_len, int n, int32_t* order_out) {
@@ -312,6 +363,88 @@ llx_status llx_migration_order(const int32_t* priority, const int32_t* seq_len, 
         return priority[a] != priority[b] ? priority[a] < priority[b] : seq_len[a] < seq_len[b];
     });
     return LLX_OK;
+}
+
+// One migration round of one (source, destination) pair as one batch (reading A31): the source offers its
+// running requests in migration order while it is still below the source threshold; each request's blocks are
+// PRE-ALLOCated on the destination, all or nothing; the first request that does not fit ends the round.
+// The output is the argument list of llx_migrate_batch.
+llx_status llx_plan_migration_batch(const llx_req_info* reqs, const int32_t* seq_len, int n, double M,
+                                    const double* headroom_for_priority, int num_priorities, int is_terminating,
+                                    double src_below, const int32_t* table_offsets, const int32_t* src_block_tables,
+                                    llx_blockmgr* dst_mgr, int dst_reserve_blocks, int32_t* chosen_out, int* n_chosen,
+                                    int32_t* req_offsets_out, int32_t* src_ids_out, int32_t* dst_ids_out, int cap_pairs,
+                                    int* n_pairs) {
+    LLX_TRY
+    if (!n_chosen || !n_pairs) return fail(LLX_ERR_INVALID_ARG, "NULL output");
+    *n_chosen = 0;
+    *n_pairs = 0;
+    if (n < 0 || cap_pairs < 0 || dst_reserve_blocks < 0 || !dst_mgr || !req_offsets_out || !headroom_for_priority || num_priorities < 1)
+        return fail(LLX_ERR_INVALID_ARG, "bad arguments (n=%d, cap_pairs=%d, dst_reserve_blocks=%d)", n, cap_pairs, dst_reserve_blocks);
+    req_offsets_out[0] = 0;
+    if (n == 0) return LLX_OK;
+    if (!reqs || !seq_len || !table_offsets || !chosen_out) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
+    if (table_offsets[0] != 0) return fail(LLX_ERR_INVALID_ARG, "table_offsets[0] = %d, must be 0", table_offsets[0]);
+    for (int r = 0; r < n; ++r)
+        if (table_offsets[r + 1] < table_offsets[r]) return fail(LLX_ERR_INVALID_ARG, "table_offsets decreases at request %d", r);
+    if (table_offsets[n] > 0 && !src_block_tables) return fail(LLX_ERR_INVALID_ARG, "src_block_tables is NULL");
+
+    // 1. candidates: the running requests, lower priority first, then shorter, then lower index (llx_migration_order)
+    std::vector<int32_t> prio((size_t)n), order((size_t)n);
+    for (int i = 0; i < n; ++i) prio[(size_t)i] = reqs[i].priority;
+    llx_status rc = llx_migration_order(prio.data(), seq_len, n, order.data());
+    if (rc != LLX_OK) return rc;
+    // 2. take requests while the source is still below its threshold and the destination can hold the next one.
+    //    First decided on a copy of the request set (nothing is reserved if an output turns out too small) ...
+    std::vector<llx_req_info> left(reqs, reqs + n);
+    std::vector<int32_t> left_id((size_t)n);
+    for (int i = 0; i < n; ++i) left_id[(size_t)i] = i;
+    long long dst_free = (long long)llx_blockmgr_num_free(dst_mgr) - dst_reserve_blocks;
+    std::vector<int32_t> chosen;
+    long long pairs = 0;
+    for (int k = 0; k < n; ++k) {
+        const int32_t r = order[(size_t)k];
+        if (reqs[r].is_queuing || reqs[r].is_fake) continue;  // nothing to migrate: no KV cache on this instance yet
+        double F = 0.0;
+        rc = llx_calc_freeness(left.data(), (int)left.size(), M, headroom_for_priority, num_priorities, is_terminating, &F, nullptr);
+        if (rc != LLX_OK) return rc;
+        if (!(F < src_below)) break;  // no longer in the source state
+        const long long nb = (long long)table_offsets[r + 1] - table_offsets[r];
+        if (nb > dst_free) break;  // PRE-ALLOC fails: the destination aborts this migration and the round ends
+        dst_free -= nb;
+        pairs += nb;
+        chosen.push_back(r);
+        for (size_t j = 0; j < left_id.size(); ++j)
+            if (left_id[j] == r) {
+                left.erase(left.begin() + (long)j);
+                left_id.erase(left_id.begin() + (long)j);
+                break;
+            }
+    }
+    if (pairs > cap_pairs) {
+        *n_pairs = (int)pairs;
+        return fail(LLX_ERR_INVALID_ARG, "%lld id pairs, outputs hold %d", pairs, cap_pairs);
+    }
+    if (pairs > 0 && (!src_ids_out || !dst_ids_out)) return fail(LLX_ERR_INVALID_ARG, "id output is NULL");
+    // ... then the PRE-ALLOC itself, request by request in the order taken (all or nothing each)
+    long long at = 0;
+    for (size_t c = 0; c < chosen.size(); ++c) {
+        const int32_t r = chosen[c];
+        const int nb = table_offsets[r + 1] - table_offsets[r];
+        rc = llx_blockmgr_alloc(dst_mgr, nb, dst_ids_out + at);
+        if (rc != LLX_OK) {  // cannot happen after the count above; give everything back and report
+            if (at > 0) llx_blockmgr_release(dst_mgr, dst_ids_out, (int)at);
+            return rc;
+        }
+        for (int i = 0; i < nb; ++i) src_ids_out[at + i] = src_block_tables[table_offsets[r] + i];
+        at += nb;
+        chosen_out[c] = r;
+        req_offsets_out[c + 1] = (int32_t)at;
+    }
+    *n_chosen = (int)chosen.size();
+    *n_pairs = (int)at;
+    return LLX_OK;
+    LLX_CATCH
 }
 
 }  // extern "C"

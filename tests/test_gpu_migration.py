@@ -50,13 +50,12 @@ def test_tiny_two_stage_migration_bit_exact(env, opts):
     s_tab = synth.block_permutation(1, TINY["num_blocks"])[:7]
     d_tab = synth.block_permutation(2, TINY["num_blocks"])[:7]
     m = 0
-    with llx.options(**opts):
-        for n in (5, 2):
-            llx.migrate_stage(src.pool, s_tab[m:m + n], dst.pool, d_tab[m:m + n])
-            om.migrate_stage(h_src, s_tab[m:m + n], h_dst, d_tab[m:m + n])
-            m += n
-            H.assert_pool_equal(dst.host(), h_dst)      # P1 mapping + P2 sentinel on every other block
-            H.assert_pool_equal(src.host(), h_src)      # P3 source intact
+    for n in (5, 2):                                    # the option set is THIS call's launch policy (llx_migrate_stage_ex)
+        llx.migrate_stage(src.pool, s_tab[m:m + n], dst.pool, d_tab[m:m + n], opts=opts)
+        om.migrate_stage(h_src, s_tab[m:m + n], h_dst, d_tab[m:m + n])
+        m += n
+        H.assert_pool_equal(dst.host(), h_dst)      # P1 mapping + P2 sentinel on every other block
+        H.assert_pool_equal(src.host(), h_src)      # P3 source intact
     untouched = np.setdiff1d(np.arange(TINY["num_blocks"]), d_tab)
     assert np.all(dst.host()[:, :, untouched] == SENT)
 
@@ -69,11 +68,36 @@ def test_ragged_tiles_and_small_tiles(env, g, opts, n):
     src, dst, h_src, h_dst = make(H, g, seed=5)
     s_ids = synth.block_permutation(11, g["num_blocks"])[:n]
     d_ids = synth.block_permutation(12, g["num_blocks"])[:n]
-    with llx.options(**opts):
-        llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids)
+    llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, opts=opts)
     om.migrate_stage(h_src, s_ids, h_dst, d_ids)
     H.assert_pool_equal(dst.host(), h_dst)
     H.assert_pool_equal(src.host(), h_src)
+
+
+@pytest.mark.parametrize("opts", [dict(copy_kernel=1, chunk_bytes=2048), dict(bandwidth_gbps=40), dict(copy_kernel=2, max_ctas=3)])
+def test_process_default_options_are_inherited_by_plain_calls(env, opts):
+    """llx_set_option sets process DEFAULTS: a plain llx_migrate_stage (no llx_launch_opts) inherits them, and a call's
+    own opts override them field by field."""
+    H, llx = env
+    src, dst, h_src, h_dst = make(H, RAGGED, seed=5)
+    s_ids = synth.block_permutation(11, RAGGED["num_blocks"])[:13]
+    d_ids = synth.block_permutation(12, RAGGED["num_blocks"])[:13]
+    with llx.options(**opts):
+        llx.migrate_stage(src.pool, s_ids[:6], dst.pool, d_ids[:6])
+        llx.migrate_stage(src.pool, s_ids[6:], dst.pool, d_ids[6:], opts=dict(copy_kernel=2, bandwidth_gbps=0, max_ctas=0))
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
+    with pytest.raises(llx.LlxError) as e:
+        llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, opts=dict(chunk_bytes=100))      # not a multiple of 16
+    assert e.value.name == "LLX_ERR_INVALID_ARG"
+    bad = llx.LaunchOpts()
+    bad.struct_size = 6
+    with pytest.raises(llx.LlxError):
+        llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, opts=bad)
+    short = llx.LaunchOpts(copy_kernel=1, route=7)      # an older, shorter struct: fields beyond struct_size are not read
+    short.struct_size = 16
+    llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, opts=short)
+    H.assert_pool_equal(dst.host(), h_dst)
 
 
 def test_whole_pool_and_ids_through_the_ring(env):
@@ -153,13 +177,12 @@ def test_pack_unpack_block_fusion(env, where, opts):                 # P5, S6
         pin = llx.PinnedStaging(nbytes)
         pin.as_numpy()[:] = 0x1111
         ptr = pin.dev_alias
-    with llx.options(**opts):
-        llx.pack(src.pool, s_ids, ptr, nbytes)
-        torch.cuda.synchronize()
-        got = stg.cpu().numpy().view(np.uint16) if where == "device" else pin.as_numpy().copy()
-        want = om.pack(h_src, s_ids)
-        assert np.array_equal(got.reshape(want.shape), want)         # staging layout [i][l][kv][tile] (A6)
-        llx.unpack(ptr, nbytes, dst.pool, d_ids)
+    llx.pack(src.pool, s_ids, ptr, nbytes, opts=opts)
+    torch.cuda.synchronize()
+    got = stg.cpu().numpy().view(np.uint16) if where == "device" else pin.as_numpy().copy()
+    want = om.pack(h_src, s_ids)
+    assert np.array_equal(got.reshape(want.shape), want)         # staging layout [i][l][kv][tile] (A6)
+    llx.unpack(ptr, nbytes, dst.pool, d_ids, opts=opts)
     om.unpack(want, h_dst, d_ids)
     H.assert_pool_equal(dst.host(), h_dst)
     direct = H.DevPool(g, fill=SENT)
@@ -190,11 +213,11 @@ def test_migrate_via_host_pipelined_route(env, where, n, chunk):    # S6: PAPER.
         ptr = pin.dev_alias
     st = torch.cuda.Stream()
     st.wait_stream(torch.cuda.current_stream())
-    with llx.options(via_host_mode=mode):
-        llx.migrate_via_host(src.pool, s_ids, dst.pool, d_ids, ptr, nbytes, chunk_blocks=chunk, stream=st)
-        if n == 37:      # a second migration right behind the first reuses the bounce buffers and events
-            llx.migrate_via_host(src.pool, s_ids[::-1], dst.pool, d_ids[::-1], ptr, nbytes, chunk_blocks=chunk + 1, stream=st)
-            llx.migrate_via_host(src.pool, s_ids, dst.pool, d_ids, ptr, nbytes, chunk_blocks=chunk, stream=st)
+    o = dict(via_host_mode=mode)
+    llx.migrate_via_host(src.pool, s_ids, dst.pool, d_ids, ptr, nbytes, chunk_blocks=chunk, stream=st, opts=o)
+    if n == 37:      # a second migration right behind the first reuses the bounce buffers and events
+        llx.migrate_via_host(src.pool, s_ids[::-1], dst.pool, d_ids[::-1], ptr, nbytes, chunk_blocks=chunk + 1, stream=st, opts=o)
+        llx.migrate_via_host(src.pool, s_ids, dst.pool, d_ids, ptr, nbytes, chunk_blocks=chunk, stream=st, opts=o)
     # work enqueued on the caller's stream afterwards must see the complete migration (the call joins its side stream)
     with torch.cuda.stream(st):
         after = dst.view.clone()
@@ -412,9 +435,8 @@ def test_migrate_stage_wait_returns_after_completion(env, opts):     # S4: the f
     for rep in range(4):                                             # flag slots and sequence numbers are reused
         s_ids = synth.block_permutation(60 + rep, g["num_blocks"])[:9]
         d_ids = synth.block_permutation(70 + rep, g["num_blocks"])[:9]
-        with llx.options(**opts):
-            llx.migrate_stage(src.pool, s_ids[:6], dst.pool, d_ids[:6], stream=st)        # earlier stage, not synchronised
-            llx.migrate_stage_wait(src.pool, s_ids[6:], dst.pool, d_ids[6:], stream=st)
+        llx.migrate_stage(src.pool, s_ids[:6], dst.pool, d_ids[:6], stream=st, opts=opts)        # earlier stage, not synchronised
+        llx.migrate_stage_wait(src.pool, s_ids[6:], dst.pool, d_ids[6:], stream=st, opts=opts)
         with torch.cuda.stream(other):                               # no synchronize of `st`: the call itself waited
             snap = dst.view.clone()
         other.synchronize()
@@ -447,11 +469,10 @@ def test_guard_bands_around_pools_and_staging_stay_intact(env, opts):
     bufs[0][guard:guard + nbytes] = torch.randint(0, 255, (nbytes,), dtype=torch.uint8, device="cuda")
     ids_s = np.array([0, nb - 1, 1, nb - 2, 5, 17, 3])               # first and last blocks of every slice
     ids_d = np.array([nb - 1, 0, nb - 2, 1, 9, 2, 30])
-    with llx.options(**opts):
-        llx.migrate_stage(src, ids_s, dst, ids_d)
-        llx.pack(src, ids_s, bufs[2].data_ptr() + guard, stg_bytes)
-        llx.unpack(bufs[2].data_ptr() + guard, stg_bytes, dst, ids_d)
-        llx.migrate_via_host(src, ids_s, dst, ids_d, bufs[2].data_ptr() + guard, stg_bytes, chunk_blocks=3)
+    llx.migrate_stage(src, ids_s, dst, ids_d, opts=opts)
+    llx.pack(src, ids_s, bufs[2].data_ptr() + guard, stg_bytes, opts=opts)
+    llx.unpack(bufs[2].data_ptr() + guard, stg_bytes, dst, ids_d, opts=opts)
+    llx.migrate_via_host(src, ids_s, dst, ids_d, bufs[2].data_ptr() + guard, stg_bytes, chunk_blocks=3, opts=opts)
     torch.cuda.synchronize()
     for raw, size in zip(bufs, (nbytes, nbytes, stg_bytes)):
         assert bool((raw[:guard] == 0x5A).all()) and bool((raw[guard + size:] == 0x5A).all()), "guard band overwritten"
@@ -513,7 +534,7 @@ def test_destination_pool_on_a_peer_gpu(env):                       # NEXT-2; ne
 
 
 def test_two_host_threads_on_two_streams(env):
-    """llx.h: "calls on distinct streams from distinct threads are safe".  Two threads migrate different requests
+    """llx.h, "Threads": data calls may be issued from several host threads at once on distinct streams.  Two threads migrate different requests
     between the same pools at the same time: long id lists (pinned id ring), pinned-host pack (shared bounce
     buffers) and the blocking final-stage call (flag slots)."""
     import threading

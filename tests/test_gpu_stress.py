@@ -1,5 +1,5 @@
 """A short soak: three host threads on their own streams issue a random mix of migration calls (all entry points,
-random option sets — the options are process-wide, so the threads also disturb each other's launch shapes) for a few
+a random launch policy PER CALL — llx_launch_opts — so the threads run different launch shapes side by side) for a few
 seconds; after every call the touched destination blocks must equal their source blocks (torch gather on the device,
 independent of the library).  90 s of the same loop (88,000 calls) ran clean on a B200 while this was written."""
 import threading
@@ -49,23 +49,22 @@ def test_random_mix_of_calls_from_three_threads():
                 s_ids = rng.permutation(NB)[:n].astype(np.int32)
                 d_ids = rng.permutation(NB)[:n].astype(np.int32)
                 kind = int(rng.integers(0, 6))
-                opts = [dict(), dict(), dict(copy_kernel=1), dict(dynamic_tail_pct=30), dict(max_ctas=int(rng.integers(1, 400))),
-                        dict(exact_residency=0)][int(rng.integers(0, 6))]
+                opts = [None, dict(), dict(copy_kernel=1), dict(dynamic_tail_pct=30), dict(max_ctas=int(rng.integers(1, 400))),
+                        dict(exact_residency=0), dict(bandwidth_gbps=int(rng.integers(2000, 6000))),
+                        dict(route=llx.ROUTE_PEER)][int(rng.integers(0, 8))]
                 if kind <= 2:
-                    with llx.options(**opts):
-                        llx.migrate_stage(src, s_ids, dst, d_ids, stream=st)
+                    llx.migrate_stage(src, s_ids, dst, d_ids, stream=st, opts=opts)
                 elif kind == 3:
-                    with llx.options(**opts):
-                        llx.migrate_stage_wait(src, s_ids, dst, d_ids, stream=st)
+                    llx.migrate_stage_wait(src, s_ids, dst, d_ids, stream=st, opts=opts)
                 else:
                     n = min(n, 300)
                     s_ids, d_ids = s_ids[:n], d_ids[:n]
                     if kind == 4:
                         llx.migrate_via_host(src, s_ids, dst, d_ids, pin.dev_alias, pin.nbytes,
-                                             chunk_blocks=int(rng.integers(0, 60)), stream=st)
+                                             chunk_blocks=int(rng.integers(0, 60)), stream=st, opts=opts)
                     else:
-                        llx.pack(src, s_ids, pin.dev_alias, pin.nbytes, stream=st)
-                        llx.unpack(pin.dev_alias, pin.nbytes, dst, d_ids, stream=st)
+                        llx.pack(src, s_ids, pin.dev_alias, pin.nbytes, stream=st, opts=opts)
+                        llx.unpack(pin.dev_alias, pin.nbytes, dst, d_ids, stream=st, opts=opts)
                 st.synchronize()
                 si = torch.from_numpy(s_ids.astype(np.int64)).cuda()
                 di = torch.from_numpy(d_ids.astype(np.int64)).cuda()
@@ -86,5 +85,6 @@ def test_random_mix_of_calls_from_three_threads():
         t.join()
     assert not errors, errors
     assert len(counts) == 3 and min(counts) > 20
-    for k in ("copy_kernel", "max_ctas", "dynamic_tail_pct", "exact_residency"):   # racing context managers may leave options set
-        llx.set_option(getattr(llx, "OPT_" + k.upper()), {"dynamic_tail_pct": 6, "exact_residency": 1}.get(k, 0))
+    # per-call policies leave the process defaults alone
+    assert [llx.get_option(o) for o in (llx.OPT_COPY_KERNEL, llx.OPT_MAX_CTAS, llx.OPT_DYNAMIC_TAIL_PCT, llx.OPT_EXACT_RESIDENCY,
+                                        llx.OPT_BANDWIDTH_GBPS)] == [0, 0, 6, 1, 0]

@@ -137,3 +137,154 @@ def test_c_pairing_and_order_equal_oracle(llx):
         assert llx.migration_order(pr, sl) == op.migration_order(pr, sl)
     with pytest.raises(llx.LlxError):
         llx.pair_instances([1.0, 2.0], 60.0, 10.0)                           # overlapping thresholds
+
+
+# ---- one migration round as one batch (reading A31, PAPER.md:225 + :142) ---------------------------------
+def random_source(rng, P=2, max_reqs=14, nb_pool=400):
+    """A seeded source instance: requests, sequence lengths, disjoint block tables (usage unit: blocks)."""
+    reqs, seq, tables = [], [], []
+    free = list(rng.permutation(nb_pool))
+    hol_given = False
+    for _ in range(int(rng.integers(0, max_reqs))):
+        if rng.random() < 0.2:
+            hol = (not hol_given) and bool(rng.random() < 0.6)
+            hol_given |= hol
+            reqs.append(op.Req(is_queuing=True, is_head_of_line=hol, priority=int(rng.integers(0, P)),
+                               demand=float(rng.integers(1, 60))))
+            seq.append(int(rng.integers(1, 900)))
+            tables.append([])
+        else:
+            nb = int(rng.integers(1, 30))
+            t = [int(free.pop()) for _ in range(nb)]
+            reqs.append(op.Req(priority=int(rng.integers(0, P)), physical_usage=float(nb)))
+            seq.append(int(rng.integers((nb - 1) * 16 + 1, nb * 16 + 1)))
+            tables.append(t)
+    return reqs, seq, tables
+
+
+def test_batch_plan_closed_form_for_equal_requests():
+    """B running requests of u blocks each, nothing queuing, no headroom: after k requests have left,
+    F_k = M/(B-k) - u, so the round takes k* = the smallest k with F_k >= T, i.e. max(0, ceil(B - M/(T+u)))
+    (and everything when even one remaining request keeps F below T: then B = 1 by A28 once all are gone)."""
+    from oracle import handshake as oh
+    for B, u, M, T in [(8, 10, 100, 5.0), (8, 10, 100, 15.0), (5, 4, 40, 2.0), (6, 7, 20, 1.0), (3, 9, 100, 0.5), (4, 10, 30, 40.0)]:
+        inst = op.Instance(M=float(M), requests=[running(u) for _ in range(B)], headroom_for_priority=[0.0])
+        tables = [list(range(r * u, (r + 1) * u)) for r in range(B)]
+        dst = oh.BlockManager(1000)
+        chosen, off, s_ids, d_ids = op.plan_migration_batch(inst, [u * 16] * B, tables, T, dst)
+        k_star = max(0, math.ceil(B - M / (T + u)))
+        if k_star >= B:                       # all running requests gone: B := 1 (A28), F = M >= T unless T > M
+            k_star = B
+        assert len(chosen) == k_star, (B, u, M, T, chosen)
+        assert chosen == list(range(k_star))                          # equal priority and length: index order
+        assert off == [u * i for i in range(k_star + 1)]
+        assert s_ids == [b for r in chosen for b in tables[r]]
+        assert d_ids == list(range(u * k_star)) and dst.num_free() == 1000 - u * k_star    # A23: a fresh manager hands out 0,1,2,...
+
+
+def test_batch_plan_special_cases():
+    from oracle import handshake as oh
+    reqs = [running(10, 1), running(30, 0), running(5, 0), op.Req(is_queuing=True, is_head_of_line=True, demand=50.0), running(5, 0)]
+    seq, tables = [160, 480, 70, 800, 80], [list(range(0, 10)), list(range(10, 40)), list(range(40, 45)), [], list(range(45, 50))]
+    inst = op.Instance(M=80.0, requests=reqs, headroom_for_priority=[0.0, 20.0])
+    # sum V = 10+20 + 30 + 5 + 50 + 5 = 120 -> F = -40/4 = -10: a source for any threshold above -10
+    assert op.calc_freeness(inst)[0] == -10.0
+    dst = oh.BlockManager(100)
+    assert op.plan_migration_batch(inst, seq, tables, -10.0, dst) == ([], [0], [], [])        # F is not BELOW the threshold
+    # lower priority first, then shorter: 2 (70 tokens), 4 (80), 1 (480), and the high-priority request 0 last
+    chosen, off, s_ids, d_ids = op.plan_migration_batch(inst, seq, tables, 1e9, dst)
+    assert chosen == [2, 4, 1, 0] and off == [0, 5, 10, 40, 50] and d_ids == list(range(50))
+    assert s_ids == tables[2] + tables[4] + tables[1] + tables[0] and dst.num_free() == 50
+    # threshold 0: after 2 leaves F = (80-115)/3, after 4: (80-110)/2 = -15, after 1: (80-80)/1 = 0 -> stop before request 0
+    dst = oh.BlockManager(100)
+    assert op.plan_migration_batch(inst, seq, tables, 0.0, dst)[0] == [2, 4, 1]
+    # the destination runs out: all-or-nothing per request, the first misfit ends the round (nothing of it is reserved)
+    dst = oh.BlockManager(100)
+    dst.allocate(70)                                                    # 30 free: 5 + 5 fit, the 30-block request does not
+    chosen, off, s_ids, d_ids = op.plan_migration_batch(inst, seq, tables, 1e9, dst)
+    assert chosen == [2, 4] and dst.num_free() == 20 and d_ids == list(range(70, 80))
+    dst = oh.BlockManager(100)
+    assert op.plan_migration_batch(inst, seq, tables, 1e9, dst, dst_reserve_blocks=91)[0] == [2]      # 9 usable: only 5 fit
+    # a terminating instance is drained whatever the threshold (fake request: F = -inf)
+    inst.is_terminating = True
+    dst = oh.BlockManager(100)
+    assert op.plan_migration_batch(inst, seq, tables, -1e300, dst)[0] == [2, 4, 1, 0]
+
+
+def brute_batch_plan(reqs, seq, tables, M, headroom, term, T, dst_free):
+    """Independent restatement of A31 from the paper's sentences, without oracle.policy: plain tuples and loops."""
+    here = [i for i in range(len(reqs))]
+    cand = [i for i in range(len(reqs)) if not reqs[i].is_queuing]
+    # "prefers the requests with lower priorities and shorter sequence lengths": repeated selection of the minimum
+    ordered = []
+    while cand:
+        best = cand[0]
+        for i in cand[1:]:
+            if (reqs[i].priority, seq[i], i) < (reqs[best].priority, seq[best], best):
+                best = i
+        ordered.append(best)
+        cand.remove(best)
+    taken = []
+    for r in ordered:
+        run = [i for i in here if not reqs[i].is_queuing]
+        V = 0.0
+        for i in here:
+            q = reqs[i]
+            if q.is_queuing:
+                V += q.demand if q.is_head_of_line else 0.0
+            else:
+                V += q.physical_usage + headroom[q.priority] / sum(1 for j in run if reqs[j].priority == q.priority)
+        F = -math.inf if term else (M - V) / max(1, len(run))
+        if F >= T or len(tables[r]) > dst_free:
+            break
+        dst_free -= len(tables[r])
+        taken.append(r)
+        here.remove(r)
+    return taken
+
+
+def test_batch_plan_equals_bruteforce_restatement_and_c(llx):
+    from oracle import handshake as oh
+    rng = np.random.default_rng(11)
+    nonempty = 0
+    for case in range(400):
+        P = int(rng.integers(1, 3))
+        headroom = [0.0] + [float(rng.integers(0, 80))] * (P - 1)
+        reqs, seq, tables = random_source(rng, P)
+        used = sum(len(t) for t in tables)
+        M = float(rng.integers(max(1, used // 2), used + 120))
+        term = bool(rng.random() < 0.1)
+        T = float(rng.integers(-20, 40))
+        nb_dst, taken_before, reserve = 300, int(rng.integers(0, 300)), int(rng.integers(0, 20))
+        o_dst, c_dst = oh.BlockManager(nb_dst), llx.BlockManager(nb_dst)
+        o_dst.allocate(taken_before), c_dst.alloc(taken_before)
+        inst = op.Instance(M=M, requests=reqs, headroom_for_priority=headroom, is_terminating=term)
+        want = op.plan_migration_batch(inst, seq, tables, T, o_dst, reserve)
+        assert want[0] == brute_batch_plan(reqs, seq, tables, M, headroom, term, T, nb_dst - taken_before - reserve), case
+        got = llx.plan_migration_batch([as_tuple(r) for r in reqs], seq, M, headroom, T, tables, c_dst, reserve, term)
+        assert got[0] == want[0] and list(got[1]) == want[1] and list(got[2]) == want[2] and list(got[3]) == want[3], case
+        assert c_dst.num_free == o_dst.num_free() == nb_dst - taken_before - len(want[3])
+        assert len(set(want[3])) == len(want[3])
+        nonempty += bool(want[0])
+    assert nonempty > 100
+
+
+def test_c_batch_plan_argument_errors_reserve_nothing(llx):
+    l = llx.lib()
+    import ctypes as C
+    mgr = llx.BlockManager(50)
+    reqs = [(0, 0, 0, 0, 0.0, 10.0), (0, 0, 0, 0, 0.0, 10.0)]
+    assert llx.plan_migration_batch(reqs, [100, 100], 5.0, [0.0], 100.0, [[1, 2, 3], [4, 5]], mgr)[0] == [0, 1]
+    assert mgr.num_free == 45
+    # outputs too small: LLX_ERR_INVALID_ARG, *n_pairs tells the size needed, nothing reserved
+    arr = (llx.binding.ReqInfo * 2)(*[llx.binding.ReqInfo(*[int(x) for x in r[:4]], r[4], r[5]) for r in reqs])
+    i32 = lambda v: (C.c_int32 * len(v))(*v)
+    hr = (C.c_double * 1)(0.0)
+    chosen, ro, so, do = i32([0, 0]), i32([0, 0, 0]), i32([0] * 4), i32([0] * 4)
+    nc, npairs = C.c_int(), C.c_int()
+    rc = l.llx_plan_migration_batch(arr, i32([100, 100]), 2, 5.0, hr, 1, 0, 100.0, i32([0, 3, 5]), i32([1, 2, 3, 4, 5]),
+                                    mgr.handle, 0, chosen, C.byref(nc), ro, so, do, 4, C.byref(npairs))
+    assert rc == -1 and npairs.value == 5 and mgr.num_free == 45
+    rc = l.llx_plan_migration_batch(arr, i32([100, 100]), 2, 5.0, hr, 1, 0, 100.0, i32([0, 3, 2]), i32([1, 2, 3, 4, 5]),
+                                    mgr.handle, 0, chosen, C.byref(nc), ro, so, do, 4, C.byref(npairs))
+    assert rc == -1 and mgr.num_free == 45                                      # offsets decrease
