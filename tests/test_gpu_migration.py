@@ -516,23 +516,6 @@ def test_default_launch_shape_with_dynamic_tail_on_a_mid_size_stage(env):
     H.assert_pool_equal(dst.host(), h_dst)
 
 
-def test_destination_pool_on_a_peer_gpu(env):                       # NEXT-2; needs two GPUs (skipped on a 1-GPU box)
-    H, llx = env
-    if torch.cuda.device_count() < 2:
-        pytest.skip("needs two GPUs with peer access")
-    g = RAGGED
-    src, _, h_src, h_dst = make(H, g, seed=14)
-    with torch.cuda.device(1):
-        dst = H.DevPool(g, fill=SENT)
-    s_ids = synth.block_permutation(1, g["num_blocks"])[:13]
-    d_ids = synth.block_permutation(2, g["num_blocks"])[:13]
-    llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids)              # kernel on device 0 stores into device 1's pool
-    torch.cuda.synchronize(0)
-    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
-    with torch.cuda.device(1):
-        H.assert_pool_equal(dst.host(), h_dst)
-
-
 def test_two_host_threads_on_two_streams(env):
     """llx.h, "Threads": data calls may be issued from several host threads at once on distinct streams.  Two threads migrate different requests
     between the same pools at the same time: long id lists (pinned id ring), pinned-host pack (shared bounce
