@@ -1,0 +1,241 @@
+"""Launch policy is per call (llx_launch_opts) and stream capture is safe or refused.
+
+PAPER.md:289-291: a migration must not slow the co-running requests (<= 1 %), so non-final stages run under a bandwidth
+budget; the final stage IS the downtime, so it runs unthrottled; a source migrates requests
+continuously.  Both policies are therefore live at once, on two streams, from two host threads."""
+import statistics
+import threading
+import time
+
+import numpy as np
+import pytest
+import torch
+
+import synth
+from oracle import kv_migration as om
+
+pytestmark = pytest.mark.gpu
+
+SENT = synth.SENTINEL_U16
+SENT_I16 = int(np.array(SENT, np.uint16).view(np.int16))
+# LLaMA-7B tiles (128 KiB, 8 MiB blocks) in pools small enough to mirror one layer at a time
+G7 = dict(layers=32, kv_heads=32, head_dim=128, block_size=16, elem_bytes=2, num_blocks=300)
+
+
+@pytest.fixture(scope="module")
+def env():
+    import gpu_harness as H
+    import paper_2406_03243_b200 as llx
+    llx.load()
+    return H, llx
+
+
+def test_budgeted_stage_and_unthrottled_final_stage_from_two_threads(env):
+    """Thread A loops a 25 GB/s-budgeted 112-block stage (llx_migrate_stage_ex); thread B times 2-block final stages
+    (llx_migrate_stage_wait).  Both bit-exact; B's median within 2x of its solo value; A's achieved rate within 10 % of
+    its budget.  With process-global options (round 1) A's budget would have throttled B's final stage to milliseconds."""
+    H, llx = env
+    g = G7
+    sample = [0, 31]
+    src, dst_a, dst_b = H.DevPool(g), H.DevPool(g, fill=SENT), H.DevPool(g, fill=SENT)
+    src.fill_device_random(77)
+    src.fill_from_synth(0, 0, layers=sample)
+    perm_s = synth.block_permutation(1, g["num_blocks"])
+    perm_d = synth.block_permutation(2, g["num_blocks"])
+    a_s, a_d = perm_s[:112], perm_d[:112]
+    b_s, b_d = perm_s[112:114], perm_d[112:114]
+    torch.cuda.synchronize()
+    st_a, st_b = torch.cuda.Stream(), torch.cuda.Stream()
+    budget = 25
+    stage_bytes = 2 * 112 * src.pool.block_bytes                      # read + written
+
+    def final_stage_us(reps):
+        out = []
+        for _ in range(reps):
+            t0 = time.perf_counter_ns()
+            llx.migrate_stage_wait(src.pool, b_s, dst_b.pool, b_d, stream=st_b)
+            out.append((time.perf_counter_ns() - t0) / 1e3)
+        return out
+
+    final_stage_us(20)
+    solo = statistics.median(final_stage_us(200))
+
+    errors, a_ms, stop = [], [], threading.Event()
+
+    def thread_a():
+        try:
+            torch.cuda.set_device(0)
+            while not stop.is_set():
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(st_a)
+                llx.migrate_stage(src.pool, a_s, dst_a.pool, a_d, stream=st_a, opts=dict(bandwidth_gbps=budget))
+                e1.record(st_a)
+                st_a.synchronize()
+                a_ms.append(e0.elapsed_time(e1))
+        except Exception as e:  # noqa: BLE001
+            errors.append(repr(e))
+
+    ta = threading.Thread(target=thread_a)
+    ta.start()
+    time.sleep(0.05)                                                   # A's first stage is in flight
+    busy = []
+    while len(a_ms) < 3 and not errors and len(busy) < 200000:         # B keeps issuing final stages while A streams
+        busy += final_stage_us(100)
+    stop.set()
+    ta.join()
+    assert not errors, errors
+    with_a = statistics.median(busy)
+    assert len(a_ms) >= 2
+    achieved = stage_bytes / (statistics.median(a_ms) * 1e-3) / 1e9
+    print(f"final stage solo {solo:.1f} us, next to a {budget} GB/s stage {with_a:.1f} us; budgeted stage achieved {achieved:.1f} GB/s")
+    assert with_a <= 2.0 * solo, (solo, with_a)
+    assert abs(achieved - budget) <= 0.10 * budget, achieved
+    assert llx.get_option(llx.OPT_BANDWIDTH_GBPS) == 0                 # nobody touched the process defaults
+    # bit-exact, both destinations, on the sampled layers (oracle) and on every layer (device gather)
+    for l in sample:
+        h_src = H.host_pool_from_synth(g, 0, 0, layers=[l])
+        for dst, (s_ids, d_ids) in ((dst_a, (a_s, a_d)), (dst_b, (b_s, b_d))):
+            h_dst = om.new_pool(1, g["num_blocks"], H.tile_elems(g), fill=SENT)
+            om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+            H.assert_pool_equal(dst.host_layer(l), h_dst)
+    for dst, (s_ids, d_ids) in ((dst_a, (a_s, a_d)), (dst_b, (b_s, b_d))):
+        si, di = torch.from_numpy(s_ids.astype(np.int64)).cuda(), torch.from_numpy(d_ids.astype(np.int64)).cuda()
+        for l in range(g["layers"]):
+            assert torch.equal(dst.view[l].index_select(1, di), src.view[l].index_select(1, si))
+
+
+def test_session_budget_applies_to_non_final_stages_only(env):
+    """llx_migration_set_stage_opts: stage 0 of a session runs under the budget, the final stage at full speed."""
+    H, llx = env
+    g = G7
+    src, dst = H.DevPool(g), H.DevPool(g, fill=SENT)
+    src.fill_device_random(78)
+    src.fill_from_synth(0, 0, layers=[7])
+    nb = g["num_blocks"]
+    src_mgr, dst_mgr = llx.BlockManager(nb), llx.BlockManager(nb)
+    table = src_mgr.alloc(40)
+    tokens = 39 * 16 + 5
+    mig = llx.Migration(src.pool, src_mgr, dst.pool, dst_mgr, 16, 2)
+    mig.set_stage_opts(dict(bandwidth_gbps=50))
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ev[0].record(st)
+    n0, fin0, ids0 = mig.stage(table, tokens, stream=st)
+    ev[1].record(st)
+    st.synchronize()
+    ev[2].record(st)
+    n1, fin1, ids1 = mig.stage(table, tokens, stream=st)
+    ev[3].record(st)
+    st.synchronize()
+    assert (n0, fin0, n1, fin1) == (38, False, 2, True)               # 39 full blocks; remaining 2 <= last_stage_max_blocks
+    t0, t1 = ev[0].elapsed_time(ev[1]), ev[2].elapsed_time(ev[3])
+    rate0 = 2 * n0 * src.pool.block_bytes / (t0 * 1e-3) / 1e9
+    rate1 = 2 * n1 * src.pool.block_bytes / (t1 * 1e-3) / 1e9
+    print(f"session: stage 0 at {rate0:.1f} GB/s under a 50 GB/s budget, final stage at {rate1:.0f} GB/s")
+    assert abs(rate0 - 50) <= 5 and rate1 > 500
+    d_table = mig.commit(table)
+    assert list(d_table) == list(ids0) + list(ids1)
+    h_src = H.host_pool_from_synth(g, 0, 0, layers=[7])
+    h_dst = om.new_pool(1, nb, H.tile_elems(g), fill=SENT)
+    om.migrate_stage(h_src, table, h_dst, d_table)
+    H.assert_pool_equal(dst.host_layer(7), h_dst)
+    with pytest.raises(llx.LlxError) as e:
+        mig2 = llx.Migration(src.pool, src_mgr, dst.pool, dst_mgr, 16, 2)
+        mig2.stage([5, 5, 6], 40)                                      # a table that names a block twice cannot be committed
+    assert e.value.name == "LLX_ERR_INVALID_ARG" and dst_mgr.num_free == nb - 40
+
+
+# ---- CUDA graphs: captured where that is safe, refused (LLX_ERR_STATE) where it is not ------------------------------
+G_LONG = dict(layers=8, kv_heads=8, head_dim=128, block_size=16, elem_bytes=2, num_blocks=800)      # 32 KiB tiles, 512 KiB blocks
+
+
+def test_captured_long_stage_replays_on_other_streams_next_to_direct_launches(env):
+    """A >= 64 MiB stage (the dynamic tail is active when it is launched directly) is captured on stream C and replayed
+    on two other streams while the same kind of stage is launched directly on C.  In round 1 the captured launch kept C's
+    claim counter: a replay running next to a direct launch shared it and chunks could be skipped silently.  Captured
+    launches now run without the dynamic tail."""
+    H, llx = env
+    g = G_LONG
+    nb = g["num_blocks"]
+    src = H.DevPool(g)
+    src.fill_device_random(5)
+    dsts = [H.DevPool(g, fill=SENT) for _ in range(3)]                  # graph replay 1, graph replay 2, direct launches
+    perm_s, perm_d = synth.block_permutation(61, nb), synth.block_permutation(62, nb)
+    n = 256                                                             # ids still by value; 128 MiB payload = 4096 chunks of 32 KiB
+    assert n * src.pool.block_bytes >= 64 << 20 and n * 2 * g["layers"] >= 148 * 16          # long stage with a tail worth claiming
+    cap_st, r1, r2 = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    for st in (cap_st, r1, r2):
+        st.wait_stream(torch.cuda.current_stream())
+    llx.migrate_stage(src.pool, perm_s[:n], dsts[2].pool, perm_d[:n], stream=cap_st)        # warm-up: first-use allocations
+    cap_st.synchronize()
+    dsts[2].view.fill_(SENT_I16)
+    torch.cuda.synchronize()
+    graphs = []
+    for k in range(2):                                                  # one graph per destination pool
+        gr = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gr, stream=cap_st):
+            llx.migrate_stage(src.pool, perm_s[:n], dsts[k].pool, perm_d[:n], stream=cap_st)
+            llx.migrate_stage(src.pool, perm_s[n:2 * n], dsts[k].pool, perm_d[n:2 * n], stream=cap_st)
+        graphs.append(gr)
+    torch.cuda.synchronize()
+    for d in dsts:
+        assert bool((d.view == SENT_I16).all())                         # capturing ran nothing
+    for rep in range(3):
+        with torch.cuda.stream(r1):
+            graphs[0].replay()
+        with torch.cuda.stream(r2):
+            graphs[1].replay()
+        llx.migrate_stage(src.pool, perm_s[:n], dsts[2].pool, perm_d[:n], stream=cap_st)    # direct, dynamic tail on
+        llx.migrate_stage(src.pool, perm_s[n:2 * n], dsts[2].pool, perm_d[n:2 * n], stream=cap_st)
+    torch.cuda.synchronize()
+    h_src = src.host()
+    h_dst = om.new_pool(g["layers"], nb, H.tile_elems(g), fill=SENT)
+    om.migrate_stage(h_src, perm_s[:2 * n], h_dst, perm_d[:2 * n])
+    for d in dsts:
+        H.assert_pool_equal(d.host(), h_dst)
+
+
+def test_calls_that_cannot_be_captured_are_refused_and_leave_the_capture_valid(env):
+    H, llx = env
+    g = dict(synth.CONFIGS["tiny"], num_blocks=700)
+    src, dst = H.DevPool(g), H.DevPool(g, fill=SENT)
+    src.fill_from_synth(9, 0)
+    h_src = H.host_pool_from_synth(g, 9, 0)
+    s_ids, d_ids = synth.block_permutation(63, 700), synth.block_permutation(64, 700)
+    pin = llx.PinnedStaging(llx.staging_bytes(src.pool, 4))
+    dev_stg = torch.zeros(llx.staging_bytes(src.pool, 4), dtype=torch.uint8, device="cuda")
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    llx.migrate_stage(src.pool, s_ids[:3], dst.pool, d_ids[:3], stream=st)                   # warm-up
+    st.synchronize()
+    dst.view.fill_(SENT_I16)
+    torch.cuda.synchronize()
+
+    def refused(fn):
+        with pytest.raises(llx.LlxError) as e:
+            fn()
+        assert e.value.name == "LLX_ERR_STATE", e.value
+
+    gr = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(gr, stream=st):
+        refused(lambda: llx.migrate_stage(src.pool, s_ids[:300], dst.pool, d_ids[:300], stream=st))          # ids through the pinned ring
+        refused(lambda: llx.migrate_stage_wait(src.pool, s_ids[:2], dst.pool, d_ids[:2], stream=st))           # a blocking call
+        refused(lambda: llx.pack(src.pool, s_ids[:4], pin.dev_alias, pin.nbytes, stream=st))                   # bounce buffers + copy engine
+        refused(lambda: llx.migrate_via_host(src.pool, s_ids[:4], dst.pool, d_ids[:4], dev_stg.data_ptr(), dev_stg.numel(), stream=st))
+        # what CAN be captured, in the same capture: it is still valid after the refusals
+        llx.migrate_stage(src.pool, s_ids[:256], dst.pool, d_ids[:256], stream=st)                             # 256 pairs: ids by value
+        llx.migrate_batch(src.pool, dst.pool, [0, 10, 44], s_ids[256:300], d_ids[256:300], stream=st)
+        llx.pack(src.pool, s_ids[:4], dev_stg.data_ptr(), dev_stg.numel(), stream=st)                          # device staging buffer
+    torch.cuda.synchronize()
+    assert bool((dst.view == SENT_I16).all())
+    other = torch.cuda.Stream()
+    with torch.cuda.stream(other):
+        gr.replay()
+    other.synchronize()
+    h_dst = om.new_pool(g["layers"], 700, H.tile_elems(g), fill=SENT)
+    om.migrate_stage(h_src, s_ids[:300], h_dst, d_ids[:300])
+    H.assert_pool_equal(dst.host(), h_dst)
+    want = om.pack(h_src, s_ids[:4])
+    assert np.array_equal(dev_stg.cpu().numpy().view(np.uint16).reshape(want.shape), want)
+    pin.free()
