@@ -159,3 +159,56 @@ def test_attention_argument_errors(env):
     with pytest.raises(llx.LlxError):
         llx.decode_attention(pool64.pool, 5, buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), 1, 1, 1.0)
     llx.decode_attention(pool64.pool, 0, 0, 0, 0, 0, 0, 0, 1.0)        # B == 0: OK, nothing launched
+
+
+def test_configs4_decode_batch_shape_within_tolerance(env):
+    """BASELINE.json configs[4]'s own decode batch — the shape the interference numbers are quoted on: B = 32, context
+    lengths uniform in [128, 4096] (synth seed 4), H = 32, D = 128, disjoint block tables in an 8448-block pool (reading
+    A12), default KV split, 2 layers.  max |o - o_fp64| <= 2e-3 on every output element.  Prints the oracle's wall time
+    ("the fp64 attention oracle is timed once")."""
+    import time
+    H, llx = env
+    g = dict(synth.CONFIGS["llama7b"], layers=2, num_blocks=32 * 256 + 128 + 128)
+    B, S, Hh, D = 32, g["block_size"], g["kv_heads"], g["head_dim"]
+    ctx = synth.context_lengths(4, B, 128, 4096)
+    bt = disjoint_tables(g, ctx, seed=6)
+    assert bt.shape[1] <= 256 and int(ctx.sum()) > 32 * 1500
+    pool = H.DevPool(g)
+    # seeded fp16 U[-1,1) generated on the device (input generation only) and read back for the oracle: a host-side
+    # fill of the 8448-block pool would spend minutes in the generator for blocks no sequence uses
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(4)
+    flat = pool.raw.view(torch.float16)
+    step = 1 << 27
+    for a in range(0, flat.numel(), step):
+        b = min(flat.numel(), a + step)
+        flat[a:b] = (torch.rand(b - a, generator=gen, device="cuda", dtype=torch.float32) * 2 - 1).half()
+    h_pool = pool.host()
+    q = synth.queries_f16(5, B, Hh, D)
+    worst, t_oracle = 0.0, 0.0
+    for layer in range(g["layers"]):
+        got = as_f64(gpu_attention(llx, pool.pool, layer, q, bt, ctx, g))
+        t0 = time.perf_counter()
+        want = decode_attention_fp64(h_pool, layer, q, bt, ctx, S, Hh, D)
+        t_oracle += time.perf_counter() - t0
+        err = np.abs(got - want).max()
+        worst = max(worst, err)
+        assert err <= TOL, f"layer {layer}: max abs err {err}"
+    print(f"configs[4] decode batch: max abs err {worst:.3e} (bound {TOL}); fp64 oracle {t_oracle / g['layers']:.1f} s per layer "
+          f"for {int(ctx.sum())} context tokens")
+
+
+def test_ctx_len_beyond_the_table_row_is_clamped(env):
+    """llx.h precondition: ctx_len <= max_blocks*block_size; a longer one is clamped in the kernels — the result is the
+    attention over the row's max_blocks*block_size tokens, not a read past the table row."""
+    H, llx = env
+    g = G64
+    pool = H.DevPool(g)
+    pool.fill_from_synth(6, 0)
+    h_pool = H.host_pool_from_synth(g, 6, 0)
+    ctx_ok = np.array([48, 32], dtype=np.int32)
+    bt = disjoint_tables(g, ctx_ok, seed=12)                             # 3 blocks per row
+    q = synth.queries_f16(7, 2, g["kv_heads"], g["head_dim"])
+    got = as_f64(gpu_attention(llx, pool.pool, 0, q, bt, np.array([10_000, 32], dtype=np.int32), g))
+    want = decode_attention_fp64(h_pool, 0, q, bt, np.array([48, 32]), g["block_size"], g["kv_heads"], g["head_dim"])
+    assert np.abs(got - want).max() <= TOL

@@ -128,7 +128,7 @@ def test_session_budget_applies_to_non_final_stages_only(env):
     n1, fin1, ids1 = mig.stage(table, tokens, stream=st)
     ev[3].record(st)
     st.synchronize()
-    assert (n0, fin0, n1, fin1) == (38, False, 2, True)               # 39 full blocks; remaining 2 <= last_stage_max_blocks
+    assert (n0, fin0, n1, fin1) == (39, False, 1, True)               # the 39 full blocks, then the partly filled one
     t0, t1 = ev[0].elapsed_time(ev[1]), ev[2].elapsed_time(ev[3])
     rate0 = 2 * n0 * src.pool.block_bytes / (t0 * 1e-3) / 1e9
     rate1 = 2 * n1 * src.pool.block_bytes / (t1 * 1e-3) / 1e9
