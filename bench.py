@@ -4,7 +4,11 @@
 One STEP = one pass of the hot path over BASELINE.json configs[1] (LLaMA-7B shape): a 2048-token request
 (128 scattered blocks of 8 MiB) migrated between two 2000-block pools in 3 stages (112, 14, then the 2
 final blocks) with 8 new tokens appended to the source between stages — S1 planning check, S3 stages,
-S8 appends and the S4 final stage, all through the C-ABI (libllx.so).
+S8 appends and the S4 final stage, all through the C-ABI (libllx.so).  The copies run on the migration
+stream, the appends on a second "decode" stream, as in the paper ("continues the computation at the same
+time"; "another CUDA stream"): a stage waits for an append only when it reads
+the appended block, i.e. the final stage does.  Both streams lie inside the event-bracketed region; nothing
+is removed from the step (`--serial-appends` puts the appends back on the migration stream for comparison).
 
     value     GB/s, bytes read + written by the three stage copies / device time of the whole step
               (pools resident in HBM; CUDA events on the launching stream; max over ranks)
@@ -102,16 +106,22 @@ class ClockSampler:
 
 
 def profiled_traffic(launch="stage0_112_blocks"):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed ncu capture."""
-    try:
-        import csv
-        with open(os.path.join(ROOT, "profiles", "r01_copy_bulk_traffic.csv")) as f:
-            for row in csv.DictReader(f):
-                if row["launch"] == launch:
-                    return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
-    except Exception:  # noqa: BLE001
-        pass
-    return None
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the newest committed
+    `ncu --set full` capture (profiles/rNN_copy_bulk_traffic.csv; its `commit` column names the commit the capture
+    was taken at — a run does not re-measure it)."""
+    import csv
+    import glob
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_copy_bulk_traffic.csv")), reverse=True):
+        try:
+            with open(path) as f:
+                for row in csv.DictReader(f):
+                    if row["launch"] == launch:
+                        return {"bytes": int(row["dram_bytes_read"]) + int(row["dram_bytes_write"]),
+                                "source": os.path.relpath(path, ROOT) + " (ncu --set full)",
+                                "commit": row.get("commit") or "round-1 capture (before the kernel-shape commits d0dd35d, ccc79b2, 2c0d0bf)"}
+        except Exception:  # noqa: BLE001
+            continue
+    return {"bytes": None, "source": None, "commit": None}
 
 
 def measured_peak():
@@ -166,12 +176,45 @@ def cpu_baseline(budget_s=12.0) -> dict:
     while sum(times) < budget_s and len(times) < 50:
         times.append(oracle_step(ctx))
     t = statistics.median(times)
+    # the final stage alone on the host (context for the paper's downtime figure)
+    om, _, src, dst, s_tab, d_tab, _ = ctx
+    fin = []
+    for _ in range(5):
+        t0 = time.perf_counter()
+        om.migrate_stage(src, s_tab[-SCHEDULE[-1]:], dst, d_tab[-SCHEDULE[-1]:])
+        fin.append(time.perf_counter() - t0)
     return {"value": step_bytes(g) / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
             "host_cores_available": len(os.sched_getaffinity(0)),
+            "final_stage_ms": statistics.median(fin) * 1e3,
             "sample": f"the whole configs[1] step (128 blocks, stages 112/14/2, 2 appends of 8 tokens) inside two "
                       f"160-block host pools instead of 2000-block ones; {len(times)} repetitions, median; "
                       f"oracle.kv_migration.staged_migration as it stands (NumPy row copies, single thread)",
             "ms_per_step": t * 1e3}
+
+
+def cpu_baseline_all_cores(budget_s=8.0) -> dict:
+    """The oracle as it stands over a thread pool: one task per layer (the oracle's pool shape keeps K and V of a layer
+    together), `host_cores_available` threads; NumPy's row copies release the GIL.  Same sample as cpu_baseline."""
+    from concurrent.futures import ThreadPoolExecutor
+    om, g, src, dst, s_tab, d_tab, values = oracle_sample_setup()
+    cores = len(os.sched_getaffinity(0))
+    L = g["layers"]
+
+    def one_layer(l):
+        om.staged_migration(src[l:l + 1], s_tab, dst[l:l + 1], d_tab, SCHEDULE, APPENDS, g["block_size"], START_TOKENS,
+                            lambda t, _l, kv: values(t, l, kv))
+
+    times = []
+    with ThreadPoolExecutor(max_workers=cores) as ex:
+        while sum(times) < budget_s and len(times) < 50:
+            t0 = time.perf_counter()
+            list(ex.map(one_layer, range(L)))
+            times.append(time.perf_counter() - t0)
+    t = statistics.median(times)
+    return {"value": step_bytes(g) / t / 1e9, "unit": UNIT, "cores": min(cores, L), "kind": "oracle",
+            "host_cores_available": cores, "ms_per_step": t * 1e3,
+            "sample": f"the cpu_baseline sample; oracle.kv_migration.staged_migration per layer over a pool of {cores} threads "
+                      f"({L} tasks), {len(times)} repetitions, median"}
 
 
 def run_reference(args):
@@ -237,6 +280,7 @@ class Workload:
                     vals[t, l, kv] = synth.append_values_f16(3, START_TOKENS + t, l, kv, te_tok)
         self.append_host = torch.from_numpy(vals.view(np.int16)).pin_memory()
         self.append_dev = self.append_host.cuda()
+        self.e_fork, self.e_app = torch.cuda.Event(), torch.cuda.Event()
         torch.cuda.synchronize()
 
     def _pool(self, nb):
@@ -246,20 +290,39 @@ class Workload:
         return raw, llx.pool_wrap(raw.data_ptr(), nbytes, g["layers"], g["kv_heads"], g["head_dim"], g["block_size"],
                                   llx.F16, nb, keepalive=raw)
 
-    def step(self, stream, ev=None):
-        """One pass of the path: stage 0, append, stage 1, append, final stage — all enqueued on `stream`."""
+    def step(self, stream, dec=None, ev=None):
+        """One pass of the path: stage 0, append, stage 1, append, final stage.
+        dec is None: everything on `stream`, in that order.  Otherwise the appends run on the decode stream `dec`
+        (forked from `stream` at the start of the step, so they stay inside the timed region) concurrently with
+        stages 0 and 1, which do not read the appended block; the final stage, which does, waits for them.
+        ev: optional {name: (start, end)} timing events around the kernels "stage0", "stage1", "final" (on `stream`)
+        and "appends" (on the stream the appends run on)."""
         llx, g = self.llx, self.g
         tokens, m = START_TOKENS, 0
         vptr = self.append_dev.data_ptr()
         tok_bytes = g["layers"] * 2 * g["kv_heads"] * g["head_dim"] * 2
+        names = ("stage0", "stage1", "final")
+        if dec is not None:
+            self.e_fork.record(stream)
+            dec.wait_event(self.e_fork)
+            if ev is not None and "appends" in ev:
+                ev["appends"][0].record(dec)
+            for k, a in enumerate(APPENDS):
+                llx.append_tokens(self.src, self.s_tab, tokens, tokens + a, vptr + (tokens - START_TOKENS) * tok_bytes, stream=dec)
+                tokens += a
+            if ev is not None and "appends" in ev:
+                ev["appends"][1].record(dec)
+            self.e_app.record(dec)
         for k, n in enumerate(SCHEDULE):
-            if ev is not None and k == 0:
-                ev[0].record(stream)
+            if dec is not None and k == len(SCHEDULE) - 1:
+                stream.wait_event(self.e_app)              # the final stage reads the block the appends wrote
+            if ev is not None and names[k] in ev:
+                ev[names[k]][0].record(stream)
             llx.migrate_stage(self.src, self.s_tab[m:m + n], self.dst, self.d_tab[m:m + n], stream=stream)
-            if ev is not None and k == 0:
-                ev[1].record(stream)
+            if ev is not None and names[k] in ev:
+                ev[names[k]][1].record(stream)
             m += n
-            if k < len(APPENDS):
+            if dec is None and k < len(APPENDS):
                 llx.append_tokens(self.src, self.s_tab, tokens, tokens + APPENDS[k],
                                   vptr + (tokens - START_TOKENS) * tok_bytes, stream=stream)
                 tokens += APPENDS[k]
@@ -293,12 +356,13 @@ def run_llx(args):
     assert llx.plan_stage(START_TOKENS + sum(APPENDS), sum(SCHEDULE[:-1]), g["block_size"], 2) == (SCHEDULE[-1], True)
     stream = torch.cuda.Stream()
     stream.wait_stream(torch.cuda.current_stream())
+    dec = None if args.serial_appends else torch.cuda.Stream()      # the source's decode stream (appends)
     sampler = ClockSampler(local)
     sampler.start()
 
     # ---- device-resident throughput -----------------------------------------------------
     for _ in range(args.warmup):
-        w.step(stream)
+        w.step(stream, dec)
     stream.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     replicas.barrier()
@@ -307,8 +371,8 @@ def run_llx(args):
     tw0 = time.perf_counter()
     e0.record(stream)
     for k in range(args.steps):
-        w.step(stream)
-    e1.record(stream)
+        w.step(stream, dec)
+    e1.record(stream)              # behind the last final stage, which waited for the decode stream's appends
     stream.synchronize()
     tw1 = time.perf_counter()
     replicas.barrier()
@@ -324,15 +388,49 @@ def run_llx(args):
     # dominant kernel (stage 0) timed on its own events, in the same step sequence (second pass: the event
     # records would otherwise sit between the kernels of the pass that defines `value`)
     k_steps = min(args.steps, 200)
-    pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k_steps)]
+    mk = lambda: (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    pairs = [mk() for _ in range(k_steps)]
     tw0 = time.perf_counter()
     for k in range(k_steps):
-        w.step(stream, pairs[k])
+        w.step(stream, dec, {"stage0": pairs[k]})
     stream.synchronize()
     sampler.window(tw0, time.perf_counter())
     stage0_ms = statistics.mean(a.elapsed_time(b) for a, b in pairs)
     stage0_bytes = 2 * SCHEDULE[0] * w.src.block_bytes
     achieved = stage0_bytes / (stage0_ms * 1e-3) / 1e9
+
+    # where the step's time goes: every kernel of the step on its own events (third pass; events between the kernels
+    # cost the PDL overlap, so the parts sum to slightly MORE than ms_per_step — the difference is reported, not hidden)
+    parts = {k: [mk() for _ in range(k_steps)] for k in ("stage0", "stage1", "final", "appends")}
+    whole = [mk() for _ in range(k_steps)]
+    for k in range(k_steps):
+        whole[k][0].record(stream)
+        w.step(stream, dec, {name: evs[k] for name, evs in parts.items()})
+        whole[k][1].record(stream)
+    stream.synchronize()
+    mean_us = lambda evs: 1e3 * statistics.mean(a.elapsed_time(b) for a, b in evs)
+    breakdown = {name + "_us": mean_us(evs) for name, evs in parts.items()}
+    breakdown["step_with_events_us"] = mean_us(whole)
+    breakdown["step_us"] = ms_local * 1e3
+    breakdown["ideal_at_measured_peak_us"] = step_bytes(g) / peak / 1e3
+    breakdown["stage_kernels_sum_us"] = breakdown["stage0_us"] + breakdown["stage1_us"] + breakdown["final_us"]
+    breakdown["outside_stage_kernels_us"] = breakdown["step_us"] - breakdown["stage_kernels_sum_us"]
+    breakdown["appends"] = ("on the decode stream, concurrent with stages 0 and 1; the final stage waits for them" if dec is not None
+                            else "serialised on the migration stream between the stages")
+
+    # the same 128 blocks as ONE stage (what a blocking copy would do; north_star's "2048-token request")
+    ss = [mk() for _ in range(min(args.steps, 100))]
+    for _ in range(3):
+        llx.migrate_stage(w.src, w.s_tab, w.dst, w.d_tab, stream=stream)
+    for a, b in ss:
+        a.record(stream)
+        llx.migrate_stage(w.src, w.s_tab, w.dst, w.d_tab, stream=stream)
+        b.record(stream)
+    stream.synchronize()
+    single_ms = statistics.mean(a.elapsed_time(b) for a, b in ss)
+    single_shot = {"GBps": step_bytes(g) / (single_ms * 1e-3) / 1e9, "ms": single_ms,
+                   "frac_of_nominal_8TBps": step_bytes(g) / (single_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+                   "frac_of_measured_peak": step_bytes(g) / (single_ms * 1e-3) / 1e9 / peak}
 
     # ---- end to end through pinned host buffers (block fusion path) -----------------------
     # llx_migrate_via_host: gather -> pinned host buffer -> scatter, chunked so that both directions of the
@@ -375,6 +473,7 @@ def run_llx(args):
     clocks = sampler.stop()
 
     block_bytes = w.src.block_bytes
+    traffic = profiled_traffic()
     suite = None
     if args.suite and world == 1:
         del w
@@ -394,8 +493,11 @@ def run_llx(args):
         "pct_of_nominal_8TBps": 100.0 * value / world / NOMINAL_HBM_GBS,
         "pct_of_measured_copy_peak": 100.0 * value / world / peak,
         "downtime_us": downtime,
+        "breakdown": breakdown,
+        "single_shot_2048": single_shot,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": profiled_traffic(), "traffic_source": "profiles/r01_copy_bulk_traffic.csv (ncu --set full)", "kernel": "llx_copy_bulk (stage 0: 112 blocks)", "peak_source": peak_src,
+                     "traffic": traffic["bytes"], "traffic_source": traffic["source"], "traffic_commit": traffic["commit"],
+                     "kernel": "llx_copy_bulk (stage 0: 112 blocks)", "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": stage0_bytes, "avg_launch_ms": stage0_ms,
                      "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS},
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": n * block_bytes,
@@ -404,7 +506,8 @@ def run_llx(args):
                 "path": "llx_migrate_via_host: gather kernel -> pinned host buffer -> scatter kernel, 64 MiB chunks, D2H and "
                         "H2D on the copy engines at the same time (host wall clock incl. stream sync)",
                 "sequential_pack_then_unpack": {"value": e2e_seq_val, "ms_per_step": e2e_seq_ms,
-                                                "path": "llx_pack (zero-copy kernel, D2H) then llx_unpack (H2D)"}},
+                                                "path": "llx_pack (gather kernel into a device bounce buffer, copy engine D2H, 64 MiB chunks) "
+                                                        "then llx_unpack (copy engine H2D, scatter kernel), one after the other"}},
         "gpu_launches": launches,
         "clocks": clocks,
         "paper_context": "Llumnix reports 20-30 ms downtime on A10 + 64 Gb/s Gloo (PAPER.md:287); no GB/s figure",
@@ -413,6 +516,7 @@ def run_llx(args):
         out["cpu_baseline"] = None
     else:
         out["cpu_baseline"] = cpu_baseline()
+        out["cpu_baseline_all_cores"] = cpu_baseline_all_cores()
     if suite is not None:
         out["suite_file"] = suite
     print(json.dumps(out))
@@ -512,6 +616,8 @@ def main():
     ap.add_argument("--suite", action="store_true", help="also run the length sweep, 30B batch and interference configs")
     ap.add_argument("--downtime-reps", type=int, default=100)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--serial-appends", action="store_true",
+                    help="enqueue the appends on the migration stream between the stages (round-1 behaviour) instead of a decode stream")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

@@ -417,6 +417,10 @@ typedef struct {
 void llx_get_counters(llx_counters* out);
 void llx_reset_counters(void);
 
+/* Waits until everything enqueued on cuda_stream (NULL: the legacy default stream) has completed; LLX_ERR_CUDA reports an
+ * asynchronous fault of that work.  For clients that do not link the CUDA runtime themselves. */
+llx_status llx_synchronize(void* cuda_stream);
+
 const char* llx_status_str(llx_status s);
 const char* llx_last_error(void); /* thread-local detail of this thread's last failed call */
 const char* llx_version(void);

@@ -16,5 +16,5 @@ from .binding import (  # noqa: F401
     BlockManager, Migration, REQ_RUNNING, REQ_FINISHED, REQ_PREEMPTED, REQ_PEER_FAILED,
     MIG_READY, MIG_COPYING, MIG_FINAL_COPYING, MIG_COMMITTED, MIG_ABORTED,
     ABORT_NONE, ABORT_FINISHED, ABORT_PREEMPTED, ABORT_PEER_FAILED, ABORT_NO_SPACE,
-    set_option, get_option, options, counters, reset_counters, version, EXPORTS,
+    set_option, get_option, options, synchronize, counters, reset_counters, version, EXPORTS,
 )

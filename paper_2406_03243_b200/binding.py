@@ -122,6 +122,7 @@ EXPORTS = {
     "llx_get_option": (C.c_longlong, [_i]),
     "llx_get_counters": (None, [C.POINTER(_Counters)]),
     "llx_reset_counters": (None, []),
+    "llx_synchronize": (_i, [_vp]),
     "llx_status_str": (C.c_char_p, [_i]),
     "llx_last_error": (C.c_char_p, []),
     "llx_version": (C.c_char_p, []),
@@ -514,6 +515,10 @@ def options(**kw):
     finally:
         for k, v in old.items():
             set_option(names[k], v)
+
+
+def synchronize(stream=None):
+    _check(load().llx_synchronize(_stream(stream)))
 
 
 def counters() -> dict:

@@ -12,8 +12,10 @@ SOURCES = [os.path.join(CSRC, "llx_api.cu"), os.path.join(CSRC, "llx_coord.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("llx_copy.cuh", "llx_attention.cuh", "llx_internal.h")] + \
     [os.path.join(os.path.dirname(HERE), "include", "llx.h")]
 
+# -cudart shared: the library uses the process's CUDA runtime (the one torch already loaded, else the toolkit's through
+# the rpath) instead of carrying a private static copy — one runtime per process, and the artefact holds our code only.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-shared", "-Xcompiler", "-fPIC", "-diag-suppress", "550"]
+              "-shared", "-Xcompiler", "-fPIC", "-diag-suppress", "550", "-cudart", "shared"]
 
 
 def _nvcc() -> str:
@@ -34,7 +36,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile libllx.so if missing or older than its sources; returns its path."""
     if not force and not is_stale():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB + ".tmp"] + SOURCES
+    nvcc = _nvcc()
+    cuda_lib = os.path.join(os.path.dirname(os.path.dirname(os.path.realpath(nvcc))), "lib64")
+    cmd = [nvcc] + NVCC_FLAGS + ["-Xlinker", "-rpath=" + cuda_lib] + (["-Xptxas", "-v"] if verbose else []) + \
+        ["-o", LIB + ".tmp"] + SOURCES
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)

@@ -1356,6 +1356,13 @@ void llx_reset_counters(void) {
     g_id_uploads = 0;
 }
 
+llx_status llx_synchronize(void* stream) {
+    llx_status rc = refuse_if_capturing((cudaStream_t)stream, "llx_synchronize");
+    if (rc != LLX_OK) return rc;
+    LLX_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    return LLX_OK;
+}
+
 const char* llx_status_str(llx_status s) {
     switch (s) {
         case LLX_OK: return "LLX_OK";
