@@ -401,7 +401,7 @@ def run_llx(args):
 
     # where the step's time goes: every kernel of the step on its own events (third pass; events between the kernels
     # cost the PDL overlap, so the parts sum to slightly MORE than ms_per_step — the difference is reported, not hidden)
-    parts = {k: [mk() for _ in range(k_steps)] for k in ("stage0", "stage1", "final", "appends")}
+    parts = {k: [mk() for _ in range(k_steps)] for k in ("stage0", "stage1", "final") + (("appends",) if dec is not None else ())}
     whole = [mk() for _ in range(k_steps)]
     for k in range(k_steps):
         whole[k][0].record(stream)
@@ -596,8 +596,8 @@ def measure_downtime(torch, llx, w, stream, reps=100):
 
 
 def run_suite(torch, llx, stream):
-    from paper_2406_03243_b200 import suite
-    res = suite.run(torch, llx, stream)
+    import bench_suite
+    res = bench_suite.run(torch, llx, stream)
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     path = os.path.join("gpurun_out", "suite.json")
     with open(os.path.join(ROOT, path), "w") as f:

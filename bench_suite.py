@@ -1,5 +1,7 @@
 """The other BASELINE.json configs, measured through the C-ABI: configs[2] length sweep, configs[3] 30B batch,
-configs[4] interference with a decode step + staging through pinned host memory.  Called by `bench.py --suite`.
+configs[4] interference with a decode step + staging through pinned host memory, plus the NEXT-row measurements
+(bandwidth budget, live migration during decode, TP-rank sharded tiles, peer route).  A measuring harness beside
+bench.py, not part of the library: `bench.py --suite` calls run(); `python bench_suite.py --only NAME` runs one leg.
 
 Everything here is measurement harness: pools are torch allocations (memory + streams only), inputs come
 from `synth`, all timing is CUDA events on the launching stream (or host wall clock where stated)."""
@@ -9,9 +11,16 @@ import gc
 import statistics
 import time
 
+import os
+import sys
+
 import numpy as np
 
-import synth
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synth  # noqa: E402
 
 SENT_I16 = int(np.array(synth.SENTINEL_U16, np.uint16).view(np.int16))
 
@@ -141,9 +150,9 @@ def reference_points(torch, llx, p: Pools, stream, nb):
         res["per_tile_memcpy_loop_ms"] = t["median_ms"]
     t = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=stream))
     res["llx_migrate_stage_GBps"] = by / t["median_ms"] / 1e6
-    for kern, name in ((1, "llx_vec16_kernel_GBps"), (2, "llx_bulk_kernel_GBps")):
-        with llx.options(copy_kernel=kern):
-            t = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=stream))
+    for o, name in ((dict(copy_kernel=1), "llx_vec16_kernel_GBps"), (dict(copy_kernel=2), "llx_bulk_kernel_GBps"),
+                    (dict(route=llx.ROUTE_PEER), "llx_peer_route_on_one_device_GBps")):
+        t = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=stream, opts=o))
         res[name] = by / t["median_ms"] / 1e6
     # device-buffer block fusion (pack then unpack through HBM)
     stg = torch.empty(llx.staging_bytes(p.src, n), dtype=torch.uint8, device="cuda")
@@ -177,11 +186,11 @@ def staging_host(torch, llx, p: Pools, stream, nb):
     res["llx_unpack_from_pinned_host_GBps"] = nbytes / t["median_ms"] / 1e6
     res["pack_frac_of_link_peak"] = res["llx_pack_to_pinned_host_GBps"] / res["link_peak_d2h_GBps"]
     res["unpack_frac_of_link_peak"] = res["llx_unpack_from_pinned_host_GBps"] / res["link_peak_h2d_GBps"]
-    with llx.options(via_host_mode=1):       # the kernels address the pinned buffer themselves
-        t = _time_stream(torch, stream, lambda: llx.pack(p.src, s_tab, pin.dev_alias, nbytes, stream=stream), reps=5, warm=1)
-        res["llx_pack_zero_copy_GBps"] = nbytes / t["median_ms"] / 1e6
-        t = _time_stream(torch, stream, lambda: llx.unpack(pin.dev_alias, nbytes, p.dst, d_tab, stream=stream), reps=5, warm=1)
-        res["llx_unpack_zero_copy_GBps"] = nbytes / t["median_ms"] / 1e6
+    zc = dict(via_host_mode=1)               # the kernels address the pinned buffer themselves
+    t = _time_stream(torch, stream, lambda: llx.pack(p.src, s_tab, pin.dev_alias, nbytes, stream=stream, opts=zc), reps=5, warm=1)
+    res["llx_pack_zero_copy_GBps"] = nbytes / t["median_ms"] / 1e6
+    t = _time_stream(torch, stream, lambda: llx.unpack(pin.dev_alias, nbytes, p.dst, d_tab, stream=stream, opts=zc), reps=5, warm=1)
+    res["llx_unpack_zero_copy_GBps"] = nbytes / t["median_ms"] / 1e6
     t = _time_stream(torch, stream, lambda: llx.migrate_via_host(p.src, s_tab, p.dst, d_tab, pin.dev_alias, nbytes, stream=stream), reps=5, warm=1)
     res["llx_migrate_via_host_roundtrip_ms"] = t["median_ms"]
     # alternative: pack into a DEVICE buffer, then one copy-engine transfer (and back)
@@ -207,9 +216,12 @@ def staging_host(torch, llx, p: Pools, stream, nb):
 
 
 # ---- configs[3]: LLaMA-30B batch --------------------------------------------------------------
-def batch_30b(torch, llx, stream):
+def batch_30b(torch, llx, stream, seed=0):
+    """seed 0 is the config's draw as specified; its sample of 64 lengths has mean 248 tokens (1023 blocks, 24.4 GiB) —
+    a fair draw of a heavy tail (the distribution's mean is 512).  seed 2 is added because its SAMPLE mean (507 tokens,
+    2064 blocks, 49 GiB) is within 10 % of the nominal 512."""
     g = dict(synth.CONFIGS["llama30b"])
-    lens, nblk, seed_used = synth.batch_request_blocks(0, 64, g["block_size"], g["num_blocks"])
+    lens, nblk, seed_used = synth.batch_request_blocks(seed, 64, g["block_size"], g["num_blocks"])
     total = int(nblk.sum())
     block_bytes = 2 * g["layers"] * g["block_size"] * g["kv_heads"] * g["head_dim"] * 2
     nb = g["num_blocks"]
@@ -276,8 +288,8 @@ def interference(torch, llx, stream_mig_unused):
             llx.decode_attention(p.src, l, q.data_ptr(), o.data_ptr(), d_bt.data_ptr(), d_ctx.data_ptr(), B, MB, scale,
                                  stream=s_dec)
 
-    def migrate():
-        llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig)
+    def migrate(o=None):
+        llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=o)
 
     decode_step()
     torch.cuda.synchronize()
@@ -289,14 +301,14 @@ def interference(torch, llx, stream_mig_unused):
         torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ma, mb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        with llx.options(max_ctas=max_ctas, bandwidth_gbps=budget):
-            a.record(s_dec)
-            ma.record(s_mig)
-            for _ in range(n_mig):
-                migrate()
-            mb.record(s_mig)
-            decode_step()
-            b.record(s_dec)
+        o = dict(max_ctas=max_ctas, bandwidth_gbps=budget)          # the launch policy of these calls only
+        a.record(s_dec)
+        ma.record(s_mig)
+        for _ in range(n_mig):
+            migrate(o)
+        mb.record(s_mig)
+        decode_step()
+        b.record(s_dec)
         torch.cuda.synchronize()
         return a.elapsed_time(b), ma.elapsed_time(mb)
 
@@ -385,12 +397,11 @@ def auto_budget(torch, llx, stream_unused=None, target_pct=1.0, rounds=12):
     def one(budget, n_mig):
         torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        with llx.options(bandwidth_gbps=budget):
-            a.record(s_dec)
-            for _ in range(n_mig):
-                llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig)
-            decode_step()
-            b.record(s_dec)
+        a.record(s_dec)
+        for _ in range(n_mig):
+            llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=dict(bandwidth_gbps=budget))
+        decode_step()
+        b.record(s_dec)
         torch.cuda.synchronize()
         return a.elapsed_time(b)
 
@@ -426,8 +437,6 @@ def auto_budget(torch, llx, stream_unused=None, target_pct=1.0, rounds=12):
            "ideal_share_pct_at_chosen": None if best is None else 100.0 * best / (int(ctx.sum()) * 2 * H * D * 2 * L / base / 1e6),
            "note": "median of per-pair ratios (step with migration / step without, alternating); null_pair_pct is the "
                    "same statistic for two steps without migration (the measurement floor)"}
-    if best is not None:
-        llx.set_option(llx.OPT_BANDWIDTH_GBPS, 0)
     del p
     _free(torch)
     return res
@@ -499,21 +508,20 @@ def live_migration(torch, llx, stream_unused=None, budgets=(0, 100, 25), start_t
         tokens_at_start = tokens
         mig = llx.Migration(p.src, src_mgr, p.dst, dst_mgr, S, 2)
         stages, during, t_start = [], [], time.perf_counter()
-        with llx.options(bandwidth_gbps=budget):
-            while True:
-                n, fin, _ = mig.stage(table_r, tokens, stream=s_mig)
-                ev = torch.cuda.Event()
-                ev.record(s_mig)
-                stages.append(n)
-                assert not fin and mig.state == llx.MIG_COPYING
-                while not ev.query():                         # decoding continues while the stage copies
-                    during.append(decode_step(p.src))
-                n_next, fin_next = llx.plan_stage(tokens, mig.blocks_migrated, S, 2)
-                if fin_next:
-                    break
+        mig.set_stage_opts(dict(bandwidth_gbps=budget))       # non-final stages only: the session runs the final stage unthrottled
+        while True:
+            n, fin, _ = mig.stage(table_r, tokens, stream=s_mig)
+            ev = torch.cuda.Event()
+            ev.record(s_mig)
+            stages.append(n)
+            assert not fin and mig.state == llx.MIG_COPYING
+            while not ev.query():                             # decoding continues while the stage copies
+                during.append(decode_step(p.src))
+            n_next, fin_next = llx.plan_stage(tokens, mig.blocks_migrated, S, 2)
+            if fin_next:
+                break
         copy_ms = (time.perf_counter() - t_start) * 1e3
         # final stage: the request is drained (no more decode steps for it), the last blocks move, it resumes on dst
-        llx.set_option(llx.OPT_BANDWIDTH_GBPS, 0)             # the final stage always runs at full speed
         t0 = time.perf_counter_ns()
         n, fin, _ = mig.stage(table_r, tokens, stream=s_mig)  # handshake round (check, plan, PRE-ALLOC) + copy
         s_mig.synchronize()
@@ -547,6 +555,50 @@ def live_migration(torch, llx, stream_unused=None, budgets=(0, 100, 25), start_t
     return out
 
 
+# ---- NEXT-2 / SURVEY 8(e): tensor-parallel rank shards of LLaMA-30B (52 heads = 4 ranks x 13 -> 52 KiB tiles) ----------
+def tp_shard_30b(torch, llx, stream_unused=None, tp=4, n=128, nb=700):
+    """Rank r of the source instance migrates to rank r of the destination, no exchange between ranks (PAPER.md:235,
+    :254).  On ONE GPU the four rank pairs are four pool pairs on four streams; reported: one rank's stage alone, and
+    the four ranks' stages in flight together (they share this GPU's HBM; on a TP=4 node each rank has its own)."""
+    g = dict(synth.CONFIGS["llama30b"])
+    g["kv_heads"] //= tp
+    pools = [Pools(torch, llx, g, nb, nb) for _ in range(tp)]
+    streams = [torch.cuda.Stream() for _ in range(tp)]
+    s_tab, d_tab = synth.block_permutation(1, nb)[:n], synth.block_permutation(2, nb)[:n]
+    by = 2 * n * pools[0].src.block_bytes
+    one = _time_stream(torch, streams[0], lambda: llx.migrate_stage(pools[0].src, s_tab, pools[0].dst, d_tab, stream=streams[0]))
+    for _ in range(2):
+        for r in range(tp):
+            llx.migrate_stage(pools[r].src, s_tab, pools[r].dst, d_tab, stream=streams[r])
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(10):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(streams[0])
+        for r in range(1, tp):
+            streams[r].wait_event(a)
+        for r in range(tp):
+            llx.migrate_stage(pools[r].src, s_tab, pools[r].dst, d_tab, stream=streams[r])
+        for r in range(1, tp):
+            e = torch.cuda.Event()
+            e.record(streams[r])
+            streams[0].wait_event(e)
+        b.record(streams[0])
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    t4 = statistics.median(ts)
+    fin = _time_stream(torch, streams[0], lambda: llx.migrate_stage(pools[0].src, s_tab[:2], pools[0].dst, d_tab[:2], stream=streams[0]), reps=20)
+    res = {"tp": tp, "kv_heads_per_rank": g["kv_heads"], "tile_KiB": pools[0].src.tile_bytes / 1024, "blocks": n,
+           "payload_per_rank_MiB": n * pools[0].src.block_bytes / 2**20,
+           "one_rank_alone_GBps": by / one["median_ms"] / 1e6, "one_rank_alone_ms": one["median_ms"],
+           "four_ranks_concurrent_total_GBps": tp * by / t4 / 1e6, "four_ranks_concurrent_ms": t4,
+           "final_stage_2_blocks_gpu_us_warm": fin["median_ms"] * 1e3,
+           "note": "one GPU stands in for the four GPUs of a TP=4 instance pair: the concurrent figure is four rank-local stages sharing ONE HBM"}
+    del pools
+    _free(torch)
+    return res
+
+
 def run(torch, llx, stream):
     res = {}
     g = synth.CONFIGS["llama7b"]
@@ -561,11 +613,13 @@ def run(torch, llx, stream):
     res["auto_budget_1pct"] = auto_budget(torch, llx, stream, target_pct=1.0)
     res["live_migration_during_decode"] = live_migration(torch, llx, stream)
     res["batch_llama30b_64req"] = batch_30b(torch, llx, stream)
+    res["batch_llama30b_64req_seed2_mean507"] = batch_30b(torch, llx, stream, seed=2)
+    res["tp4_rank_shards_llama30b"] = tp_shard_30b(torch, llx, stream)
     return res
 
 
 def main():
-    """python -m paper_2406_03243_b200.suite [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch)"""
+    """python bench_suite.py [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch | batch2 | tp)"""
     import argparse
     import json
 
@@ -590,6 +644,10 @@ def main():
         res = live_migration(torch, llx, stream)
     elif args.only == "batch":
         res = batch_30b(torch, llx, stream)
+    elif args.only == "batch2":
+        res = batch_30b(torch, llx, stream, seed=2)
+    elif args.only == "tp":
+        res = tp_shard_30b(torch, llx, stream)
     else:
         p = Pools(torch, llx, g, nb, nb)
         fn = {"sweep": length_sweep, "refs": reference_points, "staging": staging_host}[args.only]
@@ -599,5 +657,4 @@ def main():
 
 
 if __name__ == "__main__":
-    import sys
     sys.exit(main())

@@ -400,6 +400,14 @@ typedef enum {
     LLX_OPT_DYNAMIC_TAIL_BATCH = 13, /* chunks per claim of the dynamic tail (0 = auto: 4) */
     LLX_OPT_EXACT_RESIDENCY = 14, /* 1 (default): the bulk kernel asks for enough shared memory that no SM can hold more of its
                                    CTAs than intended, early-launched CTAs of the next kernel included */
+    LLX_OPT_COPY_SMEM_CARVEOUT_PCT = 15, /* PROCESS-WIDE ONLY (a property of the kernel function, not of a launch): preferred
+                                   shared-memory carve-out, in % of the SM's maximum, of the register-staged copy kernel that
+                                   serves bandwidth budgets below 500 GB/s and the host zero-copy / peer routes.  That kernel
+                                   keeps a small CTA resident on every SM for the whole stage, and an SM cannot change its
+                                   L1/shared split while a CTA is resident: with the driver's default (0) a co-running kernel
+                                   that needs shared memory waits for the end of the stage.  Default 75 (196 KB shared, 60 KB
+                                   L1): every llx kernel co-runs, the stand-in decode step loses nothing.  100: no kernel ever
+                                   waits, L1-hungry co-runners lose ~20 % */
     LLX_OPT_VIA_HOST_MODE = 11  /* llx_pack / llx_unpack / llx_migrate_via_host with a pinned-host buffer: 0 (default) copy engines
                                    through device bounce buffers; 1 the kernels address the host buffer directly (zero-copy) */
 } llx_option;

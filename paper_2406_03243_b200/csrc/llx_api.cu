@@ -66,7 +66,7 @@ int elem_bytes_of(llx_dtype d) {
 
 // ---- options / counters -------------------------------------------------------------------
 std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
-    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1};
+    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1}, g_opt_carveout{75};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
 // Range of every option: shared by llx_set_option (process defaults) and by the per-call llx_launch_opts.
@@ -87,6 +87,7 @@ bool opt_valid(int opt, long long v) {
         case LLX_OPT_DYNAMIC_TAIL_PCT: return v >= 0 && v <= 100;
         case LLX_OPT_DYNAMIC_TAIL_BATCH: return v >= 0 && v <= 4096;
         case LLX_OPT_EXACT_RESIDENCY: return v >= 0 && v <= 1;
+        case LLX_OPT_COPY_SMEM_CARVEOUT_PCT: return v >= 0 && v <= 100;
     }
     return false;
 }
@@ -170,6 +171,7 @@ struct DevInfo {
     int sm_count = 0;
     int max_smem_optin = 0;
     int smem_per_sm = 0;
+    int carveout_applied = -1;  // LLX_OPT_COPY_SMEM_CARVEOUT_PCT as last set on the register-staged copy kernel
     bool ready = false;
 };
 std::mutex g_dev_mu;
@@ -188,6 +190,21 @@ llx_status dev_info(int dev, DevInfo** out, bool capturing = false) {
         LLX_CUDA(cudaFuncSetAttribute(llx_copy_bulk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
         LLX_CUDA(cudaFuncSetAttribute(llx_copy_bulk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
         d.ready = true;
+    }
+    // Shared-memory carve-out of the register-staged copy kernel (the paced copy of NEXT-1, the host zero-copy and peer
+    // routes).  Its CTAs hold no shared memory but stay resident on EVERY SM for a whole stage (75 ms for 112 blocks at
+    // 25 GB/s), and an SM cannot change its L1/shared split while a CTA is resident: arriving on idle SMs with the
+    // driver's default preference they pin the split at "all L1", and every kernel that needs shared memory — the bulk
+    // ring of another request's final stage, a GEMM — then waits for the END OF THE STAGE on that SM (measured on B200: a
+    // 2-block final stage next to a 25 GB/s stage: median 53 us, p90 75 ms; with a preference of 64-75 % never above
+    // 0.14 ms; 87-100 % costs the L1-hungry stand-in decode attention +20-25 %, 75 % costs it nothing).  75 % asks for the
+    // 196 KB split: every llx kernel fits beside it (final stage 2 x 76 KB, long stage 113 KB) and 60 KB of L1 remain.
+    const int want_carveout = (int)g_opt_carveout.load();
+    if (d.carveout_applied != want_carveout && !capturing) {
+        const int v = want_carveout > 0 ? want_carveout : cudaSharedmemCarveoutDefault;
+        LLX_CUDA(cudaFuncSetAttribute(llx_copy_vec16<true, 4>, cudaFuncAttributePreferredSharedMemoryCarveout, v));
+        LLX_CUDA(cudaFuncSetAttribute(llx_copy_vec16<false, 4>, cudaFuncAttributePreferredSharedMemoryCarveout, v));
+        d.carveout_applied = want_carveout;
     }
     *out = &d;
     return LLX_OK;
@@ -1318,6 +1335,7 @@ llx_status llx_set_option(llx_option opt, long long v) {
         case LLX_OPT_DYNAMIC_TAIL_PCT: g_opt_dyn_pct = v; break;
         case LLX_OPT_DYNAMIC_TAIL_BATCH: g_opt_dyn_batch = v; break;
         case LLX_OPT_EXACT_RESIDENCY: g_opt_smem_pad = v; break;
+        case LLX_OPT_COPY_SMEM_CARVEOUT_PCT: g_opt_carveout = v; break;  // applied to the kernel at the next copy launch
     }
     return LLX_OK;
 }
@@ -1338,6 +1356,7 @@ long long llx_get_option(llx_option opt) {
         case LLX_OPT_DYNAMIC_TAIL_PCT: return g_opt_dyn_pct;
         case LLX_OPT_DYNAMIC_TAIL_BATCH: return g_opt_dyn_batch;
         case LLX_OPT_EXACT_RESIDENCY: return g_opt_smem_pad;
+        case LLX_OPT_COPY_SMEM_CARVEOUT_PCT: return g_opt_carveout;
     }
     return -1;
 }

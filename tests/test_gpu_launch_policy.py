@@ -89,6 +89,11 @@ def test_budgeted_stage_and_unthrottled_final_stage_from_two_threads(env):
     achieved = stage_bytes / (statistics.median(a_ms) * 1e-3) / 1e9
     print(f"final stage solo {solo:.1f} us, next to a {budget} GB/s stage {with_a:.1f} us; budgeted stage achieved {achieved:.1f} GB/s")
     assert with_a <= 2.0 * solo, (solo, with_a)
+    # and NEVER a whole stage: the budgeted copy keeps a CTA resident on every SM for ~75 ms; if it pinned the SMs'
+    # L1/shared split at "all L1" (the driver's default for a kernel without shared memory) the final stage's bulk ring
+    # would wait for the end of that stage on every SM (measured before LLX_OPT_COPY_SMEM_CARVEOUT_PCT: p90 75 ms)
+    busy.sort()
+    assert busy[int(0.99 * len(busy))] < 2000 and busy[-1] < 20000, (busy[int(0.99 * len(busy))], busy[-1])
     assert abs(achieved - budget) <= 0.10 * budget, achieved
     assert llx.get_option(llx.OPT_BANDWIDTH_GBPS) == 0                 # nobody touched the process defaults
     # bit-exact, both destinations, on the sampled layers (oracle) and on every layer (device gather)
@@ -132,8 +137,8 @@ def test_session_budget_applies_to_non_final_stages_only(env):
     t0, t1 = ev[0].elapsed_time(ev[1]), ev[2].elapsed_time(ev[3])
     rate0 = 2 * n0 * src.pool.block_bytes / (t0 * 1e-3) / 1e9
     rate1 = 2 * n1 * src.pool.block_bytes / (t1 * 1e-3) / 1e9
-    print(f"session: stage 0 at {rate0:.1f} GB/s under a 50 GB/s budget, final stage at {rate1:.0f} GB/s")
-    assert abs(rate0 - 50) <= 5 and rate1 > 500
+    print(f"session: stage 0 at {rate0:.1f} GB/s under a 50 GB/s budget, final stage {t1 * 1e3:.0f} us ({rate1:.0f} GB/s)")
+    assert abs(rate0 - 50) <= 5 and t1 < 0.2           # one 8 MiB block under the budget would take 0.34 ms
     d_table = mig.commit(table)
     assert list(d_table) == list(ids0) + list(ids1)
     h_src = H.host_pool_from_synth(g, 0, 0, layers=[7])
