@@ -270,8 +270,11 @@ class Workload:
             b = min(flat.numel(), a + step)
             flat[a:b] = (torch.rand(b - a, generator=gen, device="cuda", dtype=torch.float32) * 2 - 1).half()
         self.dst_raw.view(torch.int16).fill_(int(np.array(synth.SENTINEL_U16, np.uint16).view(np.int16)))
-        self.s_tab = synth.block_permutation(1, self.nb_src)[:128]
-        self.d_tab = synth.block_permutation(2, self.nb_dst)[:128]
+        # two requests of 128 scattered blocks each: consecutive steps migrate them alternately ("the llumlet ... starts
+        # to migrate requests to the destination continuously") — every step is one whole configs[1] request
+        ps, pd = synth.block_permutation(1, self.nb_src), synth.block_permutation(2, self.nb_dst)
+        self.s_tabs, self.d_tabs = (ps[:128], ps[128:256]), (pd[:128], pd[128:256])
+        self.s_tab, self.d_tab = self.s_tabs[0], self.d_tabs[0]
         te_tok = H * D
         vals = np.empty((16, L, 2, te_tok), dtype=np.uint16)
         for t in range(16):
@@ -280,7 +283,9 @@ class Workload:
                     vals[t, l, kv] = synth.append_values_f16(3, START_TOKENS + t, l, kv, te_tok)
         self.append_host = torch.from_numpy(vals.view(np.int16)).pin_memory()
         self.append_dev = self.append_host.cuda()
-        self.e_fork, self.e_app = torch.cuda.Event(), torch.cuda.Event()
+        self.e_mid = (torch.cuda.Event(), torch.cuda.Event())
+        self.e_app = (torch.cuda.Event(), torch.cuda.Event())
+        self.k, self.primed = 0, False
         torch.cuda.synchronize()
 
     def _pool(self, nb):
@@ -290,42 +295,55 @@ class Workload:
         return raw, llx.pool_wrap(raw.data_ptr(), nbytes, g["layers"], g["kv_heads"], g["head_dim"], g["block_size"],
                                   llx.F16, nb, keepalive=raw)
 
+    def reset_fork(self):
+        """The next step forks its decode-stream work from the migration stream AT ITS START (first step of a timed region)."""
+        self.primed = False
+
     def step(self, stream, dec=None, ev=None):
-        """One pass of the path: stage 0, append, stage 1, append, final stage.
+        """One pass of the path over the next request: stage 0, append, stage 1, append, final stage.
         dec is None: everything on `stream`, in that order.  Otherwise the appends run on the decode stream `dec`
-        (forked from `stream` at the start of the step, so they stay inside the timed region) concurrently with
-        stages 0 and 1, which do not read the appended block; the final stage, which does, waits for them.
-        ev: optional {name: (start, end)} timing events around the kernels "stage0", "stage1", "final" (on `stream`)
-        and "appends" (on the stream the appends run on)."""
+        concurrently with stages 0 and 1, which do not read the appended block; the final stage, which does, waits for
+        them (e_app).  Ordering of the decode stream against the migration stream: the appends of step k start after the
+        event e_mid(k-1), recorded on the migration stream just before the final stage of step k-1 — i.e. after the final
+        stage of step k-2, the last reader of THIS request's tail block (steps alternate between two requests).  The wait
+        and the record share one stream boundary, so stage 0 -> stage 1 and final -> next stage 0 stay adjacent kernels
+        (programmatic dependent launch).  The first step of a timed region forks at its own start instead (reset_fork).
+        ev: optional {name: (start, end)} timing events around "stage0", "stage1", "final" (on `stream`) and "appends"."""
         llx, g = self.llx, self.g
+        r = self.k % 2
+        s_tab, d_tab = self.s_tabs[r], self.d_tabs[r]
         tokens, m = START_TOKENS, 0
         vptr = self.append_dev.data_ptr()
         tok_bytes = g["layers"] * 2 * g["kv_heads"] * g["head_dim"] * 2
         names = ("stage0", "stage1", "final")
         if dec is not None:
-            self.e_fork.record(stream)
-            dec.wait_event(self.e_fork)
+            if not self.primed:
+                self.e_mid[1 - r].record(stream)
+                self.primed = True
+            dec.wait_event(self.e_mid[1 - r])
             if ev is not None and "appends" in ev:
                 ev["appends"][0].record(dec)
-            for k, a in enumerate(APPENDS):
-                llx.append_tokens(self.src, self.s_tab, tokens, tokens + a, vptr + (tokens - START_TOKENS) * tok_bytes, stream=dec)
+            for a in APPENDS:
+                llx.append_tokens(self.src, s_tab, tokens, tokens + a, vptr + (tokens - START_TOKENS) * tok_bytes, stream=dec)
                 tokens += a
             if ev is not None and "appends" in ev:
                 ev["appends"][1].record(dec)
-            self.e_app.record(dec)
+            self.e_app[r].record(dec)
         for k, n in enumerate(SCHEDULE):
             if dec is not None and k == len(SCHEDULE) - 1:
-                stream.wait_event(self.e_app)              # the final stage reads the block the appends wrote
+                stream.wait_event(self.e_app[r])           # the final stage reads the block the appends wrote
+                self.e_mid[r].record(stream)               # the next step's appends (other request) may start from here
             if ev is not None and names[k] in ev:
                 ev[names[k]][0].record(stream)
-            llx.migrate_stage(self.src, self.s_tab[m:m + n], self.dst, self.d_tab[m:m + n], stream=stream)
+            llx.migrate_stage(self.src, s_tab[m:m + n], self.dst, d_tab[m:m + n], stream=stream)
             if ev is not None and names[k] in ev:
                 ev[names[k]][1].record(stream)
             m += n
             if dec is None and k < len(APPENDS):
-                llx.append_tokens(self.src, self.s_tab, tokens, tokens + APPENDS[k],
+                llx.append_tokens(self.src, s_tab, tokens, tokens + APPENDS[k],
                                   vptr + (tokens - START_TOKENS) * tok_bytes, stream=stream)
                 tokens += APPENDS[k]
+        self.k += 1
         return tokens
 
 
@@ -369,6 +387,7 @@ def run_llx(args):
     torch.cuda.synchronize()
     c0 = llx.counters()
     tw0 = time.perf_counter()
+    w.reset_fork()
     e0.record(stream)
     for k in range(args.steps):
         w.step(stream, dec)
@@ -486,7 +505,10 @@ def run_llx(args):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u16", "data": "synthetic",
         "config": {"workload": WORKLOAD, "shape": "L32 H32 D128 S16 fp16, 2 pools x 2000 blocks (15.6 GiB each)",
-                   "request": "128 scattered blocks (2048 tokens), stages 112/14/2, 8-token appends between stages",
+                   "request": "128 scattered blocks (2048 tokens), stages 112/14/2, 8-token appends between stages; "
+                              "consecutive steps migrate two such requests alternately",
+                   "streams": ("copies on the migration stream, appends on the source's decode stream (PAPER.md:134, :235); the final "
+                               "stage waits for the appends" if dec is not None else "everything on one stream (--serial-appends)"),
                    "bytes_per_step_rd_plus_wr": step_bytes(g), "parallelism": f"replicas x{world} (no collective)",
                    "l2": "inputs larger than L2 (2.1 GB of traffic per step vs 126 MB L2), no flush needed",
                    "copy_kernel": "bulk-async smem ring (llx_copy_bulk)" if llx.get_option(llx.OPT_COPY_KERNEL) in (0, 2) else "vec16"},

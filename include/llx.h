@@ -103,6 +103,19 @@ int    llx_pool_num_blocks(const llx_pool* pool);
 /* Bytes a pool of this geometry needs (for sizing memory passed to llx_pool_wrap); 0 on bad args. */
 size_t llx_pool_bytes_for(int layers, int kv_heads, int head_dim, int block_size, llx_dtype dtype, int num_blocks);
 
+/* The destination instance as ANOTHER PROCESS (instances are separate actors; here one process per
+ * GPU / per instance): the owner of a library-allocated pool exports a handle (LLX_IPC_HANDLE_BYTES opaque bytes, sent
+ * to the peer by whatever channel the caller has), the peer opens it and gets a pool that names the SAME device memory.
+ * llx_migrate_stage / _batch into an opened pool then store straight into the other process's KV cache — on the same GPU
+ * (two instances sharing one device) or on another one (the mapping enables peer access; the copy takes the cross-GPU
+ * route).  The handle carries the pool's geometry, so the opened pool cannot disagree with the exporter's.
+ * llx_pool_destroy of an opened pool unmaps it; the exporter must keep its pool alive meanwhile.  Only pools from
+ * llx_pool_create can be exported (the handle names a whole allocation); LLX_ERR_CUDA when the handle is opened in the
+ * process that exported it (the driver refuses that). */
+#define LLX_IPC_HANDLE_BYTES 96
+llx_status llx_pool_ipc_export(const llx_pool* pool, void* handle_out);
+llx_status llx_pool_ipc_open(const void* handle, llx_pool** out);
+
 /* Plain stream-ordered copies between HOST memory and n_blocks consecutive tiles
  * pool[layer][kv][first_block ...]: how the owner of a library-allocated pool fills and
  * inspects it.  `host` holds n_blocks*tile_bytes bytes; pinned memory makes them truly async. */
@@ -404,10 +417,11 @@ typedef enum {
                                    shared-memory carve-out, in % of the SM's maximum, of the register-staged copy kernel that
                                    serves bandwidth budgets below 500 GB/s and the host zero-copy / peer routes.  That kernel
                                    keeps a small CTA resident on every SM for the whole stage, and an SM cannot change its
-                                   L1/shared split while a CTA is resident: with the driver's default (0) a co-running kernel
-                                   that needs shared memory waits for the end of the stage.  Default 75 (196 KB shared, 60 KB
-                                   L1): every llx kernel co-runs, the stand-in decode step loses nothing.  100: no kernel ever
-                                   waits, L1-hungry co-runners lose ~20 % */
+                                   L1/shared split while a CTA is resident: a co-running kernel that needs more shared memory
+                                   than the split offers waits for the END of the stage.  Default 50 (132 KB shared / 124 KB
+                                   L1): every llx kernel co-runs and the stand-in decode step loses nothing (measured; 75 costs
+                                   it +5 %, 100 +30 %).  0 = the driver's choice ("all L1").  100: not even a kernel that needs
+                                   the whole 227 KB ever waits */
     LLX_OPT_VIA_HOST_MODE = 11  /* llx_pack / llx_unpack / llx_migrate_via_host with a pinned-host buffer: 0 (default) copy engines
                                    through device bounce buffers; 1 the kernels address the host buffer directly (zero-copy) */
 } llx_option;

@@ -74,6 +74,8 @@ EXPORTS = {
     "llx_pool_bytes": (_sz, [_vp]),
     "llx_pool_num_blocks": (_i, [_vp]),
     "llx_pool_bytes_for": (_sz, [_i, _i, _i, _i, _i, _i]),
+    "llx_pool_ipc_export": (_i, [_vp, _vp]),
+    "llx_pool_ipc_open": (_i, [_vp, C.POINTER(_vp)]),
     "llx_pool_upload": (_i, [_vp, _i, _i, _i, _i, _vp, _vp]),
     "llx_pool_download": (_i, [_vp, _i, _i, _i, _i, _vp, _vp]),
     "llx_pool_fill_u16": (_i, [_vp, C.c_uint16, _vp]),
@@ -237,6 +239,24 @@ def pool_wrap(dev_ptr: int, nbytes: int, layers, kv_heads, head_dim, block_size,
     h = _vp()
     _check(load().llx_pool_wrap(dev_ptr, nbytes, layers, kv_heads, head_dim, block_size, dtype, num_blocks, C.byref(h)))
     return Pool(h.value, keepalive)
+
+
+IPC_HANDLE_BYTES = 96
+
+
+def pool_ipc_export(pool: Pool) -> bytes:
+    """Handle of a library-allocated pool for another process (llx_pool_ipc_export): send the bytes, open them there."""
+    buf = C.create_string_buffer(IPC_HANDLE_BYTES)
+    _check(load().llx_pool_ipc_export(pool.handle, buf))
+    return buf.raw
+
+
+def pool_ipc_open(handle: bytes) -> Pool:
+    if len(handle) != IPC_HANDLE_BYTES:
+        raise LlxError(-1, "LLX_ERR_INVALID_ARG", "an llx pool handle has %d bytes" % IPC_HANDLE_BYTES)
+    h = _vp()
+    _check(load().llx_pool_ipc_open(C.c_char_p(handle), C.byref(h)))
+    return Pool(h.value)
 
 
 def plan_stage(num_tokens: int, blocks_migrated: int, block_size: int, last_stage_max_blocks: int):

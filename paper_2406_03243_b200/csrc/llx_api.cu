@@ -27,6 +27,7 @@ struct llx_pool {
     long long tile_bytes = 0;
     int device = 0;
     bool owned = false;
+    bool ipc_mapped = false;  // data comes from cudaIpcOpenMemHandle: destroy unmaps it
     // decode-attention workspace (grows on demand)
     float* attn_ws = nullptr;
     size_t attn_ws_bytes = 0;
@@ -66,7 +67,7 @@ int elem_bytes_of(llx_dtype d) {
 
 // ---- options / counters -------------------------------------------------------------------
 std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
-    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1}, g_opt_carveout{75};
+    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1}, g_opt_carveout{50};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
 // Range of every option: shared by llx_set_option (process defaults) and by the per-call llx_launch_opts.
@@ -191,14 +192,8 @@ llx_status dev_info(int dev, DevInfo** out, bool capturing = false) {
         LLX_CUDA(cudaFuncSetAttribute(llx_copy_bulk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
         d.ready = true;
     }
-    // Shared-memory carve-out of the register-staged copy kernel (the paced copy of NEXT-1, the host zero-copy and peer
-    // routes).  Its CTAs hold no shared memory but stay resident on EVERY SM for a whole stage (75 ms for 112 blocks at
-    // 25 GB/s), and an SM cannot change its L1/shared split while a CTA is resident: arriving on idle SMs with the
-    // driver's default preference they pin the split at "all L1", and every kernel that needs shared memory — the bulk
-    // ring of another request's final stage, a GEMM — then waits for the END OF THE STAGE on that SM (measured on B200: a
-    // 2-block final stage next to a 25 GB/s stage: median 53 us, p90 75 ms; with a preference of 64-75 % never above
-    // 0.14 ms; 87-100 % costs the L1-hungry stand-in decode attention +20-25 %, 75 % costs it nothing).  75 % asks for the
-    // 196 KB split: every llx kernel fits beside it (final stage 2 x 76 KB, long stage 113 KB) and 60 KB of L1 remain.
+    // Shared-memory carve-out preference of the register-staged copy kernel (LLX_OPT_COPY_SMEM_CARVEOUT_PCT; see the
+    // co-residency note at paced_in_flight below).  0 = the driver's default.
     const int want_carveout = (int)g_opt_carveout.load();
     if (d.carveout_applied != want_carveout && !capturing) {
         const int v = want_carveout > 0 ? want_carveout : cudaSharedmemCarveoutDefault;
@@ -300,6 +295,67 @@ llx_status dyn_counter_get(int dev, cudaStream_t st, unsigned int** counter) {
     }
     *counter = g_dyn_counters[dev] + it->second;
     return LLX_OK;
+}
+
+// ---- co-residency of the register-staged copy kernel -----------------------------------------------------------
+// The register-staged kernel (paced copies of NEXT-1, host zero-copy and peer routes) holds no shared memory, but its
+// small CTAs stay resident on EVERY SM for a whole stage (75 ms for 112 blocks at 25 GB/s), and an SM cannot change its
+// L1/shared-memory split while any CTA is resident.  Whatever split an SM has when such a CTA arrives is pinned until
+// the END OF THE STAGE, and a kernel that needs more shared memory than that split offers waits that long.  Measured on
+// B200 with the driver's default preference ("all L1" for a kernel without shared memory): a 2-block final stage (bulk
+// ring, 2 x 76 KB of shared memory) next to a 25 GB/s stage: median 53 us, p90 75 ms; a 4096^3 bf16 GEMM: up to 75 ms.
+// Two measures:
+//  (1) the kernel asks for a 50 % carve-out (LLX_OPT_COPY_SMEM_CARVEOUT_PCT): arriving on idle SMs it leaves 132 KB of
+//      shared memory configured, enough for every llx kernel (final stage 76 KB per CTA, long stage 113 KB), and 124 KB of
+//      L1, which costs the L1-hungry stand-in decode step nothing (20 GB/s: +0.7 %; 64 %: +1.3 %, 75 %: +4.9 %, 100 %: +30 %);
+//  (2) SMs that were busy with shared-memory-free kernels when the stage arrived keep "all L1" all the same, so the library
+//      remembers the register-staged launches that may still be running (one event each) and, while any is, sends its own
+//      auto-selected copies through the register-staged kernel too: no shared memory, placed at once (a short stage takes
+//      the same time: 23.3 vs 23.6 us; a long one runs at 5.6 instead of 6.5 TB/s next to the budgeted stage).
+// Kernels of OTHER libraries that need more than 131 KB of shared memory can still wait for the end of a budgeted stage;
+// a preference of 100 removes that at the decode step's expense.
+struct PacedTracker {
+    std::mutex mu;
+    static constexpr int kSlots = 16;
+    cudaEvent_t ev[kSlots] = {};
+    bool live[kSlots] = {};
+    int next = 0;
+};
+PacedTracker g_paced[64];
+
+bool paced_in_flight(int dev) {
+    PacedTracker& t = g_paced[dev];
+    std::lock_guard<std::mutex> lk(t.mu);
+    bool any = false;
+    for (int i = 0; i < PacedTracker::kSlots; ++i) {
+        if (!t.live[i]) continue;
+        const cudaError_t q = cudaEventQuery(t.ev[i]);
+        if (q == cudaErrorNotReady) {
+            any = true;
+        } else {
+            if (q != cudaSuccess) cudaGetLastError();
+            t.live[i] = false;
+        }
+    }
+    return any;
+}
+void paced_mark(int dev, cudaStream_t st) {
+    PacedTracker& t = g_paced[dev];
+    std::lock_guard<std::mutex> lk(t.mu);
+    int slot = -1;
+    for (int i = 0; i < PacedTracker::kSlots && slot < 0; ++i)
+        if (!t.live[i]) slot = i;
+    if (slot < 0) {  // all in use: the oldest is given up (it is then no longer tracked)
+        slot = t.next;
+        t.next = (t.next + 1) % PacedTracker::kSlots;
+    }
+    if (!t.ev[slot] && cudaEventCreateWithFlags(&t.ev[slot], cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        t.ev[slot] = nullptr;
+        return;
+    }
+    t.live[slot] = cudaEventRecord(t.ev[slot], st) == cudaSuccess;
+    if (!t.live[slot]) cudaGetLastError();
 }
 
 // ---- completion flags of llx_migrate_stage_wait: a word in mapped pinned host memory that the kernel's last
@@ -423,6 +479,9 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     // 400 GB/s paced but 0.045 % at 800 and 0.060 % at 2400, while a FEW full-speed bulk CTAs stay at 0.023-0.030 %
     // (about 60 GB/s per CTA: 7 CTAs 447 GB/s, 14: 864, 29: 1623, 43: 2243).  High budgets are therefore met by the
     // CTA count of the unpaced bulk kernel, low ones by the paced kernel.
+    // while a register-staged stage may be resident on every SM, auto-selected copies avoid shared memory (see paced_in_flight)
+    const bool beside_paced = pol.kernel == 0 && kern == 2 && !capturing && paced_in_flight(device);
+    if (beside_paced) kern = 1;
     const long long budget_asked = pol.budget;
     const bool budget_by_ctas = budget_asked >= 500 && pol.kernel == 0 && kern == 2;
     const long long budget = budget_by_ctas ? 0 : budget_asked;  // from here on: > 0 means "paced"
@@ -612,6 +671,8 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     const llx_status rc_ring = ring_close(slot, st);
     if (e != cudaSuccess) return cuda_fail(e, "copy kernel launch");
     if (rc_ring != LLX_OK) return rc_ring;
+    // a register-staged stage that will be resident for a while (every paced one; unpaced ones from 8 MiB): remember it
+    if (kern == 1 && !capturing && (budget > 0 || total_bytes >= (8ll << 20))) paced_mark(device, st);
     g_launches++;
     g_copy_launches++;
     g_bytes += (unsigned long long)total_bytes;
@@ -810,9 +871,60 @@ llx_status llx_pool_wrap(void* dev_ptr, size_t bytes, int layers, int kv_heads, 
                          llx_dtype dtype, int num_blocks, llx_pool** out) {
     return make_pool(dev_ptr, bytes, false, layers, kv_heads, head_dim, block_size, dtype, num_blocks, out);
 }
+struct IpcHandle {  // LLX_IPC_HANDLE_BYTES: the CUDA handle of the allocation + the pool's geometry
+    cudaIpcMemHandle_t mem;
+    uint32_t magic;
+    int32_t layers, kv_heads, head_dim, block_size, dtype, num_blocks;
+    uint32_t reserved;
+};
+static_assert(sizeof(IpcHandle) == LLX_IPC_HANDLE_BYTES, "LLX_IPC_HANDLE_BYTES must match IpcHandle");
+constexpr uint32_t kIpcMagic = 0x4C4C5831u;  // "LLX1"
+
+llx_status llx_pool_ipc_export(const llx_pool* p, void* handle_out) {
+    if (!p || !p->data || !handle_out) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
+    if (!p->owned) return fail(LLX_ERR_INVALID_ARG, "only a pool allocated by llx_pool_create can be exported (the handle names a whole allocation)");
+    IpcHandle h;
+    memset(&h, 0, sizeof h);
+    LLX_CUDA(cudaIpcGetMemHandle(&h.mem, p->data));
+    h.magic = kIpcMagic;
+    h.layers = p->layers;
+    h.kv_heads = p->kv_heads;
+    h.head_dim = p->head_dim;
+    h.block_size = p->block_size;
+    h.dtype = (int32_t)p->dtype;
+    h.num_blocks = p->num_blocks;
+    memcpy(handle_out, &h, sizeof h);
+    return LLX_OK;
+}
+
+llx_status llx_pool_ipc_open(const void* handle, llx_pool** out) {
+    if (!out) return fail(LLX_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!handle) return fail(LLX_ERR_INVALID_ARG, "handle is NULL");
+    IpcHandle h;
+    memcpy(&h, handle, sizeof h);
+    if (h.magic != kIpcMagic) return fail(LLX_ERR_INVALID_ARG, "not an llx pool handle");
+    const size_t need = llx_pool_bytes_for(h.layers, h.kv_heads, h.head_dim, h.block_size, (llx_dtype)h.dtype, h.num_blocks);
+    if (need == 0) return fail(LLX_ERR_INVALID_ARG, "handle carries a bad geometry");
+    void* ptr = nullptr;
+    cudaError_t e = cudaIpcOpenMemHandle(&ptr, h.mem, cudaIpcMemLazyEnablePeerAccess);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(LLX_ERR_CUDA, "cudaIpcOpenMemHandle: %s", cudaGetErrorString(e));
+    }
+    llx_status rc = make_pool(ptr, need, false, h.layers, h.kv_heads, h.head_dim, h.block_size, (llx_dtype)h.dtype, h.num_blocks, out);
+    if (rc != LLX_OK) {
+        cudaIpcCloseMemHandle(ptr);
+        return rc;
+    }
+    (*out)->ipc_mapped = true;
+    return LLX_OK;
+}
+
 llx_status llx_pool_destroy(llx_pool* p) {
     if (!p) return LLX_OK;
     if (p->attn_ws) cudaFree(p->attn_ws);
+    if (p->ipc_mapped && p->data) cudaIpcCloseMemHandle(p->data);
     if (p->owned && p->data) cudaFree(p->data);
     delete p;
     return LLX_OK;
