@@ -605,9 +605,10 @@ def ncu_targets(torch, llx, stream):
       1 llx_copy_bulk   LLaMA-30B batch, 64 requests / 1023 blocks in ONE launch (208 KiB tiles)
       2 llx_copy_bulk   llx_pack of a 2048-token 7B request into a DEVICE buffer          3 llx_copy_bulk  llx_unpack of it
       4 llx_copy_vec16  paced stage, 25 GB/s budget (16 blocks of 7B)                     5 llx_copy_vec16 paced, 400 GB/s
-      6 llx_copy_bulk   long stage of Tiny-shaped 8 KiB tiles (1100 blocks, 68.75 MiB)
+      6 llx_copy_bulk   long stage of Tiny-shaped 8 KiB tiles (4000 blocks, 250 MiB: larger than L2)
       7 llx_copy_bulk   the final stage: 2 blocks of 7B (cold: a 512 MiB fill runs before it)
       8 llx_copy_vec16  peer route of a 2048-token 7B request on one device
+      9 llx_copy_vec16  zero-copy llx_pack into pinned host memory (16 blocks)           10 llx_copy_vec16 zero-copy llx_unpack
     and prints the order so that the launch list can be labelled."""
     out = []
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
@@ -640,11 +641,16 @@ def ncu_targets(torch, llx, stream):
     twice("paced_25GBps_16_blocks", lambda: llx.migrate_stage(p7.src, s7[:16], p7.dst, d7[:16], stream=stream, opts=dict(bandwidth_gbps=25)))
     twice("paced_400GBps_16_blocks", lambda: llx.migrate_stage(p7.src, s7[:16], p7.dst, d7[:16], stream=stream, opts=dict(bandwidth_gbps=400)))
     gt = dict(synth.CONFIGS["tiny"])
-    pt = Pools(torch, llx, gt, 1200, 1200)
-    st_, dt_ = synth.block_permutation(1, 1200)[:1100], synth.block_permutation(2, 1200)[:1100]
-    twice("tiny_tiles_8KiB_1100_blocks", lambda: llx.migrate_stage(pt.src, st_, pt.dst, dt_, stream=stream))
+    pt = Pools(torch, llx, gt, 4200, 4200)        # 4000 blocks = 250 MiB read + 250 MiB written: twice the 126 MB L2
+    st_, dt_ = synth.block_permutation(1, 4200)[:4000], synth.block_permutation(2, 4200)[:4000]
+    twice("tiny_tiles_8KiB_4000_blocks", lambda: llx.migrate_stage(pt.src, st_, pt.dst, dt_, stream=stream))
     twice("final_stage_2_blocks_cold", lambda: llx.migrate_stage(p7.src, s7[126:], p7.dst, d7[126:], stream=stream), cold=True)
     twice("peer_route_128_blocks", lambda: llx.migrate_stage(p7.src, s7, p7.dst, d7, stream=stream, opts=dict(route=llx.ROUTE_PEER)))
+    pin = llx.PinnedStaging(llx.staging_bytes(p7.src, 16))
+    zc = dict(via_host_mode=1)          # the kernel itself crosses the host link: the only host leg a kernel profiler can see
+    twice("pack_zero_copy_pinned_host_16_blocks", lambda: llx.pack(p7.src, s7[:16], pin.dev_alias, pin.nbytes, stream=stream, opts=zc))
+    twice("unpack_zero_copy_pinned_host_16_blocks", lambda: llx.unpack(pin.dev_alias, pin.nbytes, p7.dst, d7[:16], stream=stream, opts=zc))
+    pin.free()
     return {"order": out, "note": "each label = two consecutive launches of that shape; llx_fill / at:: kernels in between are input generation"}
 
 
