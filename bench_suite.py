@@ -555,6 +555,97 @@ def live_migration(torch, llx, stream_unused=None, budgets=(0, 100, 25), start_t
     return out
 
 
+# ---- NEXT-1, the other variant the row names: an SM partition (green contexts) instead of pacing -----------------------
+def green_partition(torch, llx, stream_unused=None, sm_counts=(8, 16)):
+    """The migration gets its own few SMs (CUDA green context: cuDevSmResourceSplitByCount), the decode step the rest;
+    inside its partition the migration runs unthrottled.  Paired slowdown of the configs[4] decode step, next to the
+    same measurement for a CTA-capped launch on plain streams (LLX_OPT_MAX_CTAS).  Needs cuda-python."""
+    try:
+        from cuda.bindings import driver as drv
+    except Exception as e:  # noqa: BLE001
+        return {"skipped": "cuda-python unavailable: " + repr(e)}
+
+    def ck(r):
+        if r[0] != drv.CUresult.CUDA_SUCCESS:
+            raise RuntimeError(str(r[0]))
+        return r[1:] if len(r) > 2 else (r[1] if len(r) == 2 else None)
+
+    g = dict(synth.CONFIGS["llama7b"])
+    L, H, D, S = g["layers"], g["kv_heads"], g["head_dim"], g["block_size"]
+    B, MB = 32, 256
+    ctx = synth.context_lengths(4, B, 128, 4096)
+    need = [-(-int(c) // S) for c in ctx]
+    nb_src, nb_dst = B * 256 + 256, g["num_blocks"]
+    if (nb_src + nb_dst) * 2 * L * S * H * D * 2 > _free(torch) - (4 << 30):
+        return {"skipped": "not enough device memory"}
+    p = Pools(torch, llx, g, nb_src, nb_dst)
+    perm = synth.block_permutation(6, nb_src)
+    bt = np.zeros((B, MB), dtype=np.int32)
+    pos = 0
+    for b, n in enumerate(need):
+        bt[b, :n] = perm[pos:pos + n]
+        pos += n
+    mig_src, mig_dst = perm[pos:pos + 128], synth.block_permutation(2, nb_dst)[:128]
+    q = torch.from_numpy(synth.queries_f16(5, B, H, D).view(np.int16)).cuda()
+    o = torch.zeros_like(q)
+    d_bt, d_ctx = torch.from_numpy(bt).cuda(), torch.from_numpy(ctx).cuda()
+    scale = 1.0 / float(np.sqrt(D))
+    mig_bytes = 2 * 128 * p.src.block_bytes
+
+    def case(s_dec, s_mig, opts, n_mig):
+        def one(nm):
+            torch.cuda.synchronize()
+            a, b_, ma, mb = (torch.cuda.Event(enable_timing=True) for _ in range(4))
+            a.record(s_dec)
+            ma.record(s_mig)
+            for _ in range(nm):
+                llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=opts)
+            mb.record(s_mig)
+            for l in range(L):
+                llx.decode_attention(p.src, l, q.data_ptr(), o.data_ptr(), d_bt.data_ptr(), d_ctx.data_ptr(), B, MB, scale, stream=s_dec)
+            b_.record(s_dec)
+            torch.cuda.synchronize()
+            return a.elapsed_time(b_), ma.elapsed_time(mb)
+        for _ in range(3):
+            one(0)
+        ratios, mig_ms = [], []
+        for _ in range(8):
+            t0, _ = one(0)
+            t1, m = one(n_mig)
+            ratios.append(t1 / t0)
+            mig_ms.append(m)
+        return {"decode_slowdown_pct": 100.0 * (statistics.median(ratios) - 1.0),
+                "migration_GBps": n_mig * mig_bytes / statistics.median(mig_ms) / 1e6 if n_mig else 0.0}
+
+    res = {"cases": []}
+    lo, hi = torch.cuda.Stream.priority_range()
+    sd, sm = torch.cuda.Stream(priority=hi), torch.cuda.Stream(priority=lo)
+    for c in sm_counts:
+        r = case(sd, sm, dict(max_ctas=c), 8)
+        res["cases"].append(dict(r, case=f"plain streams, {c} full-speed CTAs (LLX_OPT_MAX_CTAS)"))
+    dev = ck(drv.cuDeviceGet(torch.cuda.current_device()))
+    sm_res = ck(drv.cuDeviceGetDevResource(dev, drv.CUdevResourceType.CU_DEV_RESOURCE_TYPE_SM))
+    res["device_sms"] = int(sm_res.sm.smCount)
+    for c in sm_counts:
+        try:
+            groups, _, remaining = ck(drv.cuDevSmResourceSplitByCount(1, sm_res, 0, c))
+            streams = []
+            for part in (groups[0], remaining):
+                desc = ck(drv.cuDevResourceGenerateDesc([part], 1))
+                gctx = ck(drv.cuGreenCtxCreate(desc, dev, drv.CUgreenCtxCreate_flags.CU_GREEN_CTX_DEFAULT_STREAM))
+                streams.append(torch.cuda.ExternalStream(int(ck(drv.cuGreenCtxStreamCreate(gctx, drv.CUstream_flags.CU_STREAM_NON_BLOCKING, 0)))))
+        except Exception as e:  # noqa: BLE001
+            res["cases"].append({"case": f"green context with {c} SMs", "skipped": repr(e)})
+            continue
+        r = case(streams[1], streams[0], None, 8)
+        res["cases"].append(dict(r, case=f"green contexts: {int(groups[0].sm.smCount)} SMs migrate at full speed, {int(remaining.sm.smCount)} SMs decode"))
+        r = case(streams[1], streams[0], None, 0)
+        res["cases"].append(dict(r, case=f"green contexts: decode alone on its {int(remaining.sm.smCount)} SMs, paired with itself (floor)"))
+    del p
+    _free(torch)
+    return res
+
+
 # ---- NEXT-2 / SURVEY 8(e): tensor-parallel rank shards of LLaMA-30B (52 heads = 4 ranks x 13 -> 52 KiB tiles) ----------
 def tp_shard_30b(torch, llx, stream_unused=None, tp=4, n=128, nb=700):
     """Rank r of the source instance migrates to rank r of the destination, no exchange between ranks (PAPER.md:235,
@@ -605,7 +696,7 @@ def ncu_targets(torch, llx, stream):
       1 llx_copy_bulk   LLaMA-30B batch, 64 requests / 1023 blocks in ONE launch (208 KiB tiles)
       2 llx_copy_bulk   llx_pack of a 2048-token 7B request into a DEVICE buffer          3 llx_copy_bulk  llx_unpack of it
       4 llx_copy_vec16  paced stage, 25 GB/s budget (16 blocks of 7B)                     5 llx_copy_vec16 paced, 400 GB/s
-      6 llx_copy_bulk   long stage of Tiny-shaped 8 KiB tiles (4000 blocks, 250 MiB: larger than L2)
+      6 llx_copy_bulk   long stage of Tiny-shaped 8 KiB tiles (8000 blocks, 250 MiB: larger than L2)
       7 llx_copy_bulk   the final stage: 2 blocks of 7B (cold: a 512 MiB fill runs before it)
       8 llx_copy_vec16  peer route of a 2048-token 7B request on one device
       9 llx_copy_vec16  zero-copy llx_pack into pinned host memory (16 blocks)           10 llx_copy_vec16 zero-copy llx_unpack
@@ -641,9 +732,9 @@ def ncu_targets(torch, llx, stream):
     twice("paced_25GBps_16_blocks", lambda: llx.migrate_stage(p7.src, s7[:16], p7.dst, d7[:16], stream=stream, opts=dict(bandwidth_gbps=25)))
     twice("paced_400GBps_16_blocks", lambda: llx.migrate_stage(p7.src, s7[:16], p7.dst, d7[:16], stream=stream, opts=dict(bandwidth_gbps=400)))
     gt = dict(synth.CONFIGS["tiny"])
-    pt = Pools(torch, llx, gt, 4200, 4200)        # 4000 blocks = 250 MiB read + 250 MiB written: twice the 126 MB L2
-    st_, dt_ = synth.block_permutation(1, 4200)[:4000], synth.block_permutation(2, 4200)[:4000]
-    twice("tiny_tiles_8KiB_4000_blocks", lambda: llx.migrate_stage(pt.src, st_, pt.dst, dt_, stream=stream))
+    pt = Pools(torch, llx, gt, 8400, 8400)        # 8000 blocks of 32 KiB = 250 MiB read + 250 MiB written: twice the 126 MB L2
+    st_, dt_ = synth.block_permutation(1, 8400)[:8000], synth.block_permutation(2, 8400)[:8000]
+    twice("tiny_tiles_8KiB_8000_blocks", lambda: llx.migrate_stage(pt.src, st_, pt.dst, dt_, stream=stream))
     twice("final_stage_2_blocks_cold", lambda: llx.migrate_stage(p7.src, s7[126:], p7.dst, d7[126:], stream=stream), cold=True)
     twice("peer_route_128_blocks", lambda: llx.migrate_stage(p7.src, s7, p7.dst, d7, stream=stream, opts=dict(route=llx.ROUTE_PEER)))
     pin = llx.PinnedStaging(llx.staging_bytes(p7.src, 16))
@@ -670,11 +761,12 @@ def run(torch, llx, stream):
     res["batch_llama30b_64req"] = batch_30b(torch, llx, stream)
     res["batch_llama30b_64req_seed2_mean507"] = batch_30b(torch, llx, stream, seed=2)
     res["tp4_rank_shards_llama30b"] = tp_shard_30b(torch, llx, stream)
+    res["sm_partition_green_contexts"] = green_partition(torch, llx, stream)
     return res
 
 
 def main():
-    """python bench_suite.py [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch | batch2 | tp)"""
+    """python bench_suite.py [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch | batch2 | tp | green | ncu_targets)"""
     import argparse
     import json
 
@@ -683,8 +775,12 @@ def main():
     import paper_2406_03243_b200 as llx
     ap = argparse.ArgumentParser()
     ap.add_argument("--only", default="")
+    ap.add_argument("--carveout", type=int, default=-1,
+                    help="LLX_OPT_COPY_SMEM_CARVEOUT_PCT for this run (the sweep behind its default: 0, 50, 64, 75, 100)")
     args = ap.parse_args()
     llx.load()
+    if args.carveout >= 0:
+        llx.set_option(llx.OPT_COPY_SMEM_CARVEOUT_PCT, args.carveout)
     stream = torch.cuda.Stream()
     if not args.only:
         print(json.dumps(run(torch, llx, stream), indent=1))
@@ -703,6 +799,8 @@ def main():
         res = batch_30b(torch, llx, stream, seed=2)
     elif args.only == "tp":
         res = tp_shard_30b(torch, llx, stream)
+    elif args.only == "green":
+        res = green_partition(torch, llx, stream)
     elif args.only == "ncu_targets":
         res = ncu_targets(torch, llx, stream)
     else:
