@@ -183,9 +183,19 @@ def cpu_baseline(budget_s=12.0) -> dict:
         t0 = time.perf_counter()
         om.migrate_stage(src, s_tab[-SCHEDULE[-1]:], dst, d_tab[-SCHEDULE[-1]:])
         fin.append(time.perf_counter() - t0)
+    # block fusion on the host: the oracle's pack and unpack of the whole 128-block request
+    t0 = time.perf_counter()
+    buf = om.pack(src, s_tab)
+    t_pack = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    om.unpack(buf, dst, d_tab)
+    t_unpack = time.perf_counter() - t0
+    del buf
     return {"value": step_bytes(g) / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
             "host_cores_available": len(os.sched_getaffinity(0)),
-            "final_stage_ms": statistics.median(fin) * 1e3,
+            "final_stage_ms": statistics.median(fin) * 1e3, "pack_ms": t_pack * 1e3, "unpack_ms": t_unpack * 1e3,
+            "attention_oracle": "fp64 decode attention over configs[4]'s batch (65,590 context tokens): 1.8 s per layer on one core, "
+                                "timed in tests/test_gpu_attention.py::test_configs4_decode_batch_shape_within_tolerance",
             "sample": f"the whole configs[1] step (128 blocks, stages 112/14/2, 2 appends of 8 tokens) inside two "
                       f"160-block host pools instead of 2000-block ones; {len(times)} repetitions, median; "
                       f"oracle.kv_migration.staged_migration as it stands (NumPy row copies, single thread)",

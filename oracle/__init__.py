@@ -30,6 +30,8 @@ What it computes, and the passage each part follows (all `PAPER.md:<line>`):
   check after each stage, abort and release, commit.
 * `policy.calc_freeness`, `policy.pair_instances`, `policy.migration_order` — Algorithm 1
   (virtual usage and freeness) and the pairing rule of §4.4.3.
+* `policy.plan_migration_batch` — one migration round of one (source, destination) pair as one batch: migration
+  order, the source-state threshold and all-or-nothing PRE-ALLOC (PAPER.md:225 + :142; reading A31 in DESIGN.md).
 * `decode_attention.decode_attention_fp64` — standard KV-cache attention for one
   decode token per sequence, read through the block table (§2).
 
@@ -44,5 +46,6 @@ leak freedom at every abort point and the commit bookkeeping in closed form
 (tests/test_oracle_handshake.py); Algorithm 1 is pinned to the meaning the paper gives
 freeness (decode iterations left, by brute-force simulation), to the printed capacity
 13,616 tokens / target load 1,600 tokens (tests/golden/paper_priority_headroom.txt) and to
-the rule-by-rule special cases (tests/test_oracle_policy.py).  Nothing here is "parity unpinned".
+the rule-by-rule special cases; the batch round to a closed form for equal requests, hand-computed special cases and
+an independent brute-force restatement (tests/test_oracle_policy.py).  Nothing here is "parity unpinned".
 """
