@@ -117,6 +117,44 @@ def length_sweep(torch, llx, p: Pools, stream, nb):
     return out
 
 
+# ---- the latency floor under the final stage -------------------------------------------------------
+def latency_floor(torch, llx, p: Pools, stream, nb):
+    """What one launch + one synchronize cost on this box when the copy itself is negligible: a 1-block stage of a
+    Tiny-shaped pool (32 KiB payload) through the same entry point, next to the 2-block final stage of the 7B shape.
+    Host wall clock (enqueue -> synchronize returns) and CUDA-event time, 300 repetitions each."""
+    import ctypes as C
+    lib = llx.lib()
+    gt = dict(synth.CONFIGS["tiny"])
+    pt = Pools(torch, llx, gt, 64, 64)
+    out = {}
+    for label, pools, n in (("tiny_1_block_32KiB", pt, 1), ("llama7b_2_blocks_16MiB", p, 2)):
+        s_ids = np.ascontiguousarray(synth.block_permutation(7, pools.src.num_blocks)[:n], dtype=np.int32)
+        d_ids = np.ascontiguousarray(synth.block_permutation(8, pools.dst.num_blocks)[:n], dtype=np.int32)
+        sp, dp = s_ids.ctypes.data_as(C.POINTER(C.c_int32)), d_ids.ctypes.data_as(C.POINTER(C.c_int32))
+        host, enq, gpu = [], [], []
+        ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for rep in range(320):
+            stream.synchronize()
+            t0 = time.perf_counter_ns()
+            lib.llx_migrate_stage(pools.src.handle, sp, pools.dst.handle, dp, n, stream.cuda_stream)
+            t1 = time.perf_counter_ns()
+            stream.synchronize()
+            t2 = time.perf_counter_ns()
+            ea.record(stream)
+            lib.llx_migrate_stage(pools.src.handle, sp, pools.dst.handle, dp, n, stream.cuda_stream)
+            eb.record(stream)
+            stream.synchronize()
+            if rep >= 20:
+                host.append((t2 - t0) / 1e3)
+                enq.append((t1 - t0) / 1e3)
+                gpu.append(ea.elapsed_time(eb) * 1e3)
+        out[label] = {"host_us_median": statistics.median(host), "enqueue_us_median": statistics.median(enq),
+                      "sync_us_median": statistics.median(host) - statistics.median(enq), "gpu_event_us_median": statistics.median(gpu)}
+    out["note"] = ("the 32 KiB stage moves nothing worth timing: its numbers are the floor of one launch + one synchronize through this "
+                   "entry point; the final stage's excess over it is the copy itself")
+    return out
+
+
 # ---- reference points on the same data (SURVEY.md §8(d)) ---------------------------------------
 def reference_points(torch, llx, p: Pools, stream, nb):
     n = 128
@@ -751,6 +789,7 @@ def run(torch, llx, stream):
     nb = g["num_blocks"]
     p = Pools(torch, llx, g, nb, nb)
     res["length_sweep_llama7b"] = length_sweep(torch, llx, p, stream, nb)
+    res["latency_floor"] = latency_floor(torch, llx, p, stream, nb)
     res["reference_points_2048tok"] = reference_points(torch, llx, p, stream, nb)
     res["staging_pinned_host_2048tok"] = staging_host(torch, llx, p, stream, nb)
     del p
@@ -766,7 +805,7 @@ def run(torch, llx, stream):
 
 
 def main():
-    """python bench_suite.py [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch | batch2 | tp | green | ncu_targets)"""
+    """python bench_suite.py [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch | batch2 | tp | green | floor | ncu_targets)"""
     import argparse
     import json
 
@@ -805,7 +844,7 @@ def main():
         res = ncu_targets(torch, llx, stream)
     else:
         p = Pools(torch, llx, g, nb, nb)
-        fn = {"sweep": length_sweep, "refs": reference_points, "staging": staging_host}[args.only]
+        fn = {"sweep": length_sweep, "refs": reference_points, "staging": staging_host, "floor": latency_floor}[args.only]
         res = fn(torch, llx, p, stream, nb)
     print(json.dumps(res, indent=1))
     return 0
