@@ -98,7 +98,6 @@ bool opt_valid(int opt, long long v) {
 struct Policy {
     long long kernel, max_ctas, chunk, stages, byval, order, l2hint, rings, pdl, budget, via_host, dyn_pct, dyn_batch, smem_pad;
     int route;
-    bool kernel_explicit;  // the copy kernel was chosen by the caller (option or opts), not by "auto"
 };
 
 llx_status resolve_policy(const llx_launch_opts* o, Policy* p) {
@@ -146,7 +145,6 @@ llx_status resolve_policy(const llx_launch_opts* o, Policy* p) {
             p->route = o->route;
         }
     }
-    p->kernel_explicit = p->kernel != 0;
     return LLX_OK;
 }
 
