@@ -45,6 +45,24 @@ def _time_stream(torch, stream, fn, reps=10, warm=2, before=None):
     return {"median_ms": statistics.median(ts), "min_ms": ts[0]}
 
 
+def _in_thread(torch, fn):
+    """Runs `fn` (the migration's enqueue) on its own host thread, as a serving engine's migration thread would: a
+    budgeted stage is a chain of launches, and enqueueing it from the thread that launches the decode step would put its
+    host time inside the decode step's measured interval.  Returns after the thread has started; join() the result."""
+    import threading
+    dev = torch.cuda.current_device()
+    started = threading.Event()
+
+    def run():
+        torch.cuda.set_device(dev)
+        started.set()
+        fn()
+    th = threading.Thread(target=run)
+    th.start()
+    started.wait()
+    return th
+
+
 def _free(torch):
     gc.collect()
     torch.cuda.empty_cache()
@@ -290,7 +308,7 @@ def batch_30b(torch, llx, stream, seed=0):
 
 
 # ---- configs[4] first half: interference with a decode step -----------------------------------
-def interference(torch, llx, stream_mig_unused):
+def interference(torch, llx, stream_mig_unused, paced_only=False):
     g = dict(synth.CONFIGS["llama7b"])
     L, H, D, S = g["layers"], g["kv_heads"], g["head_dim"], g["block_size"]
     B = 32
@@ -340,13 +358,18 @@ def interference(torch, llx, stream_mig_unused):
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ma, mb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         o = dict(max_ctas=max_ctas, bandwidth_gbps=budget)          # the launch policy of these calls only
-        a.record(s_dec)
+
+        def enqueue_migrations():
+            for _ in range(n_mig):
+                migrate(o)
         ma.record(s_mig)
-        for _ in range(n_mig):
-            migrate(o)
-        mb.record(s_mig)
+        th = _in_thread(torch, enqueue_migrations)
+        time.sleep(0.0002)                                           # the first migration launch is on the device (same pause in both arms of a pair)
+        a.record(s_dec)
         decode_step()
         b.record(s_dec)
+        th.join()
+        mb.record(s_mig)
         torch.cuda.synchronize()
         return a.elapsed_time(b), ma.elapsed_time(mb)
 
@@ -355,7 +378,8 @@ def interference(torch, llx, stream_mig_unused):
         per-pair ratios (the isolated step drifts by +-2 % between blocks of measurements, more than the small cases)."""
         times, mig_ms, ratios = [], [], []
         for _ in range(8):
-            t0, _ = one_step(0, 0, 0)
+            one_step(0, 0, 0)          # discarded: the previous pair ended with the GPU all but idle under a long paced tail;
+            t0, _ = one_step(0, 0, 0)  # both measured steps now follow a decode step
             t1, m = one_step(n_mig, max_ctas, budget)
             times.append(t1)
             mig_ms.append(m)
@@ -378,6 +402,8 @@ def interference(torch, llx, stream_mig_unused):
     cases += [(f"looped, {c} full-speed CTAs (LLX_OPT_MAX_CTAS)", n_for(c * 33), c, 0) for c in (32, 16, 8, 4)]
     cases += [(f"looped, budget {bw} GB/s (LLX_OPT_BANDWIDTH_GBPS: " + ("few full-speed CTAs" if bw >= 500 else "paced on all SMs") + ")",
                n_for(bw), 0, bw) for bw in (2400, 1600, 800, 400, 200, 100, 65, 20)]
+    if paced_only:
+        cases = [c for c in cases if 0 < c[3] < 500]
     for label, n_mig, cap, bw in cases:
         t, m, ratio = with_migration(n_mig, cap, bw)
         res["cases"].append({"case": label, "migrations": n_mig, "max_ctas": cap, "bandwidth_budget_GBps": bw,
@@ -394,7 +420,7 @@ def interference(torch, llx, stream_mig_unused):
 
 
 # ---- NEXT-1: choose the bandwidth budget from a decode-slowdown target (<= 1 %) ----------
-def auto_budget(torch, llx, stream_unused=None, target_pct=1.0, rounds=12):
+def auto_budget(torch, llx, stream_unused=None, target_pct=1.0, rounds=16, grid=None):
     """Largest LLX_OPT_BANDWIDTH_GBPS whose decode-step slowdown stays within `target_pct`.
 
     The isolated decode step varies by about +-2 % from one measurement block to the next on a B200, more than
@@ -435,46 +461,62 @@ def auto_budget(torch, llx, stream_unused=None, target_pct=1.0, rounds=12):
     def one(budget, n_mig):
         torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+        def enqueue_migrations():
+            for _ in range(n_mig):
+                llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=dict(bandwidth_gbps=budget))
+        th = _in_thread(torch, enqueue_migrations)
+        time.sleep(0.0002)                                           # same pause in both arms of a pair
         a.record(s_dec)
-        for _ in range(n_mig):
-            llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=dict(bandwidth_gbps=budget))
         decode_step()
         b.record(s_dec)
+        th.join()
         torch.cuda.synchronize()
         return a.elapsed_time(b)
 
-    for _ in range(3):
-        one(0, 0)
-    base = statistics.median(one(0, 0) for _ in range(5))
+    grid = list(grid) if grid else [5, 8, 12, 18, 25, 35, 50, 100, 200]
 
-    def slowdown(budget):
-        n_mig = max(1, int(budget * 1e9 * base * 1e-3 * 1.6 / mig_bytes) + 1)   # keeps the copy stream busy all step long
-        ratios = []
-        for _ in range(rounds):
-            t0 = one(0, 0)
-            t1 = one(budget, n_mig)
-            ratios.append(t1 / t0)
-        return 100.0 * (statistics.median(ratios) - 1.0)
-
-    grid = [5, 8, 12, 18, 25, 35, 50, 70, 100, 140, 200, 280, 400]
-    tried, lo_i, hi_i = {}, 0, len(grid) - 1
-    tried[grid[0]] = slowdown(grid[0])
-    best = grid[0] if tried[grid[0]] <= target_pct else None
-    if best is not None:
-        while lo_i < hi_i:                       # bisection: slowdown grows with the budget
-            mid = (lo_i + hi_i + 1) // 2
-            tried[grid[mid]] = slowdown(grid[mid])
-            if tried[grid[mid]] <= target_pct:
-                lo_i, best = mid, grid[mid]
+    def measure_state():
+        for _ in range(3):
+            one(0, 0)
+        base = statistics.median(one(0, 0) for _ in range(5))
+        by_budget = {}
+        for budget in grid:
+            n_mig = max(1, int(budget * 1e9 * base * 1e-3 * 1.6 / mig_bytes) + 1)   # keeps the copy stream busy all step long
+            ratios, with_mig = [], []
+            for _ in range(rounds):
+                one(0, 0)              # discarded (see interference(): both measured steps follow a decode step)
+                t0 = one(0, 0)
+                t1 = one(budget, n_mig)
+                ratios.append(t1 / t0)
+                with_mig.append(t1)
+            by_budget[str(budget)] = {"slowdown_pct": 100.0 * (statistics.median(ratios) - 1.0), "decode_step_ms": statistics.median(with_mig)}
+        ok = [b_ for b_ in grid if by_budget[str(b_)]["slowdown_pct"] <= target_pct]
+        largest = None
+        for b_ in grid:                          # the largest budget below which every candidate holds the target
+            if by_budget[str(b_)]["slowdown_pct"] <= target_pct:
+                largest = b_
             else:
-                hi_i = mid - 1
-    null = 100.0 * (statistics.median(one(0, 0) / one(0, 0) for _ in range(rounds)) - 1.0)
-    res = {"target_slowdown_pct": target_pct, "chosen_budget_GBps": best, "decode_step_ms": base,
-           "paired_slowdown_pct_by_budget": {str(k): v for k, v in sorted(tried.items())},
-           "null_pair_pct": null, "pairs_per_candidate": rounds,
-           "ideal_share_pct_at_chosen": None if best is None else 100.0 * best / (int(ctx.sum()) * 2 * H * D * 2 * L / base / 1e6),
-           "note": "median of per-pair ratios (step with migration / step without, alternating); null_pair_pct is the "
-                   "same statistic for two steps without migration (the measurement floor)"}
+                break
+        null = 100.0 * (statistics.median(one(0, 0) / one(0, 0) for _ in range(rounds)) - 1.0)
+        return {"decode_step_alone_ms": base, "chosen_budget_GBps": largest, "by_budget": by_budget, "null_pair_pct": null,
+                "candidates_within_target": ok}
+
+    # Two states of the same GPU.  "pristine": nothing but this decode step has run in the process.  "steady": after
+    # bulk-ring (shared-memory) migrations have run — they leave the GPU in a state in which THIS decode step is
+    # 1-2 % slower for good (5.18 -> 5.25-5.28 ms; the register-staged kernel does not do it, a carve-out preference on
+    # the attention kernels does not undo it; mechanism not established).  A GPU that migrates requests is in the
+    # steady state; the pristine one is the more conservative baseline.  The decode step next to a given budget
+    # takes about the same absolute time in both.
+    res = {"target_slowdown_pct": target_pct, "pairs_per_candidate": rounds, "pristine": measure_state()}
+    for _ in range(20):
+        llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig)
+    torch.cuda.synchronize()
+    res["steady"] = measure_state()
+    res["chosen_budget_GBps"] = res["pristine"]["chosen_budget_GBps"]
+    res["note"] = ("slowdown = median of per-pair ratios (step with migration / step without, alternating, each after a discarded "
+                   "step); null_pair_pct = the same statistic for two steps without migration (the measurement floor); the "
+                   "migration is enqueued from its own host thread")
     del p
     _free(torch)
     return res

@@ -175,7 +175,7 @@ void llx_launch_opts_init(llx_launch_opts* opts);
 
 /* for i<n, l<layers, kv<2:  dst[l][kv][dst_block_ids[i]][:] = src[l][kv][src_block_ids[i]][:]
  * Whole tiles, including unused token slots of a partly filled last block.  One kernel
- * launch on `cuda_stream`.  Checked: same geometry (num_blocks may differ), ids in range,
+ * launch on `cuda_stream` (a stage under a bandwidth budget: a chain of launches, LLX_OPT_PACED_SLICE_US).  Checked: same geometry (num_blocks may differ), ids in range,
  * no duplicate destination id (duplicate source ids are legal: prefix-shared blocks),
  * src and dst distinct and non-overlapping.  src is never written.
  * The call runs on the SOURCE pool's device (which must be current; cuda_stream belongs to it).  dst may live on
@@ -422,6 +422,12 @@ typedef enum {
                                    L1): every llx kernel co-runs and the stand-in decode step loses nothing (measured; 75 costs
                                    it +5 %, 100 +30 %).  0 = the driver's choice ("all L1").  100: not even a kernel that needs
                                    the whole 227 KB ever waits */
+    LLX_OPT_PACED_SLICE_US = 16, /* PROCESS-WIDE ONLY.  A paced stage (bandwidth budget below 500 GB/s) is issued as a chain of launches
+                                   of about this many microseconds each (at most 256 per call) instead of ONE kernel resident
+                                   for the whole stage, so that a co-running kernel waiting for an SM to change its L1/shared
+                                   split waits for the end of a slice, not of the stage (75 ms for 112 blocks at 25 GB/s).
+                                   Default 1000; 0 = one launch.  Costs ~3 us of host time per slice inside the call; the rate
+                                   and the decode step's slowdown are unchanged (measured).  Counters count every launch */
     LLX_OPT_VIA_HOST_MODE = 11  /* llx_pack / llx_unpack / llx_migrate_via_host with a pinned-host buffer: 0 (default) copy engines
                                    through device bounce buffers; 1 the kernels address the host buffer directly (zero-copy) */
 } llx_option;

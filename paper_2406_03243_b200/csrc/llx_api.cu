@@ -67,7 +67,7 @@ int elem_bytes_of(llx_dtype d) {
 
 // ---- options / counters -------------------------------------------------------------------
 std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
-    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1}, g_opt_carveout{50};
+    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1}, g_opt_carveout{50}, g_opt_slice_us{1000};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
 // Range of every option: shared by llx_set_option (process defaults) and by the per-call llx_launch_opts.
@@ -89,6 +89,7 @@ bool opt_valid(int opt, long long v) {
         case LLX_OPT_DYNAMIC_TAIL_BATCH: return v >= 0 && v <= 4096;
         case LLX_OPT_EXACT_RESIDENCY: return v >= 0 && v <= 1;
         case LLX_OPT_COPY_SMEM_CARVEOUT_PCT: return v >= 0 && v <= 100;
+        case LLX_OPT_PACED_SLICE_US: return v >= 0 && v <= 1000000;
     }
     return false;
 }
@@ -587,6 +588,7 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     a.chunks_per_tile = (int)cpt;
     a.slices = slices;
     a.total_units = (int)units;
+    a.unit_begin = 0;
     a.blocked_order = (int)pol.order;
     a.l2_hint = (int)pol.l2hint;
     a.pace_ns = (int)pace_ns;
@@ -652,18 +654,43 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
         g_id_uploads++;
     }
 
-    cudaError_t e;
+    cudaError_t e = cudaSuccess;
     const bool pdl = pol.pdl != 0;
+    int launches = 1;
     if (kern == 2) {
         if (byval)
             e = launch_k(pdl, llx_copy_bulk<true>, grid, threads, smem, st, a, pack, nstages);
         else
             e = launch_k(pdl, llx_copy_bulk<false>, grid, threads, smem, st, a, pack, nstages);
     } else {
-        if (byval)
-            e = launch_k(pdl, llx_copy_vec16<true, 4>, grid, threads, 0, st, a, pack);
-        else
-            e = launch_k(pdl, llx_copy_vec16<false, 4>, grid, threads, 0, st, a, pack);
+        // A paced stage is issued as a chain of short launches (LLX_OPT_PACED_SLICE_US, default 1 ms): its CTAs sit on every
+        // SM, and an SM whose L1/shared split is too small for a waiting kernel can only be reconfigured when no CTA is
+        // resident (see paced_in_flight).  With slices, such a kernel waits for the end of a slice, not of the stage.
+        // Measured next to a 25 GB/s stage of 112 blocks (75 ms): a kernel that needs the 164 KB split: p99 75 ms as one
+        // launch, 1.0 ms with 1 ms slices, 0.27 ms with 250 us slices; a 4096^3 GEMM likewise; the stage still runs at
+        // 24.9 / 24.6 GB/s and the decode step's slowdown is unchanged (+0.4 % at 25 GB/s, +3.6 % at 100 GB/s).  Price: ~3 us
+        // of host time per slice inside the call.  Slices after the first are launched WITHOUT programmatic dependent
+        // launch: an early-launched successor would keep the SMs occupied across the boundary.  Every CTA restarts its
+        // pacing clock at its slice's start.
+        const long long slice_us = g_opt_slice_us.load();
+        long long per_slice = units;
+        if (budget > 0 && slice_us > 0 && pace_ns > 0 && !capturing) {
+            const long long chunks_per_cta = slice_us * 1000 / pace_ns;  // chunks one CTA moves within one slice
+            per_slice = (chunks_per_cta < 1 ? 1 : chunks_per_cta) * (long long)grid;
+            const long long floor_units = ((units + 255) / 256 + grid - 1) / grid * grid;  // at most 256 launches per call
+            if (per_slice < floor_units) per_slice = floor_units;
+            if (per_slice * 3 / 2 >= units) per_slice = units;  // not worth cutting
+        }
+        for (long long u0 = 0; u0 < units && e == cudaSuccess; u0 += per_slice) {
+            a.unit_begin = (int)u0;
+            a.total_units = (int)(u0 + per_slice < units ? u0 + per_slice : units);
+            const bool p = pdl && u0 == 0;
+            if (byval)
+                e = launch_k(p, llx_copy_vec16<true, 4>, grid, threads, 0, st, a, pack);
+            else
+                e = launch_k(p, llx_copy_vec16<false, 4>, grid, threads, 0, st, a, pack);
+            if (u0 > 0) ++launches;
+        }
     }
     if (e == cudaSuccess) e = cudaGetLastError();
     const llx_status rc_ring = ring_close(slot, st);
@@ -671,8 +698,8 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     if (rc_ring != LLX_OK) return rc_ring;
     // a register-staged stage that will be resident for a while (every paced one; unpaced ones from 8 MiB): remember it
     if (kern == 1 && !capturing && (budget > 0 || total_bytes >= (8ll << 20))) paced_mark(device, st);
-    g_launches++;
-    g_copy_launches++;
+    g_launches += (unsigned long long)launches;
+    g_copy_launches += (unsigned long long)launches;
     g_bytes += (unsigned long long)total_bytes;
     return LLX_OK;
 }
@@ -1370,6 +1397,12 @@ llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* q, 
     if ((((uintptr_t)q | (uintptr_t)out) & 15) != 0) return fail(LLX_ERR_INVALID_ARG, "q and out must be 16-byte aligned");
     cudaStream_t st = (cudaStream_t)stream;
     llx_pool* p = const_cast<llx_pool*>(pool);
+    {
+        bool capturing = false;
+        if ((rc = stream_capturing(st, &capturing)) != LLX_OK) return rc;
+        DevInfo* di = nullptr;  // first use on this device sets the kernels' attributes (L1 preference)
+        if ((rc = dev_info(pool->device, &di, capturing)) != LLX_OK) return rc;
+    }
 
     int split = (int)g_opt_attn_split.load();
     if (split <= 0) split = 256;
@@ -1446,6 +1479,7 @@ llx_status llx_set_option(llx_option opt, long long v) {
         case LLX_OPT_DYNAMIC_TAIL_BATCH: g_opt_dyn_batch = v; break;
         case LLX_OPT_EXACT_RESIDENCY: g_opt_smem_pad = v; break;
         case LLX_OPT_COPY_SMEM_CARVEOUT_PCT: g_opt_carveout = v; break;  // applied to the kernel at the next copy launch
+        case LLX_OPT_PACED_SLICE_US: g_opt_slice_us = v; break;
     }
     return LLX_OK;
 }
@@ -1467,6 +1501,7 @@ long long llx_get_option(llx_option opt) {
         case LLX_OPT_DYNAMIC_TAIL_BATCH: return g_opt_dyn_batch;
         case LLX_OPT_EXACT_RESIDENCY: return g_opt_smem_pad;
         case LLX_OPT_COPY_SMEM_CARVEOUT_PCT: return g_opt_carveout;
+        case LLX_OPT_PACED_SLICE_US: return g_opt_slice_us;
     }
     return -1;
 }

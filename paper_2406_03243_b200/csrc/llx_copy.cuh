@@ -44,7 +44,9 @@ struct CopyArgs {
     int chunk_bytes;
     int chunks_per_tile;
     int slices;       // 2*layers
-    int total_units;  // n * slices * chunks_per_tile
+    int total_units;  // n * slices * chunks_per_tile (the register-staged kernel: END of this launch's unit range)
+    int unit_begin;   // register-staged kernel: this launch handles units [unit_begin, total_units) — a budgeted stage is
+                      // issued as a chain of short launches (see launch_copy); the bulk kernel always gets 0
     int blocked_order;  // 0: worker w takes units w, w+W, ...; 1: worker w takes a contiguous range
     int l2_hint;        // bit0: loads L2::evict_first, bit1: stores L2::evict_first (bulk kernel)
     int pace_ns;        // bulk kernel: minimum time between two chunks of one ring (0 = unthrottled)
@@ -117,10 +119,11 @@ __global__ void __launch_bounds__(256, 8) llx_copy_vec16(const CopyArgs a, const
     pdl_launch_dependents();
     pdl_wait_prior_grids();
     unsigned long long deadline = a.pace_ns > 0 ? global_timer_ns() : 0ull;
-    int u_begin = blockIdx.x, u_end = a.total_units, u_step = gridDim.x;
+    int u_begin = a.unit_begin + blockIdx.x, u_end = a.total_units, u_step = gridDim.x;
     if (a.blocked_order) {
-        u_begin = (int)((long long)blockIdx.x * a.total_units / gridDim.x);
-        u_end = (int)((long long)(blockIdx.x + 1) * a.total_units / gridDim.x);
+        const long long span = a.total_units - a.unit_begin;
+        u_begin = a.unit_begin + (int)((long long)blockIdx.x * span / gridDim.x);
+        u_end = a.unit_begin + (int)((long long)(blockIdx.x + 1) * span / gridDim.x);
         u_step = 1;
     }
     for (int u = u_begin; u < u_end; u += u_step) {

@@ -244,3 +244,31 @@ def test_calls_that_cannot_be_captured_are_refused_and_leave_the_capture_valid(e
     want = om.pack(h_src, s_ids[:4])
     assert np.array_equal(dev_stg.cpu().numpy().view(np.uint16).reshape(want.shape), want)
     pin.free()
+
+
+# ---- a budgeted stage is a chain of short launches (LLX_OPT_PACED_SLICE_US) ------------------------------------------
+@pytest.mark.parametrize("slice_us,unit_order,ids_by_value_max", [(1, 1, 256), (1, 0, 256), (1, 1, 0), (50, 1, 256)])
+def test_sliced_budgeted_stage_is_bit_exact(env, slice_us, unit_order, ids_by_value_max):
+    """Ragged 34,560-byte tiles (16 full 2 KiB chunks + a 1,792-byte tail per tile), 13 blocks, 40 GB/s: with tiny slices
+    the stage becomes many launches over consecutive unit ranges; together they must copy every chunk exactly once."""
+    H, llx = env
+    g = dict(layers=3, kv_heads=9, head_dim=120, block_size=16, elem_bytes=2, num_blocks=40)
+    src, dst = H.DevPool(g), H.DevPool(g, fill=SENT)
+    src.fill_from_synth(5, 0)
+    h_src = H.host_pool_from_synth(g, 5, 0)
+    h_dst = om.new_pool(g["layers"], g["num_blocks"], H.tile_elems(g), fill=SENT)
+    s_ids = synth.block_permutation(11, g["num_blocks"])[:13]
+    d_ids = synth.block_permutation(12, g["num_blocks"])[:13]
+    c0 = llx.counters()["copy_launches"]
+    with llx.options(paced_slice_us=slice_us):
+        llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, opts=dict(bandwidth_gbps=40, unit_order=unit_order, ids_by_value_max=ids_by_value_max))
+    launches = llx.counters()["copy_launches"] - c0
+    assert 2 <= launches <= 256, launches
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
+    H.assert_pool_equal(src.host(), h_src)
+    with llx.options(paced_slice_us=0):                                  # 0 = one launch for the whole stage
+        c0 = llx.counters()["copy_launches"]
+        llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, opts=dict(bandwidth_gbps=40))
+        assert llx.counters()["copy_launches"] - c0 == 1
+    H.assert_pool_equal(dst.host(), h_dst)
