@@ -418,10 +418,12 @@ typedef enum {
                                    serves bandwidth budgets below 500 GB/s and the host zero-copy / peer routes.  That kernel
                                    keeps a small CTA resident on every SM for the whole stage, and an SM cannot change its
                                    L1/shared split while a CTA is resident: a co-running kernel that needs more shared memory
-                                   than the split offers waits for the END of the stage.  Default 50 (132 KB shared / 124 KB
-                                   L1): every llx kernel co-runs and the stand-in decode step loses nothing (measured; 75 costs
-                                   it +5 %, 100 +30 %).  0 = the driver's choice ("all L1").  100: not even a kernel that needs
-                                   the whole 227 KB ever waits */
+                                   than the split offers waits for the end of the launch (a slice of the stage, see
+                                   LLX_OPT_PACED_SLICE_US).  Default 50 (132 KB shared / 124 KB L1): the stand-in decode step
+                                   loses nothing (measured; 75 costs it +2..5 %, 100 +11..30 %).  0 = the driver's choice ("all
+                                   L1").  100: not even a kernel that needs the whole 227 KB ever waits.  llx's own bulk ring
+                                   (164 KB split) does not rely on this: while a register-staged stage is in flight the library
+                                   routes its auto-selected copies through the register-staged kernel */
     LLX_OPT_PACED_SLICE_US = 16, /* PROCESS-WIDE ONLY.  A paced stage (bandwidth budget below 500 GB/s) is issued as a chain of launches
                                    of about this many microseconds each (at most 256 per call) instead of ONE kernel resident
                                    for the whole stage, so that a co-running kernel waiting for an SM to change its L1/shared

@@ -303,16 +303,17 @@ llx_status dyn_counter_get(int dev, cudaStream_t st, unsigned int** counter) {
 // the END OF THE STAGE, and a kernel that needs more shared memory than that split offers waits that long.  Measured on
 // B200 with the driver's default preference ("all L1" for a kernel without shared memory): a 2-block final stage (bulk
 // ring, 2 x 76 KB of shared memory) next to a 25 GB/s stage: median 53 us, p90 75 ms; a 4096^3 bf16 GEMM: up to 75 ms.
-// Two measures:
+// Three measures:
 //  (1) the kernel asks for a 50 % carve-out (LLX_OPT_COPY_SMEM_CARVEOUT_PCT): arriving on idle SMs it leaves 132 KB of
-//      shared memory configured, enough for every llx kernel (final stage 76 KB per CTA, long stage 113 KB), and 124 KB of
-//      L1, which costs the L1-hungry stand-in decode step nothing (20 GB/s: +0.7 %; 64 %: +1.3 %, 75 %: +4.9 %, 100 %: +30 %);
-//  (2) SMs that were busy with shared-memory-free kernels when the stage arrived keep "all L1" all the same, so the library
-//      remembers the register-staged launches that may still be running (one event each) and, while any is, sends its own
-//      auto-selected copies through the register-staged kernel too: no shared memory, placed at once (a short stage takes
-//      the same time: 23.3 vs 23.6 us; a long one runs at 5.6 instead of 6.5 TB/s next to the budgeted stage).
-// Kernels of OTHER libraries that need more than 131 KB of shared memory can still wait for the end of a budgeted stage;
-// a preference of 100 removes that at the decode step's expense.
+//      shared memory configured and 124 KB of L1, which costs the L1-hungry stand-in decode step nothing (measured by
+//      preference at a 20 GB/s budget: 0/50/64 %: +0.4..0.5 %, 75 %: +2.1 %, 100 %: +11 %).  That helps kernels of other
+//      libraries up to 131 KB; llx's own bulk ring asks for the 164 KB split and still waits at 50 %, hence (2) and (3);
+//  (2) the library remembers the register-staged launches that may still be running (one event each) and, while any
+//      is, sends its own auto-selected copies through the register-staged kernel too: no shared memory, placed at once
+//      (a short stage takes the same time: 23.3 vs 23.6 us; a long one runs at 5.6 instead of 6.5 TB/s next to the
+//      budgeted stage);
+//  (3) a budgeted stage is a chain of ~1 ms launches (LLX_OPT_PACED_SLICE_US, in launch_copy): whoever waits for an SM
+//      to change its split waits for the end of a slice, not of the stage.
 struct PacedTracker {
     std::mutex mu;
     static constexpr int kSlots = 16;
