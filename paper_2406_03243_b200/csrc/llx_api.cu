@@ -495,7 +495,8 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     const int slices = 2 * layers;
 
     if (kern == 2) {
-        // Tuned on B200 (profiles/r01_copy_sweep.md, r01_dynamic_tail.md): ONE CTA per SM with one ring of 3 x 32 KiB,
+        // Tuned on B200 (round-1 CUDA-event sweeps, summarised in profiles/r01_ncu_summary.md; re-checked in round 2): ONE CTA
+        // per SM with one ring of 3 x 32 KiB,
         // every ring streaming a contiguous range of chunks and the last 6 % of the stage claimed dynamically
         // (6.57 TB/s at 112 blocks, 6.66 TB/s at >= 256).  More bytes in flight per SM lowers DRAM efficiency.
         // A short stage (the final one: 2 blocks) is latency-bound: smaller chunks over twice as many rings.
