@@ -79,6 +79,37 @@ int main(void) {
         CHECK(llx_set_option(LLX_OPT_DYNAMIC_TAIL_PCT, 6) == LLX_OK);
     }
 
+    /* one migration round of a pair as one batch (PAPER.md:225 + :142, reading A31): M = 40 blocks, three running requests
+     * of 10 / 6 / 12 blocks and a head-of-line queuing request that needs 20: F = (40 - 48)/3 < 2, so the source gives
+     * requests away, shortest first, until F >= 2 or the destination (8 free blocks, 1 kept in reserve) is full */
+    {
+        llx_blockmgr* dstm = NULL;
+        llx_req_info rq[4];
+        int32_t seq[4] = {150, 90, 180, 300}, offs[5] = {0, 10, 16, 28, 28}, tabs[28], chosen[4], ro[5], so[28], dd[28], got8[8];
+        double hr[1] = {0.0};
+        int nc = -1, np = -1;
+        llx_launch_opts lo;
+        memset(rq, 0, sizeof rq);
+        for (i = 0; i < 28; ++i) tabs[i] = 100 + i;
+        rq[0].physical_usage = 10.0;
+        rq[1].physical_usage = 6.0;
+        rq[2].physical_usage = 12.0;
+        rq[3].is_queuing = 1;
+        rq[3].is_head_of_line = 1;
+        rq[3].demand = 20.0;
+        CHECK(llx_blockmgr_create(16, &dstm) == LLX_OK && llx_blockmgr_alloc(dstm, 8, got8) == LLX_OK);
+        CHECK(llx_plan_migration_batch(rq, seq, 4, 40.0, hr, 1, 0, 2.0, offs, tabs, dstm, 1, chosen, &nc, ro, so, dd, 28, &np) == LLX_OK);
+        CHECK(nc == 1 && chosen[0] == 1 && np == 6 && ro[0] == 0 && ro[1] == 6);    /* the 6-block request fits, the 10-block one does not */
+        CHECK(so[0] == 110 && so[5] == 115 && dd[0] == 8 && dd[5] == 13 && llx_blockmgr_num_free(dstm) == 2);
+        CHECK(llx_plan_migration_batch(rq, seq, 4, 40.0, hr, 1, 0, 2.0, offs, tabs, dstm, 0, chosen, &nc, ro, so, dd, 2, &np) == LLX_OK && nc == 0);
+        CHECK(llx_plan_migration_batch(rq, seq, 4, 400.0, hr, 1, 0, 2.0, offs, tabs, dstm, 0, chosen, &nc, ro, so, dd, 28, &np) == LLX_OK && nc == 0); /* not a source */
+        llx_blockmgr_destroy(dstm);
+        llx_launch_opts_init(&lo);
+        CHECK(lo.struct_size == sizeof lo && lo.bandwidth_gbps == LLX_OPT_DEFAULT && lo.route == LLX_OPT_DEFAULT);
+        lo.chunk_bytes = 100; /* not a multiple of 16: refused before anything else is looked at */
+        CHECK(llx_migrate_stage_ex(NULL, NULL, NULL, NULL, 1, NULL, &lo) == LLX_ERR_INVALID_ARG);
+    }
+
     /* no device here or bad arguments: data calls fail loudly, never compute on the CPU */
     CHECK(llx_migrate_stage(NULL, NULL, NULL, NULL, 1, NULL) == LLX_ERR_INVALID_ARG);
     CHECK(strcmp(llx_status_str(LLX_ERR_NO_SPACE), "LLX_ERR_NO_SPACE") == 0);

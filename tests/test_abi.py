@@ -170,3 +170,56 @@ def test_host_side_under_asan_and_ubsan(tmp_path):
     r = subprocess.run([exe], capture_output=True, text=True, env=env)
     assert r.returncode == 0 and "abi_smoke ok" in r.stdout and "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr, \
         r.stdout + r.stderr[-3000:]
+
+
+def test_launch_opts_are_validated_before_any_device_work(llx):
+    """llx_launch_opts: init sets every field to LLX_OPT_DEFAULT; a bad field, an unknown route or a struct_size this
+    library does not know is LLX_ERR_INVALID_ARG — reported before the pools are even looked at (so also without a GPU)."""
+    import ctypes as C
+    o = llx.LaunchOpts()
+    assert o.struct_size == C.sizeof(llx.LaunchOpts) == 64
+    assert all(getattr(o, f) == llx.OPT_DEFAULT for f, _ in o._fields_ if f != "struct_size")
+    l = llx.lib()
+    ids = (C.c_int32 * 2)(0, 1)
+    for bad in (dict(chunk_bytes=100), dict(copy_kernel=7), dict(bandwidth_gbps=-5), dict(route=9), dict(ring_stages=1)):
+        rc = l.llx_migrate_stage_ex(None, ids, None, ids, 2, None, C.byref(llx.LaunchOpts(**bad)))
+        assert rc == -1 and b"llx_launch_opts." in l.llx_last_error(), (bad, l.llx_last_error())
+    o = llx.LaunchOpts()
+    o.struct_size = 6
+    assert l.llx_migrate_stage_ex(None, ids, None, ids, 2, None, C.byref(o)) == -1 and b"struct_size" in l.llx_last_error()
+    o.struct_size = 400
+    assert l.llx_migrate_batch_ex(None, None, ids, ids, ids, 1, None, C.byref(o)) == -1 and b"struct_size" in l.llx_last_error()
+    with pytest.raises(TypeError):
+        llx.LaunchOpts(no_such_field=1)
+    # a good policy passes validation and the call then fails on the NULL pools, not on the policy
+    rc = l.llx_migrate_stage_ex(None, ids, None, ids, 2, None, C.byref(llx.LaunchOpts(bandwidth_gbps=25, route=llx.ROUTE_PEER)))
+    assert rc == -1 and b"pool is NULL" in l.llx_last_error()
+    # the process-wide defaults that are not per-call fields
+    assert llx.get_option(llx.OPT_COPY_SMEM_CARVEOUT_PCT) == 50 and llx.get_option(llx.OPT_PACED_SLICE_US) == 1000
+    with pytest.raises(llx.LlxError):
+        llx.set_option(llx.OPT_COPY_SMEM_CARVEOUT_PCT, 101)
+
+
+def test_ipc_handle_is_checked(llx):
+    import ctypes as C
+    l = llx.lib()
+    assert llx.IPC_HANDLE_BYTES == 96
+    with pytest.raises(llx.LlxError) as e:
+        llx.pool_ipc_open(b"\0" * llx.IPC_HANDLE_BYTES)                  # no magic: not an llx handle
+    assert e.value.name == "LLX_ERR_INVALID_ARG"
+    with pytest.raises(llx.LlxError):
+        llx.pool_ipc_open(b"short")
+    out = C.c_void_p()
+    assert l.llx_pool_ipc_open(None, C.byref(out)) == -1 and l.llx_pool_ipc_export(None, None) == -1
+    # session policy: a struct of another size is refused, NULL resets
+    a, b = llx.BlockManager(8), llx.BlockManager(8)
+    mig = llx.Migration(None, a, None, b, 4, 1)
+    mig.set_stage_opts(dict(bandwidth_gbps=25))
+    mig.set_stage_opts(None)
+    bad = llx.LaunchOpts()
+    bad.struct_size = 8
+    with pytest.raises(llx.LlxError):
+        mig.set_stage_opts(bad)
+    with pytest.raises(llx.LlxError) as e:
+        mig.stage([3, 3, 4, 5], 14)                                       # a table that names a block twice (A33)
+    assert e.value.name == "LLX_ERR_INVALID_ARG" and b.num_free == 8
