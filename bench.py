@@ -12,9 +12,11 @@ is removed from the step (`--serial-appends` puts the appends back on the migrat
 
     value     GB/s, bytes read + written by the three stage copies / device time of the whole step
               (pools resident in HBM; CUDA events on the launching stream; max over ranks)
-    e2e       the same request migrated THROUGH HOST BUFFERS: llx_migrate_via_host gathers into a pinned host
-              staging buffer (D2H) and scatters from it (H2D), chunk-pipelined — the paper's GPU->CPU buffer->GPU
-              route; the plain llx_pack -> llx_unpack pair is reported beside it
+    e2e       the same request migrated THROUGH HOST BUFFERS: llx_migrate_via_host moves it into a pinned host staging
+              buffer (D2H) and out of it into the destination's blocks (H2D), both directions of the link at once — the
+              paper's GPU->CPU buffer->GPU route.  Default host leg: one pitched copy-engine transfer
+              per block (no kernel); the gather/scatter-kernel route through bounce buffers and the plain
+              llx_pack -> llx_unpack pair are reported beside it
     roofline  the dominant kernel (stage 0: 112 blocks, 1.75 GiB of traffic) against the measured HBM peak
     cpu_baseline / --impl reference   the NumPy oracle timed on the host cores on a bounded sample
 
@@ -472,6 +474,9 @@ def run_llx(args):
     def via_host():
         llx.migrate_via_host(w.src, w.s_tab, w.dst, w.d_tab, pin.dev_alias, stg_bytes, stream=stream)
 
+    def via_host_kernels():      # LLX_OPT_VIA_HOST_MODE = 3: gather / scatter kernels + bounce buffers, the copy engine crosses the link
+        llx.migrate_via_host(w.src, w.s_tab, w.dst, w.d_tab, pin.dev_alias, stg_bytes, stream=stream, opts=dict(via_host_mode=3))
+
     def pack_unpack():
         llx.pack(w.src, w.s_tab, pin.dev_alias, stg_bytes, stream=stream)       # device -> pinned host
         llx.unpack(pin.dev_alias, stg_bytes, w.dst, w.d_tab, stream=stream)     # pinned host -> device
@@ -490,11 +495,13 @@ def run_llx(args):
         return replicas.max_over_ranks((t1 - t0) * 1e3 / e2e_steps)
 
     e2e_seq_ms = host_timed(pack_unpack)
+    e2e_kern_ms = host_timed(via_host_kernels)
     c_e0 = llx.counters()
     e2e_ms = host_timed(via_host)
     e2e_launches = (llx.counters()["kernel_launches"] - c_e0["kernel_launches"]) // (e2e_steps + 2)
     e2e_val = replicas.sum_over_ranks(2 * n * w.src.block_bytes) / (e2e_ms * 1e-3) / 1e9
     e2e_seq_val = replicas.sum_over_ranks(2 * n * w.src.block_bytes) / (e2e_seq_ms * 1e-3) / 1e9
+    e2e_kern_val = replicas.sum_over_ranks(2 * n * w.src.block_bytes) / (e2e_kern_ms * 1e-3) / 1e9
     pin.free()
 
     # ---- final-stage downtime (S4): host wall clock around the C-ABI call + stream sync ----
@@ -535,8 +542,13 @@ def run_llx(args):
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": n * block_bytes,
                 "d2h_bytes_per_step": n * block_bytes, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "gpu_launches_per_step": e2e_launches,
-                "path": "llx_migrate_via_host: gather kernel -> pinned host buffer -> scatter kernel, 64 MiB chunks, D2H and "
-                        "H2D on the copy engines at the same time (host wall clock incl. stream sync)",
+                "path": "llx_migrate_via_host, default host leg: one pitched copy-engine transfer per block (2L tiles at a constant "
+                        "stride) into the pinned buffer and out of it, D2H and H2D at the same time in groups of ~16 MiB; no kernel "
+                        "on this route (host wall clock incl. stream sync)",
+                "gather_scatter_kernels_through_bounce_buffers": {
+                    "value": e2e_kern_val, "ms_per_step": e2e_kern_ms,
+                    "path": "LLX_OPT_VIA_HOST_MODE=3: gather kernel -> device bounce buffer -> copy engine D2H | H2D -> bounce "
+                            "buffer -> scatter kernel, 64 MiB chunks (round 1's route)"},
                 "sequential_pack_then_unpack": {"value": e2e_seq_val, "ms_per_step": e2e_seq_ms,
                                                 "path": "llx_pack (gather kernel into a device bounce buffer, copy engine D2H, 64 MiB chunks) "
                                                         "then llx_unpack (copy engine H2D, scatter kernel), one after the other"}},

@@ -249,6 +249,9 @@ def staging_host(torch, llx, p: Pools, stream, nb):
     res["llx_unpack_zero_copy_GBps"] = nbytes / t["median_ms"] / 1e6
     t = _time_stream(torch, stream, lambda: llx.migrate_via_host(p.src, s_tab, p.dst, d_tab, pin.dev_alias, nbytes, stream=stream), reps=5, warm=1)
     res["llx_migrate_via_host_roundtrip_ms"] = t["median_ms"]
+    t = _time_stream(torch, stream, lambda: llx.migrate_via_host(p.src, s_tab, p.dst, d_tab, pin.dev_alias, nbytes, stream=stream,
+                                                                 opts=dict(via_host_mode=3)), reps=5, warm=1)
+    res["llx_migrate_via_host_kernels_and_bounce_buffers_roundtrip_ms"] = t["median_ms"]
     # alternative: pack into a DEVICE buffer, then one copy-engine transfer (and back)
     stg = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     hbuf = torch.empty(nbytes, dtype=torch.uint8).pin_memory()

@@ -228,8 +228,8 @@ llx_status llx_staging_free_pinned(void* host_ptr);
 /* staging[i][l][kv][:] = src[l][kv][src_block_ids[i]][:]
  * With a pinned-host buffer the tiles are gathered into a library-owned device bounce buffer in ~64 MiB chunks and
  * each chunk crosses the host link on the copy engine (all on cuda_stream; first use allocates the bounce buffers and
- * synchronises the device).  LLX_OPT_VIA_HOST_MODE=1 or an explicit LLX_OPT_COPY_KERNEL makes the kernel write the
- * pinned buffer directly instead (zero-copy). */
+ * synchronises the device).  LLX_OPT_VIA_HOST_MODE selects the other host legs: 1 (or an explicit LLX_OPT_COPY_KERNEL)
+ * makes the kernel write the pinned buffer directly (zero-copy), 2 lets the copy engine gather by itself. */
 llx_status llx_pack(const llx_pool* src, const int32_t* src_block_ids, int n, void* staging, size_t staging_bytes,
                     void* cuda_stream);
 /* dst[l][kv][dst_block_ids[i]][:] = staging[i][l][kv][:]   (dst ids distinct) */
@@ -245,8 +245,9 @@ llx_status llx_unpack_ex(const void* staging, size_t staging_bytes, llx_pool* ds
  * The request is cut into chunks of `chunk_blocks` blocks (<= 0: auto, ~64 MiB); chunk k is scattered on an internal
  * stream while chunk k+1 is gathered on `cuda_stream`.  With a pinned-host buffer the chunks cross the host link on the
  * copy engines, device->host and host->device at the same time (the source and destination machines of the paper work
- * concurrently in the same way), through library-owned device bounce buffers (4 x chunk bytes, allocated on first use:
- * that call synchronises the device).  `cuda_stream` is joined with the internal streams before the call returns: work
+ * concurrently in the same way): by default as one pitched copy per block in groups of ~16 MiB (no kernel at all), with
+ * LLX_OPT_VIA_HOST_MODE = 3 or a destination on another GPU through library-owned device bounce buffers (4 x chunk
+ * bytes, allocated on first use: that call synchronises the device).  `cuda_stream` is joined with the internal streams before the call returns: work
  * enqueued on it afterwards sees the complete migration.  Checks as llx_migrate_stage + llx_pack; nothing is launched
  * when a check fails.  Calls are serialised per process (they share the internal streams). */
 llx_status llx_migrate_via_host(const llx_pool* src, const int32_t* src_block_ids, llx_pool* dst,
@@ -430,8 +431,13 @@ typedef enum {
                                    split waits for the end of a slice, not of the stage (75 ms for 112 blocks at 25 GB/s).
                                    Default 1000; 0 = one launch.  Costs ~3 us of host time per slice inside the call; the rate
                                    and the decode step's slowdown are unchanged (measured).  Counters count every launch */
-    LLX_OPT_VIA_HOST_MODE = 11  /* llx_pack / llx_unpack / llx_migrate_via_host with a pinned-host buffer: 0 (default) copy engines
-                                   through device bounce buffers; 1 the kernels address the host buffer directly (zero-copy) */
+    LLX_OPT_VIA_HOST_MODE = 11  /* the host leg of llx_pack / llx_unpack / llx_migrate_via_host with a pinned-host buffer.
+                                   0 (default) auto: llx_migrate_via_host lets the copy engines gather and scatter by themselves
+                                   (mode 2; measured 93.8 vs 84.9 GB/s), llx_pack / llx_unpack go through the bounce buffers
+                                   (mode 3; equal speed, measured).  1: the kernels address the host buffer directly (zero-copy).
+                                   2: one pitched copy-engine transfer per block (2L tiles at a constant stride): no kernel, no
+                                   bounce buffer, no SM.  3: a gather / scatter kernel per 64 MiB chunk into / out of device bounce
+                                   buffers, the copy engine crosses the link */
 } llx_option;
 /* Process-wide DEFAULTS: what a later call uses for every policy field it does not set itself (llx_launch_opts).
  * For experiments and process-wide tuning; per-request policy belongs in the call.  LLX_ERR_INVALID_ARG for a bad value. */

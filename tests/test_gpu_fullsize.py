@@ -218,12 +218,23 @@ def test_llama7b_2048_tokens_through_the_pinned_host_buffer(env):
         H.assert_pool_equal(dst.host_layer(l), h_dst)
         assert np.array_equal(buf[:, l], want[:, 0])                 # the pinned buffer holds the fused blocks (A6)
     check_untouched_and_mapping_on_device(src, dst, s_tab, d_tab, range(L))
+    # the same request once more through the other host leg (gather / scatter kernels + bounce buffers, 64 MiB chunks)
+    d3 = synth.block_permutation(10, g["num_blocks"])
+    d3 = d3[~np.isin(d3, d_tab)][:128]
+    pin.as_numpy()[:] = 0
+    llx.migrate_via_host(src.pool, s_tab, dst.pool, d3, pin.dev_alias, nbytes, stream=st, opts=dict(via_host_mode=3))
+    st.synchronize()
+    buf = pin.as_numpy().reshape(128, L, 2, te)
+    for l in sample_layers[:1]:
+        h_src = H.host_pool_from_synth(g, 0, 0, layers=[l])
+        assert np.array_equal(buf[:, l], om.pack(h_src, s_tab)[:, 0])
+    check_untouched_and_mapping_on_device(src, dst, np.concatenate([s_tab, s_tab]), np.concatenate([d_tab, d3]), range(0, L, 3))
     # the two halves on their own: pack into the buffer, unpack into other destination blocks
     d2 = synth.block_permutation(9, g["num_blocks"])
-    d2 = d2[~np.isin(d2, d_tab)][:128]
+    d2 = d2[~np.isin(d2, np.concatenate([d_tab, d3]))][:128]
     pin.as_numpy()[:] = 0
     llx.pack(src.pool, s_tab, pin.dev_alias, nbytes, stream=st)
     llx.unpack(pin.dev_alias, nbytes, dst.pool, d2, stream=st)
     st.synchronize()
-    check_untouched_and_mapping_on_device(src, dst, np.concatenate([s_tab, s_tab]), np.concatenate([d_tab, d2]), range(0, L, 5))
+    check_untouched_and_mapping_on_device(src, dst, np.concatenate([s_tab, s_tab, s_tab]), np.concatenate([d_tab, d3, d2]), range(0, L, 5))
     pin.free()

@@ -160,7 +160,7 @@ def test_batch_equals_sequential_and_oracle(env):                   # P7, S5
 
 
 @pytest.mark.parametrize("where", ["device", "pinned"])
-@pytest.mark.parametrize("opts", [dict(), dict(copy_kernel=1), dict(copy_kernel=2)])
+@pytest.mark.parametrize("opts", [dict(), dict(copy_kernel=1), dict(copy_kernel=2), dict(via_host_mode=3), dict(via_host_mode=2)])
 def test_pack_unpack_block_fusion(env, where, opts):                 # P5, S6
     H, llx = env
     g = RAGGED
@@ -193,11 +193,11 @@ def test_pack_unpack_block_fusion(env, where, opts):                 # P5, S6
         pin.free()
 
 
-@pytest.mark.parametrize("where", ["device", "pinned", "pinned_zero_copy"])
+@pytest.mark.parametrize("where", ["device", "pinned", "pinned_zero_copy", "pinned_strided_ce", "pinned_bounce"])
 @pytest.mark.parametrize("n,chunk", [(1, 0), (11, 0), (11, 1), (13, 4), (37, 5), (40, 64)])
 def test_migrate_via_host_pipelined_route(env, where, n, chunk):    # S6: PAPER.md:235-237 in one call
     H, llx = env
-    mode = 1 if where == "pinned_zero_copy" else 0
+    mode = {"pinned_zero_copy": 1, "pinned_strided_ce": 2, "pinned_bounce": 3}.get(where, 0)
     where = where.split("_")[0]
     g = RAGGED
     src, dst, h_src, h_dst = make(H, g, seed=10)
