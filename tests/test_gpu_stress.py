@@ -2,6 +2,7 @@
 a random launch policy PER CALL — llx_launch_opts — so the threads run different launch shapes side by side) for a few
 seconds; after every call the touched destination blocks must equal their source blocks (torch gather on the device,
 independent of the library).  90 s of the same loop (88,000 calls) ran clean on a B200 while this was written."""
+import os
 import threading
 import time
 
@@ -13,7 +14,7 @@ pytestmark = pytest.mark.gpu
 
 G = dict(layers=4, kv_heads=8, head_dim=128, block_size=16)     # 32 KiB tiles, 256 KiB blocks
 NB = 3000
-SECONDS = 6.0
+SECONDS = float(os.environ.get("LLX_STRESS_SECONDS", "6"))        # a longer soak: LLX_STRESS_SECONDS=120 python -m pytest tests/test_gpu_stress.py -m gpu
 
 
 def test_random_mix_of_calls_from_three_threads():
