@@ -207,7 +207,8 @@ def reference_points(torch, llx, p: Pools, stream, nb):
     t = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=stream))
     res["llx_migrate_stage_GBps"] = by / t["median_ms"] / 1e6
     for o, name in ((dict(copy_kernel=1), "llx_vec16_kernel_GBps"), (dict(copy_kernel=2), "llx_bulk_kernel_GBps"),
-                    (dict(route=llx.ROUTE_PEER), "llx_peer_route_on_one_device_GBps")):
+                    (dict(route=llx.ROUTE_PEER), "llx_peer_route_on_one_device_GBps"),
+                    (dict(route=llx.ROUTE_COPY_ENGINE), "llx_copy_engine_route_on_one_device_GBps")):
         t = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_tab, p.dst, d_tab, stream=stream, opts=o))
         res[name] = by / t["median_ms"] / 1e6
     # device-buffer block fusion (pack then unpack through HBM)

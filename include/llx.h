@@ -147,8 +147,13 @@ llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, i
 #define LLX_OPT_DEFAULT (-1)
 typedef enum {
     LLX_ROUTE_AUTO = 0, /* peer route exactly when the pools live on different GPUs */
-    LLX_ROUTE_PEER = 1  /* take the cross-GPU route (kernel choice, launch shape, addressing of SURVEY NEXT-2) although both
+    LLX_ROUTE_PEER = 1, /* take the cross-GPU route (kernel choice, launch shape, addressing of SURVEY NEXT-2) although both
                            pools are on one device: how a single-GPU box executes that branch.  Results are unchanged. */
+    LLX_ROUTE_COPY_ENGINE = 2 /* llx_migrate_stage / _batch only: no kernel at all — one pitched copy-engine transfer per block
+                           (2L tiles at the pools' slice strides), same or different GPUs.  No SM is used on either GPU, so
+                           a migration to another GPU cannot slow a decode step's kernels except through HBM and the link;
+                           on ONE GPU it is the slow way (measured there: 1.9 TB/s against the kernels' 6.6).  Unmeasured over NVLink.
+                           llx_migrate_stage_wait falls back to the stream synchronize */
 } llx_route;
 typedef struct llx_launch_opts {
     uint32_t struct_size;      /* sizeof(llx_launch_opts) as the caller compiled it; set by llx_launch_opts_init */

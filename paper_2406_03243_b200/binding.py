@@ -29,7 +29,7 @@ class ReqInfo(C.Structure):
 
 
 OPT_DEFAULT = -1
-ROUTE_AUTO, ROUTE_PEER = 0, 1
+ROUTE_AUTO, ROUTE_PEER, ROUTE_COPY_ENGINE = 0, 1, 2
 
 
 class LaunchOpts(C.Structure):

@@ -142,7 +142,8 @@ llx_status resolve_policy(const llx_launch_opts* o, Policy* p) {
         LLX_FIELD(via_host_mode, LLX_OPT_VIA_HOST_MODE, via_host)
 #undef LLX_FIELD
         if (offsetof(llx_launch_opts, route) + sizeof(int32_t) <= o->struct_size && o->route != LLX_OPT_DEFAULT) {
-            if (o->route != LLX_ROUTE_AUTO && o->route != LLX_ROUTE_PEER) return fail(LLX_ERR_INVALID_ARG, "llx_launch_opts.route = %d", (int)o->route);
+            if (o->route != LLX_ROUTE_AUTO && o->route != LLX_ROUTE_PEER && o->route != LLX_ROUTE_COPY_ENGINE)
+                return fail(LLX_ERR_INVALID_ARG, "llx_launch_opts.route = %d", (int)o->route);
             p->route = o->route;
         }
     }
@@ -1044,6 +1045,19 @@ void llx_launch_opts_init(llx_launch_opts* o) {
     o->struct_size = (uint32_t)sizeof *o;
 }
 
+// LLX_ROUTE_COPY_ENGINE: pool -> pool with one pitched copy-engine transfer per block (2L tiles at the pools' slice
+// strides).  No kernel and no SM on either GPU: meant for a destination on another GPU, where the link is the bound.
+static llx_status ce_pool_to_pool(const llx_pool* src, const int32_t* src_ids, llx_pool* dst, const int32_t* dst_ids, long long n,
+                                  cudaStream_t st) {
+    const size_t tile = (size_t)src->tile_bytes, rows = 2 * (size_t)src->layers;
+    const size_t sp = (size_t)src->num_blocks * tile, dp = (size_t)dst->num_blocks * tile;
+    for (long long i = 0; i < n; ++i)
+        LLX_CUDA(cudaMemcpy2DAsync(dst->data + (size_t)dst_ids[i] * tile, dp, src->data + (size_t)src_ids[i] * tile, sp, tile, rows,
+                                   cudaMemcpyDefault, st));
+    g_bytes += (unsigned long long)n * rows * tile;
+    return LLX_OK;
+}
+
 static llx_status migrate_stage_checked(const Policy& pol, const llx_pool* src, const int32_t* src_ids, llx_pool* dst,
                                         const int32_t* dst_ids, int n, void* stream) {
     llx_status rc = check_pair(src, dst);
@@ -1054,6 +1068,7 @@ static llx_status migrate_stage_checked(const Policy& pol, const llx_pool* src, 
     if ((rc = check_range(src_ids, n, src->num_blocks, "src")) != LLX_OK) return rc;
     if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
     if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
+    if (pol.route == LLX_ROUTE_COPY_ENGINE) return ce_pool_to_pool(src, src_ids, dst, dst_ids, n, (cudaStream_t)stream);
     return launch_copy(pol, pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
                        (cudaStream_t)stream);
 }
@@ -1155,6 +1170,7 @@ llx_status llx_migrate_batch_ex(const llx_pool* src, llx_pool* dst, const int32_
     if ((rc = check_range(src_ids, n, src->num_blocks, "src")) != LLX_OK) return rc;
     if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
     if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
+    if (pol.route == LLX_ROUTE_COPY_ENGINE) return ce_pool_to_pool(src, src_ids, dst, dst_ids, n, (cudaStream_t)stream);
     // every (block, layer, K|V) tile is independent, so the requests are flattened into one grid
     return launch_copy(pol, pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
                        (cudaStream_t)stream);

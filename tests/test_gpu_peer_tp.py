@@ -60,6 +60,33 @@ def test_peer_route_on_one_device_is_bit_exact(env, g, opts):
     H.assert_pool_equal(src.host(), h_src)
 
 
+@pytest.mark.parametrize("g", [RAGGED, SMALLTILE])
+def test_copy_engine_route_is_bit_exact(env, g):
+    """LLX_ROUTE_COPY_ENGINE: no kernel at all, one pitched transfer per block; stage, batch, the blocking final stage
+    and a stream capture (memcpy nodes) — all bit-exact, and not one llx kernel launched."""
+    H, llx = env
+    src, dst, h_src, h_dst = make(H, g, seed=24)
+    s_ids = synth.block_permutation(35, g["num_blocks"])[:19]
+    d_ids = synth.block_permutation(36, g["num_blocks"])[:19]
+    o = dict(route=llx.ROUTE_COPY_ENGINE)
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    c0 = llx.counters()
+    llx.migrate_stage(src.pool, s_ids[:9], dst.pool, d_ids[:9], stream=st, opts=o)
+    llx.migrate_batch(src.pool, dst.pool, [0, 3, 3, 6], s_ids[9:15], d_ids[9:15], stream=st, opts=o)
+    llx.migrate_stage_wait(src.pool, s_ids[15:17], dst.pool, d_ids[15:17], stream=st, opts=o)
+    c1 = llx.counters()
+    assert c1["kernel_launches"] == c0["kernel_launches"] and c1["bytes_moved"] - c0["bytes_moved"] == 17 * src.pool.block_bytes
+    gr = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(gr, stream=st):
+        llx.migrate_stage(src.pool, s_ids[17:], dst.pool, d_ids[17:], stream=st, opts=o)
+    gr.replay()
+    torch.cuda.synchronize()
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
+    H.assert_pool_equal(src.host(), h_src)
+
+
 def test_peer_route_long_id_list_and_blocking_final_stage(env):
     """> 256 pairs through the (per-device) id ring on the peer route, then the blocking final-stage call, which falls
     back to the stream synchronize because the peer route's kernel carries no completion flag."""
