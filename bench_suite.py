@@ -526,13 +526,16 @@ def auto_budget(torch, llx, stream_unused=None, target_pct=1.0, rounds=16, grid=
 
 
 # ---- interference under SUSTAINED decoding: the state a serving GPU is in ---------------------------------------
-def interference_sustained(torch, llx, stream_unused=None, budgets=(12, 25, 50, 100, 200, 400), seg_steps=150, segments=4):
+def interference_sustained(torch, llx, stream_unused=None, budgets=(12, 25, 50, 100, 200, 400), alt_budgets=(25, 100, 400), seg_steps=150, segments=4):
     """The configs[4] decode step run back to back without pause, as a serving engine does.  After ~0.5 s of that the
     B200 sits at its power cap (about 1000 W, SM clock 1965 -> ~1600 MHz, NVML reason sw_power_cap) and the step takes
     5.5 ms instead of the 5.2 ms of a GPU that idles between measurements — the "pristine" and "steady" baselines of
     auto_budget are two points on that curve.  Here the decode loop never stops; a host thread keeps budgeted
     16-block stages in flight during the ON segments and none during the OFF segments; the first and last 20 steps of
-    every segment are dropped.  slowdown = median ON step / median OFF step - 1."""
+    every segment are dropped.  slowdown = median ON step / median OFF step - 1.
+    Two other mechanisms at the same byte rate, to separate what the KERNEL costs from what the BYTES cost: the same
+    blocks moved by the copy engine (LLX_ROUTE_COPY_ENGINE: no SM at all) and by the full-speed bulk kernel, one block
+    per interval, paced by the host thread."""
     import threading
     g = dict(synth.CONFIGS["llama7b"])
     L, H, D, S = g["layers"], g["kv_heads"], g["head_dim"], g["block_size"]
@@ -591,32 +594,55 @@ def interference_sustained(torch, llx, stream_unused=None, budgets=(12, 25, 50, 
     res["decode_step_first_ms"] = statistics.median(first)
     res["sustained_clocks"] = clocks()
     res["cases"] = []
-    for budget in budgets:
-        on, off = [], []
-        for _ in range(segments):
-            t = run_steps(seg_steps)
-            off += t[20:-20]
-            stop = threading.Event()
+    block_rw = 2 * p.src.block_bytes
 
-            def feeder():
-                torch.cuda.set_device(dev)
-                while not stop.is_set():
-                    llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=dict(bandwidth_gbps=budget))
-                    llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=dict(bandwidth_gbps=budget))
-                    ev = torch.cuda.Event()
-                    ev.record(s_mig)
-                    while not ev.query() and not stop.is_set():
-                        time.sleep(0.0005)
-            th = threading.Thread(target=feeder)
-            th.start()
-            run_steps(10)                             # the first stage is on the device
-            t = run_steps(seg_steps)
-            on += t[20:-20]
-            stop.set()
-            th.join()
-            s_mig.synchronize()
-        res["cases"].append({"bandwidth_budget_GBps": budget, "decode_step_off_ms": statistics.median(off), "decode_step_on_ms": statistics.median(on),
-                             "slowdown_pct": 100.0 * (statistics.median(on) / statistics.median(off) - 1.0), "steps_each": len(on)})
+    def feeder_paced_kernel(budget, stop):           # the library's budget: paced register-staged kernel on every SM
+        while not stop.is_set():
+            llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=dict(bandwidth_gbps=budget))
+            llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=dict(bandwidth_gbps=budget))
+            ev = torch.cuda.Event()
+            ev.record(s_mig)
+            while not ev.query() and not stop.is_set():
+                time.sleep(0.0005)
+
+    def feeder_per_block(opts):                      # one block per interval, paced by the HOST: no resident kernel at all
+        def feed(budget, stop):
+            i, t_next, interval = 0, time.perf_counter(), block_rw / (budget * 1e9)
+            while not stop.is_set():
+                k = i % len(mig_src)
+                llx.migrate_stage(p.src, mig_src[k:k + 1], p.dst, mig_dst[k:k + 1], stream=s_mig, opts=opts)
+                i += 1
+                t_next += interval
+                d = t_next - time.perf_counter()
+                if d > 0:
+                    time.sleep(d)
+        return feed
+
+    mechanisms = [("paced kernel on every SM (bandwidth_gbps)", feeder_paced_kernel, budgets),
+                  ("copy engine, one block per interval paced by the host (no SM at all)", feeder_per_block(dict(route=llx.ROUTE_COPY_ENGINE)), alt_budgets),
+                  ("full-speed bulk kernel, one block per interval paced by the host", feeder_per_block(None), alt_budgets)]
+    for label, feed, bl in mechanisms:
+        for budget in bl:
+            on, off = [], []
+            for _ in range(segments):
+                t = run_steps(seg_steps)
+                off += t[20:-20]
+                stop = threading.Event()
+
+                def run_feeder():
+                    torch.cuda.set_device(dev)
+                    feed(budget, stop)
+                th = threading.Thread(target=run_feeder)
+                th.start()
+                run_steps(10)                         # the first stage is on the device
+                t = run_steps(seg_steps)
+                on += t[20:-20]
+                stop.set()
+                th.join()
+                s_mig.synchronize()
+            res["cases"].append({"mechanism": label, "bandwidth_budget_GBps": budget, "decode_step_off_ms": statistics.median(off),
+                                 "decode_step_on_ms": statistics.median(on),
+                                 "slowdown_pct": 100.0 * (statistics.median(on) / statistics.median(off) - 1.0), "steps_each": len(on)})
     res["end_clocks"] = clocks()
     res["note"] = "decode loop never pauses; ON = budgeted 16-block stages kept in flight by a host thread; 20 steps dropped at both ends of every segment"
     del p
