@@ -262,7 +262,7 @@ def run_reference(args):
 class Workload:
     """Two LLaMA-7B-shaped pools on the current device and the configs[1] request."""
 
-    def __init__(self, torch, llx, cfg="llama7b", num_blocks=None, src_blocks=None):
+    def __init__(self, torch, llx, cfg="llama7b", num_blocks=None, src_blocks=None, overlap=True):
         g = dict(synth.CONFIGS[cfg])
         if num_blocks:
             g["num_blocks"] = num_blocks
@@ -297,6 +297,11 @@ class Workload:
         self.append_dev = self.append_host.cuda()
         self.e_mid = (torch.cuda.Event(), torch.cuda.Event())
         self.e_app = (torch.cuda.Event(), torch.cuda.Event())
+        # Non-final stages are declared independent of the kernel before them (llx_launch_opts.overlap_prev): stage 0 reads
+        # and writes other blocks than the previous request's final stage, stage 1 other blocks than stage 0, and full
+        # blocks are never written again.  Completion order on the stream is unchanged.  The final stage
+        # keeps plain stream order (it reads the block the appends wrote).
+        self.stage_opts = llx.LaunchOpts(overlap_prev=1) if overlap else None
         self.k, self.primed = 0, False
         torch.cuda.synchronize()
 
@@ -347,7 +352,8 @@ class Workload:
                 self.e_mid[r].record(stream)               # the next step's appends (other request) may start from here
             if ev is not None and names[k] in ev:
                 ev[names[k]][0].record(stream)
-            llx.migrate_stage(self.src, s_tab[m:m + n], self.dst, d_tab[m:m + n], stream=stream)
+            llx.migrate_stage(self.src, s_tab[m:m + n], self.dst, d_tab[m:m + n], stream=stream,
+                              opts=self.stage_opts if k < len(SCHEDULE) - 1 else None)
             if ev is not None and names[k] in ev:
                 ev[names[k]][1].record(stream)
             m += n
@@ -381,7 +387,7 @@ def run_llx(args):
     world, rank, local = dist_setup(torch, args.gpus)
     peak, peak_src = measured_peak()
 
-    w = Workload(torch, llx)
+    w = Workload(torch, llx, overlap=not args.no_overlap and not args.serial_appends)
     g = w.g
     assert llx.plan_stage(START_TOKENS + sum(APPENDS), sum(SCHEDULE[:-1]), g["block_size"], 2) == (SCHEDULE[-1], True)
     stream = torch.cuda.Stream()
@@ -526,6 +532,10 @@ def run_llx(args):
                               "consecutive steps migrate two such requests alternately",
                    "streams": ("copies on the migration stream, appends on the source's decode stream (PAPER.md:134, :235); the final "
                                "stage waits for the appends" if dec is not None else "everything on one stream (--serial-appends)"),
+                   "stage_order": ("stages 0 and 1 are launched with llx_launch_opts.overlap_prev=1 (independent of the kernel "
+                                   "before them: disjoint blocks; they may start while it drains, completion order kept); "
+                                   "the final stage in plain stream order" if w.stage_opts is not None
+                                   else "plain stream order for every stage"),
                    "bytes_per_step_rd_plus_wr": step_bytes(g), "parallelism": f"replicas x{world} (no collective)",
                    "l2": "inputs larger than L2 (2.1 GB of traffic per step vs 126 MB L2), no flush needed",
                    "copy_kernel": "bulk-async smem ring (llx_copy_bulk)" if llx.get_option(llx.OPT_COPY_KERNEL) in (0, 2) else "vec16"},
@@ -660,6 +670,8 @@ def main():
     ap.add_argument("--suite", action="store_true", help="also run the length sweep, 30B batch and interference configs")
     ap.add_argument("--downtime-reps", type=int, default=100)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-overlap", action="store_true",
+                    help="launch every stage in plain stream order (no llx_launch_opts.overlap_prev on stages 0 and 1)")
     ap.add_argument("--serial-appends", action="store_true",
                     help="enqueue the appends on the migration stream between the stages (round-1 behaviour) instead of a decode stream")
     args = ap.parse_args()

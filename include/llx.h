@@ -172,6 +172,7 @@ typedef struct llx_launch_opts {
     int32_t exact_residency;   /* LLX_OPT_EXACT_RESIDENCY */
     int32_t via_host_mode;     /* LLX_OPT_VIA_HOST_MODE */
     int32_t route;             /* llx_route; LLX_OPT_DEFAULT = LLX_ROUTE_AUTO */
+    int32_t overlap_prev;      /* LLX_OPT_OVERLAP_PREV: 1 = this copy is independent of the previous kernel on its stream */
 } llx_launch_opts;
 /* Sets struct_size and every field to LLX_OPT_DEFAULT. */
 void llx_launch_opts_init(llx_launch_opts* opts);
@@ -436,6 +437,17 @@ typedef enum {
                                    split waits for the end of a slice, not of the stage (75 ms for 112 blocks at 25 GB/s).
                                    Default 1000; 0 = one launch.  Costs ~3 us of host time per slice inside the call; the rate
                                    and the decode step's slowdown are unchanged (measured).  Counters count every launch */
+    LLX_OPT_OVERLAP_PREV = 17,  /* 1: the caller states that this copy is INDEPENDENT of the kernel enqueued just before it on
+                                   cuda_stream — it reads no byte that kernel writes and writes no byte that kernel reads or
+                                   writes.  True for consecutive stages of one request (disjoint blocks on both sides; full
+                                   blocks are never written again) and for stages of different requests
+                                   (PAPER.md:225).  The copy may then START while that kernel's slowest CTAs are still running
+                                   (the wait of the programmatic dependent launch moves from the kernel's prologue to its end),
+                                   which hides the ~3 us an SM otherwise idles between two stages.  COMPLETION order is kept:
+                                   when this copy has completed, everything enqueued before it on the stream has completed, so
+                                   events, synchronises and later kernels see both.  Dependencies that cross streams (an event
+                                   wait before the call) are honoured as always.  Only the unthrottled bulk ring with
+                                   LLX_OPT_PDL uses it; every other kernel / route ignores it.  Default 0: plain stream order */
     LLX_OPT_VIA_HOST_MODE = 11  /* the host leg of llx_pack / llx_unpack / llx_migrate_via_host with a pinned-host buffer.
                                    0 (default) auto: llx_migrate_via_host lets the copy engines gather and scatter by themselves
                                    (mode 2; measured 93.8 vs 84.9 GB/s), llx_pack / llx_unpack go through the bounce buffers

@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(HERE, "libllx.so")
 F16, BF16, U8 = 0, 1, 2
 (OPT_COPY_KERNEL, OPT_MAX_CTAS, OPT_CHUNK_BYTES, OPT_RING_STAGES, OPT_IDS_BY_VALUE_MAX, OPT_ATTN_SPLIT_TOKENS,
  OPT_UNIT_ORDER, OPT_L2_HINT, OPT_RINGS_PER_CTA, OPT_PDL, OPT_BANDWIDTH_GBPS, OPT_VIA_HOST_MODE, OPT_DYNAMIC_TAIL_PCT,
- OPT_DYNAMIC_TAIL_BATCH, OPT_EXACT_RESIDENCY, OPT_COPY_SMEM_CARVEOUT_PCT, OPT_PACED_SLICE_US) = range(17)
+ OPT_DYNAMIC_TAIL_BATCH, OPT_EXACT_RESIDENCY, OPT_COPY_SMEM_CARVEOUT_PCT, OPT_PACED_SLICE_US,
+ OPT_OVERLAP_PREV) = range(18)
 
 _vp, _i, _sz, _i32p = C.c_void_p, C.c_int, C.c_size_t, C.POINTER(C.c_int32)
 
@@ -38,7 +39,7 @@ class LaunchOpts(C.Structure):
     _fields_ = [("struct_size", C.c_uint32)] + [(k, C.c_int32) for k in (
         "bandwidth_gbps", "max_ctas", "copy_kernel", "chunk_bytes", "ring_stages", "rings_per_cta", "ids_by_value_max",
         "unit_order", "l2_hint", "pdl", "dynamic_tail_pct", "dynamic_tail_batch", "exact_residency", "via_host_mode",
-        "route")]
+        "route", "overlap_prev")]
 
     def __init__(self, **kw):
         super().__init__()
@@ -527,7 +528,8 @@ def options(**kw):
                  rings_per_cta=OPT_RINGS_PER_CTA, pdl=OPT_PDL, bandwidth_gbps=OPT_BANDWIDTH_GBPS,
                  via_host_mode=OPT_VIA_HOST_MODE, dynamic_tail_pct=OPT_DYNAMIC_TAIL_PCT,
                  dynamic_tail_batch=OPT_DYNAMIC_TAIL_BATCH, exact_residency=OPT_EXACT_RESIDENCY,
-                 copy_smem_carveout_pct=OPT_COPY_SMEM_CARVEOUT_PCT, paced_slice_us=OPT_PACED_SLICE_US)
+                 copy_smem_carveout_pct=OPT_COPY_SMEM_CARVEOUT_PCT, paced_slice_us=OPT_PACED_SLICE_US,
+                 overlap_prev=OPT_OVERLAP_PREV)
     old = {k: get_option(names[k]) for k in kw}
     try:
         for k, v in kw.items():

@@ -67,7 +67,7 @@ int elem_bytes_of(llx_dtype d) {
 
 // ---- options / counters -------------------------------------------------------------------
 std::atomic<long long> g_opt_kernel{0}, g_opt_max_ctas{0}, g_opt_chunk{0}, g_opt_stages{0}, g_opt_byval{kIdsByValueCap},
-    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1}, g_opt_carveout{50}, g_opt_slice_us{1000};
+    g_opt_attn_split{0}, g_opt_order{1}, g_opt_l2hint{0}, g_opt_rings{0}, g_opt_pdl{1}, g_opt_budget{0}, g_opt_via_host{0}, g_opt_dyn_pct{6}, g_opt_dyn_batch{0}, g_opt_smem_pad{1}, g_opt_carveout{50}, g_opt_slice_us{1000}, g_opt_overlap{0};
 std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g_id_uploads{0};
 
 // Range of every option: shared by llx_set_option (process defaults) and by the per-call llx_launch_opts.
@@ -90,6 +90,7 @@ bool opt_valid(int opt, long long v) {
         case LLX_OPT_EXACT_RESIDENCY: return v >= 0 && v <= 1;
         case LLX_OPT_COPY_SMEM_CARVEOUT_PCT: return v >= 0 && v <= 100;
         case LLX_OPT_PACED_SLICE_US: return v >= 0 && v <= 1000000;
+        case LLX_OPT_OVERLAP_PREV: return v >= 0 && v <= 1;
     }
     return false;
 }
@@ -97,7 +98,7 @@ bool opt_valid(int opt, long long v) {
 // The launch policy of ONE call: the process defaults overridden by whatever the call's llx_launch_opts sets.
 // Resolved once at the entry point and passed down by value, so concurrent callers never see each other's policy.
 struct Policy {
-    long long kernel, max_ctas, chunk, stages, byval, order, l2hint, rings, pdl, budget, via_host, dyn_pct, dyn_batch, smem_pad;
+    long long kernel, max_ctas, chunk, stages, byval, order, l2hint, rings, pdl, budget, via_host, dyn_pct, dyn_batch, smem_pad, overlap;
     int route;
 };
 
@@ -116,6 +117,7 @@ llx_status resolve_policy(const llx_launch_opts* o, Policy* p) {
     p->dyn_pct = g_opt_dyn_pct.load();
     p->dyn_batch = g_opt_dyn_batch.load();
     p->smem_pad = g_opt_smem_pad.load();
+    p->overlap = g_opt_overlap.load();
     p->route = LLX_ROUTE_AUTO;
     if (o) {
         // a caller compiled against an older, shorter struct is served: fields beyond its struct_size keep the defaults
@@ -140,6 +142,7 @@ llx_status resolve_policy(const llx_launch_opts* o, Policy* p) {
         LLX_FIELD(dynamic_tail_batch, LLX_OPT_DYNAMIC_TAIL_BATCH, dyn_batch)
         LLX_FIELD(exact_residency, LLX_OPT_EXACT_RESIDENCY, smem_pad)
         LLX_FIELD(via_host_mode, LLX_OPT_VIA_HOST_MODE, via_host)
+        LLX_FIELD(overlap_prev, LLX_OPT_OVERLAP_PREV, overlap)
 #undef LLX_FIELD
         if (offsetof(llx_launch_opts, route) + sizeof(int32_t) <= o->struct_size && o->route != LLX_OPT_DEFAULT) {
             if (o->route != LLX_ROUTE_AUTO && o->route != LLX_ROUTE_PEER && o->route != LLX_ROUTE_COPY_ENGINE)
@@ -595,6 +598,9 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     a.blocked_order = (int)pol.order;
     a.l2_hint = (int)pol.l2hint;
     a.pace_ns = (int)pace_ns;
+    // LLX_OPT_OVERLAP_PREV: only the unthrottled bulk ring starts before the previous kernel has finished, and only with
+    // programmatic dependent launch (without it the stream serialises the kernels anyway)
+    a.defer_wait = (kern == 2 && pol.overlap != 0 && pol.pdl != 0 && budget <= 0) ? 1 : 0;
     a.dyn_units = 0;
     a.dyn_batch = 1;
     a.dyn_claims = 0;
@@ -1557,6 +1563,7 @@ llx_status llx_set_option(llx_option opt, long long v) {
         case LLX_OPT_EXACT_RESIDENCY: g_opt_smem_pad = v; break;
         case LLX_OPT_COPY_SMEM_CARVEOUT_PCT: g_opt_carveout = v; break;  // applied to the kernel at the next copy launch
         case LLX_OPT_PACED_SLICE_US: g_opt_slice_us = v; break;
+        case LLX_OPT_OVERLAP_PREV: g_opt_overlap = v; break;
     }
     return LLX_OK;
 }
@@ -1579,6 +1586,7 @@ long long llx_get_option(llx_option opt) {
         case LLX_OPT_EXACT_RESIDENCY: return g_opt_smem_pad;
         case LLX_OPT_COPY_SMEM_CARVEOUT_PCT: return g_opt_carveout;
         case LLX_OPT_PACED_SLICE_US: return g_opt_slice_us;
+        case LLX_OPT_OVERLAP_PREV: return g_opt_overlap;
     }
     return -1;
 }

@@ -7,6 +7,7 @@
 //   the source's check after each stage ("has completed or been preempted")
 //   abort when the other side fails
 //   release on the source + commit on the destination after the final stage
+#include <cstring>
 #include <new>
 #include <vector>
 
@@ -211,7 +212,9 @@ llx_status llx_migration_stage(llx_migration* g, const int32_t* table, int table
         // the final stage is the downtime: never throttled; earlier stages follow the session's policy
         llx_launch_opts o;
         if (g->has_opts) o = g->stage_opts; else llx_launch_opts_init(&o);
-        if (fin) o.bandwidth_gbps = 0, o.max_ctas = 0;
+        // ... and never started early: it reads the block the source was still appending to (stream order against the
+        // appends must hold), while a non-final stage only reads full blocks nobody writes any more (A3)
+        if (fin) o.bandwidth_gbps = 0, o.max_ctas = 0, o.overlap_prev = 0;
         rc = llx_migrate_stage_ex(g->src, table + m, g->dst, ids.data(), n, stream, (g->has_opts || fin) ? &o : nullptr);
         if (rc != LLX_OK) {  // nothing was launched: give the reservation back, the session stays where it was
             llx_blockmgr_release(g->dst_mgr, ids.data(), n);
@@ -236,9 +239,12 @@ llx_status llx_migration_set_stage_opts(llx_migration* g, const llx_launch_opts*
         g->has_opts = false;
         return LLX_OK;
     }
-    if (opts->struct_size != sizeof(llx_launch_opts))
+    // a caller compiled against an older, shorter struct is served (as in the *_ex calls): later fields keep the defaults
+    if (opts->struct_size < 2 * sizeof(int32_t) || opts->struct_size > sizeof(llx_launch_opts) || (opts->struct_size % sizeof(int32_t)) != 0)
         return fail(LLX_ERR_INVALID_ARG, "llx_launch_opts.struct_size = %u (this library: %zu); use llx_launch_opts_init", opts->struct_size, sizeof(llx_launch_opts));
-    g->stage_opts = *opts;
+    llx_launch_opts_init(&g->stage_opts);
+    memcpy(&g->stage_opts, opts, opts->struct_size);
+    g->stage_opts.struct_size = (uint32_t)sizeof(llx_launch_opts);
     g->has_opts = true;
     return LLX_OK;
 }

@@ -50,6 +50,8 @@ struct CopyArgs {
     int blocked_order;  // 0: worker w takes units w, w+W, ...; 1: worker w takes a contiguous range
     int l2_hint;        // bit0: loads L2::evict_first, bit1: stores L2::evict_first (bulk kernel)
     int pace_ns;        // bulk kernel: minimum time between two chunks of one ring (0 = unthrottled)
+    int defer_wait;     // bulk kernel, LLX_OPT_OVERLAP_PREV: the copy is independent of the previous kernel of its stream, so
+                        // griddepcontrol.wait moves from the prologue to just before the first dynamic claim / the exit
     // bulk kernel, blocked order: the last dyn_units units are not pre-assigned; rings that finish their
     // contiguous range early claim them in batches of dyn_batch from *dyn_counter (evens out the tail)
     int dyn_units, dyn_batch;
@@ -252,7 +254,14 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     pdl_launch_dependents();
-    pdl_wait_prior_grids();
+    // A copy the caller declared independent of the previous kernel (stages of disjoint blocks) starts
+    // streaming as soon as its CTA is resident, i.e. while the previous stage's slowest rings are still draining.  The
+    // wait is only deferred, never dropped: (1) a ring executes it before its first claim from the dynamic-tail counter,
+    // which the previous launch shares and resets with its last claim; (2) every ring executes it before it exits, so
+    // "this kernel has completed" still implies "everything before it on the stream has completed" (completion stays
+    // transitive although the start is not ordered).
+    bool waited = a.defer_wait == 0;
+    if (waited) pdl_wait_prior_grids();
 
     const int ring = blockIdx.x * rings_per_cta + warp;
     const int nrings = gridDim.x * rings_per_cta;
@@ -278,6 +287,10 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
         }
         if (d_next < d_end) return d_next++;
         if (dyn_done) return -1;
+        if (!waited) {
+            pdl_wait_prior_grids();
+            waited = true;
+        }
         const unsigned int b = atomicAdd(a.dyn_counter, 1u);
         if (b == a.dyn_claims - 1) *a.dyn_counter = 0;  // every ring fails exactly once: this was the launch's last claim
         const long long lo = (long long)b * a.dyn_batch;
@@ -347,6 +360,7 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
         }
     }
     bulk_wait_all();  // this ring's stores are complete
+    if (!waited) pdl_wait_prior_grids();
     if (a.done_counter) {
         __threadfence();
         if (atomicAdd(a.done_counter, 1u) == a.done_rings - 1) {  // every ring has finished its stores

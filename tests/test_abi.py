@@ -177,11 +177,12 @@ def test_launch_opts_are_validated_before_any_device_work(llx):
     library does not know is LLX_ERR_INVALID_ARG — reported before the pools are even looked at (so also without a GPU)."""
     import ctypes as C
     o = llx.LaunchOpts()
-    assert o.struct_size == C.sizeof(llx.LaunchOpts) == 64
+    assert o.struct_size == C.sizeof(llx.LaunchOpts) == 68
     assert all(getattr(o, f) == llx.OPT_DEFAULT for f, _ in o._fields_ if f != "struct_size")
     l = llx.lib()
     ids = (C.c_int32 * 2)(0, 1)
-    for bad in (dict(chunk_bytes=100), dict(copy_kernel=7), dict(bandwidth_gbps=-5), dict(route=9), dict(ring_stages=1)):
+    for bad in (dict(chunk_bytes=100), dict(copy_kernel=7), dict(bandwidth_gbps=-5), dict(route=9), dict(ring_stages=1),
+                dict(overlap_prev=2)):
         rc = l.llx_migrate_stage_ex(None, ids, None, ids, 2, None, C.byref(llx.LaunchOpts(**bad)))
         assert rc == -1 and b"llx_launch_opts." in l.llx_last_error(), (bad, l.llx_last_error())
     o = llx.LaunchOpts()
@@ -211,15 +212,19 @@ def test_ipc_handle_is_checked(llx):
         llx.pool_ipc_open(b"short")
     out = C.c_void_p()
     assert l.llx_pool_ipc_open(None, C.byref(out)) == -1 and l.llx_pool_ipc_export(None, None) == -1
-    # session policy: a struct of another size is refused, NULL resets
+    # session policy: a struct size the library cannot read is refused (an older, shorter struct is served), NULL resets
     a, b = llx.BlockManager(8), llx.BlockManager(8)
     mig = llx.Migration(None, a, None, b, 4, 1)
     mig.set_stage_opts(dict(bandwidth_gbps=25))
     mig.set_stage_opts(None)
     bad = llx.LaunchOpts()
-    bad.struct_size = 8
-    with pytest.raises(llx.LlxError):
-        mig.set_stage_opts(bad)
+    for size in (6, 400):
+        bad.struct_size = size
+        with pytest.raises(llx.LlxError):
+            mig.set_stage_opts(bad)
+    older = llx.LaunchOpts(bandwidth_gbps=25, overlap_prev=1)
+    older.struct_size = 64                                               # round 2's struct before overlap_prev was added
+    mig.set_stage_opts(older)
     with pytest.raises(llx.LlxError) as e:
         mig.stage([3, 3, 4, 5], 14)                                       # a table that names a block twice (A33)
     assert e.value.name == "LLX_ERR_INVALID_ARG" and b.num_free == 8

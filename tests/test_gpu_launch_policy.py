@@ -272,3 +272,105 @@ def test_sliced_budgeted_stage_is_bit_exact(env, slice_us, unit_order, ids_by_va
         llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, opts=dict(bandwidth_gbps=40))
         assert llx.counters()["copy_launches"] - c0 == 1
     H.assert_pool_equal(dst.host(), h_dst)
+
+
+def test_overlapped_stages_are_bit_exact_and_complete_in_stream_order(env):
+    """LLX_OPT_OVERLAP_PREV (llx_launch_opts.overlap_prev): a stage the caller declares independent of the previous
+    kernel may START before that kernel has finished, but completion stays ordered.  A chain of stages over disjoint
+    blocks — long ones with the dynamic tail (whose claim counter consecutive launches share), a short one right behind
+    a long one (it could finish first if the deferred wait were dropped), a batch launch and a stage of more than 256
+    pairs — is enqueued back to back with the flag, then ONE event behind the last, smallest kernel is waited for: every
+    byte of every stage must be there, equal to the oracle's, and the untouched blocks keep the sentinel."""
+    H, llx = env
+    g = G7
+    sample = [0, 17, 31]
+    src, dst = H.DevPool(g), H.DevPool(g, fill=SENT)
+    src.fill_device_random(5)
+    src.fill_from_synth(0, 0, layers=sample)
+    perm_s = synth.block_permutation(11, g["num_blocks"])
+    perm_d = synth.block_permutation(12, g["num_blocks"])
+    cuts = [0, 112, 126, 128, 200, 264, 266, 267]                     # 112, 14, 2, 72 (batch), 64, 2, 1 blocks
+    stream = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    ov = dict(overlap_prev=1)
+    for rep in range(3):                                                # the same chain three times: the counter is reused
+        dst.view.fill_(SENT_I16)
+        torch.cuda.synchronize()
+        done = torch.cuda.Event()
+        for k in range(len(cuts) - 1):
+            a, b = cuts[k], cuts[k + 1]
+            if b - a == 72:
+                off = [0, 10, 10, 41, 72]                               # four requests, one of them empty
+                llx.migrate_batch(src.pool, dst.pool, off, perm_s[a:b], perm_d[a:b], stream=stream, opts=ov)
+            else:
+                llx.migrate_stage(src.pool, perm_s[a:b], dst.pool, perm_d[a:b], stream=stream, opts=ov)
+        done.record(stream)
+        done.synchronize()                                              # NOT a device synchronize: only what the stream orders
+        got = dst.view[sample].cpu().numpy().view(np.uint16)
+        h_src = H.host_pool_from_synth(g, 0, 0, layers=sample)
+        want = om.new_pool(len(sample), g["num_blocks"], src.te, fill=SENT)
+        om.migrate_stage(h_src, perm_s[:cuts[-1]], want, perm_d[:cuts[-1]])
+        H.assert_pool_equal(got, want)
+    # layers the host does not mirror: every copied block equals its source block, element-wise on the device
+    idx_s = torch.from_numpy(np.asarray(perm_s[:cuts[-1]], dtype=np.int64)).cuda()
+    idx_d = torch.from_numpy(np.asarray(perm_d[:cuts[-1]], dtype=np.int64)).cuda()
+    for l in range(g["layers"]):
+        assert torch.equal(dst.view[l].index_select(1, idx_d), src.view[l].index_select(1, idx_s)), l
+
+
+def test_overlap_keeps_completion_transitive_behind_a_long_stage(env):
+    """The property the deferred wait exists for: 'kernel N+1 has completed' implies 'kernel N has completed'.  A
+    256-block stage (about 650 us) is followed by a ONE-block stage with overlap_prev=1 (about 10 us of work) and an
+    event; as soon as the event has fired the long stage's LAST blocks are read back — they must already be complete.
+    Repeated with fresh sentinel fills so that a stale pass cannot hide a miss.  Also: a stream-captured pair of
+    overlapped stages replays bit-exactly (the flag touches no host state)."""
+    H, llx = env
+    g = dict(G7, num_blocks=600)
+    src, dst = H.DevPool(g), H.DevPool(g, fill=SENT)
+    src.fill_device_random(9)
+    perm_s = synth.block_permutation(21, g["num_blocks"])
+    perm_d = synth.block_permutation(22, g["num_blocks"])
+    n_long = 256
+    stream = torch.cuda.Stream()
+    idx_s = torch.from_numpy(np.asarray(perm_s[:n_long + 1], dtype=np.int64)).cuda()
+    idx_d = torch.from_numpy(np.asarray(perm_d[:n_long + 1], dtype=np.int64)).cuda()
+    want = [src.view[l].index_select(1, idx_s) for l in (0, 31)]
+    torch.cuda.synchronize()
+    for rep in range(20):
+        dst.view[:, :, :, ::512].fill_(SENT_I16)                        # cheap invalidation: one word per KiB of every tile
+        torch.cuda.synchronize()
+        ev = torch.cuda.Event()
+        llx.migrate_stage(src.pool, perm_s[:n_long], dst.pool, perm_d[:n_long], stream=stream, opts=dict(ids_by_value_max=256))
+        llx.migrate_stage(src.pool, perm_s[n_long:n_long + 1], dst.pool, perm_d[n_long:n_long + 1], stream=stream,
+                          opts=dict(overlap_prev=1))
+        ev.record(stream)
+        ev.synchronize()
+        check = torch.cuda.Stream()                                     # an unrelated stream: no implicit ordering helps
+        with torch.cuda.stream(check):
+            got = [dst.view[l].index_select(1, idx_d) for l in (0, 31)]
+        check.synchronize()
+        for gl, wl in zip(got, want):
+            assert torch.equal(gl, wl), rep
+    # capture: two overlapped stages in one graph, replayed on another stream
+    a, b = perm_s[300:364], perm_s[364:380]
+    da, db = perm_d[300:364], perm_d[364:380]
+    cap = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(cap):
+        llx.migrate_stage(src.pool, a, dst.pool, da, stream=cap, opts=dict(overlap_prev=1))     # warm-up outside the capture
+        cap.synchronize()
+        graph.capture_begin()
+        llx.migrate_stage(src.pool, a, dst.pool, da, stream=cap, opts=dict(overlap_prev=1))
+        llx.migrate_stage(src.pool, b, dst.pool, db, stream=cap, opts=dict(overlap_prev=1))
+        graph.capture_end()
+    dst.view.fill_(SENT_I16)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(stream):
+        graph.replay()
+    stream.synchronize()
+    i_s = torch.from_numpy(np.asarray(perm_s[300:380], dtype=np.int64)).cuda()
+    i_d = torch.from_numpy(np.asarray(perm_d[300:380], dtype=np.int64)).cuda()
+    for l in range(g["layers"]):
+        assert torch.equal(dst.view[l].index_select(1, i_d), src.view[l].index_select(1, i_s)), l
+    untouched = np.setdiff1d(np.arange(g["num_blocks"]), np.asarray(perm_d[300:380]))
+    assert bool((dst.view[:, :, torch.from_numpy(untouched).cuda()] == SENT_I16).all())
