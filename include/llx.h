@@ -137,6 +137,18 @@ llx_status llx_pool_fill_u16(llx_pool* pool, uint16_t pattern, void* cuda_stream
 llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, int last_stage_max_blocks, int* n,
                           int* is_final);
 
+/* How many stages a migration will take, from MEASURED rates ("copying is generally much faster than the
+ * computation", so "the number of new blocks is typically small"; "the migration only takes two stages").
+ * While stage k copies n_k blocks at copy_blocks_per_s, the request decodes decode_tokens_per_s * n_k / copy_blocks_per_s
+ * tokens, i.e. the next stage has  n_{k+1} = max(1, ceil(n_k * decode_tokens_per_s / (copy_blocks_per_s * block_size)))
+ * blocks; the sequence ends with the first stage of ONE block (the final stage).  Writes n_0 = n0, n_1, ... to sizes_out
+ * (HOST int32[cap]) and their count to *n_stages.  A caller picks a bandwidth budget for the non-final stages with it:
+ * copy_blocks_per_s = budget / (2 * block_bytes); if the sequence has not reached 1 within cap entries (the last entry
+ * is > 1), decoding outruns the copy at that budget.  LLX_ERR_INVALID_ARG: n0 < 1, a rate that is not finite,
+ * copy_blocks_per_s <= 0, decode_tokens_per_s < 0, block_size <= 0, cap < 1.  Host arithmetic only. */
+llx_status llx_predict_stage_sizes(int n0, double copy_blocks_per_s, double decode_tokens_per_s, int block_size,
+                                   int32_t* sizes_out, int cap, int* n_stages);
+
 /* ---- launch policy of ONE call -------------------------------------------------------------------------------
  *
  * The paper's own scenario needs two policies at once: non-final stages must not slow the co-running requests

@@ -81,6 +81,7 @@ EXPORTS = {
     "llx_pool_download": (_i, [_vp, _i, _i, _i, _i, _vp, _vp]),
     "llx_pool_fill_u16": (_i, [_vp, C.c_uint16, _vp]),
     "llx_plan_stage": (_i, [_i, _i, _i, _i, C.POINTER(_i), C.POINTER(_i)]),
+    "llx_predict_stage_sizes": (_i, [_i, C.c_double, C.c_double, _i, _i32p, _i, C.POINTER(_i)]),
     "llx_launch_opts_init": (None, [C.POINTER(LaunchOpts)]),
     "llx_migrate_stage": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp]),
     "llx_migrate_stage_ex": (_i, [_vp, _i32p, _vp, _i32p, _i, _vp, C.POINTER(LaunchOpts)]),
@@ -265,6 +266,13 @@ def plan_stage(num_tokens: int, blocks_migrated: int, block_size: int, last_stag
     n, f = _i(), _i()
     _check(load().llx_plan_stage(num_tokens, blocks_migrated, block_size, last_stage_max_blocks, C.byref(n), C.byref(f)))
     return n.value, bool(f.value)
+
+
+def predict_stage_sizes(n0: int, copy_blocks_per_s: float, decode_tokens_per_s: float, block_size: int, cap: int = 64):
+    """-> [n_0, n_1, ...]: the stage sizes a migration takes at these measured rates (llx_predict_stage_sizes)."""
+    out, k = (C.c_int32 * cap)(), _i()
+    _check(load().llx_predict_stage_sizes(n0, copy_blocks_per_s, decode_tokens_per_s, block_size, out, cap, C.byref(k)))
+    return [int(out[i]) for i in range(k.value)]
 
 
 def migrate_stage(src: Pool, src_block_ids, dst: Pool, dst_block_ids, stream=None, opts=None):

@@ -4,6 +4,7 @@
 #include "../../include/llx.h"
 
 #include <atomic>
+#include <cmath>
 #include <cstdarg>
 #include <cstddef>
 #include <new>
@@ -1045,6 +1046,29 @@ llx_status llx_plan_stage(int num_tokens, int blocks_migrated, int block_size, i
     return LLX_OK;
 }
 
+llx_status llx_predict_stage_sizes(int n0, double copy_blocks_per_s, double decode_tokens_per_s, int block_size,
+                                   int32_t* sizes_out, int cap, int* n_stages) {
+    if (!sizes_out || !n_stages) return fail(LLX_ERR_INVALID_ARG, "NULL output");
+    *n_stages = 0;
+    if (n0 < 1 || block_size <= 0 || cap < 1 || !(copy_blocks_per_s > 0.0) || !(decode_tokens_per_s >= 0.0) ||
+        !std::isfinite(copy_blocks_per_s) || !std::isfinite(decode_tokens_per_s))
+        return fail(LLX_ERR_INVALID_ARG, "bad arguments (n0=%d, copy=%g blocks/s, decode=%g tokens/s, S=%d, cap=%d)", n0,
+                    copy_blocks_per_s, decode_tokens_per_s, block_size, cap);
+    int k = 0;
+    long long cur = n0;
+    sizes_out[k++] = (int32_t)cur;
+    while (cur > 1 && k < cap) {
+        // stage k lasts cur / c seconds, the request decodes r * cur / c tokens meanwhile = that many / S new blocks
+        double nxt = std::ceil((double)cur * decode_tokens_per_s / (copy_blocks_per_s * (double)block_size));
+        if (nxt < 1.0) nxt = 1.0;
+        if (nxt > 2147483647.0) return fail(LLX_ERR_INVALID_ARG, "stage sizes diverge (decoding outruns the copy)");
+        cur = (long long)nxt;
+        sizes_out[k++] = (int32_t)cur;
+    }
+    *n_stages = k;
+    return LLX_OK;
+}
+
 void llx_launch_opts_init(llx_launch_opts* o) {
     if (!o) return;
     memset(o, 0xFF, sizeof *o);  // every int32 field = -1 = LLX_OPT_DEFAULT
@@ -1101,6 +1125,7 @@ llx_status llx_migrate_stage_wait_ex(const llx_pool* src, const int32_t* src_ids
     if (rc != LLX_OK) return rc;
     pol.budget = 0;  // the final stage is the downtime: never throttled, whatever the defaults say
     pol.max_ctas = 0;
+    pol.overlap = 0;  // and it reads the block the source appended to last: plain stream order
     if (n <= 0 || !src) return migrate_stage_checked(pol, src, src_ids, dst, dst_ids, n, stream);  // nothing to wait for / argument error
     if ((rc = refuse_if_capturing((cudaStream_t)stream, "llx_migrate_stage_wait (a blocking call)")) != LLX_OK) return rc;
     DoneSlot* slot = nullptr;

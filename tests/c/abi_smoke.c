@@ -26,6 +26,13 @@ int main(void) {
     CHECK(llx_plan_stage(2032, 0, 16, 2, &n, &fin) == LLX_OK && n == 127 && fin == 0);
     CHECK(llx_plan_stage(2048, 126, 16, 2, &n, &fin) == LLX_OK && n == 2 && fin == 1);
     CHECK(llx_plan_stage(16, 2, 16, 2, &n, &fin) == LLX_ERR_INVALID_ARG);
+    {   /* stage sizes from measured rates: the paper's regime gives two stages */
+        int32_t sizes[8];
+        int k = 0;
+        CHECK(llx_predict_stage_sizes(128, 950.0, 15.4, 16, sizes, 8, &k) == LLX_OK && k == 2 && sizes[0] == 128 && sizes[1] == 1);
+        CHECK(llx_predict_stage_sizes(64, 4.0, 16.0, 16, sizes, 8, &k) == LLX_OK && k == 4 && sizes[3] == 1);
+        CHECK(llx_predict_stage_sizes(64, 4.0, 16.0, 16, sizes, 0, &k) == LLX_ERR_INVALID_ARG);
+    }
 
     /* the handshake without pools: coordination only */
     CHECK(llx_blockmgr_create(16, &a) == LLX_OK && llx_blockmgr_create(6, &b) == LLX_OK);

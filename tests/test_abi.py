@@ -121,6 +121,66 @@ def test_plan_stage_matches_oracle_on_every_state(llx):
             llx.plan_stage(*bad)
 
 
+def test_predicted_stage_sizes_match_oracle_and_a_time_stepped_simulation(llx):
+    """llx_predict_stage_sizes (the planner "driven by measured copy / decode rates")
+    against oracle.stage_sizes on seeded rates, and both against a pin that shares nothing with the recurrence: a
+    time-stepped simulation in exact rational arithmetic that copies blocks one by one while a decoder appends tokens."""
+    from fractions import Fraction
+
+    import numpy as np
+
+    from oracle import kv_migration as om
+
+    def simulate(n0, c, r, S, cap):
+        # stage k copies n_k blocks one after the other (1/c s each); tokens decoded in the stage's duration, counted
+        # exactly, turn into ceil(tokens / S) new blocks (at least the one open block of the final stage)
+        c, r = Fraction(c), Fraction(r)
+        sizes, n = [n0], n0
+        while n > 1 and len(sizes) < cap:
+            duration = sum((1 / c for _ in range(n)), Fraction(0)) if n <= 5000 else n / c
+            tokens = r * duration
+            blocks = -((-tokens.numerator) // (tokens.denominator * S))     # ceil(tokens / S) on exact rationals
+            n = max(1, int(blocks))
+            sizes.append(n)
+        return sizes
+
+    rng = np.random.default_rng(7)
+    for _ in range(300):
+        n0 = int(rng.integers(1, 600))
+        S = int(rng.choice([4, 16, 32]))
+        c = float(rng.integers(1, 4000)) / 4.0                                # quarter-integers: exact in binary and as Fraction
+        r = float(rng.integers(0, 4000)) / 4.0
+        if rng.random() < 0.8:                                                # mostly the convergent regime: c*S > r
+            c = max(c, float(int(2 * r / S) + 1))
+        want = om.stage_sizes(n0, c, r, S, max_stages=12)
+        if max(want) > 2**31 - 1:                                             # decoding outruns the copy: sizes leave int32
+            with pytest.raises(llx.LlxError):
+                llx.predict_stage_sizes(n0, c, r, S, cap=12)
+        else:
+            # (quotients below 2^31 with denominators below 2^17 are at least 7e-6 from an integer unless they are one:
+            # double rounding cannot move the ceiling, so the exact simulation and the double recurrence must agree)
+            assert want == simulate(n0, c, r, S, 12), (n0, c, r, S)
+            assert llx.predict_stage_sizes(n0, c, r, S, cap=12) == want, (n0, c, r, S)
+    # the paper's regime (PAPER.md:287): copy much faster than decode -> two stages, whatever the length
+    for n0 in (16, 128, 512):
+        assert llx.predict_stage_sizes(n0, 950.0, 15.4, 16) == [n0, 1]
+    # B200, LLaMA-7B blocks of 8 MiB: 6.5 TB/s rd+wr = 387,000 blocks/s unthrottled; 12 GB/s budget = 715 blocks/s;
+    # one request decoding at ~180 tokens/s (5.5 ms per step): two stages in both cases
+    assert llx.predict_stage_sizes(128, 387000.0, 180.0, 16) == [128, 1]
+    assert llx.predict_stage_sizes(128, 715.0, 180.0, 16) == [128, 3, 1]
+    assert llx.predict_stage_sizes(1, 1.0, 1.0, 16) == [1]
+    assert llx.predict_stage_sizes(64, 4.0, 16.0, 16) == [64, 16, 4, 1]
+    assert llx.predict_stage_sizes(64, 1.0, 64.0, 16, cap=5) == [64, 256, 1024, 4096, 16384]   # decoding outruns the copy
+    for bad in [(0, 1.0, 1.0, 16), (4, 0.0, 1.0, 16), (4, 1.0, -1.0, 16), (4, 1.0, 1.0, 0), (4, float("nan"), 1.0, 16),
+                (4, float("inf"), 1.0, 16)]:
+        with pytest.raises(llx.LlxError):
+            llx.predict_stage_sizes(*bad)
+    import ctypes as C
+    k = C.c_int()
+    assert llx.lib().llx_predict_stage_sizes(4, 1.0, 1.0, 16, (C.c_int32 * 1)(), 0, C.byref(k)) == -1     # cap = 0
+    assert llx.lib().llx_predict_stage_sizes(4, 1.0, 1.0, 16, None, 4, C.byref(k)) == -1
+
+
 def test_header_is_plain_c99_and_a_c_client_links_and_runs(llx, tmp_path):
     """The boundary is a C ABI: the header compiles as C99 with -pedantic, and a C program (tests/c/abi_smoke.c)
     drives the host-only entry points — planner, block manager, handshake, Algorithm 1 — through libllx.so."""
