@@ -385,6 +385,30 @@ llx_status llx_plan_migration_batch(const llx_req_info* reqs, const int32_t* seq
                                     int32_t* req_offsets_out, int32_t* src_ids_out, int32_t* dst_ids_out, int cap_pairs,
                                     int* n_pairs);
 
+/* ---- NEXT-1: the bandwidth budget of the non-final stages, chosen from what the engine observes ------------------
+ *
+ * live migration costs the co-running requests "nearly zero (up to 1%)".  On the paper's hardware that
+ * holds because the copy is slow; on a B200 the copy can take the whole HBM, so the share has to be CHOSEN
+ * (llx_launch_opts.bandwidth_gbps), and the budget that holds a given slowdown depends on the co-running batch, the
+ * GPU's power state and what else runs — only the engine sees that.  The engine therefore reports every decode step's
+ * duration, saying whether a budgeted stage was in flight, and asks the controller for the budget of the next stage.
+ * Rule (A34): every `window` steps observed WITH a migration,
+ *     s = median(those steps) / median(the last 2*window steps observed WITHOUT one) - 1
+ *     budget <- clamp(budget * f, min_gbps, max_gbps),   f = 2 if s <= target/4, else clamp(target / s, 1/2, 2).
+ * Steps with a migration are ignored until a step without one has been reported.  Host arithmetic only; one controller
+ * per decode loop; not thread-safe per object.  The final stage is never budgeted. */
+typedef struct llx_budget_ctl llx_budget_ctl;
+/* target_slowdown_pct > 0; 1 <= min_gbps <= start_gbps <= max_gbps <= 100000; 2 <= window <= 256. */
+llx_status llx_budget_ctl_create(double target_slowdown_pct, int min_gbps, int max_gbps, int start_gbps, int window,
+                                 llx_budget_ctl** out);
+llx_status llx_budget_ctl_destroy(llx_budget_ctl* ctl);
+/* One decode step took step_ms (> 0, finite); migrating != 0: a budgeted stage was in flight during it.
+ * *budget_gbps (may be NULL) = the budget to give the next non-final stage. */
+llx_status llx_budget_ctl_observe(llx_budget_ctl* ctl, double step_ms, int migrating, int* budget_gbps);
+int    llx_budget_ctl_gbps(const llx_budget_ctl* ctl);              /* current budget, GB/s read + written; -1 on NULL */
+double llx_budget_ctl_last_slowdown_pct(const llx_budget_ctl* ctl); /* s of the last adjustment in %, NaN before the first */
+int    llx_budget_ctl_adjustments(const llx_budget_ctl* ctl);       /* adjustments made so far; -1 on NULL */
+
 /* ---- S8: append-only growth while decoding continues --------------- */
 
 /* Writes the K and V vectors of tokens t0..t1-1 of one request into their slots: token t
@@ -459,7 +483,10 @@ typedef enum {
                                    when this copy has completed, everything enqueued before it on the stream has completed, so
                                    events, synchronises and later kernels see both.  Dependencies that cross streams (an event
                                    wait before the call) are honoured as always.  Only the unthrottled bulk ring with
-                                   LLX_OPT_PDL uses it; every other kernel / route ignores it.  Default 0: plain stream order */
+                                   LLX_OPT_PDL uses it; every other kernel / route ignores it, and so do llx_migrate_stage_wait
+                                   and a session's final stage (they read the block the source appended to last) and the routes
+                                   whose own kernels depend on one another (llx_migrate_via_host, pinned-host llx_pack /
+                                   llx_unpack).  Default 0: plain stream order */
     LLX_OPT_VIA_HOST_MODE = 11  /* the host leg of llx_pack / llx_unpack / llx_migrate_via_host with a pinned-host buffer.
                                    0 (default) auto: llx_migrate_via_host lets the copy engines gather and scatter by themselves
                                    (mode 2; measured 93.8 vs 84.9 GB/s), llx_pack / llx_unpack go through the bounce buffers

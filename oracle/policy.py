@@ -141,3 +141,56 @@ def plan_migration_batch(instance: Instance, seq_len, block_tables, src_below: f
         req_offsets.append(len(src_ids))
         remaining.remove(r)
     return chosen, req_offsets, src_ids, dst_ids
+
+
+# --------------------------------------------------------------------------
+# Bandwidth budget of the non-final stages, chosen from the decode steps the engine observes
+# ("nearly zero (up to 1%) overhead" on the co-running requests).
+# The paper states the bound, not a mechanism — on its hardware the copy is too slow to matter.  Reading A34
+# (DESIGN.md): a multiplicative feedback rule on medians of observed step times.
+# --------------------------------------------------------------------------
+def _median(xs):
+    s = sorted(xs)
+    n = len(s)
+    return s[n // 2] if n % 2 else (s[n // 2 - 1] + s[n // 2]) / 2.0
+
+
+class BudgetController:
+    """budget <- clamp(budget * f, min, max) every `window` steps observed WITH a migration in flight, where
+        s = median(those steps) / median(the last 2*window steps observed WITHOUT one) - 1     (the slowdown)
+        f = 2                      if s <= target / 4      (cost within noise of zero: probe upwards)
+            clamp(target / s, 1/2, 2)   otherwise
+    Steps with a migration are dropped until at least one step without has been seen."""
+
+    def __init__(self, target_pct: float, min_gbps: int, max_gbps: int, start_gbps: int, window: int):
+        if not (target_pct > 0 and 1 <= min_gbps <= start_gbps <= max_gbps and 2 <= window <= 256):
+            raise ValueError("bad arguments")
+        self.target = target_pct / 100.0
+        self.lo, self.hi, self.window = float(min_gbps), float(max_gbps), window
+        self.budget = float(start_gbps)
+        self.base, self.mig = [], []
+        self.last_slowdown_pct = math.nan
+        self.adjustments = 0
+
+    def gbps(self) -> int:
+        return int(math.floor(self.budget + 0.5))
+
+    def observe(self, step_ms: float, migrating: bool) -> int:
+        if not (step_ms > 0 and math.isfinite(step_ms)):
+            raise ValueError("step_ms")
+        if not migrating:
+            self.base.append(step_ms)
+            if len(self.base) > 2 * self.window:
+                self.base.pop(0)
+            return self.gbps()
+        if not self.base:
+            return self.gbps()
+        self.mig.append(step_ms)
+        if len(self.mig) >= self.window:
+            s = _median(self.mig) / _median(self.base) - 1.0
+            f = 2.0 if s <= self.target / 4.0 else min(2.0, max(0.5, self.target / s))
+            self.budget = min(self.hi, max(self.lo, self.budget * f))
+            self.last_slowdown_pct = 100.0 * s
+            self.adjustments += 1
+            self.mig = []
+        return self.gbps()

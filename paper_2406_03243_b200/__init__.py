@@ -13,7 +13,7 @@ from .binding import (  # noqa: F401
     plan_stage, predict_stage_sizes, migrate_stage, migrate_stage_wait, migrate_batch, staging_bytes, PinnedStaging, pack, unpack, migrate_via_host,
     append_tokens, decode_attention,
     calc_freeness, pair_instances, migration_order, plan_migration_batch,
-    BlockManager, Migration, REQ_RUNNING, REQ_FINISHED, REQ_PREEMPTED, REQ_PEER_FAILED,
+    BlockManager, Migration, BudgetController, REQ_RUNNING, REQ_FINISHED, REQ_PREEMPTED, REQ_PEER_FAILED,
     MIG_READY, MIG_COPYING, MIG_FINAL_COPYING, MIG_COMMITTED, MIG_ABORTED,
     ABORT_NONE, ABORT_FINISHED, ABORT_PREEMPTED, ABORT_PEER_FAILED, ABORT_NO_SPACE,
     set_option, get_option, options, synchronize, counters, reset_counters, version, EXPORTS,

@@ -109,6 +109,12 @@ EXPORTS = {
     "llx_migration_commit": (_i, [_vp, _i32p, _i, _i, _i32p, _i, C.POINTER(_i)]),
     "llx_migration_abort": (_i, [_vp, _i]),
     "llx_migration_set_stage_opts": (_i, [_vp, C.POINTER(LaunchOpts)]),
+    "llx_budget_ctl_create": (_i, [C.c_double, _i, _i, _i, _i, C.POINTER(_vp)]),
+    "llx_budget_ctl_destroy": (_i, [_vp]),
+    "llx_budget_ctl_observe": (_i, [_vp, C.c_double, _i, C.POINTER(_i)]),
+    "llx_budget_ctl_gbps": (_i, [_vp]),
+    "llx_budget_ctl_last_slowdown_pct": (C.c_double, [_vp]),
+    "llx_budget_ctl_adjustments": (_i, [_vp]),
     "llx_migration_state": (_i, [_vp]),
     "llx_migration_abort_reason": (_i, [_vp]),
     "llx_migration_blocks_migrated": (_i, [_vp]),
@@ -397,6 +403,30 @@ class BlockManager:
         with contextlib.suppress(Exception):
             if self._h:
                 load().llx_blockmgr_destroy(self._h)
+                self._h = 0
+
+
+class BudgetController:
+    """The bandwidth budget of the non-final stages chosen from the decode steps the engine observes (llx_budget_ctl*)."""
+
+    def __init__(self, target_slowdown_pct: float, min_gbps: int, max_gbps: int, start_gbps: int, window: int = 8):
+        h = _vp()
+        _check(load().llx_budget_ctl_create(float(target_slowdown_pct), min_gbps, max_gbps, start_gbps, window, C.byref(h)))
+        self._h = h.value
+
+    gbps = property(lambda self: load().llx_budget_ctl_gbps(self._h))
+    last_slowdown_pct = property(lambda self: load().llx_budget_ctl_last_slowdown_pct(self._h))
+    adjustments = property(lambda self: load().llx_budget_ctl_adjustments(self._h))
+
+    def observe(self, step_ms: float, migrating: bool) -> int:
+        b = _i()
+        _check(load().llx_budget_ctl_observe(self._h, float(step_ms), 1 if migrating else 0, C.byref(b)))
+        return b.value
+
+    def __del__(self):
+        with contextlib.suppress(Exception):
+            if self._h:
+                load().llx_budget_ctl_destroy(self._h)
                 self._h = 0
 
 

@@ -1260,8 +1260,10 @@ llx_status llx_pack_ex(const llx_pool* src, const int32_t* src_ids, int n, void*
         if ((rc = refuse_if_capturing((cudaStream_t)stream, "llx_pack into pinned host memory")) != LLX_OK) return rc;
         return ce_blocks(true, src, src_ids, 0, n, stg, (cudaStream_t)stream);
     }
-    if (stg.host_memory && (pol.via_host == 0 || pol.via_host == 3) && pol.kernel == 0)
+    if (stg.host_memory && (pol.via_host == 0 || pol.via_host == 3) && pol.kernel == 0) {
+        pol.overlap = 0;  // a chain of dependent kernels and transfers through one bounce buffer: plain stream order
         return staged_through_bounce(pol, true, src, src_ids, n, stg, (cudaStream_t)stream);
+    }
     return launch_copy(pol, pool_side(src, src_ids), stg, n, src->layers, src->tile_bytes, src->device, (cudaStream_t)stream);
     LLX_CATCH
 }
@@ -1291,8 +1293,10 @@ llx_status llx_unpack_ex(const void* staging, size_t staging_bytes, llx_pool* ds
         if ((rc = refuse_if_capturing((cudaStream_t)stream, "llx_unpack from pinned host memory")) != LLX_OK) return rc;
         return ce_blocks(false, dst, dst_ids, 0, n, stg, (cudaStream_t)stream);
     }
-    if (stg.host_memory && (pol.via_host == 0 || pol.via_host == 3) && pol.kernel == 0)
+    if (stg.host_memory && (pol.via_host == 0 || pol.via_host == 3) && pol.kernel == 0) {
+        pol.overlap = 0;  // see llx_pack_ex
         return staged_through_bounce(pol, false, dst, dst_ids, n, stg, (cudaStream_t)stream);
+    }
     return launch_copy(pol, stg, pool_side(dst, dst_ids), n, dst->layers, dst->tile_bytes, dst->device, (cudaStream_t)stream);
     LLX_CATCH
 }
@@ -1307,6 +1311,7 @@ llx_status llx_migrate_via_host_ex(const llx_pool* src, const int32_t* src_ids, 
     Policy pol;
     llx_status rc = resolve_policy(opts, &pol);
     if (rc != LLX_OK) return rc;
+    pol.overlap = 0;  // the scatter of a chunk reads what its gather wrote: the route's own kernels keep plain stream order
     if ((rc = check_pair(src, dst)) != LLX_OK) return rc;
     if (n < 0) return fail(LLX_ERR_INVALID_ARG, "n = %d", n);
     if (n == 0) return LLX_OK;

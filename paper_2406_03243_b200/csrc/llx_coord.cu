@@ -454,3 +454,84 @@ llx_status llx_plan_migration_batch(const llx_req_info* reqs, const int32_t* seq
 }
 
 }  // extern "C"
+
+// ---- NEXT-1: the bandwidth budget chosen from the decode steps the engine observes (A34) ----
+#include <cmath>
+
+struct llx_budget_ctl {
+    double target = 0.0, lo = 0.0, hi = 0.0, budget = 0.0, last_slowdown_pct = NAN;
+    int window = 0, adjustments = 0;
+    std::vector<double> base, mig;  // the last 2*window steps without a migration; the steps with one since the last adjustment
+};
+
+static double median_of(std::vector<double> v) {  // by value: sorted copy
+    std::sort(v.begin(), v.end());
+    const size_t n = v.size();
+    return (n % 2) ? v[n / 2] : (v[n / 2 - 1] + v[n / 2]) / 2.0;
+}
+static int rounded_gbps(const llx_budget_ctl* c) { return (int)std::floor(c->budget + 0.5); }
+
+extern "C" {
+
+llx_status llx_budget_ctl_create(double target_slowdown_pct, int min_gbps, int max_gbps, int start_gbps, int window,
+                                 llx_budget_ctl** out) {
+    LLX_TRY
+    if (!out) return fail(LLX_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!(target_slowdown_pct > 0.0) || !std::isfinite(target_slowdown_pct) || min_gbps < 1 || start_gbps < min_gbps ||
+        max_gbps < start_gbps || max_gbps > 100000 || window < 2 || window > 256)
+        return fail(LLX_ERR_INVALID_ARG, "bad arguments (target=%g %%, budget %d <= %d <= %d GB/s, window=%d)", target_slowdown_pct,
+                    min_gbps, start_gbps, max_gbps, window);
+    llx_budget_ctl* c = new (std::nothrow) llx_budget_ctl();
+    if (!c) return fail(LLX_ERR_OOM, "host allocation failed");
+    c->target = target_slowdown_pct / 100.0;
+    c->lo = (double)min_gbps;
+    c->hi = (double)max_gbps;
+    c->budget = (double)start_gbps;
+    c->window = window;
+    try {
+        c->base.reserve((size_t)2 * window + 1);
+        c->mig.reserve((size_t)window + 1);
+    } catch (...) {
+        delete c;
+        throw;
+    }
+    *out = c;
+    return LLX_OK;
+    LLX_CATCH
+}
+
+llx_status llx_budget_ctl_destroy(llx_budget_ctl* c) {
+    delete c;
+    return LLX_OK;
+}
+
+llx_status llx_budget_ctl_observe(llx_budget_ctl* c, double step_ms, int migrating, int* budget_gbps) {
+    LLX_TRY
+    if (!c) return fail(LLX_ERR_INVALID_ARG, "controller is NULL");
+    if (!(step_ms > 0.0) || !std::isfinite(step_ms)) return fail(LLX_ERR_INVALID_ARG, "step_ms = %g", step_ms);
+    if (!migrating) {
+        c->base.push_back(step_ms);
+        if (c->base.size() > (size_t)2 * c->window) c->base.erase(c->base.begin());
+    } else if (!c->base.empty()) {  // a step with a migration means nothing before a step without one has been seen
+        c->mig.push_back(step_ms);
+        if (c->mig.size() >= (size_t)c->window) {
+            const double s = median_of(c->mig) / median_of(c->base) - 1.0;
+            double f = 2.0;  // cost within noise of zero: probe upwards
+            if (!(s <= c->target / 4.0)) f = std::min(2.0, std::max(0.5, c->target / s));
+            c->budget = std::min(c->hi, std::max(c->lo, c->budget * f));
+            c->last_slowdown_pct = 100.0 * s;
+            c->adjustments += 1;
+            c->mig.clear();
+        }
+    }
+    if (budget_gbps) *budget_gbps = rounded_gbps(c);
+    return LLX_OK;
+    LLX_CATCH
+}
+
+int llx_budget_ctl_gbps(const llx_budget_ctl* c) { return c ? rounded_gbps(c) : -1; }
+double llx_budget_ctl_last_slowdown_pct(const llx_budget_ctl* c) { return c ? c->last_slowdown_pct : NAN; }
+int llx_budget_ctl_adjustments(const llx_budget_ctl* c) { return c ? c->adjustments : -1; }
+
+}  // extern "C"

@@ -108,22 +108,57 @@ def test_llama7b_2048_tokens_three_stages_with_appends(env):
     assert tokens == 2048 and llx.counters()["copy_launches"] == launches0 + 3
     torch.cuda.synchronize()
 
-    # destination: every word of every layer against the oracle
-    for l in range(L):
-        got = dst.host_layer(l)[0]
-        rows = got[:, d_tab]
-        if not np.array_equal(rows, want_dst_rows[l]):
-            kv, i, e = np.argwhere(rows != want_dst_rows[l])[0]
-            raise AssertionError(f"layer {l} kv {kv} block {d_tab[i]} elem {e}: expected 0x{int(want_dst_rows[l][kv, i, e]):04x} "
-                                 f"got 0x{int(rows[kv, i, e]):04x}")
-        assert np.all(got[:, untouched] == SENT), f"layer {l}: an unreserved destination block was written"
-    # source: bit-identical to its state before the migration except the tail block, which holds the oracle's appends
-    before_v = src_before.view(torch.int16).view(L, 2, nb, te)
-    keep = torch.from_numpy(np.setdiff1d(np.arange(nb), [tail_block])).cuda()
-    for l in range(L):
-        assert torch.equal(src.view[l].index_select(1, keep), before_v[l].index_select(1, keep)), l
-        assert np.array_equal(src.view[l, :, tail_block].cpu().numpy().view(np.uint16), want_src_tail[l]), l
-    check_untouched_and_mapping_on_device(src, dst, s_tab, d_tab, range(L))
+    def verify():
+        # destination: every word of every layer against the oracle
+        for l in range(L):
+            got = dst.host_layer(l)[0]
+            rows = got[:, d_tab]
+            if not np.array_equal(rows, want_dst_rows[l]):
+                kv, i, e = np.argwhere(rows != want_dst_rows[l])[0]
+                raise AssertionError(f"layer {l} kv {kv} block {d_tab[i]} elem {e}: expected 0x{int(want_dst_rows[l][kv, i, e]):04x} "
+                                     f"got 0x{int(rows[kv, i, e]):04x}")
+            assert np.all(got[:, untouched] == SENT), f"layer {l}: an unreserved destination block was written"
+        # source: bit-identical to its state before the migration except the tail block, which holds the oracle's appends
+        before_v = src_before.view(torch.int16).view(L, 2, nb, te)
+        keep = torch.from_numpy(np.setdiff1d(np.arange(nb), [tail_block])).cuda()
+        for l in range(L):
+            assert torch.equal(src.view[l].index_select(1, keep), before_v[l].index_select(1, keep)), l
+            assert np.array_equal(src.view[l, :, tail_block].cpu().numpy().view(np.uint16), want_src_tail[l]), l
+        check_untouched_and_mapping_on_device(src, dst, s_tab, d_tab, range(L))
+
+    verify()
+
+    # The same request again exactly as bench.py issues it: nothing synchronised between the stages, stages 0 and 1
+    # launched with llx_launch_opts.overlap_prev = 1 (they may start while the kernel before them drains), the appends
+    # on the source's decode stream, the final stage waiting for them through an event.
+    all_vals = np.empty((sum(appends), L, 2, te_tok), dtype=np.uint16)
+    for j in range(sum(appends)):
+        for l in range(L):
+            for kv in range(2):
+                all_vals[j, l, kv] = values(2032 + j, l, kv)
+    dev_all = torch.from_numpy(all_vals.view(np.int16)).cuda()
+    tok_bytes = L * 2 * te_tok * 2
+    mig, dec = torch.cuda.Stream(), torch.cuda.Stream()
+    ov = llx.LaunchOpts(overlap_prev=1)
+    for rep in range(3):
+        src.raw.copy_(src_before)
+        dst.view.fill_(SENT_I16)
+        torch.cuda.synchronize()
+        e_app = torch.cuda.Event()
+        t = 2032
+        for a in appends:
+            llx.append_tokens(src.pool, s_tab, t, t + a, dev_all.data_ptr() + (t - 2032) * tok_bytes, stream=dec)
+            t += a
+        e_app.record(dec)
+        llx.migrate_stage(src.pool, s_tab[:112], dst.pool, d_tab[:112], stream=mig, opts=ov)
+        llx.migrate_stage(src.pool, s_tab[112:126], dst.pool, d_tab[112:126], stream=mig, opts=ov)
+        mig.wait_event(e_app)
+        llx.migrate_stage(src.pool, s_tab[126:], dst.pool, d_tab[126:], stream=mig)
+        mig.synchronize()
+        if rep == 2:
+            verify()
+        else:
+            check_untouched_and_mapping_on_device(src, dst, s_tab, d_tab, (0, 31))
 
 
 @pytest.mark.parametrize("tokens", [256, 8192])

@@ -52,8 +52,14 @@ def test_random_mix_of_calls_from_three_threads():
                 kind = int(rng.integers(0, 6))
                 opts = [None, dict(), dict(copy_kernel=1), dict(dynamic_tail_pct=30), dict(max_ctas=int(rng.integers(1, 400))),
                         dict(exact_residency=0), dict(bandwidth_gbps=int(rng.integers(2000, 6000))),
-                        dict(route=llx.ROUTE_PEER)][int(rng.integers(0, 8))]
-                if kind <= 2:
+                        dict(route=llx.ROUTE_PEER), dict(overlap_prev=1), dict(overlap_prev=1, dynamic_tail_pct=30)][int(rng.integers(0, 10))]
+                overlap = bool(opts) and opts.get("overlap_prev") == 1
+                if kind <= 2 and overlap and n >= 2:
+                    # two stages over disjoint halves, the second one allowed to start while the first drains
+                    h = n // 2
+                    llx.migrate_stage(src, s_ids[:h], dst, d_ids[:h], stream=st, opts=opts)
+                    llx.migrate_stage(src, s_ids[h:], dst, d_ids[h:], stream=st, opts=opts)
+                elif kind <= 2:
                     llx.migrate_stage(src, s_ids, dst, d_ids, stream=st, opts=opts)
                 elif kind == 3:
                     llx.migrate_stage_wait(src, s_ids, dst, d_ids, stream=st, opts=opts)
@@ -65,7 +71,8 @@ def test_random_mix_of_calls_from_three_threads():
                                              chunk_blocks=int(rng.integers(0, 60)), stream=st, opts=opts)
                     else:
                         llx.pack(src, s_ids, pin.dev_alias, pin.nbytes, stream=st, opts=opts)
-                        llx.unpack(pin.dev_alias, pin.nbytes, dst, d_ids, stream=st, opts=opts)
+                        # unpack READS what pack wrote: never declared independent of it
+                        llx.unpack(pin.dev_alias, pin.nbytes, dst, d_ids, stream=st, opts=None if overlap else opts)
                 st.synchronize()
                 si = torch.from_numpy(s_ids.astype(np.int64)).cuda()
                 di = torch.from_numpy(d_ids.astype(np.int64)).cuda()

@@ -288,3 +288,108 @@ def test_c_batch_plan_argument_errors_reserve_nothing(llx):
     rc = l.llx_plan_migration_batch(arr, i32([100, 100]), 2, 5.0, hr, 1, 0, 100.0, i32([0, 3, 2]), i32([1, 2, 3, 4, 5]),
                                     mgr.handle, 0, chosen, C.byref(nc), ro, so, do, 4, C.byref(npairs))
     assert rc == -1 and mgr.num_free == 45                                      # offsets decrease
+
+
+# ---- the budget controller (reading A34): pinned by what it must achieve on plants with a known answer ----------
+def _drive(ctl, cost, base_ms=5.0, rounds=40, noise=None):
+    """Alternate `window` steps without a migration and `window` steps with one whose slowdown is cost(budget)."""
+    rng = np.random.default_rng(3)
+    for _ in range(rounds):
+        for migrating in (False, True):
+            for _ in range(ctl.window):
+                t = base_ms * (1.0 + (cost(ctl.gbps()) if migrating else 0.0))
+                if noise:
+                    t *= 1.0 + noise * float(rng.standard_normal())
+                ctl.observe(t, migrating)
+    return ctl.gbps()
+
+
+def test_budget_controller_finds_the_budget_where_the_cost_equals_the_target():
+    """Affine plant s(B) = a + b*B (what DESIGN.md section 5.2a measures: a floor from the write turn-arounds plus a share
+    of the DRAM bytes).  The fixed point is B* = (t - a) / b; the rule must reach it from either side."""
+    from oracle.policy import BudgetController
+    t = 0.01
+    for a, b in ((0.0, 0.0004), (0.004, 0.00025), (0.007, 0.00025), (0.002, 0.00002)):
+        star = (t - a) / b
+        for start in (1, 8, 64, 400):
+            ctl = BudgetController(1.0, 1, 1000, start, 8)
+            got = _drive(ctl, lambda B: a + b * B)
+            assert abs(got - star) <= max(1.0, 0.03 * star), (a, b, start, got, star)
+    # the measured sustained-decoding curve of DESIGN.md section 5.2a (12 -> 1.0 %, 25 -> 1.5 %, 50 -> 2.2 %, 100 -> 3.35 %),
+    # linearly interpolated: the 1 % budget is 12 GB/s
+    xs, ys = [0, 12, 25, 50, 100, 200, 400], [0.0, 0.010, 0.015, 0.022, 0.0335, 0.0585, 0.0865]
+    ctl = BudgetController(1.0, 1, 1000, 100, 8)
+    assert abs(_drive(ctl, lambda B: float(np.interp(B, xs, ys))) - 12) <= 1
+
+
+def test_budget_controller_limits_and_single_steps():
+    from oracle.policy import BudgetController
+    # a floor above the target: the budget goes to its minimum and stays there
+    ctl = BudgetController(1.0, 5, 1000, 200, 4)
+    assert _drive(ctl, lambda B: 0.02 + 0.0001 * B) == 5
+    # no measurable cost: doubles at every adjustment up to the maximum
+    ctl = BudgetController(1.0, 1, 300, 10, 4)
+    seen = []
+    for _ in range(7):
+        for m in (False, True):
+            for _ in range(4):
+                ctl.observe(5.0, m)
+        seen.append(ctl.gbps())
+    assert seen == [20, 40, 80, 160, 300, 300, 300]
+    # one adjustment, by hand: slowdown 2 % at target 1 % halves; 1 % keeps; 0.5 % doubles; 10 % is clamped to a half
+    for slow, want in ((0.02, 50), (0.01, 100), (0.005, 200), (0.10, 50), (0.0125, 80)):
+        ctl = BudgetController(1.0, 1, 1000, 100, 4)
+        for _ in range(4):
+            ctl.observe(4.0, False)
+        for _ in range(4):
+            ctl.observe(4.0 * (1.0 + slow), True)
+        assert ctl.gbps() == want and abs(ctl.last_slowdown_pct - 100 * slow) < 1e-9 and ctl.adjustments == 1
+    # medians: one wild step among eight does not move the decision; steps with a migration before any baseline are dropped
+    ctl = BudgetController(1.0, 1, 1000, 100, 8)
+    for k in range(8):
+        ctl.observe(40.0 if k == 3 else 4.0, True)
+    assert ctl.adjustments == 0
+    for k in range(8):
+        ctl.observe(9.0 if k == 5 else 4.0, False)
+    for k in range(8):
+        ctl.observe(30.0 if k == 2 else 4.04, True)
+    assert ctl.gbps() == 100 and ctl.adjustments == 1
+    # with 1 % noise on every step the rule still settles within 35 % of the fixed point (B* = 40)
+    ctl = BudgetController(1.0, 1, 1000, 300, 16)
+    got = _drive(ctl, lambda B: 0.00025 * B, rounds=60, noise=0.002)
+    assert 26 <= got <= 54, got
+    for bad in ((0.0, 1, 10, 5, 8), (1.0, 0, 10, 5, 8), (1.0, 5, 4, 5, 8), (1.0, 1, 10, 11, 8), (1.0, 1, 10, 5, 1)):
+        with pytest.raises(ValueError):
+            BudgetController(*bad)
+
+
+def test_library_budget_controller_equals_the_oracle_on_seeded_step_sequences():
+    """llx_budget_ctl_* (C++) against oracle.policy.BudgetController: the same budget and the same slowdown estimate
+    after EVERY observation of 200 seeded sequences (random parameters, step times, migrating flags, outliers)."""
+    import paper_2406_03243_b200 as llx
+    from oracle.policy import BudgetController
+    rng = np.random.default_rng(11)
+    for case in range(200):
+        target = float(rng.choice([0.5, 1.0, 2.0, 5.0]))
+        lo = int(rng.integers(1, 20))
+        hi = int(rng.integers(lo, 2000))
+        start = int(rng.integers(lo, hi + 1))
+        window = int(rng.integers(2, 20))
+        a, b = BudgetController(target, lo, hi, start, window), llx.BudgetController(target, lo, hi, start, window)
+        base = float(rng.uniform(0.5, 20.0))
+        slope = float(rng.uniform(0.0, 0.001))
+        for _ in range(int(rng.integers(10, 400))):
+            mig = bool(rng.random() < 0.5)
+            t = base * (1.0 + (slope * a.gbps() if mig else 0.0)) * float(rng.uniform(0.97, 1.03))
+            if rng.random() < 0.03:
+                t *= 5.0
+            assert a.observe(t, mig) == b.observe(t, mig) == b.gbps, case
+            assert a.adjustments == b.adjustments
+            assert (math.isnan(a.last_slowdown_pct) and math.isnan(b.last_slowdown_pct)) or a.last_slowdown_pct == b.last_slowdown_pct
+    with pytest.raises(llx.LlxError):
+        llx.BudgetController(0.0, 1, 10, 5, 8)
+    with pytest.raises(llx.LlxError):
+        llx.BudgetController(1.0, 1, 10, 5, 8).observe(float("nan"), True)
+    with pytest.raises(llx.LlxError):
+        llx.BudgetController(1.0, 1, 10, 5, 8).observe(-1.0, False)
+    assert llx.lib().llx_budget_ctl_gbps(None) == -1 and llx.lib().llx_budget_ctl_adjustments(None) == -1
