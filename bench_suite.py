@@ -650,6 +650,100 @@ def interference_sustained(torch, llx, stream_unused=None, budgets=(12, 25, 50, 
     return res
 
 
+# ---- the budget chosen behind the ABI: llx_budget_ctl driven by a decode loop that never pauses ---------------
+def budget_controller_live(torch, llx, stream_unused=None, target_pct=1.0, window=16, rounds=24, start_gbps=200):
+    """SURVEY NEXT-1 "chosen automatically so decode slowdown <= 1 %", as an engine would run it: the configs[4] decode
+    loop never stops (power-capped steady state, see interference_sustained); it reports every step's duration to
+    llx_budget_ctl_observe.  Rounds alternate 2*window steps without a migration and window steps with budgeted
+    16-block stages kept in flight by a host thread at the controller's current budget (3 steps dropped after every
+    switch).  The trajectory is printed; the budget the controller settles on is then measured like interference_sustained
+    measures a fixed budget (4 segments ON / OFF of 150 steps)."""
+    import threading
+    g = dict(synth.CONFIGS["llama7b"])
+    L, H, D, S = g["layers"], g["kv_heads"], g["head_dim"], g["block_size"]
+    B, MB = 32, 256
+    ctx = synth.context_lengths(4, B, 128, 4096)
+    need = [-(-int(c) // S) for c in ctx]
+    nb_src, nb_dst = B * 256 + 256, g["num_blocks"]
+    if (nb_src + nb_dst) * 2 * L * S * H * D * 2 > _free(torch) - (4 << 30):
+        return {"skipped": "not enough device memory"}
+    p = Pools(torch, llx, g, nb_src, nb_dst)
+    perm = synth.block_permutation(6, nb_src)
+    bt = np.zeros((B, MB), dtype=np.int32)
+    pos = 0
+    for b, n in enumerate(need):
+        bt[b, :n] = perm[pos:pos + n]
+        pos += n
+    mig_src, mig_dst = perm[pos:pos + 16], synth.block_permutation(2, nb_dst)[:16]
+    q = torch.from_numpy(synth.queries_f16(5, B, H, D).view(np.int16)).cuda()
+    o = torch.zeros_like(q)
+    d_bt, d_ctx = torch.from_numpy(bt).cuda(), torch.from_numpy(ctx).cuda()
+    scale = 1.0 / float(np.sqrt(D))
+    lo, hi = torch.cuda.Stream.priority_range()
+    s_dec, s_mig = torch.cuda.Stream(priority=hi), torch.cuda.Stream(priority=lo)
+    dev = torch.cuda.current_device()
+
+    def run_steps(n):
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(n + 1)]
+        evs[0].record(s_dec)
+        for k in range(n):
+            for l in range(L):
+                llx.decode_attention(p.src, l, q.data_ptr(), o.data_ptr(), d_bt.data_ptr(), d_ctx.data_ptr(), B, MB, scale, stream=s_dec)
+            evs[k + 1].record(s_dec)
+            if k % 8 == 7:
+                evs[k - 6].synchronize()
+        s_dec.synchronize()
+        return [evs[k].elapsed_time(evs[k + 1]) for k in range(n)]
+
+    def feeder(budget_of, stop):
+        torch.cuda.set_device(dev)
+        while not stop.is_set():
+            o_ = dict(bandwidth_gbps=budget_of())
+            llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=o_)
+            llx.migrate_stage(p.src, mig_src, p.dst, mig_dst, stream=s_mig, opts=o_)
+            ev = torch.cuda.Event()
+            ev.record(s_mig)
+            while not ev.query() and not stop.is_set():
+                time.sleep(0.0005)
+
+    def with_feeder(budget_of, n_steps):
+        stop = threading.Event()
+        th = threading.Thread(target=feeder, args=(budget_of, stop))
+        th.start()
+        run_steps(3)
+        t = run_steps(n_steps)
+        stop.set()
+        th.join()
+        s_mig.synchronize()
+        return t
+
+    run_steps(300)                                    # into the power-capped steady state
+    ctl = llx.BudgetController(target_pct, 1, 2000, start_gbps, window)
+    trajectory = []
+    for r in range(rounds):
+        run_steps(3)
+        for t in run_steps(2 * window):
+            ctl.observe(t, False)
+        before = ctl.gbps
+        for t in with_feeder(lambda: before, window):
+            ctl.observe(t, True)
+        trajectory.append({"budget_GBps": before, "observed_slowdown_pct": round(ctl.last_slowdown_pct, 3), "next_budget_GBps": ctl.gbps})
+    tail = [x["budget_GBps"] for x in trajectory[rounds // 2:]]
+    chosen = int(statistics.median(tail))
+    on, off = [], []
+    for _ in range(4):
+        off += run_steps(150)[20:-20]
+        on += with_feeder(lambda: chosen, 150)[20:-20]
+    res = {"target_slowdown_pct": target_pct, "window_steps": window, "start_budget_GBps": start_gbps, "trajectory": trajectory,
+           "settled_budget_GBps": {"median_of_second_half": chosen, "min": min(tail), "max": max(tail)},
+           "verification_at_settled_budget": {"decode_step_off_ms": statistics.median(off), "decode_step_on_ms": statistics.median(on),
+                                              "slowdown_pct": 100.0 * (statistics.median(on) / statistics.median(off) - 1.0), "steps_each": len(on)},
+           "note": "decode loop never pauses; the controller sees event-timed steps, 2*window without and window with a migration per round"}
+    del p
+    _free(torch)
+    return res
+
+
 # ---- the paper's Fig. 10 situation on one B200: a request migrates WHILE its batch keeps decoding -------------
 def live_migration(torch, llx, stream_unused=None, budgets=(0, 100, 25), start_tokens=2040):
     """One request of a 32-sequence decode batch is migrated live (§6.2): the decode loop keeps
@@ -967,6 +1061,7 @@ def run(torch, llx, stream):
     res["interference_decode_batch32"] = interference(torch, llx, stream)
     res["auto_budget_1pct"] = auto_budget(torch, llx, stream, target_pct=1.0)
     res["interference_sustained_decoding"] = interference_sustained(torch, llx, stream)
+    res["budget_controller_live_1pct"] = budget_controller_live(torch, llx, stream)
     res["live_migration_during_decode"] = live_migration(torch, llx, stream)
     res["batch_llama30b_64req"] = batch_30b(torch, llx, stream)
     res["batch_llama30b_64req_seed2_mean507"] = batch_30b(torch, llx, stream, seed=2)
@@ -976,7 +1071,7 @@ def run(torch, llx, stream):
 
 
 def main():
-    """python bench_suite.py [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch | batch2 | sustained | tp | green | floor | ncu_targets)"""
+    """python bench_suite.py [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch | batch2 | sustained | controller | tp | green | floor | ncu_targets)"""
     import argparse
     import json
 
@@ -1011,6 +1106,8 @@ def main():
         res = tp_shard_30b(torch, llx, stream)
     elif args.only == "sustained":
         res = interference_sustained(torch, llx, stream)
+    elif args.only == "controller":
+        res = budget_controller_live(torch, llx, stream)
     elif args.only == "green":
         res = green_partition(torch, llx, stream)
     elif args.only == "ncu_targets":
