@@ -651,7 +651,7 @@ def interference_sustained(torch, llx, stream_unused=None, budgets=(12, 25, 50, 
 
 
 # ---- the budget chosen behind the ABI: llx_budget_ctl driven by a decode loop that never pauses ---------------
-def budget_controller_live(torch, llx, stream_unused=None, target_pct=1.0, window=16, rounds=24, start_gbps=200):
+def budget_controller_live(torch, llx, stream_unused=None, target_pct=1.0, window=16, rounds=24, start_gbps=200, drop=3):
     """SURVEY NEXT-1 "chosen automatically so decode slowdown <= 1 %", as an engine would run it: the configs[4] decode
     loop never stops (power-capped steady state, see interference_sustained); it reports every step's duration to
     llx_budget_ctl_observe.  Rounds alternate 2*window steps without a migration and window steps with budgeted
@@ -840,8 +840,14 @@ def live_migration(torch, llx, stream_unused=None, budgets=(0, 100, 25), start_t
         llx.decode_attention(p.src, L - 1, q.data_ptr(), o_src.data_ptr(), d_bt.data_ptr(), d_ctx1.data_ptr(), 1, MB, scale, stream=s_dec)
         llx.decode_attention(p.dst, L - 1, q.data_ptr(), o_dst.data_ptr(), d_bt1.data_ptr(), d_ctx1.data_ptr(), 1, MB, scale, stream=s_dec)
         s_dec.synchronize()
+        # the same count from the MEASURED rates (llx_predict_stage_sizes): copy rate of the non-final
+        # stages in blocks/s, decode rate of this request = one token per step
+        copy_rate = sum(stages[:-1]) / (copy_ms * 1e-3)
+        decode_rate = 1e3 / (statistics.median(during) if during else before)
         out["runs"].append({
             "bandwidth_budget_GBps": budget, "stages_blocks": stages, "num_stages": len(stages),
+            "predicted_stage_sizes_from_measured_rates": llx.predict_stage_sizes(stages[0], copy_rate, decode_rate, S),
+            "measured_copy_blocks_per_s": copy_rate, "measured_decode_tokens_per_s": decode_rate,
             "tokens_at_start": tokens_at_start, "tokens_at_commit": tokens, "decode_steps_during_migration": len(during),
             "copy_phase_ms": copy_ms, "downtime_us_final_stage": downtime_us, "commit_us": commit_us,
             "decode_step_ms_before": before, "decode_step_ms_during": statistics.median(during) if during else None,
