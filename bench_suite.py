@@ -170,7 +170,34 @@ def latency_floor(torch, llx, p: Pools, stream, nb):
                       "sync_us_median": statistics.median(host) - statistics.median(enq), "gpu_event_us_median": statistics.median(gpu)}
     out["note"] = ("the 32 KiB stage moves nothing worth timing: its numbers are the floor of one launch + one synchronize through this "
                    "entry point; the final stage's excess over it is the copy itself")
+    out["c99_client"] = c_client_downtime()
     return out
+
+
+def c_client_downtime(reps=300):
+    """The same two measurements by a plain C99 program (bench_downtime.c: llx.h and libllx.so only, legacy default stream,
+    clock_gettime): what the library costs with no Python and no ctypes in the timed interval."""
+    import json
+    import shutil
+    import subprocess
+    import tempfile
+    gcc = shutil.which("gcc")
+    if not gcc:
+        return {"skipped": "gcc unavailable"}
+    root = os.path.dirname(os.path.abspath(__file__))
+    libdir = os.path.join(root, "paper_2406_03243_b200")
+    with tempfile.TemporaryDirectory() as tmp:
+        exe = os.path.join(tmp, "bench_downtime")
+        r = subprocess.run([gcc, "-std=c99", "-O2", "-Wall", "-Wextra", "-Werror", "-pedantic", "-I", os.path.join(root, "include"),
+                            os.path.join(root, "bench_downtime.c"), "-o", exe, "-L", libdir, "-lllx", "-Wl,-rpath," + libdir],
+                           capture_output=True, text=True)
+        if r.returncode != 0:
+            return {"error": r.stderr[-500:]}
+        r = subprocess.run([exe, str(reps)], capture_output=True, text=True, timeout=600)
+        try:
+            return json.loads(r.stdout)
+        except Exception:  # noqa: BLE001
+            return {"error": (r.stdout + r.stderr)[-500:]}
 
 
 # ---- reference points on the same data (SURVEY.md §8(d)) ---------------------------------------
@@ -710,7 +737,7 @@ def budget_controller_live(torch, llx, stream_unused=None, target_pct=1.0, windo
         stop = threading.Event()
         th = threading.Thread(target=feeder, args=(budget_of, stop))
         th.start()
-        run_steps(3)
+        run_steps(drop)
         t = run_steps(n_steps)
         stop.set()
         th.join()
@@ -721,7 +748,7 @@ def budget_controller_live(torch, llx, stream_unused=None, target_pct=1.0, windo
     ctl = llx.BudgetController(target_pct, 1, 2000, start_gbps, window)
     trajectory = []
     for r in range(rounds):
-        run_steps(3)
+        run_steps(drop)
         for t in run_steps(2 * window):
             ctl.observe(t, False)
         before = ctl.gbps

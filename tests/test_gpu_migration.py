@@ -22,7 +22,9 @@ KERNELS = [dict(copy_kernel=2), dict(copy_kernel=1), dict(copy_kernel=2, chunk_b
            dict(bandwidth_gbps=40), dict(bandwidth_gbps=3000), dict(copy_kernel=2, unit_order=0), dict(copy_kernel=1, unit_order=0),
            dict(copy_kernel=2, l2_hint=3, rings_per_cta=2), dict(pdl=0),
            dict(copy_kernel=2, dynamic_tail_pct=30, max_ctas=2, chunk_bytes=1024),
-           dict(copy_kernel=2, dynamic_tail_pct=100, max_ctas=3, chunk_bytes=512, ring_stages=3, rings_per_cta=2)]
+           dict(copy_kernel=2, dynamic_tail_pct=100, max_ctas=3, chunk_bytes=512, ring_stages=3, rings_per_cta=2),
+           dict(overlap_prev=1), dict(overlap_prev=1, copy_kernel=2, dynamic_tail_pct=50, max_ctas=2, chunk_bytes=1024),
+           dict(overlap_prev=1, copy_kernel=1), dict(overlap_prev=1, pdl=0)]
 
 
 @pytest.fixture(scope="module")
@@ -471,7 +473,8 @@ def test_guard_bands_around_pools_and_staging_stay_intact(env, opts):
     ids_d = np.array([nb - 1, 0, nb - 2, 1, 9, 2, 30])
     llx.migrate_stage(src, ids_s, dst, ids_d, opts=opts)
     llx.pack(src, ids_s, bufs[2].data_ptr() + guard, stg_bytes, opts=opts)
-    llx.unpack(bufs[2].data_ptr() + guard, stg_bytes, dst, ids_d, opts=opts)
+    # unpack READS what pack wrote: it is never declared independent of the kernel before it
+    llx.unpack(bufs[2].data_ptr() + guard, stg_bytes, dst, ids_d, opts={k: v for k, v in opts.items() if k != "overlap_prev"})
     llx.migrate_via_host(src, ids_s, dst, ids_d, bufs[2].data_ptr() + guard, stg_bytes, chunk_blocks=3, opts=opts)
     torch.cuda.synchronize()
     for raw, size in zip(bufs, (nbytes, nbytes, stg_bytes)):
