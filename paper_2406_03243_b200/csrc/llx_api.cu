@@ -3,6 +3,8 @@
 // this file only checks arguments, stages the block ids and enqueues.  There is no CPU path.
 #include "../../include/llx.h"
 
+#include <cuda.h>  // CUtensorMap types only: cuTensorMapEncodeTiled is fetched through cudaGetDriverEntryPoint, libcuda is not linked
+
 #include <atomic>
 #include <cmath>
 #include <cstdarg>
@@ -32,6 +34,10 @@ struct llx_pool {
     // decode-attention workspace (grows on demand)
     float* attn_ws = nullptr;
     size_t attn_ws_bytes = 0;
+    // small tiles (<= 16 KiB): a 4-D tensor map over the pool, dims (row, rows of a tile, block, slice), whose box is the
+    // tiles of ONE block in tma_k consecutive (layer, K|V) slices; 0 = no map (large tiles, no driver entry point)
+    int tma_k = 0;
+    llx::TensorMap tmap;
 };
 
 namespace llx {
@@ -74,7 +80,7 @@ std::atomic<unsigned long long> g_launches{0}, g_copy_launches{0}, g_bytes{0}, g
 // Range of every option: shared by llx_set_option (process defaults) and by the per-call llx_launch_opts.
 bool opt_valid(int opt, long long v) {
     switch (opt) {
-        case LLX_OPT_COPY_KERNEL: return v >= 0 && v <= 2;
+        case LLX_OPT_COPY_KERNEL: return v >= 0 && v <= 3;
         case LLX_OPT_MAX_CTAS: return v >= 0 && v <= (1 << 20);
         case LLX_OPT_CHUNK_BYTES: return v >= 0 && (v % 16) == 0 && v <= (200 << 10);
         case LLX_OPT_RING_STAGES: return v >= 0 && v != 1 && v <= 14;
@@ -194,6 +200,8 @@ llx_status dev_info(int dev, DevInfo** out, bool capturing = false) {
         LLX_CUDA(cudaDeviceGetAttribute(&d.smem_per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
         LLX_CUDA(cudaFuncSetAttribute(llx_copy_bulk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
         LLX_CUDA(cudaFuncSetAttribute(llx_copy_bulk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
+        LLX_CUDA(cudaFuncSetAttribute(llx_copy_tma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
+        LLX_CUDA(cudaFuncSetAttribute(llx_copy_tma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, d.max_smem_optin));
         d.ready = true;
     }
     // Shared-memory carve-out preference of the register-staged copy kernel (LLX_OPT_COPY_SMEM_CARVEOUT_PCT; see the
@@ -460,6 +468,7 @@ struct Side {
     long long slice_stride, item_stride;
     bool host_memory;  // staging in mapped host memory
     int device = -1;   // pool side: the device its memory lives on (-1: staging)
+    const llx_pool* pool = nullptr;  // pool side: the pool (its tensor map serves the small-tile kernel)
 };
 
 // `device` = the device the kernel runs on = the current device (the source pool's for a migration).
@@ -491,8 +500,25 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     const bool budget_by_ctas = budget_asked >= 500 && pol.kernel == 0 && kern == 2;
     const long long budget = budget_by_ctas ? 0 : budget_asked;  // from here on: > 0 means "paced"
     if (budget > 0 && pol.kernel != 2) kern = 1;
-
+    // The tensor-map kernel (copy_kernel = 3): pool -> pool on one device, tiles of at most 16 KiB, both pools described
+    // by tensor maps with the same box (same geometry => same box).  One unit = one block in tma_k consecutive slices.
+    const bool tensor_possible = src.pool && dst.pool && src.ids && dst.ids && !peer && !src.host_memory && !dst.host_memory &&
+                                 src.pool->tma_k >= 2 && dst.pool->tma_k == src.pool->tma_k;
+    bool tensor = false;
+    if (kern == 3) {
+        if (!tensor_possible)
+            return fail(LLX_ERR_INVALID_ARG, "copy_kernel = 3 (tensor-map kernel) needs a pool-to-pool copy on one device with tiles of at most 16 KiB");
+        kern = 2;
+        tensor = true;
+    }
     const long long total_bytes = n * 2 * layers * tile_bytes;
+    // auto: long stages of 8-16 KiB tiles (measured on B200, stages of 0.25-2.6 GiB: 16 KiB tiles 6.18 -> 6.45 TB/s, 8 KiB
+    // tiles 6.45 -> 6.53 and 5.10 -> 5.20 with only 4 slices; 4 KiB tiles 6.55 either way: four 1-D rings per SM keep up)
+    if (pol.kernel == 0 && kern == 2 && tensor_possible && budget_asked <= 0 && pol.chunk <= 0 && pol.rings <= 0 && pol.stages <= 0 &&
+        pol.max_ctas <= 0 && tile_bytes >= 8192 && total_bytes >= (64ll << 20))
+        tensor = true;
+    const int tma_k = tensor ? src.pool->tma_k : 1;
+
     long long chunk = pol.chunk;
     int nstages = (int)pol.stages;
     int threads = 256, grid = 0, long_per_sm = 1;
@@ -509,6 +535,7 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
         if (chunk <= 0) chunk = budget > 0 ? 2048 : short_stage ? 8192 : 32768;  // paced: a 4 KiB ring stays below the L1 carve-out step
         if (chunk > tile_bytes) chunk = tile_bytes;
         chunk &= ~15ll;
+        if (tensor) chunk = tma_k * tile_bytes;  // one box = one ring stage
         // Small tiles cap the chunk, and one thread cannot issue small bulk copies fast enough to keep its SM's share
         // of HBM busy (measured, long stages: 8 KiB tiles 3.5 TB/s with one ring per SM, 6.0 TB/s with two; 4 KiB
         // tiles 2.0 -> 6.0 TB/s with four): more CTAs per SM, ~64-96 KiB in flight per SM in every case.
@@ -538,8 +565,8 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
         if (chunk > tile_bytes) chunk = tile_bytes;
         chunk &= ~15ll;
     }
-    const long long cpt = (tile_bytes + chunk - 1) / chunk;
-    const long long units = n * slices * cpt;
+    const long long cpt = tensor ? 1 : (tile_bytes + chunk - 1) / chunk;
+    const long long units = tensor ? n * (slices / tma_k) : n * slices * cpt;
     if (units >= (1ll << 31)) return fail(LLX_ERR_INVALID_ARG, "stage too large: %lld units", units);
 
     if (kern == 2) {
@@ -590,10 +617,11 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     a.src_indexed = src.ids != nullptr;
     a.dst_indexed = dst.ids != nullptr;
     a.src_ids = a.dst_ids = nullptr;
-    a.tile_bytes = (int)tile_bytes;
+    a.tile_bytes = (int)(tensor ? chunk : tile_bytes);
     a.chunk_bytes = (int)chunk;
     a.chunks_per_tile = (int)cpt;
-    a.slices = slices;
+    a.slices = tensor ? slices / tma_k : slices;
+    a.tma_k = tma_k;
     a.total_units = (int)units;
     a.unit_begin = 0;
     a.blocked_order = (int)pol.order;
@@ -667,7 +695,12 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     cudaError_t e = cudaSuccess;
     const bool pdl = pol.pdl != 0;
     int launches = 1;
-    if (kern == 2) {
+    if (kern == 2 && tensor) {
+        if (byval)
+            e = launch_k(pdl, llx_copy_tma<true>, grid, threads, smem, st, a, pack, nstages, src.pool->tmap, dst.pool->tmap);
+        else
+            e = launch_k(pdl, llx_copy_tma<false>, grid, threads, smem, st, a, pack, nstages, src.pool->tmap, dst.pool->tmap);
+    } else if (kern == 2) {
         if (byval)
             e = launch_k(pdl, llx_copy_bulk<true>, grid, threads, smem, st, a, pack, nstages);
         else
@@ -715,7 +748,7 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
 }
 
 Side pool_side(const llx_pool* p, const int32_t* ids) {
-    return Side{p->data, ids, (long long)p->num_blocks * p->tile_bytes, p->tile_bytes, false, p->device};
+    return Side{p->data, ids, (long long)p->num_blocks * p->tile_bytes, p->tile_bytes, false, p->device, p};
 }
 llx_status staging_side(const void* staging, int layers, long long tile_bytes, Side* out) {
     cudaPointerAttributes at;
@@ -857,6 +890,51 @@ llx_status ce_blocks(bool to_host, const llx_pool* pool, const int32_t* ids, int
     return LLX_OK;
 }
 
+// ---- tensor map of a small-tile pool (llx_copy_tma) ---------------------------------------------------------------
+// One tile is at most 16 KiB here, so a 1-D bulk copy moves little per instruction and one thread cannot issue them fast
+// enough for its SM's share of HBM.  The pool is therefore also described to the TMA unit as a 4-D
+// tensor of 8-byte elements — (row of <= 2 KiB, rows of a tile, block, slice) — with a box that spans ONE block in tma_k
+// consecutive (layer, K|V) slices: one instruction then moves tma_k tiles (<= 32 KiB), gathered by the TMA unit itself.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q = cudaDriverEntryPointSymbolNotFound;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            p = nullptr;
+        }
+        return (EncodeTiledFn)p;
+    }();
+    return fn;
+}
+void build_tensor_map(llx_pool* p) {
+    static_assert(sizeof(CUtensorMap) == sizeof(llx::TensorMap), "CUtensorMap is 128 bytes");
+    p->tma_k = 0;
+    const long long tile = p->tile_bytes, slices = 2ll * p->layers;
+    if (tile > (16 << 10)) return;
+    int k = 0;
+    for (int c = 2; c <= 256 && c <= slices; ++c)
+        if (slices % c == 0 && c * tile <= (32 << 10) && (c * tile) % 128 == 0) k = c;
+    long long row = 0;
+    for (long long d = 16; d <= 2048 && d <= tile; d += 16)
+        if (tile % d == 0) row = d;
+    if (k < 2 || row == 0 || tile / row > 256) return;
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return;
+    const cuuint64_t dims[4] = {(cuuint64_t)(row / 8), (cuuint64_t)(tile / row), (cuuint64_t)p->num_blocks, (cuuint64_t)slices};
+    const cuuint64_t strides[3] = {(cuuint64_t)row, (cuuint64_t)tile, (cuuint64_t)p->num_blocks * (cuuint64_t)tile};
+    const cuuint32_t box[4] = {(cuuint32_t)(row / 8), (cuuint32_t)(tile / row), 1u, (cuuint32_t)k};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    if (strides[2] >= (1ull << 40)) return;
+    const CUresult r = enc(reinterpret_cast<CUtensorMap*>(&p->tmap), CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, p->data, dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r == CUDA_SUCCESS) p->tma_k = k;
+}
+
 llx_status make_pool(void* ptr, size_t bytes, bool owned, int layers, int kv_heads, int head_dim, int block_size,
                      llx_dtype dtype, int num_blocks, llx_pool** out) {
     if (!out) return fail(LLX_ERR_INVALID_ARG, "out is NULL");
@@ -899,6 +977,7 @@ llx_status make_pool(void* ptr, size_t bytes, bool owned, int layers, int kv_hea
     p->tile_bytes = (long long)block_size * kv_heads * head_dim * p->elem_bytes;
     p->device = dev;
     p->owned = owned;
+    build_tensor_map(p);
     *out = p;
     return LLX_OK;
 }

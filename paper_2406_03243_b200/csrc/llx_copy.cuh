@@ -50,6 +50,8 @@ struct CopyArgs {
     int blocked_order;  // 0: worker w takes units w, w+W, ...; 1: worker w takes a contiguous range
     int l2_hint;        // bit0: loads L2::evict_first, bit1: stores L2::evict_first (bulk kernel)
     int pace_ns;        // bulk kernel: minimum time between two chunks of one ring (0 = unthrottled)
+    int tma_k;          // tensor-map kernel: (layer, K|V) slices one 4-D box covers; there a unit = (pair, group of tma_k slices),
+                        // slices = groups per block, chunks_per_tile = 1, chunk_bytes = tile_bytes = tma_k * the pool's tile
     int defer_wait;     // bulk kernel, LLX_OPT_OVERLAP_PREV: the copy is independent of the previous kernel of its stream, so
                         // griddepcontrol.wait moves from the prologue to just before the first dynamic claim / the exit
     // bulk kernel, blocked order: the last dyn_units units are not pre-assigned; rings that finish their
@@ -238,8 +240,45 @@ __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wa
 // padded to 128 B, then [rings_per_cta][nstages][chunk_bytes] data.  Lane 0 of each warp is the ring's only
 // working thread.  Striped order: ring r handles units r, r+nrings, ...  Blocked order: ring r streams the
 // contiguous range [r*Ts/W, (r+1)*Ts/W) of the first Ts = total - dyn_units units, then claims batches of the rest.
-template <bool BYVAL>
-__global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack ids, int nstages) {
+//
+// The ring is the same for both ways of moving a unit; a Mover supplies them:
+//   BulkMover   : one 1-D bulk copy per unit (a chunk of one tile), any tile size that is a multiple of 16 bytes;
+//   TensorMover : one 4-D tensor-map box per unit = the tiles of ONE block in tma_k consecutive (layer, K|V) slices
+//                 (cp.async.bulk.tensor.4d, SASS UTMALDG / UTMASTG): small tiles travel tma_k at a time.
+struct BulkMover {
+    uint64_t pol;
+    bool hint_ld, hint_st;
+    __device__ __forceinline__ void load(const CopyArgs&, const UnitAddr& ua, int, int, uint32_t dst_smem, uint32_t bar) const {
+        if (hint_ld)
+            bulk_g2s_hint(dst_smem, ua.src, (uint32_t)ua.len, bar, pol);
+        else
+            bulk_g2s(dst_smem, ua.src, (uint32_t)ua.len, bar);
+    }
+    __device__ __forceinline__ void store(const CopyArgs&, const UnitAddr& ua, int, int, uint32_t src_smem) const {
+        if (hint_st)
+            bulk_s2g_hint(ua.dst, src_smem, (uint32_t)ua.len, pol);
+        else
+            bulk_s2g(ua.dst, src_smem, (uint32_t)ua.len);
+    }
+};
+struct TensorMover {
+    const void* src_map;  // CUtensorMap in the kernel parameters (__grid_constant__)
+    const void* dst_map;
+    __device__ __forceinline__ void load(const CopyArgs& a, const UnitAddr&, int item, int group, uint32_t dst_smem, uint32_t bar) const {
+        asm volatile(
+            "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(dst_smem),
+            "l"(src_map), "r"(0), "r"(0), "r"(item), "r"(group * a.tma_k), "r"(bar)
+            : "memory");
+    }
+    __device__ __forceinline__ void store(const CopyArgs& a, const UnitAddr&, int item, int group, uint32_t src_smem) const {
+        asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4}], [%5];" ::"l"(dst_map), "r"(0),
+                     "r"(0), "r"(item), "r"(group * a.tma_k), "r"(src_smem)
+                     : "memory");
+    }
+};
+
+template <bool BYVAL, class Mover>
+__device__ __forceinline__ void ring_copy(const CopyArgs& a, const IdPack& ids, int nstages, const Mover mover) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int warp = threadIdx.x >> 5;
     const int rings_per_cta = blockDim.x >> 5;
@@ -302,26 +341,23 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
         d_end = d_next + a.dyn_batch < a.total_units ? d_next + a.dyn_batch : a.total_units;
         return d_next++;
     };
-    const uint64_t pol = policy_evict_first();
-    const bool hint_ld = a.l2_hint & 1, hint_st = a.l2_hint & 2;
     unsigned long long deadline = a.pace_ns > 0 ? global_timer_ns() : 0ull;
 
-    auto addr_of = [&](int u) -> UnitAddr {
-        int i, slice, c;
+    // unit u -> both addresses (1-D mover) and (item, slice) on both sides (tensor mover)
+    auto addr_of = [&](int u, int& item_s, int& item_d, int& slice) -> UnitAddr {
+        int i, c;
         unit_coords(a, u, i, slice, c);
-        int item_s = i, item_d = i;
+        item_s = item_d = i;
         if (a.src_indexed) item_s = BYVAL ? ids.src[i] : __ldg(a.src_ids + i);
         if (a.dst_indexed) item_d = BYVAL ? ids.dst[i] : __ldg(a.dst_ids + i);
         return unit_addr(a, slice, c, item_s, item_d);
     };
     auto issue_load = [&](int s, int u) {
         unit_of[s] = u;
-        UnitAddr ua = addr_of(u);
+        int item_s, item_d, slice;
+        UnitAddr ua = addr_of(u, item_s, item_d, slice);
         mbar_expect_tx(bar0 + s * 8, (uint32_t)ua.len);
-        if (hint_ld)
-            bulk_g2s_hint(buf0 + s * a.chunk_bytes, ua.src, (uint32_t)ua.len, bar0 + s * 8, pol);
-        else
-            bulk_g2s(buf0 + s * a.chunk_bytes, ua.src, (uint32_t)ua.len, bar0 + s * 8);
+        mover.load(a, ua, item_s, slice, buf0 + s * a.chunk_bytes, bar0 + s * 8);
     };
 
     int issued = 0;
@@ -333,11 +369,9 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
     for (int k = 0; k < issued; ++k) {
         const int s = k % nstages;
         mbar_wait(bar0 + s * 8, (uint32_t)((k / nstages) & 1));
-        UnitAddr ua = addr_of(unit_of[s]);
-        if (hint_st)
-            bulk_s2g_hint(ua.dst, buf0 + s * a.chunk_bytes, (uint32_t)ua.len, pol);
-        else
-            bulk_s2g(ua.dst, buf0 + s * a.chunk_bytes, (uint32_t)ua.len);
+        int item_s, item_d, slice;
+        UnitAddr ua = addr_of(unit_of[s], item_s, item_d, slice);
+        mover.store(a, ua, item_d, slice, buf0 + s * a.chunk_bytes);
         bulk_commit();
         if (a.pace_ns > 0) {  // bandwidth budget: this ring may start its next chunk only at its next deadline
             deadline += (unsigned long long)a.pace_ns;
@@ -369,6 +403,28 @@ __global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack i
             *a.done_flag = a.done_value;
         }
     }
+}
+
+template <bool BYVAL>
+__global__ void llx_copy_bulk(const CopyArgs a, const __grid_constant__ IdPack ids, int nstages) {
+    BulkMover m;
+    m.pol = policy_evict_first();
+    m.hint_ld = a.l2_hint & 1;
+    m.hint_st = a.l2_hint & 2;
+    ring_copy<BYVAL>(a, ids, nstages, m);
+}
+
+// 128 opaque bytes with the alignment the TMA unit needs: a CUtensorMap, declared here without the driver header
+struct alignas(64) TensorMap {
+    unsigned long long opaque[16];
+};
+template <bool BYVAL>
+__global__ void llx_copy_tma(const CopyArgs a, const __grid_constant__ IdPack ids, int nstages,
+                             const __grid_constant__ TensorMap src_map, const __grid_constant__ TensorMap dst_map) {
+    TensorMover m;
+    m.src_map = &src_map;
+    m.dst_map = &dst_map;
+    ring_copy<BYVAL>(a, ids, nstages, m);
 }
 
 // ------------------------------------------------------------------------------------------
