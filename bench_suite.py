@@ -1077,7 +1077,40 @@ def ncu_targets(torch, llx, stream):
     twice("pack_zero_copy_pinned_host_16_blocks", lambda: llx.pack(p7.src, s7[:16], pin.dev_alias, pin.nbytes, stream=stream, opts=zc))
     twice("unpack_zero_copy_pinned_host_16_blocks", lambda: llx.unpack(pin.dev_alias, pin.nbytes, p7.dst, d7[:16], stream=stream, opts=zc))
     pin.free()
+    # small tiles: the 1-D ring next to the tensor-map kernel (the default for these two stages is the tensor-map kernel)
+    twice("tiny_tiles_8KiB_8000_blocks_ring_1d", lambda: llx.migrate_stage(pt.src, st_, pt.dst, dt_, stream=stream, opts=dict(copy_kernel=2)))
+    del p7, pt
+    _free(torch)
+    g16 = dict(layers=32, kv_heads=4, head_dim=128, block_size=16, elem_bytes=2, num_blocks=4400)
+    p16 = Pools(torch, llx, g16, 4400, 4400)
+    s16, d16 = synth.block_permutation(1, 4400)[:4000], synth.block_permutation(2, 4400)[:4000]
+    twice("tiles_16KiB_4000_blocks_ring_1d", lambda: llx.migrate_stage(p16.src, s16, p16.dst, d16, stream=stream, opts=dict(copy_kernel=2)))
+    twice("tiles_16KiB_4000_blocks_tensor_map", lambda: llx.migrate_stage(p16.src, s16, p16.dst, d16, stream=stream))
     return {"order": out, "note": "each label = two consecutive launches of that shape; llx_fill / at:: kernels in between are input generation"}
+
+
+# ---- small tiles (TP-sharded / GQA caches): the 1-D ring next to the tensor-map kernel ------------------------------
+def small_tiles(torch, llx, stream):
+    """Long pool-to-pool stages of 4, 8 and 16 KiB tiles (one KV head per rank ... four), scattered ids, by CUDA events:
+    copy_kernel = 2 (1-D bulk ring; 4 / 2 / 1 CTAs per SM) against copy_kernel = 3 (the same ring fed by 4-D tensor-map
+    boxes of 32 KiB) and against what the library picks by itself."""
+    out = []
+    for label, L, H, nb, n in (("4 KiB tiles, 64 slices (1 KV head of 128)", 32, 1, 33000, 30000),
+                               ("8 KiB tiles, 4 slices (Tiny)", 2, 4, 8400, 8000),
+                               ("8 KiB tiles, 80 slices (2 KV heads of 128)", 40, 2, 9000, 8000),
+                               ("16 KiB tiles, 64 slices (4 KV heads of 128)", 32, 4, 4400, 4000)):
+        D = 64 if H == 4 and L == 2 else 128
+        g = dict(layers=L, kv_heads=H, head_dim=D, block_size=16, elem_bytes=2, num_blocks=nb)
+        p = Pools(torch, llx, g, nb, nb)
+        s_ids, d_ids = synth.block_permutation(1, nb)[:n], synth.block_permutation(2, nb)[:n]
+        row = {"shape": label, "blocks": n, "payload_MiB": n * p.src.block_bytes / 2**20}
+        for name, o in (("ring_1d", dict(copy_kernel=2)), ("tensor_map", dict(copy_kernel=3)), ("default", None)):
+            t = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_ids, p.dst, d_ids, stream=stream, opts=o), reps=12, warm=3)
+            row[name + "_GBps"] = 2 * n * p.src.block_bytes / (t["median_ms"] * 1e-3) / 1e9
+        out.append(row)
+        del p
+        _free(torch)
+    return out
 
 
 def run(torch, llx, stream):
@@ -1099,12 +1132,13 @@ def run(torch, llx, stream):
     res["batch_llama30b_64req"] = batch_30b(torch, llx, stream)
     res["batch_llama30b_64req_seed2_mean507"] = batch_30b(torch, llx, stream, seed=2)
     res["tp4_rank_shards_llama30b"] = tp_shard_30b(torch, llx, stream)
+    res["small_tiles_ring_1d_vs_tensor_map"] = small_tiles(torch, llx, stream)
     res["sm_partition_green_contexts"] = green_partition(torch, llx, stream)
     return res
 
 
 def main():
-    """python bench_suite.py [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch | batch2 | sustained | controller | tp | green | floor | ncu_targets)"""
+    """python bench_suite.py [--only NAME]   (NAME: sweep | refs | staging | interference | autobudget | live | batch | batch2 | sustained | controller | tp | small | green | floor | ncu_targets)"""
     import argparse
     import json
 
@@ -1143,6 +1177,8 @@ def main():
         res = budget_controller_live(torch, llx, stream)
     elif args.only == "green":
         res = green_partition(torch, llx, stream)
+    elif args.only == "small":
+        res = small_tiles(torch, llx, stream)
     elif args.only == "ncu_targets":
         res = ncu_targets(torch, llx, stream)
     else:

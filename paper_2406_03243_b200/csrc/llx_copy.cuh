@@ -11,14 +11,16 @@
 // (slice_stride = tile_bytes, item_stride = 2*layers*tile_bytes).  migrate = pool->pool,
 // pack = pool->buffer, unpack = buffer->pool: one kernel body serves S3, S4, S5 and S6.
 //
-// Two implementations, selected by the host (LLX_OPT_COPY_KERNEL):
+// Three implementations, selected by the host (LLX_OPT_COPY_KERNEL):
 //   llx_copy_vec16 : 256-thread CTAs, 16-byte LDG/STG, UNROLL independent loads in flight per
 //                    thread before the first store; lane 0 fetches the pair's block ids and
 //                    broadcasts them with __shfl_sync.
 //   llx_copy_bulk  : one elected thread per warp drives a ring of shared-memory stages with the
 //                    bulk async-copy engine (cp.async.bulk global->shared completing on an
 //                    mbarrier, shared->global in bulk groups): no registers or LSU issue slots
-//                    per byte, 16 KiB per instruction.
+//                    per byte, up to 32 KiB per instruction.
+//   llx_copy_tma   : the same ring, fed by 4-D tensor-map boxes (cp.async.bulk.tensor): one instruction moves
+//                    the tiles of one block in several (layer, K|V) slices — for pools whose tiles are small.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
