@@ -532,6 +532,33 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
         // (6.57 TB/s at 112 blocks, 6.66 TB/s at >= 256).  More bytes in flight per SM lowers DRAM efficiency.
         // A short stage (the final one: 2 blocks) is latency-bound: smaller chunks over twice as many rings.
         const bool short_stage = total_bytes < (64ll << 20) && !budget_by_ctas;
+        // Long stages of tiles that are not a multiple of 32 KiB (any head count that is not a multiple of 8: 13 heads of
+        // a TP=4 rank of LLaMA-30B = 52 KiB).  "32 KiB, then the rest" leaves a short chunk per tile that occupies a whole
+        // ring stage, so fewer bytes are in flight and DRAM idles: 52 KiB tiles ran at 6.13 TB/s, 40 KiB at 5.4, 36 KiB at 5.0.
+        // Measured over 13 tile sizes from 20 to 208 KiB (one ring per SM): what matters is (a) chunks of EQUAL size and
+        // (b) about 62 KiB of loads in flight per SM — (stages - 1) x chunk; 52 KiB is too little, 78 KiB already too
+        // much — with chunks of at least 13 KiB.  So: split the tile into m equal chunks, m from ceil(tile / 32 KiB) up, and
+        // take the (m, stages) whose loads in flight are closest to 62 KiB, the larger chunk on a tie.  Multiples of 32 KiB keep
+        // 3 x 32 KiB; 52 KiB -> 4 x 13 KiB, 6 stages: 6.48 TB/s; 40 KiB -> 2 x 20 KiB, 4 stages: 6.41; 36 KiB: 6.18; 72 KiB: 6.49;
+        // 80 KiB: 6.55; 208 KiB -> 10 x 20.8 KiB, 4 stages: 6.67 (from 6.63).
+        bool equal_split = false;
+        if (chunk <= 0 && nstages <= 0 && pol.rings <= 0 && !tensor && !short_stage && budget <= 0 && tile_bytes > 16384) {
+            const long long target = 62ll << 10, m0 = (tile_bytes + 32767) / 32768;
+            long long best = -1;
+            for (long long m = m0; m <= m0 + 12; ++m) {
+                const long long c = ((tile_bytes + m - 1) / m + 15) & ~15ll;
+                if (m > m0 && c < 13312) break;
+                for (int sg = 3; sg <= 8 && c * sg <= (160ll << 10); ++sg) {
+                    const long long fl = (sg - 1) * c, score = fl > target ? fl - target : target - fl;
+                    if (best < 0 || score < best) {
+                        best = score;
+                        chunk = c;
+                        nstages = sg;
+                    }
+                }
+            }
+            equal_split = true;
+        }
         if (chunk <= 0) chunk = budget > 0 ? 2048 : short_stage ? 8192 : 32768;  // paced: a 4 KiB ring stays below the L1 carve-out step
         if (chunk > tile_bytes) chunk = tile_bytes;
         chunk &= ~15ll;
@@ -539,7 +566,7 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
         // Small tiles cap the chunk, and one thread cannot issue small bulk copies fast enough to keep its SM's share
         // of HBM busy (measured, long stages: 8 KiB tiles 3.5 TB/s with one ring per SM, 6.0 TB/s with two; 4 KiB
         // tiles 2.0 -> 6.0 TB/s with four): more CTAs per SM, ~64-96 KiB in flight per SM in every case.
-        long_per_sm = chunk >= 16384 ? 1 : chunk >= 8192 ? 2 : 4;
+        long_per_sm = (chunk >= 16384 || equal_split) ? 1 : chunk >= 8192 ? 2 : 4;
         if (nstages <= 0) nstages = budget > 0 ? 2 : short_stage ? 4 : chunk >= 32768 ? 3 : chunk >= 16384 ? 6 : 4;
         int rings = (int)pol.rings;
         if (rings <= 0) rings = 1;

@@ -519,6 +519,35 @@ def test_default_launch_shape_with_dynamic_tail_on_a_mid_size_stage(env):
     H.assert_pool_equal(dst.host(), h_dst)
 
 
+@pytest.mark.parametrize("heads", [5, 9, 10, 13, 17, 26])          # 20, 36, 40, 52 (a TP=4 rank of LLaMA-30B), 68, 104 KiB tiles
+def test_long_stage_of_tiles_that_are_no_multiple_of_32k_is_split_into_equal_chunks(env, heads):
+    """>= 64 MiB of tiles whose size is not a multiple of 32 KiB: the default launch shape cuts every tile into m equal chunks
+    (13-31 KiB, the last one a few bytes shorter) with 3-6 ring stages.  A second, overlapped stage and a
+    pack / unpack round trip of the same shape follow; every word against the oracle."""
+    H, llx = env
+    te_bytes = 16 * heads * 128 * 2
+    n = (70 << 20) // (2 * 2 * te_bytes) + 1
+    g = dict(layers=2, kv_heads=heads, head_dim=128, block_size=16, elem_bytes=2, num_blocks=2 * n + 20)
+    src = H.DevPool(g)
+    src.fill_device_random(40 + heads)
+    dst = H.DevPool(g, fill=SENT)
+    assert 2 * g["layers"] * src.pool.tile_bytes * n >= 64 << 20
+    nb = g["num_blocks"]
+    ps, pd = synth.block_permutation(5, nb), synth.block_permutation(6, nb)
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    llx.migrate_stage(src.pool, ps[:n], dst.pool, pd[:n], stream=st)
+    stg = torch.empty(llx.staging_bytes(src.pool, n), dtype=torch.uint8, device="cuda")
+    llx.pack(src.pool, ps[n:2 * n], stg.data_ptr(), stg.numel(), stream=st, opts=dict(overlap_prev=1))
+    llx.unpack(stg.data_ptr(), stg.numel(), dst.pool, pd[n:2 * n], stream=st)
+    st.synchronize()
+    h_src = src.host()
+    h_dst = om.new_pool(g["layers"], nb, H.tile_elems(g), fill=SENT)
+    om.migrate_stage(h_src, ps[:2 * n], h_dst, pd[:2 * n])
+    H.assert_pool_equal(dst.host(), h_dst)
+    assert np.array_equal(stg.cpu().numpy().view(np.uint16).reshape(n, g["layers"], 2, -1), om.pack(h_src, ps[n:2 * n]))
+
+
 def test_two_host_threads_on_two_streams(env):
     """llx.h, "Threads": data calls may be issued from several host threads at once on distinct streams.  Two threads migrate different requests
     between the same pools at the same time: long id lists (pinned id ring), pinned-host pack (shared bounce
