@@ -1086,6 +1086,15 @@ def ncu_targets(torch, llx, stream):
     s16, d16 = synth.block_permutation(1, 4400)[:4000], synth.block_permutation(2, 4400)[:4000]
     twice("tiles_16KiB_4000_blocks_ring_1d", lambda: llx.migrate_stage(p16.src, s16, p16.dst, d16, stream=stream, opts=dict(copy_kernel=2)))
     twice("tiles_16KiB_4000_blocks_tensor_map", lambda: llx.migrate_stage(p16.src, s16, p16.dst, d16, stream=stream))
+    del p16
+    _free(torch)
+    # a TP=4 rank shard of LLaMA-30B (13 heads, 52 KiB tiles): "32 KiB, then the rest" next to the computed shape (4 equal chunks, 6 stages)
+    g52 = dict(synth.CONFIGS["llama30b"], kv_heads=13, num_blocks=400)
+    p52 = Pools(torch, llx, g52, 400, 400)
+    s52, d52 = synth.block_permutation(1, 400)[:128], synth.block_permutation(2, 400)[:128]
+    twice("tp4_shard_52KiB_128_blocks_32K_then_rest", lambda: llx.migrate_stage(p52.src, s52, p52.dst, d52, stream=stream,
+                                                                                 opts=dict(chunk_bytes=32768, ring_stages=3)))
+    twice("tp4_shard_52KiB_128_blocks", lambda: llx.migrate_stage(p52.src, s52, p52.dst, d52, stream=stream))
     return {"order": out, "note": "each label = two consecutive launches of that shape; llx_fill / at:: kernels in between are input generation"}
 
 
