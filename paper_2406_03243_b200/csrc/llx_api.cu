@@ -538,7 +538,7 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
         // Measured over 13 tile sizes from 20 to 208 KiB (one ring per SM): what matters is (a) chunks of EQUAL size and
         // (b) about 62 KiB of loads in flight per SM — (stages - 1) x chunk; 52 KiB is too little, 78 KiB already too
         // much — with chunks of at least 13 KiB.  So: split the tile into m equal chunks, m from ceil(tile / 32 KiB) up, and
-        // take the (m, stages) whose loads in flight are closest to 62 KiB, the larger chunk on a tie.  Multiples of 32 KiB keep
+        // take the (m, stages) whose loads in flight are closest to 62 KiB, the larger chunk unless a smaller one is 2 KiB closer.  Multiples of 32 KiB keep
         // 3 x 32 KiB; 52 KiB -> 4 x 13 KiB, 6 stages: 6.48 TB/s; 40 KiB -> 2 x 20 KiB, 4 stages: 6.41; 36 KiB: 6.18; 72 KiB: 6.49;
         // 80 KiB: 6.55; 208 KiB -> 10 x 20.8 KiB, 4 stages: 6.67 (from 6.63).
         bool equal_split = false;
@@ -550,7 +550,7 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
                 if (m > m0 && c < 13312) break;
                 for (int sg = 3; sg <= 8 && c * sg <= (160ll << 10); ++sg) {
                     const long long fl = (sg - 1) * c, score = fl > target ? fl - target : target - fl;
-                    if (best < 0 || score < best) {
+                    if (best < 0 || score + 2048 < best) {  // a smaller chunk has to be clearly closer (2 KiB) to replace a larger one
                         best = score;
                         chunk = c;
                         nstages = sg;
