@@ -1077,15 +1077,16 @@ def ncu_targets(torch, llx, stream):
     twice("pack_zero_copy_pinned_host_16_blocks", lambda: llx.pack(p7.src, s7[:16], pin.dev_alias, pin.nbytes, stream=stream, opts=zc))
     twice("unpack_zero_copy_pinned_host_16_blocks", lambda: llx.unpack(pin.dev_alias, pin.nbytes, p7.dst, d7[:16], stream=stream, opts=zc))
     pin.free()
-    # small tiles: the 1-D ring next to the tensor-map kernel (the default for these two stages is the tensor-map kernel)
-    twice("tiny_tiles_8KiB_8000_blocks_ring_1d", lambda: llx.migrate_stage(pt.src, st_, pt.dst, dt_, stream=stream, opts=dict(copy_kernel=2)))
+    # small tiles: the tensor-map kernel (copy_kernel = 3) next to the default, the 1-D ring
+    twice("tiny_tiles_8KiB_8000_blocks_tensor_map", lambda: llx.migrate_stage(pt.src, st_, pt.dst, dt_, stream=stream, opts=dict(copy_kernel=3)))
     del p7, pt
     _free(torch)
     g16 = dict(layers=32, kv_heads=4, head_dim=128, block_size=16, elem_bytes=2, num_blocks=4400)
     p16 = Pools(torch, llx, g16, 4400, 4400)
     s16, d16 = synth.block_permutation(1, 4400)[:4000], synth.block_permutation(2, 4400)[:4000]
-    twice("tiles_16KiB_4000_blocks_ring_1d", lambda: llx.migrate_stage(p16.src, s16, p16.dst, d16, stream=stream, opts=dict(copy_kernel=2)))
-    twice("tiles_16KiB_4000_blocks_tensor_map", lambda: llx.migrate_stage(p16.src, s16, p16.dst, d16, stream=stream))
+    twice("tiles_16KiB_4000_blocks_6_stages_round1", lambda: llx.migrate_stage(p16.src, s16, p16.dst, d16, stream=stream, opts=dict(ring_stages=6)))
+    twice("tiles_16KiB_4000_blocks", lambda: llx.migrate_stage(p16.src, s16, p16.dst, d16, stream=stream))
+    twice("tiles_16KiB_4000_blocks_tensor_map", lambda: llx.migrate_stage(p16.src, s16, p16.dst, d16, stream=stream, opts=dict(copy_kernel=3)))
     del p16
     _free(torch)
     # a TP=4 rank shard of LLaMA-30B (13 heads, 52 KiB tiles): "32 KiB, then the rest" next to the computed shape (4 equal chunks, 6 stages)
@@ -1101,8 +1102,9 @@ def ncu_targets(torch, llx, stream):
 # ---- small tiles (TP-sharded / GQA caches): the 1-D ring next to the tensor-map kernel ------------------------------
 def small_tiles(torch, llx, stream):
     """Long pool-to-pool stages of 4, 8 and 16 KiB tiles (one KV head per rank ... four), scattered ids, by CUDA events:
-    copy_kernel = 2 (1-D bulk ring; 4 / 2 / 1 CTAs per SM) against copy_kernel = 3 (the same ring fed by 4-D tensor-map
-    boxes of 32 KiB) and against what the library picks by itself."""
+    copy_kernel = 2 (1-D bulk ring; 4 / 2 / 1 CTAs per SM, ring depth from the loads-in-flight rule) against copy_kernel = 3
+    (the same ring fed by 4-D tensor-map boxes of 32 KiB), against what the library picks by itself (the 1-D ring) and
+    against the 1-D ring with round 1's ring depths (4 / 4 / 6 stages)."""
     out = []
     for label, L, H, nb, n in (("4 KiB tiles, 64 slices (1 KV head of 128)", 32, 1, 33000, 30000),
                                ("8 KiB tiles, 4 slices (Tiny)", 2, 4, 8400, 8000),
@@ -1113,7 +1115,9 @@ def small_tiles(torch, llx, stream):
         p = Pools(torch, llx, g, nb, nb)
         s_ids, d_ids = synth.block_permutation(1, nb)[:n], synth.block_permutation(2, nb)[:n]
         row = {"shape": label, "blocks": n, "payload_MiB": n * p.src.block_bytes / 2**20}
-        for name, o in (("ring_1d", dict(copy_kernel=2)), ("tensor_map", dict(copy_kernel=3)), ("default", None)):
+        old_depth = 6 if p.src.tile_bytes >= 16384 else 4
+        for name, o in (("ring_1d", dict(copy_kernel=2)), ("tensor_map", dict(copy_kernel=3)), ("default", None),
+                        ("ring_1d_round1_depth", dict(copy_kernel=2, ring_stages=old_depth))):
             t = _time_stream(torch, stream, lambda: llx.migrate_stage(p.src, s_ids, p.dst, d_ids, stream=stream, opts=o), reps=12, warm=3)
             row[name + "_GBps"] = 2 * n * p.src.block_bytes / (t["median_ms"] * 1e-3) / 1e9
         out.append(row)

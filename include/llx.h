@@ -438,7 +438,7 @@ typedef enum {
     LLX_OPT_COPY_KERNEL = 0,    /* 0 auto, 1 = 16-byte LDG/STG kernel, 2 = bulk-async (1-D TMA) smem ring, 3 = the same ring fed by 4-D
                                    tensor-map boxes (cp.async.bulk.tensor: one instruction moves the tiles of one block in several
                                    (layer, K|V) slices) — pool-to-pool copies on one device with tiles of at most 16 KiB only,
-                                   LLX_ERR_INVALID_ARG elsewhere; auto takes it for long stages of 8-16 KiB tiles */
+                                   LLX_ERR_INVALID_ARG elsewhere; never taken by auto (it ties the 1-D ring, measured) */
     LLX_OPT_MAX_CTAS = 1,       /* cap on the copy grid (0 = auto: fill the GPU); the throttle of SURVEY NEXT-1 */
     LLX_OPT_CHUNK_BYTES = 2,    /* bytes of one tile one CTA moves per step (multiple of 16; 0 = auto) */
     LLX_OPT_RING_STAGES = 3,    /* smem stages per ring of the bulk-async kernel (0 = auto) */

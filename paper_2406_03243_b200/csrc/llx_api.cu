@@ -512,11 +512,9 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
         tensor = true;
     }
     const long long total_bytes = n * 2 * layers * tile_bytes;
-    // auto: long stages of 8-16 KiB tiles (measured on B200, stages of 0.25-2.6 GiB: 16 KiB tiles 6.18 -> 6.45 TB/s, 8 KiB
-    // tiles 6.45 -> 6.53 and 5.10 -> 5.20 with only 4 slices; 4 KiB tiles 6.55 either way: four 1-D rings per SM keep up)
-    if (pol.kernel == 0 && kern == 2 && tensor_possible && budget_asked <= 0 && pol.chunk <= 0 && pol.rings <= 0 && pol.stages <= 0 &&
-        pol.max_ctas <= 0 && tile_bytes >= 8192 && total_bytes >= (64ll << 20))
-        tensor = true;
+    // Never taken by itself: once the 1-D ring's depth follows the loads-in-flight rule below, the two tie on every small
+    // tile measured (4 KiB: 6.55 / 6.53 TB/s, 8 KiB: 6.48 / 6.48, 16 KiB: 6.53 / 6.51, 12 KiB: 6.41 / 6.38, 3.75 KiB: 6.17 / 6.02);
+    // the tensor-map kernel gets there with ONE ring per SM instead of two or four.
     const int tma_k = tensor ? src.pool->tma_k : 1;
 
     long long chunk = pol.chunk;
@@ -566,8 +564,18 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
         // Small tiles cap the chunk, and one thread cannot issue small bulk copies fast enough to keep its SM's share
         // of HBM busy (measured, long stages: 8 KiB tiles 3.5 TB/s with one ring per SM, 6.0 TB/s with two; 4 KiB
         // tiles 2.0 -> 6.0 TB/s with four): more CTAs per SM, ~64-96 KiB in flight per SM in every case.
-        long_per_sm = (chunk >= 16384 || equal_split) ? 1 : chunk >= 8192 ? 2 : 4;
-        if (nstages <= 0) nstages = budget > 0 ? 2 : short_stage ? 4 : chunk >= 32768 ? 3 : chunk >= 16384 ? 6 : 4;
+        long_per_sm = (chunk >= 16384 || equal_split || tensor) ? 1 : chunk >= 8192 ? 2 : 4;
+        if (nstages <= 0 && budget <= 0 && !short_stage) {
+            // ring depth from the same measurement as above: ~62 KiB of loads in flight per SM, over all rings of the SM.
+            // 32 KiB chunks: 3 stages; 16 KiB: 5 (6.19 -> 6.54 TB/s; 6 stages = 80 KiB in flight is already too much);
+            // two rings of 8 KiB or four of 4 KiB: 5 each; a 24 KiB tensor-map box: 4 (6.18 -> 6.38)
+            const long long per_stage = (long long)long_per_sm * chunk;
+            nstages = 1 + (int)(((62ll << 10) + per_stage / 2) / per_stage);
+            if (nstages < 3) nstages = 3;
+            if (nstages > 8) nstages = 8;
+            if (long_per_sm == 4) nstages = 4;  // four rings of 4 KiB: 48 KiB in flight measured best (6.55 vs 6.45 TB/s with 5 stages)
+        }
+        if (nstages <= 0) nstages = budget > 0 ? 2 : 4;
         int rings = (int)pol.rings;
         if (rings <= 0) rings = 1;
         threads = 32 * rings;

@@ -1,6 +1,6 @@
 """The tensor-map copy kernel (llx_copy_tma: cp.async.bulk.tensor.4d, one box = one block in several (layer, K|V) slices)
-against the oracle.  It serves pool-to-pool stages of small tiles (<= 16 KiB: TP-sharded or GQA caches, Tiny): selected with
-copy_kernel = 3, and by itself for long stages of 8-16 KiB tiles.  Same definition as every other route (PAPER.md:134,
+against the oracle.  It serves pool-to-pool stages of small tiles (<= 16 KiB: TP-sharded or GQA caches, Tiny), selected with
+copy_kernel = 3 (the default stays the 1-D ring, which ties it once its depth is right: DESIGN.md section 5.1b).  Same definition as every other route (PAPER.md:134,
 :237): dst[l][kv][dst_ids[i]] = src[l][kv][src_ids[i]], whole tiles, everything else untouched."""
 import numpy as np
 import pytest
@@ -97,9 +97,11 @@ def test_tensor_map_kernel_batch_capture_and_guard_bands(env):
         assert bool((raw[:guard] == 0x5A).all()) and bool((raw[guard + nbytes:] == 0x5A).all()), "guard band overwritten"
 
 
-def test_long_stage_of_16k_tiles_takes_the_tensor_map_kernel_by_itself(env):
-    """Default options, >= 64 MiB of 16 KiB tiles: the library picks the tensor-map kernel; an overlapped
-    short stage right behind it takes the 1-D ring.  Pools of different sizes (A21)."""
+@pytest.mark.parametrize("opts", [None, dict(copy_kernel=3)])
+def test_long_stage_of_16k_tiles_by_the_default_ring_and_by_the_tensor_map_kernel(env, opts):
+    """>= 64 MiB of 16 KiB tiles with the default options (1-D ring, one CTA per SM, 5 stages of 16 KiB) and with the
+    tensor-map kernel (boxes of two tiles, 3 stages); an overlapped short stage right behind it.  Pools of different
+    sizes (A21)."""
     H, llx = env
     g = dict(layers=16, kv_heads=4, head_dim=128, block_size=16, elem_bytes=2, num_blocks=900)
     src = H.DevPool(g)
@@ -110,7 +112,7 @@ def test_long_stage_of_16k_tiles_takes_the_tensor_map_kernel_by_itself(env):
     s_ids, d_ids = synth.block_permutation(3, 900)[:n + 20], synth.block_permutation(4, 1000)[:n + 20]
     st = torch.cuda.Stream()
     st.wait_stream(torch.cuda.current_stream())
-    llx.migrate_stage(src.pool, s_ids[:n], dst.pool, d_ids[:n], stream=st)
+    llx.migrate_stage(src.pool, s_ids[:n], dst.pool, d_ids[:n], stream=st, opts=opts)
     llx.migrate_stage(src.pool, s_ids[n:], dst.pool, d_ids[n:], stream=st, opts=dict(overlap_prev=1))
     st.synchronize()
     h_src = src.host()
