@@ -12,14 +12,15 @@ import torch
 
 pytestmark = pytest.mark.gpu
 
-G = dict(layers=4, kv_heads=8, head_dim=128, block_size=16)     # 32 KiB tiles, 256 KiB blocks
 NB = 3000
-SECONDS = float(os.environ.get("LLX_STRESS_SECONDS", "6"))        # a longer soak: LLX_STRESS_SECONDS=120 python -m pytest tests/test_gpu_stress.py -m gpu
+SECONDS = float(os.environ.get("LLX_STRESS_SECONDS", "4"))        # per geometry; a longer soak: LLX_STRESS_SECONDS=120 python -m pytest tests/test_gpu_stress.py -m gpu
 
 
-def test_random_mix_of_calls_from_three_threads():
+@pytest.mark.parametrize("heads", [8, 13])                         # 32 KiB tiles (3 x 32 KiB ring) and 52 KiB tiles (equal chunks of 13 KiB, 6 stages)
+def test_random_mix_of_calls_from_three_threads(heads):
     import paper_2406_03243_b200 as llx
     llx.load()
+    G = dict(layers=4, kv_heads=heads, head_dim=128, block_size=16)
     te = G["block_size"] * G["kv_heads"] * G["head_dim"]
 
     def pool():
