@@ -32,6 +32,8 @@ What it computes, and the passage each part follows (all `PAPER.md:<line>`):
   (virtual usage and freeness) and the pairing rule of §4.4.3.
 * `policy.plan_migration_batch` — one migration round of one (source, destination) pair as one batch: migration
   order, the source-state threshold and all-or-nothing PRE-ALLOC (PAPER.md:225 + :142; reading A31 in DESIGN.md).
+* `policy.BudgetController` — the bandwidth budget of non-final stages chosen from observed decode steps so that their
+  slowdown stays at a target (PAPER.md:289-291 states the bound, not a mechanism: reading A34 in DESIGN.md).
 * `decode_attention.decode_attention_fp64` — standard KV-cache attention for one
   decode token per sequence, read through the block table (§2).
 
@@ -47,5 +49,9 @@ leak freedom at every abort point and the commit bookkeeping in closed form
 freeness (decode iterations left, by brute-force simulation), to the printed capacity
 13,616 tokens / target load 1,600 tokens (tests/golden/paper_priority_headroom.txt) and to
 the rule-by-rule special cases; the batch round to a closed form for equal requests, hand-computed special cases and
-an independent brute-force restatement (tests/test_oracle_policy.py).  Nothing here is "parity unpinned".
+an independent brute-force restatement (tests/test_oracle_policy.py); `stage_sizes` also to an exact-rational time-stepped
+simulation that shares nothing with the recurrence (tests/test_abi.py); `BudgetController` to the closed-form fixed point of an
+affine cost, B* = (target - a) / b, reached from either side, to hand-computed single adjustments, to its limits (floor above
+the target -> minimum; no cost -> doubling up to the maximum) and to one outlier per window (tests/test_oracle_policy.py).
+Nothing here is "parity unpinned".
 """
