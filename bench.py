@@ -668,7 +668,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", choices=["llx", "reference"], default="llx")
     ap.add_argument("--suite", action="store_true", help="also run the length sweep, 30B batch and interference configs")
-    ap.add_argument("--downtime-reps", type=int, default=100)
+    ap.add_argument("--downtime-reps", type=int, default=200)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-overlap", action="store_true",
                     help="launch every stage in plain stream order (no llx_launch_opts.overlap_prev on stages 0 and 1)")
