@@ -323,7 +323,7 @@ llx_status dyn_counter_get(int dev, cudaStream_t st, unsigned int** counter) {
 //      libraries up to 131 KB; llx's own bulk ring asks for the 164 KB split and still waits at 50 %, hence (2) and (3);
 //  (2) the library remembers the register-staged launches that may still be running (one event each) and, while any
 //      is, sends its own auto-selected copies through the register-staged kernel too: no shared memory, placed at once
-//      (a short stage takes the same time: 23.3 vs 23.6 us; a long one runs at 5.6 instead of 6.5 TB/s next to the
+//      (a short stage takes the same time: 23.3 vs 23.6 us; a long one runs at 6.1 instead of 6.5 TB/s next to the
 //      budgeted stage);
 //  (3) a budgeted stage is a chain of ~1 ms launches (LLX_OPT_PACED_SLICE_US, in launch_copy): whoever waits for an SM
 //      to change its split waits for the end of a slice, not of the stage.
@@ -625,7 +625,10 @@ llx_status launch_copy(const Policy& pol, const Side& src, const Side& dst, long
     } else if (budget <= 0) {
         // A side in host memory is bound by the host link (~52 GB/s): one CTA per SM already saturates it
         // (measured: 52.7 GB/s with 74..296 CTAs, 51.5 with 1184) and leaves the SMs to whatever else is running.
-        grid = (src.host_memory || dst.host_memory) ? di->sm_count : di->sm_count * 8;
+        // Device <-> device: FOUR CTAs per SM, i.e. 4 x 256 threads x 4 loads x 16 B = 64 KiB of loads in flight per SM — the
+        // same optimum as the bulk ring's (~62 KiB).  Round 1 launched eight (128 KiB in flight): 5.57 TB/s for 128 blocks of
+        // LLaMA-7B, 5.80 for 512; four: 6.05 and 6.14-6.22; three or five are slower again.
+        grid = (src.host_memory || dst.host_memory) ? di->sm_count : di->sm_count * 4;
     }
     long long cap = pol.max_ctas;
     if (cap <= 0 && budget_by_ctas) cap = (budget_asked + 30) / 60;
