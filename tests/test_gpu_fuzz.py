@@ -69,10 +69,17 @@ def test_random_geometries_ids_and_policies_against_the_oracle(env, seed):
         h_dst = om.new_pool(L, nb, words, fill=SENT)
         nbytes = llx.pool_bytes_for(L, g["kv_heads"], g["head_dim"], g["block_size"], dtype, nb)
         assert nbytes == h_src.nbytes
-        d_src = torch.from_numpy(h_src.view(np.int16)).cuda()
-        d_dst = torch.from_numpy(h_dst.view(np.int16).copy()).cuda()
-        src = llx.pool_wrap(d_src.data_ptr(), nbytes, L, g["kv_heads"], g["head_dim"], g["block_size"], dtype, nb, keepalive=d_src)
-        dst = llx.pool_wrap(d_dst.data_ptr(), nbytes, L, g["kv_heads"], g["head_dim"], g["block_size"], dtype, nb, keepalive=d_dst)
+        # both pools sit between 8 KiB guard bands (compute-sanitizer is closed on this pool of machines): a copy that
+        # strayed outside a pool — a box, a chunk, a remainder — would hit them
+        GUARD = 8192
+        raw_s = torch.full((nbytes + 2 * GUARD,), 0x5A, dtype=torch.uint8, device="cuda")
+        raw_d = torch.full((nbytes + 2 * GUARD,), 0x5A, dtype=torch.uint8, device="cuda")
+        d_src = raw_s[GUARD:GUARD + nbytes].view(torch.int16)
+        d_dst = raw_d[GUARD:GUARD + nbytes].view(torch.int16)
+        d_src.copy_(torch.from_numpy(h_src.view(np.int16).reshape(-1)))
+        d_dst.copy_(torch.from_numpy(h_dst.view(np.int16).reshape(-1)))
+        src = llx.pool_wrap(d_src.data_ptr(), nbytes, L, g["kv_heads"], g["head_dim"], g["block_size"], dtype, nb, keepalive=raw_s)
+        dst = llx.pool_wrap(d_dst.data_ptr(), nbytes, L, g["kv_heads"], g["head_dim"], g["block_size"], dtype, nb, keepalive=raw_d)
         stream = torch.cuda.Stream()
         stream.wait_stream(torch.cuda.current_stream())
         free_dst = list(rng.permutation(nb))
@@ -106,9 +113,11 @@ def test_random_geometries_ids_and_policies_against_the_oracle(env, seed):
                 assert e.name == "LLX_ERR_INVALID_ARG" and opts is not None and (opts.get("copy_kernel") in (2, 3)), (label, str(e))
                 free_dst.extend(int(x) for x in d_ids)
                 stream.synchronize()
-                assert np.array_equal(d_dst.cpu().numpy().view(np.uint16), h_dst), label
+                assert np.array_equal(d_dst.cpu().numpy().view(np.uint16), h_dst.reshape(-1)), label
                 continue
             om.migrate_stage(h_src, s_ids, h_dst, d_ids)
             stream.synchronize()
-            assert np.array_equal(d_dst.cpu().numpy().view(np.uint16), h_dst), label
-            assert np.array_equal(d_src.cpu().numpy().view(np.uint16), h_src), label
+            assert np.array_equal(d_dst.cpu().numpy().view(np.uint16), h_dst.reshape(-1)), label
+            assert np.array_equal(d_src.cpu().numpy().view(np.uint16), h_src.reshape(-1)), label
+            for raw in (raw_s, raw_d):
+                assert bool((raw[:GUARD] == 0x5A).all()) and bool((raw[GUARD + nbytes:] == 0x5A).all()), ("guard band overwritten", label)
