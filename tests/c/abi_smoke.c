@@ -33,6 +33,20 @@ int main(void) {
         CHECK(llx_predict_stage_sizes(64, 4.0, 16.0, 16, sizes, 8, &k) == LLX_OK && k == 4 && sizes[3] == 1);
         CHECK(llx_predict_stage_sizes(64, 4.0, 16.0, 16, sizes, 0, &k) == LLX_ERR_INVALID_ARG);
     }
+    {   /* the budget controller (<= 1 %): 2 % observed at a 1 % target halves the budget, 1 % keeps it */
+        llx_budget_ctl* ctl = NULL;
+        int i, budget = 0;
+        CHECK(llx_budget_ctl_create(0.0, 1, 1000, 100, 4, &ctl) == LLX_ERR_INVALID_ARG && ctl == NULL);
+        CHECK(llx_budget_ctl_create(1.0, 1, 1000, 100, 4, &ctl) == LLX_OK && llx_budget_ctl_gbps(ctl) == 100);
+        for (i = 0; i < 4; ++i) CHECK(llx_budget_ctl_observe(ctl, 4.08, 1, &budget) == LLX_OK && budget == 100); /* no baseline yet: dropped */
+        for (i = 0; i < 8; ++i) CHECK(llx_budget_ctl_observe(ctl, 4.0, 0, &budget) == LLX_OK);
+        for (i = 0; i < 4; ++i) CHECK(llx_budget_ctl_observe(ctl, 4.08, 1, &budget) == LLX_OK);
+        CHECK(budget == 50 && llx_budget_ctl_adjustments(ctl) == 1 && llx_budget_ctl_last_slowdown_pct(ctl) > 1.99);
+        for (i = 0; i < 4; ++i) CHECK(llx_budget_ctl_observe(ctl, 4.04, 1, NULL) == LLX_OK);
+        CHECK(llx_budget_ctl_gbps(ctl) == 50 && llx_budget_ctl_adjustments(ctl) == 2);
+        CHECK(llx_budget_ctl_observe(ctl, -1.0, 0, NULL) == LLX_ERR_INVALID_ARG && llx_budget_ctl_observe(NULL, 1.0, 0, NULL) == LLX_ERR_INVALID_ARG);
+        CHECK(llx_budget_ctl_destroy(ctl) == LLX_OK && llx_budget_ctl_destroy(NULL) == LLX_OK);
+    }
 
     /* the handshake without pools: coordination only */
     CHECK(llx_blockmgr_create(16, &a) == LLX_OK && llx_blockmgr_create(6, &b) == LLX_OK);
