@@ -432,6 +432,38 @@ llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* dev
                                 const int32_t* dev_block_tables, const int32_t* dev_ctx_lens, int B, int max_blocks,
                                 float scale, void* cuda_stream);
 
+/* The same attention for callers that are not allowed to allocate device memory.
+ *
+ * Who that is: a serving engine that has handed all of the GPU's free memory to its KV-cache pool at start-up (so a
+ * later cudaMalloc fails or trips its out-of-memory accounting), a decode loop on a latency budget (cudaMalloc and
+ * cudaFree may synchronise the whole device and stall every stream, the migration's included), and code that runs
+ * where the CUDA allocator must not be entered at all (inside a host callback of a stream, or under a memory-pool
+ * policy that forbids growth after initialisation).  llx_decode_attention grows a per-pool workspace with
+ * cudaMalloc/cudaFree whenever a larger shape arrives; this entry point never does.
+ *
+ * Arguments, result and preconditions are exactly those of llx_decode_attention.  The split-KV partials
+ * (B * kv_heads * ceil(max_blocks*block_size / split) rows of (head_dim + 4) floats, split = LLX_OPT_ATTN_SPLIT_TOKENS,
+ * 256 by default) go into ONE fixed array of LLX_ATTN_STATIC_WS_BYTES that is part of the library image: every GPU
+ * that loads libllx.so holds those bytes from the moment the library's code is loaded on it until the process exits,
+ * whether or not this function is ever called.  16 MiB covers BASELINE.json configs[4]'s decode batch (32 sequences x
+ * 32 heads x up to 4096 tokens of context, head_dim 128: 8.25 MiB) with room for a batch of 62 at that length.
+ *
+ *   - A shape whose partials need more than LLX_ATTN_STATIC_WS_BYTES is refused with LLX_ERR_INVALID_ARG before anything
+ *     is launched (llx_last_error gives the bytes needed and the limit); nothing is allocated instead.  A larger
+ *     LLX_OPT_ATTN_SPLIT_TOKENS shrinks the need.
+ *   - No cudaMalloc, cudaFree, cudaHostAlloc or other allocating routine is called, on the first call or any later one.
+ *   - First call on each device: with that device current (the pool's device — the call checks it) the library looks up
+ *     the array's device address once and keeps it.  Make that first call during start-up, before any stream capture.
+ *   - The array is shared by every pool, stream and thread of the process on that device and keeps what the last call
+ *     left in it.  Nothing in it has to start at zero: a call writes every partial it later reads.  Two calls that are
+ *     in flight on the GPU at the same time (different streams, or different threads) race on it and both may return
+ *     wrong outputs silently: order all calls of one device on one stream, or with events.  It does not touch the
+ *     per-pool workspace, so it may overlap llx_decode_attention calls freely. */
+#define LLX_ATTN_STATIC_WS_BYTES (16u << 20)
+llx_status llx_decode_attention_static_ws(const llx_pool* pool, int layer, const void* dev_q, void* dev_out,
+                                          const int32_t* dev_block_tables, const int32_t* dev_ctx_lens, int B,
+                                          int max_blocks, float scale, void* cuda_stream);
+
 /* ---- tuning, counters, errors ----------------------------------------------------------- */
 
 typedef enum {

@@ -11,7 +11,7 @@ from .binding import (  # noqa: F401
     OPT_UNIT_ORDER, OPT_L2_HINT, OPT_RINGS_PER_CTA, OPT_PDL, OPT_BANDWIDTH_GBPS, OPT_VIA_HOST_MODE, OPT_DYNAMIC_TAIL_PCT, OPT_DYNAMIC_TAIL_BATCH, OPT_EXACT_RESIDENCY, OPT_COPY_SMEM_CARVEOUT_PCT, OPT_PACED_SLICE_US, OPT_OVERLAP_PREV,
     pool_create, pool_wrap, pool_bytes_for, pool_ipc_export, pool_ipc_open, IPC_HANDLE_BYTES,
     plan_stage, predict_stage_sizes, migrate_stage, migrate_stage_wait, migrate_batch, staging_bytes, PinnedStaging, pack, unpack, migrate_via_host,
-    append_tokens, decode_attention,
+    append_tokens, decode_attention, decode_attention_static_ws, ATTN_STATIC_WS_BYTES,
     calc_freeness, pair_instances, migration_order, plan_migration_batch,
     BlockManager, Migration, BudgetController, REQ_RUNNING, REQ_FINISHED, REQ_PREEMPTED, REQ_PEER_FAILED,
     MIG_READY, MIG_COPYING, MIG_FINAL_COPYING, MIG_COMMITTED, MIG_ABORTED,

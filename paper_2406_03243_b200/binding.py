@@ -128,6 +128,7 @@ EXPORTS = {
                                       _i32p, _i32p, _vp, _i, _i32p, C.POINTER(_i), _i32p, _i32p, _i32p, _i, C.POINTER(_i)]),
     "llx_append_tokens": (_i, [_vp, _i32p, _i, _i, _i, _vp, _vp]),
     "llx_decode_attention": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _i, _i, C.c_float, _vp]),
+    "llx_decode_attention_static_ws": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _i, _i, C.c_float, _vp]),
     "llx_set_option": (_i, [_i, C.c_longlong]),
     "llx_get_option": (C.c_longlong, [_i]),
     "llx_get_counters": (None, [C.POINTER(_Counters)]),
@@ -546,6 +547,20 @@ def decode_attention(pool: Pool, layer: int, dev_q: int, dev_out: int, dev_block
                      B: int, max_blocks: int, scale: float, stream=None):
     _check(load().llx_decode_attention(pool.handle, layer, dev_q, dev_out, dev_block_tables, dev_ctx_lens,
                                        B, max_blocks, scale, _stream(stream)))
+
+
+ATTN_STATIC_WS_BYTES = 16 << 20   # LLX_ATTN_STATIC_WS_BYTES of include/llx.h
+
+
+def decode_attention_static_ws(pool: Pool, layer: int, dev_q: int, dev_out: int, dev_block_tables: int, dev_ctx_lens: int,
+                               B: int, max_blocks: int, scale: float, stream=None):
+    """llx_decode_attention for a caller that must not allocate device memory while it runs (an engine that gave all
+    free HBM to its KV pool, a decode loop that cannot afford cudaMalloc's device-wide stall): same arguments and
+    result, the split-KV partials live in a fixed ATTN_STATIC_WS_BYTES array inside the library instead of a
+    cudaMalloc'ed per-pool workspace.  Larger shapes raise LLX_ERR_INVALID_ARG; calls that overlap on the GPU race on
+    the shared array; make the first call on a device outside any stream capture (include/llx.h has the details)."""
+    _check(load().llx_decode_attention_static_ws(pool.handle, layer, dev_q, dev_out, dev_block_tables, dev_ctx_lens,
+                                                 B, max_blocks, scale, _stream(stream)))
 
 
 def set_option(opt: int, value: int):

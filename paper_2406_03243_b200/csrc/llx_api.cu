@@ -1690,6 +1690,103 @@ llx_status llx_decode_attention(const llx_pool* pool, int layer, const void* q, 
     return LLX_OK;
 }
 
+}  // extern "C"
+
+// ---- llx_decode_attention_static_ws: the split-KV partials in memory that is part of the library image ----------
+// For callers that cannot allocate device memory once they are running (llx.h says who and why).  The array below is
+// device memory the driver sets aside on every GPU when it loads this library's code there; it stays until the process
+// exits.  Nothing in it needs an initial value: llx_attn_partial writes the (acc, m, l) row of every split that has
+// tokens and llx_attn_merge reads exactly those rows, so stale rows of an earlier call are never read.
+static __device__ __align__(256) unsigned char g_attn_static_ws[LLX_ATTN_STATIC_WS_BYTES];
+
+namespace {
+// `g_attn_static_ws` in HOST code is only the handle the runtime registered for the symbol, not an address the GPU can
+// use; the device address comes from cudaGetSymbolAddress, per device (every device has its own copy of the array).
+std::mutex g_attn_static_mu;
+float* g_attn_static_ptr[64] = {};
+
+// `dev` is the current device (check_pool has verified that the pool lives on it).  Allocates nothing.
+llx_status attn_static_ws(int dev, float** out) {
+    if (dev < 0 || dev >= 64) return fail(LLX_ERR_INVALID_ARG, "device %d unsupported", dev);
+    std::lock_guard<std::mutex> lk(g_attn_static_mu);
+    if (!g_attn_static_ptr[dev]) {
+        void* ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_attn_static_ws);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(static attention workspace)");
+        if (!ptr || ((uintptr_t)ptr & 255) != 0) return fail(LLX_ERR_CUDA, "static attention workspace: bad device address %p", ptr);
+        g_attn_static_ptr[dev] = (float*)ptr;
+    }
+    *out = g_attn_static_ptr[dev];
+    return LLX_OK;
+}
+}  // namespace
+
+extern "C" {
+
+llx_status llx_decode_attention_static_ws(const llx_pool* pool, int layer, const void* q, void* out, const int32_t* block_tables,
+                                          const int32_t* ctx_lens, int B, int max_blocks, float scale, void* stream) {
+    llx_status rc = check_pool(pool, "pool");
+    if (rc != LLX_OK) return rc;
+    if (pool->dtype != LLX_F16) return fail(LLX_ERR_INVALID_ARG, "decode attention needs an fp16 pool");
+    if (pool->head_dim != 64 && pool->head_dim != 128) return fail(LLX_ERR_INVALID_ARG, "head_dim %d unsupported (64 or 128)", pool->head_dim);
+    if (layer < 0 || layer >= pool->layers) return fail(LLX_ERR_INVALID_ARG, "layer %d not in [0,%d)", layer, pool->layers);
+    if (B < 0 || max_blocks < 0) return fail(LLX_ERR_INVALID_ARG, "B = %d, max_blocks = %d", B, max_blocks);
+    if (B == 0) return LLX_OK;
+    if (!q || !out || !block_tables || !ctx_lens) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
+    if ((((uintptr_t)q | (uintptr_t)out) & 15) != 0) return fail(LLX_ERR_INVALID_ARG, "q and out must be 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+
+    int split = (int)g_opt_attn_split.load();
+    if (split <= 0) split = 256;
+    const int D = pool->head_dim, H = pool->kv_heads;
+    const long long max_tokens = (long long)max_blocks * pool->block_size;
+    long long max_splits = (max_tokens + split - 1) / split;
+    if (max_splits < 1) max_splits = 1;
+    if (max_splits > 65535 || B > 65535) return fail(LLX_ERR_INVALID_ARG, "grid too large");
+    // the size check comes before the address look-up: a shape that does not fit is refused without touching the GPU
+    const unsigned long long need = (unsigned long long)B * H * max_splits * (D + 4) * sizeof(float);
+    if (need > LLX_ATTN_STATIC_WS_BYTES)
+        return fail(LLX_ERR_INVALID_ARG,
+                    "llx_decode_attention_static_ws: the partials of B = %d, kv_heads = %d, %lld KV splits of %d tokens need %llu bytes; "
+                    "the fixed workspace holds %u (LLX_ATTN_STATIC_WS_BYTES) and this call never allocates: shrink the batch or "
+                    "raise LLX_OPT_ATTN_SPLIT_TOKENS, or use llx_decode_attention",
+                    B, H, max_splits, split, need, (unsigned)LLX_ATTN_STATIC_WS_BYTES);
+    float* ws = nullptr;
+    if ((rc = attn_static_ws(pool->device, &ws)) != LLX_OK) return rc;
+
+    AttnArgs a;
+    a.k_base = (const unsigned char*)llx_pool_data(pool, layer, 0);
+    a.v_base = (const unsigned char*)llx_pool_data(pool, layer, 1);
+    a.q = (const __half*)q;
+    a.out = (__half*)out;
+    a.block_tables = block_tables;
+    a.ctx_lens = ctx_lens;
+    a.part = ws;
+    a.tile_bytes = pool->tile_bytes;
+    a.H = H;
+    a.S = pool->block_size;
+    a.max_blocks = max_blocks;
+    a.max_splits = (int)max_splits;
+    a.split_tokens = split;
+    a.scale_log2 = scale * 1.4426950408889634f;
+    const int hpw = 32 / (D / 8);
+    const int head_groups = (H + kAttnWarps * hpw - 1) / (kAttnWarps * hpw);
+    dim3 grid1((unsigned)max_splits, head_groups, B), grid2(H, B);
+    cudaError_t e;
+    const bool pdl = g_opt_pdl.load() != 0;
+    if (D == 128) {
+        e = launch_k(pdl, llx_attn_partial<128>, grid1, kAttnWarps * 32, 0, st, a);
+        if (e == cudaSuccess) e = launch_k(pdl, llx_attn_merge<128>, grid2, 128, 0, st, a);
+    } else {
+        e = launch_k(pdl, llx_attn_partial<64>, grid1, kAttnWarps * 32, 0, st, a);
+        if (e == cudaSuccess) e = launch_k(pdl, llx_attn_merge<64>, grid2, 64, 0, st, a);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "attention kernel launch");
+    LLX_CUDA(cudaGetLastError());
+    g_launches += 2;
+    return LLX_OK;
+}
+
 llx_status llx_set_option(llx_option opt, long long v) {
     if (!opt_valid((int)opt, v)) return fail(LLX_ERR_INVALID_ARG, "option %d: bad value %lld", (int)opt, v);
     switch (opt) {
