@@ -532,8 +532,8 @@ def run_llx(args):
                               "consecutive steps migrate two such requests alternately",
                    "streams": ("copies on the migration stream, appends on the source's decode stream (PAPER.md:134, :235); the final "
                                "stage waits for the appends" if dec is not None else "everything on one stream (--serial-appends)"),
-                   "stage_order": ("stages 0 and 1 are launched with llx_launch_opts.overlap_prev=1 (independent of the kernel "
-                                   "before them: disjoint blocks; they may start while it drains, completion order kept); "
+                   "stage_order": ("stages 0 and 1 are launched with llx_launch_opts.overlap_prev=1 (independent of every launch back "
+                                   "to the previous final stage: disjoint blocks; they may start while it drains, completion order kept); "
                                    "the final stage in plain stream order" if w.stage_opts is not None
                                    else "plain stream order for every stage"),
                    "bytes_per_step_rd_plus_wr": step_bytes(g), "parallelism": f"replicas x{world} (no collective)",

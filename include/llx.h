@@ -184,7 +184,7 @@ typedef struct llx_launch_opts {
     int32_t exact_residency;   /* LLX_OPT_EXACT_RESIDENCY */
     int32_t via_host_mode;     /* LLX_OPT_VIA_HOST_MODE */
     int32_t route;             /* llx_route; LLX_OPT_DEFAULT = LLX_ROUTE_AUTO */
-    int32_t overlap_prev;      /* LLX_OPT_OVERLAP_PREV: 1 = this copy is independent of the previous kernel on its stream */
+    int32_t overlap_prev;      /* LLX_OPT_OVERLAP_PREV: 1 = this copy is independent of every launch back to the last one without the flag */
 } llx_launch_opts;
 /* Sets struct_size and every field to LLX_OPT_DEFAULT. */
 void llx_launch_opts_init(llx_launch_opts* opts);
@@ -508,11 +508,18 @@ typedef enum {
                                    split waits for the end of a slice, not of the stage (75 ms for 112 blocks at 25 GB/s).
                                    Default 1000; 0 = one launch.  Costs ~3 us of host time per slice inside the call; the rate
                                    and the decode step's slowdown are unchanged (measured).  Counters count every launch */
-    LLX_OPT_OVERLAP_PREV = 17,  /* 1: the caller states that this copy is INDEPENDENT of the kernel enqueued just before it on
-                                   cuda_stream — it reads no byte that kernel writes and writes no byte that kernel reads or
-                                   writes.  True for consecutive stages of one request (disjoint blocks on both sides; full
+    LLX_OPT_OVERLAP_PREV = 17,  /* 1: the caller states that this copy is INDEPENDENT of every launch on cuda_stream from the most
+                                   recent one made WITHOUT overlap_prev (an llx call that left the flag at 0, or any work that
+                                   is not an llx kernel) up to the one enqueued just before it — it reads no byte they write and
+                                   writes no byte they read or write.  So in a chain  F, O1, O2  (F plain; O1, O2 with the flag)
+                                   O2 must be independent of O1 AND of F: an overlapped kernel lets its successor launch before
+                                   it has waited itself, so O2 may run next to F.  Everything enqueued BEFORE F has completed
+                                   when O1 or O2 starts: every llx kernel that does not defer its wait lets dependents launch
+                                   only after that wait has returned, so a plain launch fences the start of what follows it
+                                   (a small or CTA-capped plain launch included).
+                                   True for consecutive non-final stages of one request (disjoint blocks on both sides; full
                                    blocks are never written again) and for stages of different requests
-                                   (PAPER.md:225).  The copy may then START while that kernel's slowest CTAs are still running
+                                   (PAPER.md:225).  The copy may then START while those kernels' slowest CTAs are still running
                                    (the wait of the programmatic dependent launch moves from the kernel's prologue to its end),
                                    which hides the ~3 us an SM otherwise idles between two stages.  COMPLETION order is kept:
                                    when this copy has completed, everything enqueued before it on the stream has completed, so

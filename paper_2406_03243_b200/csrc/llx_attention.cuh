@@ -213,8 +213,8 @@ __global__ void __maxnreg__(112) llx_attn_partial(const AttnArgs a) {
 // grid (H, B), D threads: out[b][h][d] = sum_s 2^(m_s-M) acc_s[d] / sum_s 2^(m_s-M) l_s
 template <int D>
 __global__ void __launch_bounds__(D) llx_attn_merge(const AttnArgs a) {
-    griddep_launch();
-    griddep_wait();
+    griddep_wait();    // wait first, then let dependents launch (llx_copy.cuh, ring_copy): a kernel behind this one
+    griddep_launch();  // never starts before llx_attn_partial has completed
     const int h = blockIdx.x, b = blockIdx.y, d = threadIdx.x;
     const int ctx = min(a.ctx_lens[b], a.max_blocks * a.S);  // llx.h: a longer ctx_len is clamped, never followed past the table row
     const int ns = (ctx + a.split_tokens - 1) / a.split_tokens;

@@ -122,8 +122,8 @@ template <bool BYVAL, int UNROLL>
 __global__ void __launch_bounds__(256, 8) llx_copy_vec16(const CopyArgs a, const __grid_constant__ IdPack ids) {
     const int lane = threadIdx.x & 31;
     const int nt = blockDim.x;
+    pdl_wait_prior_grids();   // wait first, then let dependents launch: see ring_copy
     pdl_launch_dependents();
-    pdl_wait_prior_grids();
     unsigned long long deadline = a.pace_ns > 0 ? global_timer_ns() : 0ull;
     int u_begin = a.unit_begin + blockIdx.x, u_end = a.total_units, u_step = gridDim.x;
     if (a.blocked_order) {
@@ -294,15 +294,19 @@ __device__ __forceinline__ void ring_copy(const CopyArgs& a, const IdPack& ids, 
     for (int s = 0; s < nstages; ++s) mbar_init(bar0 + s * 8, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    pdl_launch_dependents();
     // A copy the caller declared independent of the previous kernel (stages of disjoint blocks) starts
     // streaming as soon as its CTA is resident, i.e. while the previous stage's slowest rings are still draining.  The
     // wait is only deferred, never dropped: (1) a ring executes it before its first claim from the dynamic-tail counter,
     // which the previous launch shares and resets with its last claim; (2) every ring executes it before it exits, so
     // "this kernel has completed" still implies "everything before it on the stream has completed" (completion stays
     // transitive although the start is not ordered).
+    // Every llx kernel that does NOT defer lets its dependents launch only AFTER its own wait has returned: when a kernel
+    // behind it starts, everything in front of it has completed.  A launch without overlap_prev is thus a fence for the
+    // start of whatever follows, and a deferred copy can only ever run next to the launches back to (and including) the
+    // last such launch — the set llx.h asks the caller to declare it independent of.
     bool waited = a.defer_wait == 0;
     if (waited) pdl_wait_prior_grids();
+    pdl_launch_dependents();
 
     const int ring = blockIdx.x * rings_per_cta + warp;
     const int nrings = gridDim.x * rings_per_cta;
@@ -442,8 +446,8 @@ struct AppendArgs {
 };
 template <bool BYVAL>
 __global__ void __launch_bounds__(128) llx_append_kernel(const AppendArgs a, const __grid_constant__ IdPack ids) {
+    pdl_wait_prior_grids();   // wait first, then let dependents launch: see ring_copy
     pdl_launch_dependents();
-    pdl_wait_prior_grids();
     const int u = blockIdx.x;  // (tok, slice)
     const int slice = u % a.slices;
     const int k = u / a.slices;

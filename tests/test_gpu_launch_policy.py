@@ -278,8 +278,8 @@ def test_overlapped_stages_are_bit_exact_and_complete_in_stream_order(env):
     """LLX_OPT_OVERLAP_PREV (llx_launch_opts.overlap_prev): a stage the caller declares independent of the previous
     kernel may START before that kernel has finished, but completion stays ordered.  A chain of stages over disjoint
     blocks — long ones with the dynamic tail (whose claim counter consecutive launches share), a short one right behind
-    a long one (it could finish first if the deferred wait were dropped), a batch launch and a stage of more than 256
-    pairs — is enqueued back to back with the flag, then ONE event behind the last, smallest kernel is waited for: every
+    a long one (it could finish first if the deferred wait were dropped) and a batch launch (the stage of more than 256
+    pairs, whose ids go through the pinned ring, is test_overlapped_stage_of_more_than_256_pairs below) — is enqueued back to back with the flag, then ONE event behind the last, smallest kernel is waited for: every
     byte of every stage must be there, equal to the oracle's, and the untouched blocks keep the sentinel."""
     H, llx = env
     g = G7
@@ -316,6 +316,95 @@ def test_overlapped_stages_are_bit_exact_and_complete_in_stream_order(env):
     idx_d = torch.from_numpy(np.asarray(perm_d[:cuts[-1]], dtype=np.int64)).cuda()
     for l in range(g["layers"]):
         assert torch.equal(dst.view[l].index_select(1, idx_d), src.view[l].index_select(1, idx_s)), l
+
+
+def test_overlapped_stage_of_more_than_256_pairs(env):
+    """An overlapped stage whose id list does not fit the kernel parameters (> 256 pairs): the ids travel through the
+    pinned ring and a device buffer, the copy of the ids is ordinary stream work in FRONT of the kernel.  Chain: a plain
+    40-block stage, then 300 pairs with overlap_prev=1, then 8 pairs with overlap_prev=1; one event behind the last."""
+    H, llx = env
+    g = dict(G7, num_blocks=360)
+    sample = [0, 13, 31]
+    src, dst = H.DevPool(g), H.DevPool(g, fill=SENT)
+    src.fill_device_random(15)
+    src.fill_from_synth(0, 0, layers=sample)
+    perm_s = synth.block_permutation(31, g["num_blocks"])
+    perm_d = synth.block_permutation(32, g["num_blocks"])
+    cuts = [0, 40, 340, 348]
+    stream = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for rep in range(3):
+        dst.view.fill_(SENT_I16)
+        torch.cuda.synchronize()
+        c0 = llx.counters()
+        for k in range(3):
+            a, b = cuts[k], cuts[k + 1]
+            llx.migrate_stage(src.pool, perm_s[a:b], dst.pool, perm_d[a:b], stream=stream, opts=None if k == 0 else dict(overlap_prev=1))
+        done = torch.cuda.Event()
+        done.record(stream)
+        done.synchronize()
+        c1 = llx.counters()
+        assert c1["id_uploads"] - c0["id_uploads"] == 1 and c1["copy_launches"] - c0["copy_launches"] == 3
+        got = dst.view[sample].cpu().numpy().view(np.uint16)
+        want = om.new_pool(len(sample), g["num_blocks"], src.te, fill=SENT)
+        om.migrate_stage(H.host_pool_from_synth(g, 0, 0, layers=sample), perm_s[:cuts[-1]], want, perm_d[:cuts[-1]])
+        H.assert_pool_equal(got, want)
+    idx_s = torch.from_numpy(np.asarray(perm_s[:cuts[-1]], dtype=np.int64)).cuda()
+    idx_d = torch.from_numpy(np.asarray(perm_d[:cuts[-1]], dtype=np.int64)).cuda()
+    for l in range(g["layers"]):
+        assert torch.equal(dst.view[l].index_select(1, idx_d), src.view[l].index_select(1, idx_s)), l
+
+
+@pytest.mark.parametrize("middle", ["capped_stage", "append", "attention"])
+def test_plain_launch_fences_the_start_of_an_overlapped_stage(env, middle):
+    """llx.h, LLX_OPT_OVERLAP_PREV: an overlapped copy has to be independent of the launches back to the last PLAIN one
+    only — what lies in front of that plain launch has completed when the copy starts, however small the plain launch is.
+    Chain on one stream: A = a 64-block stage X -> Y capped at 4 CTAs (milliseconds, 144 SMs stay free); P = a plain launch
+    that also leaves nearly every SM free (a 1-block stage capped at 2 CTAs / a 1-token append / a 1-sequence attention)
+    and touches none of A's blocks; B = a full-width stage Y -> Z with overlap_prev=1 that reads what A wrote.  B is
+    independent of P, as the contract asks, but not of A.  With kernels that let dependents launch BEFORE their own wait
+    (round 2) P's CTAs released B at once, B found the free SMs and copied Y while A had written a fraction of it — with
+    those kernels the capped-stage and append variants fail in the first repetitions (sentinel words in Z; the attention
+    variant always held, llx_attn_partial waited first already); now P's CTAs release B only after A has completed.  Every word of Z
+    is compared, 10 times with Y and Z invalidated in between."""
+    H, llx = env
+    g = dict(G7, num_blocks=160)
+    X, Y, Z = H.DevPool(g), H.DevPool(g, fill=SENT), H.DevPool(g, fill=SENT)
+    X.fill_device_random(19)
+    perm_x = synth.block_permutation(41, g["num_blocks"])
+    perm_y = synth.block_permutation(42, g["num_blocks"])
+    perm_z = synth.block_permutation(43, g["num_blocks"])
+    n = 64
+    ax, ay, bz = perm_x[:n], perm_y[:n], perm_z[:n]
+    # P's own blocks: outside everything A and B touch
+    px, py = perm_x[n + 1:n + 2], perm_y[n + 1:n + 2]
+    te_tok = g["kv_heads"] * g["head_dim"]
+    vals = torch.zeros(g["layers"] * 2 * te_tok, dtype=torch.int16, device="cuda")
+    q = torch.zeros(g["kv_heads"] * g["head_dim"], dtype=torch.int16, device="cuda")
+    o = torch.zeros_like(q)
+    bt = torch.tensor([int(px[0])], dtype=torch.int32, device="cuda")
+    ctx = torch.tensor([16], dtype=torch.int32, device="cuda")
+    i_x = torch.from_numpy(np.asarray(ax, dtype=np.int64)).cuda()
+    i_z = torch.from_numpy(np.asarray(bz, dtype=np.int64)).cuda()
+    want = [X.view[l].index_select(1, i_x) for l in range(g["layers"])]
+    stream = torch.cuda.Stream()
+    llx.decode_attention(X.pool, 0, q.data_ptr(), o.data_ptr(), bt.data_ptr(), ctx.data_ptr(), 1, 1, 1.0, stream=stream)  # workspace
+    torch.cuda.synchronize()
+    for rep in range(10):
+        Y.view[:, :, :, ::256].fill_(SENT_I16)                          # one word per 512 B of every tile
+        Z.view[:, :, :, ::256].fill_(SENT_I16)
+        torch.cuda.synchronize()
+        llx.migrate_stage(X.pool, ax, Y.pool, ay, stream=stream, opts=dict(max_ctas=4, copy_kernel=2))  # A
+        if middle == "capped_stage":
+            llx.migrate_stage(X.pool, px, Y.pool, py, stream=stream, opts=dict(max_ctas=2))            # P
+        elif middle == "append":
+            llx.append_tokens(X.pool, px, 3, 4, vals.data_ptr(), stream=stream)
+        else:
+            llx.decode_attention(X.pool, 0, q.data_ptr(), o.data_ptr(), bt.data_ptr(), ctx.data_ptr(), 1, 1, 1.0, stream=stream)
+        llx.migrate_stage(Y.pool, ay, Z.pool, bz, stream=stream, opts=dict(overlap_prev=1))             # B reads what A wrote
+        stream.synchronize()
+        for l in range(g["layers"]):
+            assert torch.equal(Z.view[l].index_select(1, i_z), want[l]), (rep, l)
 
 
 def test_overlap_keeps_completion_transitive_behind_a_long_stage(env):
