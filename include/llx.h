@@ -108,7 +108,10 @@ size_t llx_pool_bytes_for(int layers, int kv_heads, int head_dim, int block_size
  * to the peer by whatever channel the caller has), the peer opens it and gets a pool that names the SAME device memory.
  * llx_migrate_stage / _batch into an opened pool then store straight into the other process's KV cache — on the same GPU
  * (two instances sharing one device) or on another one (the mapping enables peer access; the copy takes the cross-GPU
- * route).  The handle carries the pool's geometry, so the opened pool cannot disagree with the exporter's.
+ * route).  The handle carries the pool's geometry, so the opened pool cannot disagree with the exporter's: its last
+ * 4 bytes are a checksum (32-bit FNV-1a of the 92 bytes in front of them) and llx_pool_ipc_open also compares the geometry
+ * with the size of the allocation it has just mapped — a truncated, corrupted or stale handle (one that names more
+ * blocks or layers than the exporter's allocation holds) is LLX_ERR_INVALID_ARG, not a pool that writes past the mapping.
  * llx_pool_destroy of an opened pool unmaps it; the exporter must keep its pool alive meanwhile.  Only pools from
  * llx_pool_create can be exported (the handle names a whole allocation); LLX_ERR_CUDA when the handle is opened in the
  * process that exported it (the driver refuses that). */
@@ -165,7 +168,16 @@ typedef enum {
                            (2L tiles at the pools' slice strides), same or different GPUs.  No SM is used on either GPU, so
                            a migration to another GPU cannot slow a decode step's kernels except through HBM and the link;
                            on ONE GPU it is the slow way (measured there: 1.9 TB/s against the kernels' 6.6).  Unmeasured over NVLink.
-                           llx_migrate_stage_wait falls back to the stream synchronize */
+                           llx_migrate_stage_wait falls back to the stream synchronize.  The copy engines cannot be paced or
+                           capped: with a non-zero bandwidth_gbps or max_ctas (from the call or the process defaults) the
+                           call returns LLX_ERR_INVALID_ARG instead of running unthrottled; every other launch-policy field
+                           (copy_kernel, chunk_bytes, ring_stages, overlap_prev, ...) has no meaning here and is ignored.
+                           Counters: bytes_moved grows, kernel_launches / copy_launches do not (no kernel ran).  The same
+                           holds for the copy-engine host legs (LLX_OPT_VIA_HOST_MODE 2, and 0 for llx_migrate_via_host):
+                           budget and CTA cap do not apply to them (the link, not HBM, is their bound; they are NOT refused),
+                           an explicit copy_kernel selects the kernel + bounce route instead.  A pool whose slice stride
+                           num_blocks*tile_bytes exceeds the pitch limit of a pitched transfer (2^31-1 bytes) is served
+                           tile by tile (2L transfers per block); llx_migrate_via_host's AUTO then prefers the bounce route */
 } llx_route;
 typedef struct llx_launch_opts {
     uint32_t struct_size;      /* sizeof(llx_launch_opts) as the caller compiled it; set by llx_launch_opts_init */

@@ -914,16 +914,45 @@ llx_status staged_through_bounce(const Policy& pol, bool to_host, const llx_pool
 // LLX_OPT_VIA_HOST_MODE = 2: the copy engine gathers / scatters by itself.  One block is 2L tiles at a constant
 // stride (num_blocks*tile_bytes) in the pool and 2L consecutive tiles in the staging buffer: ONE pitched copy per block
 // (cudaMemcpy2DAsync: width = tile_bytes, height = 2L) crosses the link with no kernel, no bounce buffer and no SM.
+// A pitched transfer's pitch is limited (cudaDevAttrMaxPitch, 2^31-1 bytes on B200), and a pool's slice stride
+// num_blocks*tile_bytes passes that in big pools (LLaMA-7B tiles: from 16384 blocks = 128 GiB of pool; fewer layers, sooner).
+// Such a pool is served tile by tile: 2L plain copies per block instead of one pitched one — still the copy engines, no
+// kernel, more calls.  (llx_migrate_via_host's AUTO route prefers the bounce route there, see below.)
+bool pitch_ok(const llx_pool* pool) {
+    static std::atomic<long long> cache[64];
+    const int dev = pool->device;
+    long long lim = (dev >= 0 && dev < 64) ? cache[dev].load() : 0;
+    if (lim <= 0) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxPitch, dev) != cudaSuccess || v <= 0) {
+            cudaGetLastError();
+            v = 0x7fffffff;
+        }
+        lim = v;
+        if (dev >= 0 && dev < 64) cache[dev] = lim;
+    }
+    return (long long)pool->num_blocks * pool->tile_bytes <= lim;
+}
+
 llx_status ce_blocks(bool to_host, const llx_pool* pool, const int32_t* ids, int first, int count, const Side& stg, cudaStream_t st) {
     const size_t tile = (size_t)pool->tile_bytes, pool_pitch = (size_t)pool->num_blocks * tile;
     const size_t rows = 2 * (size_t)pool->layers, block_bytes = rows * tile;
+    const bool pitched = pitch_ok(pool);
     for (int i = first; i < first + count; ++i) {
         unsigned char* p = pool->data + (size_t)ids[i] * tile;
         unsigned char* h = const_cast<unsigned char*>(stg.base) + (size_t)i * block_bytes;
-        if (to_host)
+        if (!pitched) {
+            for (size_t r = 0; r < rows; ++r) {
+                if (to_host)
+                    LLX_CUDA(cudaMemcpyAsync(h + r * tile, p + r * pool_pitch, tile, cudaMemcpyDefault, st));
+                else
+                    LLX_CUDA(cudaMemcpyAsync(p + r * pool_pitch, h + r * tile, tile, cudaMemcpyDefault, st));
+            }
+        } else if (to_host) {
             LLX_CUDA(cudaMemcpy2DAsync(h, tile, p, pool_pitch, tile, rows, cudaMemcpyDefault, st));
-        else
+        } else {
             LLX_CUDA(cudaMemcpy2DAsync(p, pool_pitch, h, tile, tile, rows, cudaMemcpyDefault, st));
+        }
     }
     return LLX_OK;
 }
@@ -1044,10 +1073,38 @@ struct IpcHandle {  // LLX_IPC_HANDLE_BYTES: the CUDA handle of the allocation +
     cudaIpcMemHandle_t mem;
     uint32_t magic;
     int32_t layers, kv_heads, head_dim, block_size, dtype, num_blocks;
-    uint32_t reserved;
+    uint32_t checksum;  // FNV-1a over every byte in front of it: a truncated, stale or corrupted handle is refused
 };
 static_assert(sizeof(IpcHandle) == LLX_IPC_HANDLE_BYTES, "LLX_IPC_HANDLE_BYTES must match IpcHandle");
-constexpr uint32_t kIpcMagic = 0x4C4C5831u;  // "LLX1"
+constexpr uint32_t kIpcMagic = 0x4C4C5832u;  // "LLX2" (round 3: the last word became the checksum)
+
+uint32_t ipc_checksum(const IpcHandle& h) {
+    const unsigned char* b = reinterpret_cast<const unsigned char*>(&h);
+    uint32_t x = 2166136261u;
+    for (size_t i = 0; i < offsetof(IpcHandle, checksum); ++i) x = (x ^ b[i]) * 16777619u;
+    return x;
+}
+
+// Size of the allocation (or IPC mapping) that contains `ptr`, 0 when the driver cannot say.  cuMemGetAddressRange is
+// fetched like cuTensorMapEncodeTiled: libcuda is not linked.
+size_t mapped_range_bytes(const void* ptr) {
+    typedef CUresult (*RangeFn)(CUdeviceptr*, size_t*, CUdeviceptr);
+    static RangeFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q = cudaDriverEntryPointSymbolNotFound;
+        if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            p = nullptr;
+        }
+        return (RangeFn)p;
+    }();
+    if (!fn) return 0;
+    CUdeviceptr base = 0;
+    size_t size = 0;
+    if (fn(&base, &size, (CUdeviceptr)(uintptr_t)ptr) != CUDA_SUCCESS) return 0;
+    const size_t skip = (size_t)((uintptr_t)ptr - (uintptr_t)base);
+    return size > skip ? size - skip : 0;
+}
 
 llx_status llx_pool_ipc_export(const llx_pool* p, void* handle_out) {
     if (!p || !p->data || !handle_out) return fail(LLX_ERR_INVALID_ARG, "NULL argument");
@@ -1062,6 +1119,7 @@ llx_status llx_pool_ipc_export(const llx_pool* p, void* handle_out) {
     h.block_size = p->block_size;
     h.dtype = (int32_t)p->dtype;
     h.num_blocks = p->num_blocks;
+    h.checksum = ipc_checksum(h);
     memcpy(handle_out, &h, sizeof h);
     return LLX_OK;
 }
@@ -1073,6 +1131,7 @@ llx_status llx_pool_ipc_open(const void* handle, llx_pool** out) {
     IpcHandle h;
     memcpy(&h, handle, sizeof h);
     if (h.magic != kIpcMagic) return fail(LLX_ERR_INVALID_ARG, "not an llx pool handle");
+    if (h.checksum != ipc_checksum(h)) return fail(LLX_ERR_INVALID_ARG, "llx pool handle is corrupted or truncated (checksum mismatch)");
     const size_t need = llx_pool_bytes_for(h.layers, h.kv_heads, h.head_dim, h.block_size, (llx_dtype)h.dtype, h.num_blocks);
     if (need == 0) return fail(LLX_ERR_INVALID_ARG, "handle carries a bad geometry");
     void* ptr = nullptr;
@@ -1081,7 +1140,16 @@ llx_status llx_pool_ipc_open(const void* handle, llx_pool** out) {
         cudaGetLastError();
         return fail(LLX_ERR_CUDA, "cudaIpcOpenMemHandle: %s", cudaGetErrorString(e));
     }
-    llx_status rc = make_pool(ptr, need, false, h.layers, h.kv_heads, h.head_dim, h.block_size, (llx_dtype)h.dtype, h.num_blocks, out);
+    // The geometry came with the handle; the mapping is what the exporter really allocated.  A handle that names more
+    // blocks or layers than that (stale: the exporter re-created its pool; or forged with a matching checksum) would let
+    // stages write past the mapping into whatever the other process keeps behind it.
+    const size_t mapped = mapped_range_bytes(ptr);
+    if (mapped != 0 && mapped < need) {
+        cudaIpcCloseMemHandle(ptr);
+        return fail(LLX_ERR_INVALID_ARG, "llx pool handle names a pool of %zu bytes but the exporter's allocation has %zu", need, mapped);
+    }
+    llx_status rc = make_pool(ptr, mapped != 0 ? mapped : need, false, h.layers, h.kv_heads, h.head_dim, h.block_size, (llx_dtype)h.dtype,
+                              h.num_blocks, out);
     if (rc != LLX_OK) {
         cudaIpcCloseMemHandle(ptr);
         return rc;
@@ -1198,10 +1266,28 @@ static llx_status ce_pool_to_pool(const llx_pool* src, const int32_t* src_ids, l
                                   cudaStream_t st) {
     const size_t tile = (size_t)src->tile_bytes, rows = 2 * (size_t)src->layers;
     const size_t sp = (size_t)src->num_blocks * tile, dp = (size_t)dst->num_blocks * tile;
-    for (long long i = 0; i < n; ++i)
-        LLX_CUDA(cudaMemcpy2DAsync(dst->data + (size_t)dst_ids[i] * tile, dp, src->data + (size_t)src_ids[i] * tile, sp, tile, rows,
-                                   cudaMemcpyDefault, st));
+    const bool pitched = pitch_ok(src) && pitch_ok(dst);  // else tile by tile: see pitch_ok
+    for (long long i = 0; i < n; ++i) {
+        unsigned char* d = dst->data + (size_t)dst_ids[i] * tile;
+        const unsigned char* s = src->data + (size_t)src_ids[i] * tile;
+        if (pitched) {
+            LLX_CUDA(cudaMemcpy2DAsync(d, dp, s, sp, tile, rows, cudaMemcpyDefault, st));
+        } else {
+            for (size_t r = 0; r < rows; ++r) LLX_CUDA(cudaMemcpyAsync(d + r * dp, s + r * sp, tile, cudaMemcpyDefault, st));
+        }
+    }
     g_bytes += (unsigned long long)n * rows * tile;
+    return LLX_OK;
+}
+
+// The copy engines cannot be paced or capped by this library: a budget or CTA cap that silently did nothing would defeat
+// its purpose (<= 1 % on the co-running batch), so the combination is refused instead of ignored.
+static llx_status ce_route_policy_ok(const Policy& pol) {
+    if (pol.budget > 0 || pol.max_ctas > 0)
+        return fail(LLX_ERR_INVALID_ARG,
+                    "LLX_ROUTE_COPY_ENGINE runs no kernel and cannot honour bandwidth_gbps = %lld / max_ctas = %lld (from this "
+                    "call's llx_launch_opts or the process defaults): pace the calls on the host, or use the kernel route",
+                    pol.budget, pol.max_ctas);
     return LLX_OK;
 }
 
@@ -1215,7 +1301,10 @@ static llx_status migrate_stage_checked(const Policy& pol, const llx_pool* src, 
     if ((rc = check_range(src_ids, n, src->num_blocks, "src")) != LLX_OK) return rc;
     if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
     if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
-    if (pol.route == LLX_ROUTE_COPY_ENGINE) return ce_pool_to_pool(src, src_ids, dst, dst_ids, n, (cudaStream_t)stream);
+    if (pol.route == LLX_ROUTE_COPY_ENGINE) {
+        if ((rc = ce_route_policy_ok(pol)) != LLX_OK) return rc;
+        return ce_pool_to_pool(src, src_ids, dst, dst_ids, n, (cudaStream_t)stream);
+    }
     return launch_copy(pol, pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
                        (cudaStream_t)stream);
 }
@@ -1318,7 +1407,10 @@ llx_status llx_migrate_batch_ex(const llx_pool* src, llx_pool* dst, const int32_
     if ((rc = check_range(src_ids, n, src->num_blocks, "src")) != LLX_OK) return rc;
     if ((rc = check_range(dst_ids, n, dst->num_blocks, "dst")) != LLX_OK) return rc;
     if ((rc = check_unique(dst_ids, n, dst->num_blocks)) != LLX_OK) return rc;
-    if (pol.route == LLX_ROUTE_COPY_ENGINE) return ce_pool_to_pool(src, src_ids, dst, dst_ids, n, (cudaStream_t)stream);
+    if (pol.route == LLX_ROUTE_COPY_ENGINE) {
+        if ((rc = ce_route_policy_ok(pol)) != LLX_OK) return rc;
+        return ce_pool_to_pool(src, src_ids, dst, dst_ids, n, (cudaStream_t)stream);
+    }
     // every (block, layer, K|V) tile is independent, so the requests are flattened into one grid
     return launch_copy(pol, pool_side(src, src_ids), pool_side(dst, dst_ids), n, src->layers, src->tile_bytes, src->device,
                        (cudaStream_t)stream);
@@ -1375,7 +1467,9 @@ llx_status llx_pack_ex(const llx_pool* src, const int32_t* src_ids, int n, void*
     if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "staging buffer overlaps the pool");
     if (stg.host_memory && pol.via_host == 2 && pol.kernel == 0) {
         if ((rc = refuse_if_capturing((cudaStream_t)stream, "llx_pack into pinned host memory")) != LLX_OK) return rc;
-        return ce_blocks(true, src, src_ids, 0, n, stg, (cudaStream_t)stream);
+        if ((rc = ce_blocks(true, src, src_ids, 0, n, stg, (cudaStream_t)stream)) != LLX_OK) return rc;
+        g_bytes += (unsigned long long)llx_staging_bytes(src, n);  // copy-engine transfers count bytes, not launches
+        return LLX_OK;
     }
     if (stg.host_memory && (pol.via_host == 0 || pol.via_host == 3) && pol.kernel == 0) {
         pol.overlap = 0;  // a chain of dependent kernels and transfers through one bounce buffer: plain stream order
@@ -1408,7 +1502,9 @@ llx_status llx_unpack_ex(const void* staging, size_t staging_bytes, llx_pool* ds
     if (a0 < b1 && b0 < a1) return fail(LLX_ERR_ALIAS, "staging buffer overlaps the pool");
     if (stg.host_memory && pol.via_host == 2 && pol.kernel == 0) {
         if ((rc = refuse_if_capturing((cudaStream_t)stream, "llx_unpack from pinned host memory")) != LLX_OK) return rc;
-        return ce_blocks(false, dst, dst_ids, 0, n, stg, (cudaStream_t)stream);
+        if ((rc = ce_blocks(false, dst, dst_ids, 0, n, stg, (cudaStream_t)stream)) != LLX_OK) return rc;
+        g_bytes += (unsigned long long)llx_staging_bytes(dst, n);
+        return LLX_OK;
     }
     if (stg.host_memory && (pol.via_host == 0 || pol.via_host == 3) && pol.kernel == 0) {
         pol.overlap = 0;  // see llx_pack_ex
@@ -1459,7 +1555,10 @@ llx_status llx_migrate_via_host_ex(const llx_pool* src, const int32_t* src_ids, 
     // after 16 MiB instead of 64: 22.9 ms per GiB each way = 93.8 GB/s against 25.3 ms = 84.9 GB/s for the bounce route
     // on the same box (the full-duplex floor of the link is 21.6 ms).  The bounce route stays for a destination on
     // another GPU and as mode 3; zero-copy kernels are mode 1.
-    const bool strided_ce = stg.host_memory && src->device == dst->device && (pol.via_host == 2 || pol.via_host == 0);
+    // A pool whose slice stride exceeds the pitch limit (pitch_ok) cannot take pitched transfers: AUTO then keeps the bounce
+    // route (85 GB/s; tile-by-tile copy-engine transfers are 2L calls per block); an explicit mode 2 gets tile by tile.
+    const bool strided_ce = stg.host_memory && src->device == dst->device &&
+                            (pol.via_host == 2 || (pol.via_host == 0 && pol.kernel == 0 && pitch_ok(src) && pitch_ok(dst)));
     const bool bounce = stg.host_memory && !strided_ce && pol.via_host != 1;
     if (strided_ce && chunk_blocks <= 0) {  // small groups: the first host->device copy starts after 16 MiB, not 64
         chunk_blocks = (int)((16ll << 20) / block_bytes);

@@ -270,6 +270,13 @@ def test_ipc_handle_is_checked(llx):
     assert e.value.name == "LLX_ERR_INVALID_ARG"
     with pytest.raises(llx.LlxError):
         llx.pool_ipc_open(b"short")
+    # the right magic ("LLX2") but no valid checksum behind it: refused before any CUDA call is made
+    import struct
+    forged = b"\x11" * 64 + struct.pack("<I6iI", 0x4C4C5832, 32, 32, 128, 16, 0, 2000, 0)
+    assert len(forged) == llx.IPC_HANDLE_BYTES
+    with pytest.raises(llx.LlxError) as e:
+        llx.pool_ipc_open(forged)
+    assert e.value.name == "LLX_ERR_INVALID_ARG" and "checksum" in str(e.value)
     out = C.c_void_p()
     assert l.llx_pool_ipc_open(None, C.byref(out)) == -1 and l.llx_pool_ipc_export(None, None) == -1
     # session policy: a struct size the library cannot read is refused (an older, shorter struct is served), NULL resets

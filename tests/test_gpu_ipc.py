@@ -21,6 +21,14 @@ def _ids():
     return synth.block_permutation(51, G["num_blocks"])[:N], synth.block_permutation(52, G["num_blocks"])[:N]
 
 
+def _fnv1a(b: bytes) -> int:
+    """The handle's last word as llx.h describes it (32-bit FNV-1a of the 92 bytes in front of it)."""
+    x = 2166136261
+    for c in b:
+        x = ((x ^ c) * 16777619) & 0xFFFFFFFF
+    return x
+
+
 def destination_instance(conn, device):
     """Runs in the child: owns the destination pool; never calls a copy itself."""
     try:
@@ -71,6 +79,18 @@ def test_migration_into_another_process_pool():
         assert isinstance(handle, bytes) and len(handle) == llx.IPC_HANDLE_BYTES, handle
         src = H.DevPool(G)
         src.fill_from_synth(31, 0)
+        # a damaged handle is refused by its checksum; a handle that names a larger pool than the exporter allocated,
+        # with a checksum made to match (a stale or forged handle), is refused against the size of the real mapping
+        flipped = bytearray(handle)
+        flipped[64 + 4 + 20] ^= 0x40                            # num_blocks: 40 -> 104
+        with pytest.raises(llx.LlxError) as e:
+            llx.pool_ipc_open(bytes(flipped))
+        assert e.value.name == "LLX_ERR_INVALID_ARG" and "checksum" in str(e.value)
+        flipped[92:96] = _fnv1a(bytes(flipped[:92])).to_bytes(4, "little")
+        with pytest.raises(llx.LlxError) as e:
+            llx.pool_ipc_open(bytes(flipped))
+        assert e.value.name == "LLX_ERR_INVALID_ARG" and "allocation has" in str(e.value), str(e.value)
+        assert _fnv1a(handle[:92]).to_bytes(4, "little") == handle[92:96]
         dst = llx.pool_ipc_open(handle)
         assert dst.num_blocks == G["num_blocks"] and dst.tile_bytes == src.pool.tile_bytes
         s_ids, d_ids = _ids()

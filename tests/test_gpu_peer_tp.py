@@ -87,6 +87,53 @@ def test_copy_engine_route_is_bit_exact(env, g):
     H.assert_pool_equal(src.host(), h_src)
 
 
+def test_copy_engine_route_refuses_a_budget_and_counts_bytes(env):
+    """llx.h, LLX_ROUTE_COPY_ENGINE: the copy engines cannot be paced or capped, so a call that asks for both the route and
+    a bandwidth budget / CTA cap (per call, or inherited from the process defaults) is refused before anything is enqueued
+    instead of running unthrottled.  The copy-engine host legs (llx_pack / llx_unpack mode 2) count their bytes like the
+    pool-to-pool route; an explicit copy_kernel makes llx_migrate_via_host take its kernel route (as llx_pack does)."""
+    H, llx = env
+    g = RAGGED
+    src, dst, h_src, h_dst = make(H, g, seed=25)
+    s_ids = synth.block_permutation(37, g["num_blocks"])[:6]
+    d_ids = synth.block_permutation(38, g["num_blocks"])[:6]
+    for bad in (dict(bandwidth_gbps=25), dict(max_ctas=4)):
+        with pytest.raises(llx.LlxError) as e:
+            llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, opts=dict(route=llx.ROUTE_COPY_ENGINE, **bad))
+        assert e.value.name == "LLX_ERR_INVALID_ARG" and "LLX_ROUTE_COPY_ENGINE" in str(e.value)
+        with pytest.raises(llx.LlxError):
+            llx.migrate_batch(src.pool, dst.pool, [0, 6], s_ids, d_ids, opts=dict(route=llx.ROUTE_COPY_ENGINE, **bad))
+    with llx.options(bandwidth_gbps=25):                                  # inherited from the process default
+        with pytest.raises(llx.LlxError):
+            llx.migrate_stage(src.pool, s_ids, dst.pool, d_ids, opts=dict(route=llx.ROUTE_COPY_ENGINE))
+    torch.cuda.synchronize()
+    H.assert_pool_equal(dst.host(), h_dst)                                # refused: not a byte moved
+    nbytes = llx.staging_bytes(src.pool, 6)
+    pin = llx.PinnedStaging(nbytes)
+    c0 = llx.counters()
+    llx.pack(src.pool, s_ids, pin.dev_alias, nbytes, opts=dict(via_host_mode=2))
+    llx.unpack(pin.dev_alias, nbytes, dst.pool, d_ids, opts=dict(via_host_mode=2))
+    c1 = llx.counters()
+    assert c1["kernel_launches"] == c0["kernel_launches"] and c1["bytes_moved"] - c0["bytes_moved"] == 2 * nbytes
+    torch.cuda.synchronize()
+    om.migrate_stage(h_src, s_ids, h_dst, d_ids)
+    H.assert_pool_equal(dst.host(), h_dst)
+    # explicit copy_kernel: llx_migrate_via_host runs its kernels (pack into / unpack from the bounce buffers)
+    s2 = synth.block_permutation(37, g["num_blocks"])[6:12]
+    d2 = synth.block_permutation(38, g["num_blocks"])[6:12]
+    c0 = llx.counters()
+    llx.migrate_via_host(src.pool, s2, dst.pool, d2, pin.dev_alias, nbytes)                      # auto: copy engines only
+    c1 = llx.counters()
+    assert c1["kernel_launches"] == c0["kernel_launches"]
+    llx.migrate_via_host(src.pool, s2, dst.pool, d2, pin.dev_alias, nbytes, opts=dict(copy_kernel=1))
+    c2 = llx.counters()
+    assert c2["copy_launches"] - c1["copy_launches"] >= 2
+    torch.cuda.synchronize()
+    om.migrate_stage(h_src, s2, h_dst, d2)
+    H.assert_pool_equal(dst.host(), h_dst)
+    pin.free()
+
+
 def test_peer_route_long_id_list_and_blocking_final_stage(env):
     """> 256 pairs through the (per-device) id ring on the peer route, then the blocking final-stage call, which falls
     back to the stream synchronize because the peer route's kernel carries no completion flag."""
