@@ -143,7 +143,6 @@ def oracle_sample_setup(pool_blocks=160):
     from oracle import kv_migration as om
     g = synth.CONFIGS["llama7b"]
     te = g["block_size"] * g["kv_heads"] * g["head_dim"]
-    rng = np.random.default_rng(0)
     src = om.new_pool(g["layers"], pool_blocks, te)
     for l in range(g["layers"]):
         # seeded fp16 bit patterns; one slice generated and rolled per layer to keep the setup short
@@ -154,7 +153,11 @@ def oracle_sample_setup(pool_blocks=160):
     s_tab = synth.block_permutation(1, pool_blocks)[:128]
     d_tab = synth.block_permutation(2, pool_blocks)[:128]
     te_tok = g["kv_heads"] * g["head_dim"]
-    vals = rng.integers(0, 0x3C00, size=(16, g["layers"], 2, te_tok), dtype=np.uint16)
+    vals = np.empty((16, g["layers"], 2, te_tok), dtype=np.uint16)      # the appended tokens: the generator the tests use
+    for t in range(16):
+        for l in range(g["layers"]):
+            for kv in range(2):
+                vals[t, l, kv] = synth.append_values_f16(3, START_TOKENS + t, l, kv, te_tok)
     values = lambda t, l, kv: vals[t - START_TOKENS, l, kv]
     return om, g, src, dst, s_tab, d_tab, values
 
@@ -169,6 +172,26 @@ def oracle_step(ctx):
 def step_bytes(g) -> int:
     block_bytes = 2 * g["layers"] * g["block_size"] * g["kv_heads"] * g["head_dim"] * g["elem_bytes"]
     return 2 * sum(SCHEDULE) * block_bytes          # read + written
+
+
+def attention_oracle_sample() -> dict:
+    """oracle.decode_attention.decode_attention_fp64 timed on ONE sequence of 2048 context tokens, one layer, LLaMA-7B heads
+    (a bounded sample of configs[4]'s decode batch: 32 sequences, 128..4096 tokens, 32 layers)."""
+    from oracle.decode_attention import decode_attention_fp64
+    g = synth.CONFIGS["llama7b"]
+    S, H, D = g["block_size"], g["kv_heads"], g["head_dim"]
+    nb, te = 128, S * H * D
+    pool = np.empty((1, 2, nb, te), dtype=np.uint16)
+    for kv in range(2):
+        pool[0, kv] = synth.slice_values_f16(4, 0, 0, kv, nb, te)
+    q = synth.queries_f16(5, 1, H, D)
+    bt = synth.block_permutation(6, nb)[:nb].reshape(1, nb).astype(np.int32)
+    ctx = np.array([nb * S], dtype=np.int32)
+    t0 = time.perf_counter()
+    decode_attention_fp64(pool, 0, q, bt, ctx, S, H, D)
+    dt = time.perf_counter() - t0
+    return {"kind": "oracle", "cores": 1, "sample": "one sequence of 2048 context tokens, one layer, 32 heads x 128 dims (fp64)",
+            "ms": dt * 1e3, "context_tokens_per_s": nb * S / dt}
 
 
 def cpu_baseline(budget_s=12.0) -> dict:
@@ -196,8 +219,7 @@ def cpu_baseline(budget_s=12.0) -> dict:
     return {"value": step_bytes(g) / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
             "host_cores_available": len(os.sched_getaffinity(0)),
             "final_stage_ms": statistics.median(fin) * 1e3, "pack_ms": t_pack * 1e3, "unpack_ms": t_unpack * 1e3,
-            "attention_oracle": "fp64 decode attention over configs[4]'s batch (65,590 context tokens): 1.8 s per layer on one core, "
-                                "timed in tests/test_gpu_attention.py::test_configs4_decode_batch_shape_within_tolerance",
+            "attention_oracle": attention_oracle_sample(),
             "sample": f"the whole configs[1] step (128 blocks, stages 112/14/2, 2 appends of 8 tokens) inside two "
                       f"160-block host pools instead of 2000-block ones; {len(times)} repetitions, median; "
                       f"oracle.kv_migration.staged_migration as it stands (NumPy row copies, single thread)",
@@ -235,19 +257,19 @@ def run_reference(args):
         return 0
     ctx = oracle_sample_setup()
     g = ctx[1]
-    for _ in range(min(args.warmup, 2)):
+    for _ in range(args.warmup):
         oracle_step(ctx)
-    steps = min(args.steps, 40)
+    steps = min(args.steps, 2000)       # ~0.13 s per step: the default 1000 steps take about two minutes
     t0 = time.perf_counter()
     for _ in range(steps):
         oracle_step(ctx)
     dt = (time.perf_counter() - t0) / steps
     val = step_bytes(g) / dt / 1e9
     sample = ("configs[1] step (128 blocks, stages 112/14/2, appends 8+8) inside two 160-block host pools; "
-              f"{steps} timed steps (capped at 40 to bound the run)")
+              f"{steps} timed steps after {args.warmup} warm-up steps")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-        "warmup": min(args.warmup, 2), "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u16", "data": "synthetic",
         "config": {"workload": WORKLOAD, "pools": "2 x 160 host blocks (sample)", "note": "CPU oracle, host memory"},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
@@ -469,6 +491,24 @@ def run_llx(args):
                    "frac_of_nominal_8TBps": step_bytes(g) / (single_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
                    "frac_of_measured_peak": step_bytes(g) / (single_ms * 1e-3) / 1e9 / peak}
 
+    # the step as round 1 defined it: every stage in plain stream order, the appends serialised between the
+    # stages on the migration stream — so that rounds stay comparable
+    saved_opts, w.stage_opts = w.stage_opts, None
+    r1_steps = min(args.steps, 200)
+    for _ in range(5):
+        w.step(stream, None)
+    stream.synchronize()
+    r0, r1 = mk()
+    r0.record(stream)
+    for _ in range(r1_steps):
+        w.step(stream, None)
+    r1.record(stream)
+    stream.synchronize()
+    w.stage_opts = saved_opts
+    r1_ms = r0.elapsed_time(r1) / r1_steps
+    round1_def = {"ms_per_step": r1_ms, "value": step_bytes(g) / (r1_ms * 1e-3) / 1e9, "steps": r1_steps,
+                  "definition": "plain stream order, appends between the stages on the migration stream (bench.py --serial-appends)"}
+
     # ---- end to end through pinned host buffers (block fusion path) -----------------------
     # llx_migrate_via_host: gather -> pinned host buffer -> scatter, chunked so that both directions of the
     # host link are busy at once; the sequential llx_pack -> llx_unpack pair is timed beside it.
@@ -509,6 +549,10 @@ def run_llx(args):
     e2e_seq_val = replicas.sum_over_ranks(2 * n * w.src.block_bytes) / (e2e_seq_ms * 1e-3) / 1e9
     e2e_kern_val = replicas.sum_over_ranks(2 * n * w.src.block_bytes) / (e2e_kern_ms * 1e-3) / 1e9
     pin.free()
+    link = None
+    if world == 1:
+        import bench_suite
+        link = bench_suite.link_peak(torch)      # the host link's own peak, measured in this run
 
     # ---- final-stage downtime (S4): host wall clock around the C-ABI call + stream sync ----
     downtime = measure_downtime(torch, llx, w, stream, reps=args.downtime_reps)
@@ -517,9 +561,16 @@ def run_llx(args):
     block_bytes = w.src.block_bytes
     traffic = profiled_traffic()
     suite = None
-    if args.suite and world == 1:
+    configs = None
+    overlap_on = w.stage_opts is not None
+    if world == 1 and (args.suite or not args.no_configs):
         del w
-        suite = run_suite(torch, llx, stream)
+        import bench_suite
+        bench_suite._free(torch)
+        if not args.no_configs:
+            configs = bench_suite.baseline_configs(torch, llx, stream)      # configs[2..4] + reference points, bounded
+        if args.suite:
+            suite = run_suite(torch, llx, stream)
 
     if rank != 0:
         return 0
@@ -534,13 +585,14 @@ def run_llx(args):
                                "stage waits for the appends" if dec is not None else "everything on one stream (--serial-appends)"),
                    "stage_order": ("stages 0 and 1 are launched with llx_launch_opts.overlap_prev=1 (independent of every launch back "
                                    "to the previous final stage: disjoint blocks; they may start while it drains, completion order kept); "
-                                   "the final stage in plain stream order" if w.stage_opts is not None
+                                   "the final stage in plain stream order" if overlap_on
                                    else "plain stream order for every stage"),
                    "bytes_per_step_rd_plus_wr": step_bytes(g), "parallelism": f"replicas x{world} (no collective)",
                    "l2": "inputs larger than L2 (2.1 GB of traffic per step vs 126 MB L2), no flush needed",
                    "copy_kernel": "bulk-async smem ring (llx_copy_bulk)" if llx.get_option(llx.OPT_COPY_KERNEL) in (0, 2) else "vec16"},
         "pct_of_nominal_8TBps": 100.0 * value / world / NOMINAL_HBM_GBS,
         "pct_of_measured_copy_peak": 100.0 * value / world / peak,
+        "value_round1_definition": round1_def,
         "downtime_us": downtime,
         "breakdown": breakdown,
         "single_shot_2048": single_shot,
@@ -548,10 +600,16 @@ def run_llx(args):
                      "traffic": traffic["bytes"], "traffic_source": traffic["source"], "traffic_commit": traffic["commit"],
                      "kernel": "llx_copy_bulk (stage 0: 112 blocks)", "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": stage0_bytes, "avg_launch_ms": stage0_ms,
-                     "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS},
+                     "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
+                     "whole_step_frac_of_nominal_8TBps": value / world / NOMINAL_HBM_GBS,
+                     "downtime_us": {k: downtime[k] for k in ("host_median", "host_p99", "host_wait_call_median", "gpu_median") if k in downtime},
+                     "configs": configs if configs is not None else "not run (--no-configs, or N > 1)"},
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": n * block_bytes,
                 "d2h_bytes_per_step": n * block_bytes, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "gpu_launches_per_step": e2e_launches,
+                "link_peak_gbs": link,
+                "frac_of_link_duplex": (e2e_val / link["duplex_GBps_both_directions_summed"]) if link else None,
+                "kernel_route_frac_of_link_duplex": (e2e_kern_val / link["duplex_GBps_both_directions_summed"]) if link else None,
                 "path": "llx_migrate_via_host, default host leg: one pitched copy-engine transfer per block (2L tiles at a constant "
                         "stride) into the pinned buffer and out of it, D2H and H2D at the same time in groups of ~16 MiB; no kernel "
                         "on this route (host wall clock incl. stream sync)",
@@ -670,6 +728,8 @@ def main():
     ap.add_argument("--suite", action="store_true", help="also run the length sweep, 30B batch and interference configs")
     ap.add_argument("--downtime-reps", type=int, default=200)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true",
+                    help="skip the bounded legs over BASELINE.json configs[2..4] and the reference points (about a minute)")
     ap.add_argument("--no-overlap", action="store_true",
                     help="launch every stage in plain stream order (no llx_launch_opts.overlap_prev on stages 0 and 1)")
     ap.add_argument("--serial-appends", action="store_true",

@@ -339,7 +339,21 @@ def batch_30b(torch, llx, stream, seed=0):
 
 
 # ---- configs[4] first half: interference with a decode step -----------------------------------
-def interference(torch, llx, stream_mig_unused, paced_only=False):
+def _power_state(torch):
+    """SM clock, power draw and clock-event reasons right now (NVML), or None."""
+    try:
+        import pynvml
+        pynvml.nvmlInit()
+        h = pynvml.nvmlDeviceGetHandleByIndex(torch.cuda.current_device())
+        return {"sm_mhz": pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM), "power_w": pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0,
+                "reasons": hex(pynvml.nvmlDeviceGetCurrentClocksEventReasons(h))}
+    except Exception:  # noqa: BLE001
+        return None
+
+
+def interference(torch, llx, stream_mig_unused, paced_only=False, budgets=None):
+    """budgets: None = the full case list; a tuple of GB/s = the bounded list of bench.py's default line (one unthrottled
+    migration at the step's start, then a looped migration under each budget)."""
     g = dict(synth.CONFIGS["llama7b"])
     L, H, D, S = g["layers"], g["kv_heads"], g["head_dim"], g["block_size"]
     B = 32
@@ -435,12 +449,16 @@ def interference(torch, llx, stream_mig_unused, paced_only=False):
                n_for(bw), 0, bw) for bw in (2400, 1600, 800, 400, 200, 100, 65, 20)]
     if paced_only:
         cases = [c for c in cases if 0 < c[3] < 500]
+    if budgets is not None:
+        cases = [cases[0]] + [(f"looped, budget {bw} GB/s (paced on all SMs)", n_for(bw), 0, bw) for bw in budgets]
+    res["power_state_before_cases"] = _power_state(torch)
     for label, n_mig, cap, bw in cases:
         t, m, ratio = with_migration(n_mig, cap, bw)
         res["cases"].append({"case": label, "migrations": n_mig, "max_ctas": cap, "bandwidth_budget_GBps": bw,
                              "decode_step_ms": t, "slowdown_pct": 100.0 * (ratio - 1.0),
                              "migration_GBps_while_overlapped": n_mig * mig_bytes / m / 1e6,
                              "bandwidth_share_pct": 100.0 * min(1.0, t / m) * n_mig * mig_bytes / (kv_bytes_step + min(1.0, t / m) * n_mig * mig_bytes)})
+    res["power_state_after_cases"] = _power_state(torch)
     res["note"] = ("slowdown = median of per-pair ratios (step with migration / isolated step right before it); any concurrent kernel of another "
                    "stream costs ~3.5 % (floor, independent of its rate: launch gaps of the 64-launch step grow), a co-resident "
                    "CTA holding > ~6 KB shared memory costs +30 % (L1 carve-out), and a few full-speed CTAs make their SMs "
@@ -1123,6 +1141,82 @@ def small_tiles(torch, llx, stream):
         out.append(row)
         del p
         _free(torch)
+    return out
+
+
+def link_peak(torch, nbytes=1 << 30, reps=10):
+    """Host-link peak measured in THIS run: best of `reps` plain 1 GiB pinned copy-engine transfers each way, and both ways
+    at once on two streams (the full-duplex floor a round trip through the host is held against)."""
+    dev_a = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    dev_b = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    host_a = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    host_b = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    res = {"bytes_each_way": nbytes, "reps": reps}
+    with torch.cuda.stream(s1):
+        t = _time_stream(torch, s1, lambda: host_a.copy_(dev_a, non_blocking=True), reps=reps, warm=1)
+        res["d2h_GBps"] = nbytes / t["min_ms"] / 1e6
+        t = _time_stream(torch, s1, lambda: dev_b.copy_(host_b, non_blocking=True), reps=reps, warm=1)
+        res["h2d_GBps"] = nbytes / t["min_ms"] / 1e6
+    both = []
+    for _ in range(reps + 1):
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(s1)
+        s2.wait_event(a)
+        with torch.cuda.stream(s1):
+            host_a.copy_(dev_a, non_blocking=True)
+        with torch.cuda.stream(s2):
+            dev_b.copy_(host_b, non_blocking=True)
+        s1.wait_stream(s2)
+        b.record(s1)
+        torch.cuda.synchronize()
+        both.append(a.elapsed_time(b))
+    t_both = min(both[1:])
+    res["duplex_ms_per_GiB_each_way"] = t_both * (1 << 30) / nbytes
+    res["duplex_GBps_both_directions_summed"] = 2 * nbytes / t_both / 1e6
+    del dev_a, dev_b, host_a, host_b
+    return res
+
+
+def baseline_configs(torch, llx, stream):
+    """The BASELINE.json configs other than configs[1], bounded for bench.py's default line (about a minute in all):
+    configs[2] the length sweep, configs[3] the LLaMA-30B batch (the config's draw and the draw whose sample mean is the
+    nominal 512 tokens), configs[4] the batch-32 decode step alone / next to an unthrottled migration / next to a 25 and
+    a 12 GB/s budget (paired, with the power state), SURVEY 8(d)'s reference points.  Numbers only; the long notes stay
+    in the full legs (`bench.py --suite`)."""
+    out = {}
+    g = synth.CONFIGS["llama7b"]
+    nb = g["num_blocks"]
+    p = Pools(torch, llx, g, nb, nb)
+    sweep = length_sweep(torch, llx, p, stream, nb)
+    out["configs2_length_sweep_llama7b"] = [
+        {"tokens": r["tokens"], "single_shot_GBps": round(r["single_shot_GBps"], 1), "stage0_GBps": round(r["stage0_GBps"], 1),
+         "final_stage_gpu_us_cold": round(r["final_stage_gpu_us_cold"], 2), "final_stage_host_us_median": round(r["final_stage_host_us_median"], 2),
+         "blocking_copy_downtime_us": round(r["blocking_copy_downtime_us"], 1)} for r in sweep]
+    refs = reference_points(torch, llx, p, stream, nb)
+    out["reference_points_2048tok_GBps"] = {k: round(v, 1) for k, v in refs.items() if k.endswith("_GBps")}
+    del p
+    _free(torch)
+    b = {}
+    for name, seed in (("seed0_as_specified", 0), ("seed2_sample_mean_507tok", 2)):
+        r = batch_30b(torch, llx, stream, seed=seed)
+        b[name] = r if "skipped" in r else {k: (round(r[k], 2) if isinstance(r[k], float) else r[k]) for k in
+                                            ("total_blocks", "payload_GiB", "mean_tokens", "one_launch_ms", "one_launch_GBps", "sequential_GBps")}
+    out["configs3_batch_llama30b_64req"] = b
+    r = interference(torch, llx, stream, budgets=(25, 12))
+    if "skipped" in r:
+        out["configs4_interference_decode_batch32"] = r
+    else:
+        out["configs4_interference_decode_batch32"] = {
+            "decode_step_alone_ms": round(r["decode_step_alone_ms"], 4), "decode_attention_GBps": round(r["decode_attention_GBps"], 1),
+            "migration_alone_GBps": round(r["migration_alone_GBps"], 1),
+            "cases": [{"case": c["case"], "budget_GBps": c["bandwidth_budget_GBps"], "decode_step_ms": round(c["decode_step_ms"], 4),
+                       "slowdown_pct": round(c["slowdown_pct"], 2), "migration_GBps": round(c["migration_GBps_while_overlapped"], 1)}
+                      for c in r["cases"]],
+            "power_state_before": r["power_state_before_cases"], "power_state_after": r["power_state_after_cases"],
+            "method": "paired: each step next to a migration follows an isolated step; median of 8 per-pair ratios"}
     return out
 
 

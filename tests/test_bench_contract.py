@@ -49,5 +49,19 @@ def test_llx_arm_prints_the_contract_line_with_roofline_e2e_and_clocks():
     assert e["unit"] == "GB/s" and e["h2d_bytes_per_step"] == e["d2h_bytes_per_step"] == 1 << 30 and 0 < e["value"] < 0.2 * d["value"]
     cb = d["cpu_baseline"]
     assert cb["kind"] == "oracle" and cb["cores"] == 1 and 0 < cb["value"] < d["value"]
+    assert cb["attention_oracle"]["ms"] > 0                                  # a timed sample, not a sentence
+    # every BASELINE.json config and both halves of the metric are in the ONE line ("do this" item 1)
+    cf = r["configs"]
+    assert [x["tokens"] for x in cf["configs2_length_sweep_llama7b"]] == [256, 512, 1024, 2048, 4096, 8192]
+    assert all(x["single_shot_GBps"] > 1000 and 0 < x["final_stage_gpu_us_cold"] < 100 for x in cf["configs2_length_sweep_llama7b"])
+    assert all(v.get("one_launch_GBps", 0) > 1000 or "skipped" in v for v in cf["configs3_batch_llama30b_64req"].values())
+    c4 = cf["configs4_interference_decode_batch32"]
+    assert "skipped" in c4 or ([c["budget_GBps"] for c in c4["cases"]] == [0, 25, 12] and c4["decode_step_alone_ms"] > 0)
+    assert {"torch_contiguous_copy_GBps", "per_tile_memcpy_loop_GBps"} <= set(cf["reference_points_2048tok_GBps"])
+    assert r["downtime_us"]["host_median"] > 0 and r["downtime_us"]["gpu_median"] > 0
+    lp = e["link_peak_gbs"]
+    assert lp["d2h_GBps"] > 10 and lp["h2d_GBps"] > 10 and 0.3 < e["frac_of_link_duplex"] < 1.05
+    v1 = d["value_round1_definition"]
+    assert 0.8 * d["value"] < v1["value"] <= 1.02 * d["value"]
     assert {"sm_mhz", "sm_max_mhz", "reasons"} <= set(d["clocks"])
     assert not {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"} & set(d["clocks"]["reasons"])
