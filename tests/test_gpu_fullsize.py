@@ -161,9 +161,9 @@ def test_llama7b_2048_tokens_three_stages_with_appends(env):
             check_untouched_and_mapping_on_device(src, dst, s_tab, d_tab, (0, 31))
 
 
-@pytest.mark.parametrize("tokens", [256, 8192])
+@pytest.mark.parametrize("tokens", [256, 512, 1024, 2048, 4096, 8192])
 def test_llama7b_length_sweep_ends_single_shot_vs_two_stage(env, tokens):
-    """configs[2] end points: single-shot copy == (n-2, 2) staged copy == oracle on sampled layers."""
+    """configs[2], every length of the sweep: single-shot copy == (n-2, 2) staged copy == oracle on sampled layers."""
     H, llx = env
     g = synth.CONFIGS["llama7b"]
     if free_gib() < 50:
